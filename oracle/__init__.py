@@ -1,0 +1,15 @@
+"""CPU fp64 oracle for the DIMOS neighbour-list + nonbonded hot path.
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product package never imports this.
+"""
+from .dimos_oracle import (  # noqa: F401
+    METHOD_EWALD_REAL,
+    METHOD_RF,
+    NonbondedResult,
+    lorentz_berthelot,
+    needs_rebuild,
+    neighbor_pairs,
+    nonbonded,
+    num_threads,
+)

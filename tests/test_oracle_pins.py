@@ -1,0 +1,350 @@
+"""Pins for the CPU fp64 oracle (oracle/dimos_oracle.c): closed forms, textbook points, invariants,
+finite differences, brute force vs cell list vs scipy.  None of these re-type the oracle's own
+expression for a quantity and compare it with itself: each checks the oracle against something the
+paper or the mathematics fixes independently (SURVEY.md §8(c) "What pins each part")."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2503_20541_b200 import workloads as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+KE = wl.COULOMB_CONST
+Q = {"O": wl.Q_O, "H": wl.Q_H}
+TYPE = {"O": 0, "H": 1}
+BIGBOX = np.array([50.0, 50.0, 50.0])
+
+
+def lj_table():
+    return oracle.lorentz_berthelot([wl.SIGMA_O, 0.0], [wl.EPS_O, 0.0])
+
+
+def two_particles(kind_a, kind_b, r, r_cut, method=oracle.METHOD_RF, excluded=False, direction=None, **kw):
+    """Energy components and radial force on atom 0 along +d for an isolated pair in a huge box."""
+    if direction is None:
+        direction = np.array([0.3, -0.5, 0.81])
+    u = direction / np.linalg.norm(direction)
+    pos = np.array([[10.0, 11.0, 12.0] + r * u, [10.0, 11.0, 12.0]])
+    excl = np.array([[0, 1]], dtype=np.int32) if excluded else None
+    res = oracle.nonbonded(pos, [Q[kind_a], Q[kind_b]], [TYPE[kind_a], TYPE[kind_b]], lj_table(), BIGBOX, r_cut,
+                           method=method, excl_pairs=excl, algorithm="bruteforce", **kw)
+    f_radial = float(res.F[0] @ u)
+    # transverse components must vanish and Newton III must hold
+    assert np.allclose(res.F[0] - f_radial * u, 0.0, atol=1e-9 * max(1.0, abs(f_radial)))
+    assert np.allclose(res.F[0] + res.F[1], 0.0, atol=1e-9 * max(1.0, abs(f_radial)))
+    return res, f_radial
+
+
+# --- golden closed-form values (SURVEY.md §8(c), 30-digit mpmath, independent of this repo) --------------
+def _golden_rows():
+    rows = []
+    with open(os.path.join(GOLDEN, "two_particle_closed_forms.txt")) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            kind, pair, r, rc, qty, val = line.split()
+            rows.append((kind, pair, float(r), float(rc), qty, float(val)))
+    return rows
+
+
+@pytest.mark.parametrize("row", _golden_rows(), ids=lambda r: f"{r[0]}-{r[1]}-{r[2]}-{r[4]}")
+def test_two_particle_golden(row):
+    kind, pair, r, rc, qty, val = row
+    method = oracle.METHOD_RF if kind == "rf" else oracle.METHOD_EWALD_REAL
+    res, f = two_particles(pair[0], pair[1], r, rc, method=method, excluded=(kind == "excl"))
+    got = {
+        "U": res.E[0], "U_LJ": res.E[1], "U_RF": res.E[2], "U_COUL": res.E[2], "f": f, "r_dot_f": r * f,
+    }[qty]
+    if kind == "excl":
+        assert res.E[1] == 0.0 and res.E[2] == 0.0  # excluded pair: no LJ, no pair Coulomb
+        assert res.E[3] == res.E[0]
+    assert got == pytest.approx(val, rel=2e-13, abs=1e-15)
+
+
+# --- textbook points of Eq. (4) ---------------------------------------------------------------------------
+def test_lj_zero_crossing_and_minimum():
+    tab = lj_table()
+    pos = lambda r: np.array([[5.0 + r, 5.0, 5.0], [5.0, 5.0, 5.0]])
+    zero = [0.0, 0.0]
+    r0 = wl.SIGMA_O
+    res = oracle.nonbonded(pos(r0), zero, [0, 0], tab, BIGBOX, 1.0, algorithm="bruteforce")
+    assert abs(res.E[1]) < 1e-12 and res.E[2] == 0.0  # U_LJ(sigma) = 0
+    rmin = 2.0 ** (1.0 / 6.0) * wl.SIGMA_O
+    res = oracle.nonbonded(pos(rmin), zero, [0, 0], tab, BIGBOX, 1.0, algorithm="bruteforce")
+    assert res.E[1] == pytest.approx(-wl.EPS_O, rel=1e-14)  # well depth -eps at 2^(1/6) sigma
+    assert np.abs(res.F).max() < 1e-11  # force vanishes at the minimum
+    # repulsive inside the minimum, attractive outside
+    inside = oracle.nonbonded(pos(0.9 * rmin), zero, [0, 0], tab, BIGBOX, 1.0, algorithm="bruteforce")
+    outside = oracle.nonbonded(pos(1.1 * rmin), zero, [0, 0], tab, BIGBOX, 1.0, algorithm="bruteforce")
+    assert inside.F[0, 0] > 0 and outside.F[0, 0] < 0
+
+
+def test_lorentz_berthelot_eq5():
+    tab = oracle.lorentz_berthelot([0.3, 0.1, 0.25], [0.5, 2.0, 0.0])
+    assert tab[0, 1, 0] == pytest.approx(0.2) and tab[1, 0, 0] == pytest.approx(0.2)
+    assert tab[0, 1, 1] == pytest.approx(1.0) and tab[1, 0, 1] == pytest.approx(1.0)
+    assert tab[0, 2, 1] == 0.0 and tab[2, 2, 1] == 0.0  # eps = 0 type has no LJ with anything
+    assert tab[2, 2, 0] == pytest.approx(0.25)
+    water = lj_table()
+    assert water[0, 0, 0] == wl.SIGMA_O and water[0, 0, 1] == pytest.approx(wl.EPS_O)
+    assert water[0, 1, 1] == 0.0 and water[1, 1, 1] == 0.0  # LJ on O only (configs[0])
+
+
+# --- reaction field, Eq. (8) ------------------------------------------------------------------------------
+@pytest.mark.parametrize("eps_rf,rc", [(78.5, 0.9), (78.5, 1.0), (2.0, 1.3), (1.0, 0.8)])
+def test_rf_energy_vanishes_at_cutoff_and_force_limit(eps_rf, rc):
+    # U_RFA(r_c) = 0 for any eps_rf, r_c (only holds with reading C-1); force limit 3 k_e qq / ((2eps+1) rc^2)
+    r = rc * (1.0 - 1e-12)
+    res, f = two_particles("H", "H", r, rc, eps_rf=eps_rf)
+    assert abs(res.E[2]) < 1e-8
+    assert f == pytest.approx(3.0 * KE * wl.Q_H**2 / ((2 * eps_rf + 1) * rc * rc), rel=1e-9)
+    # just outside the cutoff: nothing at all
+    res, f = two_particles("H", "H", rc * (1 + 1e-12), rc, eps_rf=eps_rf)
+    assert res.E[0] == 0.0 and f == 0.0 and res.n_pairs == 0
+
+
+def test_rf_with_unit_dielectric_is_shifted_coulomb():
+    # eps_rf = 1 => k_rf = 0, c_rf = 1/r_c: the textbook shifted Coulomb potential k_e qq (1/r - 1/r_c)
+    res, f = two_particles("H", "H", 0.5, 2.0, eps_rf=1.0)
+    assert res.E[2] == pytest.approx(KE * wl.Q_H**2 * (1 / 0.5 - 1 / 2.0), rel=1e-14)
+    assert f == pytest.approx(KE * wl.Q_H**2 / 0.25, rel=1e-14)  # pure Coulomb force
+
+
+def test_coulomb_constant_enters_linearly():
+    a, _ = two_particles("O", "H", 0.4, 1.0, coulomb_const=1.0)
+    b, _ = two_particles("O", "H", 0.4, 1.0, coulomb_const=KE)
+    assert b.E[2] == pytest.approx(KE * a.E[2], rel=1e-14)
+    assert b.E[1] == a.E[1]
+
+
+# --- Ewald real space + exclusion correction --------------------------------------------------------------
+@pytest.mark.parametrize("r", [0.09572, 0.2, 0.55, 0.97])
+def test_ewald_real_plus_excluded_complement_is_plain_coulomb(r):
+    # erfc + erf = 1: [k qq erfc(ar)/r] - [-k qq erf(ar)/r] = k qq / r, same for the forces
+    real, f_real = two_particles("O", "H", r, 1.0, method=oracle.METHOD_EWALD_REAL)
+    corr, f_corr = two_particles("O", "H", r, 1.0, method=oracle.METHOD_EWALD_REAL, excluded=True)
+    qq = wl.Q_O * wl.Q_H
+    assert real.E[2] - corr.E[3] == pytest.approx(KE * qq / r, rel=1e-13)
+    assert f_real - f_corr == pytest.approx(KE * qq / r**2, rel=1e-12)
+
+
+def test_ewald_exclusion_correction_small_r_limit_and_no_cutoff():
+    alpha = 3.12
+    corr, _ = two_particles("H", "H", 1e-7, 1.0, method=oracle.METHOD_EWALD_REAL, excluded=True, alpha=alpha)
+    assert corr.E[3] == pytest.approx(-2 * alpha * KE * wl.Q_H**2 / math.sqrt(math.pi), rel=1e-9)
+    # correction applies to excluded pairs beyond r_cut too (reading C-15)
+    far, _ = two_particles("H", "H", 1.7, 1.0, method=oracle.METHOD_EWALD_REAL, excluded=True, alpha=alpha)
+    assert far.E[3] == pytest.approx(-KE * wl.Q_H**2 * math.erf(alpha * 1.7) / 1.7, rel=1e-13)
+    # alpha -> 0 turns the real-space term into plain Coulomb
+    plain, f = two_particles("H", "H", 0.4, 1.0, method=oracle.METHOD_EWALD_REAL, alpha=1e-9)
+    assert plain.E[2] == pytest.approx(KE * wl.Q_H**2 / 0.4, rel=1e-8)
+
+
+# --- small periodic systems -------------------------------------------------------------------------------
+def small_box(m=24, edge=2.2, seed=7):
+    return wl.make_water_box(m, edge, seed)
+
+
+def energy(pos, wb, box=None, method=oracle.METHOD_RF, r_cut=1.0, algorithm="bruteforce"):
+    box = wb.box if box is None else box
+    return oracle.nonbonded(pos, wb.charge, wb.type, lj_table(), box, r_cut, method=method,
+                            excl_pairs=wb.excl_pairs, algorithm=algorithm)
+
+
+def _no_pair_near_cutoff(pos, box, r_cut, margin):
+    inner = oracle.neighbor_pairs(pos, box, r_cut - margin, None, "bruteforce")
+    outer = oracle.neighbor_pairs(pos, box, r_cut + margin, None, "bruteforce")
+    return len(inner) == len(outer)
+
+
+@pytest.mark.parametrize("method", [oracle.METHOD_RF, oracle.METHOD_EWALD_REAL])
+def test_forces_are_minus_finite_difference_gradient(method):
+    wb = small_box()
+    pos = wb.pos.astype(np.float64)
+    assert _no_pair_near_cutoff(pos, wb.box, 1.0, 1e-4)
+    res = energy(pos, wb, method=method)
+    h = 1e-6
+    rng = np.random.default_rng(3)
+    for i in rng.choice(wb.n_atoms, size=10, replace=False):
+        for a in range(3):
+            p, m = pos.copy(), pos.copy()
+            p[i, a] += h
+            m[i, a] -= h
+            fd = -(energy(p, wb, method=method).E[0] - energy(m, wb, method=method).E[0]) / (2 * h)
+            assert res.F[i, a] == pytest.approx(fd, rel=2e-6, abs=2e-4)
+
+
+@pytest.mark.parametrize("method", [oracle.METHOD_RF, oracle.METHOD_EWALD_REAL])
+def test_newton_third_law_and_virial_symmetry(method):
+    wb = small_box(m=40, edge=2.4, seed=11)
+    res = energy(wb.pos, wb, method=method)
+    assert np.abs(res.F.sum(axis=0)).max() < 1e-9
+    assert np.abs(res.W - res.W.T).max() < 1e-9
+    assert res.E[0] == pytest.approx(res.E[1] + res.E[2] + res.E[3], rel=1e-15)
+
+
+@pytest.mark.parametrize("method", [oracle.METHOD_RF, oracle.METHOD_EWALD_REAL])
+def test_virial_is_minus_strain_derivative_of_energy(method):
+    # W_aa = -dE/d(eps_aa) under x_a -> (1+eps) x_a, L_a -> (1+eps) L_a with r_c fixed; tr W = -dE/dlambda
+    wb = small_box(m=30, edge=2.3, seed=5)
+    pos = wb.pos.astype(np.float64)
+    assert _no_pair_near_cutoff(pos, wb.box, 1.0, 1e-4)
+    res = energy(pos, wb, method=method)
+    h = 1e-7
+    for a in range(3):
+        def scaled(s):
+            p, b = pos.copy(), wb.box.copy()
+            p[:, a] *= s
+            b[a] *= s
+            return energy(p, wb, box=b, method=method).E[0]
+        fd = -(scaled(1 + h) - scaled(1 - h)) / (2 * h)
+        assert res.W[a, a] == pytest.approx(fd, rel=1e-5, abs=1e-3)
+    fd_iso = -(energy(pos * (1 + h), wb, box=wb.box * (1 + h), method=method).E[0]
+               - energy(pos * (1 - h), wb, box=wb.box * (1 - h), method=method).E[0]) / (2 * h)
+    assert np.trace(res.W) == pytest.approx(fd_iso, rel=1e-5, abs=1e-3)
+
+
+def test_translation_and_periodic_image_invariance():
+    wb = small_box()
+    pos = wb.pos.astype(np.float64)
+    ref = energy(pos, wb)
+    shift = np.array([0.37, -5.21, 13.9])  # arbitrary, larger than the box in two components
+    moved = energy(pos + shift, wb)
+    assert moved.E[0] == pytest.approx(ref.E[0], rel=1e-11)
+    assert np.allclose(moved.F, ref.F, rtol=0, atol=1e-7)
+    assert moved.n_pairs == ref.n_pairs
+    img = pos.copy()
+    img[5] += np.array([wb.box[0], 0.0, -2 * wb.box[2]])
+    imaged = energy(img, wb)
+    assert imaged.E[0] == pytest.approx(ref.E[0], rel=1e-12)
+    assert np.allclose(imaged.F, ref.F, rtol=0, atol=1e-8)
+    # neighbour set unchanged as well
+    a = oracle.neighbor_pairs(pos, wb.box, 1.1, wb.excl_pairs, "bruteforce")
+    b = oracle.neighbor_pairs(img, wb.box, 1.1, wb.excl_pairs, "bruteforce")
+    assert np.array_equal(a, b)
+
+
+def test_exclusions_single_and_double_water():
+    one = wl.make_water_box(1, 3.0, 1)
+    res = energy(one.pos, one)
+    assert res.n_pairs == 0 and res.E[0] == 0.0 and np.all(res.F == 0.0)
+    assert len(oracle.neighbor_pairs(one.pos, one.box, 1.1, one.excl_pairs, "bruteforce")) == 0
+    # without the exclusion list the three intramolecular pairs appear
+    assert len(oracle.neighbor_pairs(one.pos, one.box, 1.1, None, "bruteforce")) == 3
+    two = wl.make_water_box(8, 0.9 * 2, 2)  # 2x2x2 lattice sites, all 8 used -> pick the first two molecules
+    pos = two.pos[:6].astype(np.float64)
+    pos[3:6] = pos[0:3] + np.array([0.3, 0.05, -0.02])
+    pairs = oracle.neighbor_pairs(pos, np.array([5.0, 5.0, 5.0]), 1.1, two.excl_pairs[:6], "bruteforce")
+    assert len(pairs) == 9 and all(i < 3 <= j for i, j in pairs)  # exactly the 9 intermolecular pairs
+    res = oracle.nonbonded(pos, two.charge[:6], two.type[:6], lj_table(), [5.0, 5.0, 5.0], 1.0,
+                           excl_pairs=two.excl_pairs[:6], algorithm="bruteforce")
+    assert res.n_pairs == 9
+
+
+# --- the two enumerations agree; the set agrees with scipy ------------------------------------------------
+@pytest.mark.parametrize("case", ["config0", "config1", "slab_n2", "ewald_small"])
+def test_celllist_equals_bruteforce(case):
+    if case == "config0":  # degenerate 1x1x1 grid, r_nl > L/2
+        wb, rc, skin, method = wl.make_config(0), 0.9, 0.1, oracle.METHOD_RF
+        box = wb.box
+    elif case == "config1":
+        wb, rc, skin, method = wl.make_config(1), 1.0, 0.1, oracle.METHOD_RF
+        box = wb.box
+    elif case == "slab_n2":  # 2 cells along x and y, 3 along z: stencil de-duplication
+        wb, rc, skin, method = wl.make_water_box(150, 2.5, 21), 1.0, 0.1, oracle.METHOD_RF
+        box = np.array([2.5, 2.3, 3.4])
+    else:
+        wb, rc, skin, method = wl.make_water_box(100, 2.2, 4), 1.0, 0.1, oracle.METHOD_EWALD_REAL
+        box = wb.box
+    tab = lj_table()
+    kw = dict(method=method, excl_pairs=wb.excl_pairs, band=1e-5)
+    b = oracle.nonbonded(wb.pos, wb.charge, wb.type, tab, box, rc, algorithm="bruteforce", **kw)
+    c = oracle.nonbonded(wb.pos, wb.charge, wb.type, tab, box, rc, algorithm="celllist", **kw)
+    assert b.n_pairs == c.n_pairs
+    scale = np.sqrt((b.F**2).sum(axis=1).mean())
+    assert np.abs(b.F - c.F).max() < 1e-12 * scale
+    assert np.allclose(b.E, c.E, rtol=1e-12, atol=1e-9)
+    assert np.allclose(b.W, c.W, rtol=1e-12, atol=1e-8)
+    assert np.array_equal(b.allow, c.allow)
+    pb = oracle.neighbor_pairs(wb.pos, box, rc + skin, wb.excl_pairs, "bruteforce")
+    pc = oracle.neighbor_pairs(wb.pos, box, rc + skin, wb.excl_pairs, "celllist")
+    assert np.array_equal(pb, pc)
+
+
+def test_neighbor_set_matches_scipy_kdtree():
+    from scipy.spatial import cKDTree
+
+    wb = wl.make_config(1)  # 9,000 atoms
+    r_nl = 1.1
+    pos = wb.pos.astype(np.float64)
+    tree = cKDTree(pos, boxsize=wb.box)
+    kd = tree.query_pairs(r_nl, output_type="ndarray")
+    kd = np.sort(kd, axis=1)
+    n = wb.n_atoms
+    key = kd[:, 0].astype(np.int64) * n + kd[:, 1]
+    excl_key = wb.excl_pairs[:, 0].astype(np.int64) * n + wb.excl_pairs[:, 1]
+    key = np.setdiff1d(key, excl_key)
+    # scipy uses r <= r_nl, the oracle r < r_nl: remove ties (none expected) by checking sizes
+    mine = oracle.neighbor_pairs(pos, wb.box, r_nl, wb.excl_pairs, "celllist")
+    mine_key = mine[:, 0].astype(np.int64) * n + mine[:, 1]
+    assert np.array_equal(np.sort(key), mine_key)  # oracle output is lexicographically sorted already
+    assert np.all(np.diff(mine_key) > 0)
+
+
+def test_config0_matches_surveyors_independent_numbers():
+    vals = {}
+    with open(os.path.join(GOLDEN, "config0_magnitudes.txt")) as fh:
+        for line in fh:
+            if not line.startswith("#") and line.strip():
+                k, v = line.split()
+                vals[k] = float(v)
+    wb = wl.make_config(0)
+    res = oracle.nonbonded(wb.pos, wb.charge, wb.type, lj_table(), wb.box, 0.9, excl_pairs=wb.excl_pairs,
+                           algorithm="bruteforce")
+    assert res.n_pairs == int(vals["pairs_lt_rcut"])
+    assert len(oracle.neighbor_pairs(wb.pos, wb.box, 1.0, wb.excl_pairs, "bruteforce")) == int(vals["pairs_lt_rnl"])
+    assert res.E[0] == pytest.approx(vals["E_total_approx"], abs=0.6)
+    assert np.sqrt((res.F**2).sum(axis=1).mean()) == pytest.approx(vals["rmsF_approx"], abs=0.6)
+
+
+# --- rebuild trigger, PAPER.md:175 ------------------------------------------------------------------------
+def test_needs_rebuild_definition_and_strictness():
+    ref = np.zeros((5, 3))
+    pos = ref.copy()
+    skin = 0.1
+    assert oracle.needs_rebuild(pos, ref, skin) == (False, 0.0)
+    pos[3] = [0.03, 0.04, 0.0]  # |dr| = 0.05 = skin/2 exactly: strict ">" => no rebuild
+    flag, m = oracle.needs_rebuild(pos, ref, skin)
+    assert m == pytest.approx(0.05) and flag is False
+    pos[3] = [0.03, 0.04, 0.001]
+    assert oracle.needs_rebuild(pos, ref, skin)[0] is True
+    # Euclidean norm, not max-norm: every component is < skin/2 but |dr| = 0.0520 > 0.05
+    pos[3] = [0.03, 0.03, 0.03]
+    assert oracle.needs_rebuild(pos, ref, skin)[0] is True
+    pos[3] = [0.028, 0.028, 0.028]  # |dr| = 0.0485 < 0.05
+    assert oracle.needs_rebuild(pos, ref, skin)[0] is False
+    # raw coordinates: a jump by a whole box length counts as displacement (caller must not re-wrap, §8(b))
+    pos[3] = [2.0, 0.0, 0.0]
+    assert oracle.needs_rebuild(pos, ref, skin) == (True, 2.0)
+
+
+def test_verlet_list_validity_invariant():
+    # a list built with radius r_c + r_g holds every pair within r_c for as long as
+    # no atom has moved more than r_g/2.
+    wb = small_box(m=60, edge=2.6, seed=9)
+    rc, skin = 1.0, 0.1
+    pos0 = wb.pos.astype(np.float64)
+    listed = oracle.neighbor_pairs(pos0, wb.box, rc + skin, wb.excl_pairs, "bruteforce")
+    n = wb.n_atoms
+    listed_key = set((listed[:, 0].astype(np.int64) * n + listed[:, 1]).tolist())
+    rng = np.random.default_rng(0)
+    step = rng.standard_normal(pos0.shape)
+    step *= (0.5 * skin * 0.999) / np.linalg.norm(step, axis=1, keepdims=True)  # every atom moves just under skin/2
+    pos1 = pos0 + step
+    assert oracle.needs_rebuild(pos1, pos0, skin)[0] is False
+    now = oracle.neighbor_pairs(pos1, wb.box, rc, wb.excl_pairs, "bruteforce")
+    now_key = set((now[:, 0].astype(np.int64) * n + now[:, 1]).tolist())
+    assert now_key <= listed_key
