@@ -1,0 +1,211 @@
+/*
+ * dimos.h -- C ABI of libdimos_b200: the per-step hot path of the DIMOS method (arXiv 2503.20541)
+ * as hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * What the library computes (PAPER.md = /root/reference/PAPER.md, section III A 2):
+ *   - the Verlet neighbour list of radius r_nl = r_c + r_g built in O(N) from a cell list
+ *     (PAPER.md:173-177), with excluded pairs filtered at list level;
+ *   - the rebuild trigger "any atom moved more than r_g/2 since construction";
+ *   - the short-range nonbonded pair sum over that list: Lennard-Jones 12-6 (Eq. 4)
+ *     plus reaction-field electrostatics (Eq. 8) or the Ewald direct-space term
+ *     erfc(alpha r)/r (Eq. 10) with its intramolecular exclusion correction,
+ *     under the minimum-image convention, returning per-atom forces, energy
+ *     components and the virial.
+ * Readings of points the paper leaves open are listed in DESIGN.md (C-1 ... C-20).
+ *
+ * Conventions
+ *   Units: nm, ps, amu, e, kJ/mol; forces kJ mol^-1 nm^-1.
+ *   "dev" pointers are CUDA device pointers on the context's device, "host" pointers are host
+ *   memory.  All arrays are contiguous, row-major.  The element type of pos / charge / F is
+ *   `float` for DIMOS_F32 and DIMOS_MIXED contexts and `double` for DIMOS_F64 contexts.
+ *   The caller owns every array it passes in; the library owns only its opaque handles and the
+ *   workspace they hold (obtained through the dimos_allocator callbacks when given, so that the
+ *   caller's framework -- torch's caching allocator in the Python binding -- owns device memory).
+ *   All device work is enqueued on the `stream` argument (a cudaStream_t passed as void*; NULL is
+ *   the legacy default stream).  A call does not synchronise with the host unless stated.
+ *   Every call returns a dimos_status (0 = DIMOS_OK, negative = error); on error no output array
+ *   is guaranteed to be written.  dimos_last_error(ctx) gives a human-readable message.
+ *   Calls on one context must not overlap in time (no internal locking).
+ *   There is no CPU fallback: without a usable CUDA device every compute call fails with
+ *   DIMOS_ECUDA.
+ */
+#ifndef DIMOS_H_
+#define DIMOS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define DIMOS_API __attribute__((visibility("default")))
+#else
+#define DIMOS_API
+#endif
+
+typedef struct dimos_ctx dimos_ctx; /* opaque, library-owned */
+typedef struct dimos_nl dimos_nl;   /* opaque neighbour list, library-owned, tied to its ctx */
+
+typedef enum {
+    DIMOS_OK = 0,
+    DIMOS_EINVAL = -1,    /* bad argument (NULL pointer, N <= 0, non-finite box, unsupported value) */
+    DIMOS_EBOX = -2,      /* r_cut > min(box)/2: more than one image inside the cutoff (reading C-3) */
+    DIMOS_ENOMEM = -3,    /* host or device allocation failed */
+    DIMOS_EOVERFLOW = -4, /* an internal capacity was exceeded even after growing (see message) */
+    DIMOS_ECUDA = -5,     /* CUDA runtime error, or no CUDA device */
+    DIMOS_ESTALE = -6     /* N, box or r_cut differ from the values the list was built with */
+} dimos_status;
+
+/* Element type of pos/charge/F and arithmetic of the pair kernel (reading C-11):
+ *   DIMOS_F32   float in/out, float pair math, per-thread float partial sums, fp64 final reduction
+ *   DIMOS_F64   double everywhere
+ *   DIMOS_MIXED float in/out, float pair math, energy and virial accumulated in fp64 from the
+ *               first add */
+typedef enum { DIMOS_F32 = 0, DIMOS_F64 = 1, DIMOS_MIXED = 2 } dimos_precision;
+
+/* Electrostatics of the pair sum: reaction field (Eq. 8) or Ewald direct space (Eq. 10, nearest
+ * image only, reading C-14) plus the exclusion correction (reading C-15). */
+typedef enum { DIMOS_RF = 0, DIMOS_EWALD_REAL = 1 } dimos_method;
+
+/* Device-memory callbacks.  alloc returns a device pointer aligned to >= 256 bytes, or NULL;
+ * free_ releases a pointer returned by alloc.  Both are called from the thread that calls the
+ * library, only from dimos_nl_build / dimos_create / dimos_destroy / dimos_nl_destroy, never
+ * while a kernel of this library that uses the block is pending on a stream other than the
+ * one given to alloc.  Pass NULL instead of a dimos_allocator to use cudaMalloc/cudaFree. */
+typedef struct {
+    void* (*alloc)(size_t bytes, void* stream, void* user);
+    void (*free_)(void* ptr, void* user);
+    void* user;
+} dimos_allocator;
+
+typedef struct {
+    double r_cut;         /* r_c, nm; must equal the r_cut the list was built with */
+    double eps_rf;        /* reaction-field dielectric (DIMOS_RF); reading C-1 */
+    double alpha;         /* Ewald splitting parameter, nm^-1 (DIMOS_EWALD_REAL) */
+    double coulomb_const; /* k_e = 1/(4 pi eps0), kJ mol^-1 nm e^-2 (138.935456, reading C-2) */
+    int32_t method;       /* dimos_method */
+} dimos_nb_params;
+
+typedef struct {
+    int64_t n_atoms;
+    int64_t n_units;         /* i-clusters of DIMOS_UNIT atoms (incl. one partial unit per cell) */
+    int64_t n_slots;         /* n_units * DIMOS_UNIT (sorted atom slots incl. padding) */
+    int64_t n_entries;       /* (unit, j-atom) list entries, excluding chunk padding */
+    int64_t n_entries_padded;/* entries incl. padding to 32-wide chunks (what the kernel streams) */
+    int64_t n_pair_slots;    /* n_entries_padded * DIMOS_UNIT pair evaluations per force call */
+    int64_t list_bytes;      /* bytes of list data streamed per force call */
+    int64_t workspace_bytes; /* device bytes held by the list */
+    int32_t n_cells[3];
+    int32_t pbc_mode;        /* 0 = image shift from cell offsets, 1 = per-pair minimum image */
+    int32_t row_capacity;    /* entries per unit row */
+    int32_t n_rebuild_grow;  /* times the build was repeated with a larger capacity */
+} dimos_nl_stats_t;
+
+#define DIMOS_UNIT 8 /* atoms per i-cluster ("unit") of the cluster-pair list */
+
+/* Create a context bound to CUDA device `device` with the given precision.
+ * allocator may be NULL.  *out receives the handle. */
+DIMOS_API int dimos_create(dimos_ctx** out, int device, int precision, const dimos_allocator* allocator);
+
+/* Destroy a context and every list built with it (the caller must have synchronised the streams
+ * that used it). */
+DIMOS_API int dimos_destroy(dimos_ctx* ctx);
+
+/* dimos_nl_build -- PAPER.md:173-177, 243.
+ * Bins the N atoms into cells of edge >= r_cut + skin by counting sort (periodic wrap, positions
+ * need not lie inside [0,L)), forms compact units of DIMOS_UNIT atoms inside each cell, and builds
+ * for every unit the list of j-atoms that have at least one atom of the unit within
+ * r_nl = r_cut + skin (strict <, reading C-4), each unordered atom pair being owned by exactly
+ * one unit, with a per-entry bitmask that removes excluded pairs, the i >= j half of
+ * intra-unit pairs and padding atoms.
+ *   pos           dev, N x 3, float or double per the context precision; read
+ *   N             number of atoms, 1 .. 2^31-1
+ *   box           host, 3 doubles: orthorhombic box edges in nm
+ *   r_cut, skin   nm; r_cut > 0, skin >= 0, r_cut <= min(box)/2 else DIMOS_EBOX
+ *   excl_pairs    dev, n_excl x 2 int32, each row (i, j) with i < j, rows unique (reading C-17);
+ *                 may be NULL when n_excl == 0.  At most 32 exclusion partners per atom.
+ *   pos_at_build  dev, N x 3, same type as pos, caller-owned; written with a copy of pos (the
+ *                 reference positions of the rebuild trigger)
+ *   stream        cudaStream_t
+ *   inout         *inout == NULL: a new list is created and returned; otherwise the given list
+ *                 (built with the same ctx) is rebuilt in place, reusing its workspace.
+ * Synchronises the stream once (to read the list size / overflow flag), and again per capacity
+ * growth.  Also retains a device copy of excl_pairs for the Ewald exclusion correction. */
+DIMOS_API int dimos_nl_build(dimos_ctx* ctx, const void* pos, int64_t N, const double* box, double r_cut,
+                             double skin, const int32_t* excl_pairs, int64_t n_excl, void* pos_at_build,
+                             void* stream, dimos_nl** inout);
+
+/* Free one list (optional; dimos_destroy frees all lists of a context). */
+DIMOS_API int dimos_nl_destroy(dimos_ctx* ctx, dimos_nl* nl);
+
+/* dimos_nl_needs_rebuild -- PAPER.md:175, reading C-5.
+ * flag = [ max_i |pos_i - pos_at_build_i| > skin/2 ], Euclidean norm of the raw (unwrapped)
+ * coordinate difference, strict >, compared as squares in the context's element type.
+ *   pos, pos_at_build  dev, N x 3
+ *   flag_dev           dev, one int32, written with 0 or 1 (required)
+ *   flag_host          host, one int32; if non-NULL the stream is synchronised and the flag copied
+ *                      there, if NULL the call does not synchronise. */
+DIMOS_API int dimos_nl_needs_rebuild(dimos_ctx* ctx, const void* pos, const void* pos_at_build, int64_t N,
+                                     double skin, int32_t* flag_dev, int32_t* flag_host, void* stream);
+
+/* dimos_nonbonded -- PAPER.md:189-213, 222, 243; SURVEY/DESIGN reading C-7 for the virial.
+ * Evaluates, over the pairs of the list that are not excluded and have minimum-image r < r_cut
+ * (strict, fp32 r^2 in F32/MIXED contexts), the Lennard-Jones energy (Eq. 4) and the Coulomb
+ * energy by the chosen method, and their forces.  The list must be valid for `pos` (no atom moved
+ * more than skin/2 since dimos_nl_build), which the caller checks with dimos_nl_needs_rebuild.
+ *   pos      dev, N x 3
+ *   charge   dev, N (e)
+ *   type     dev, N int32 in [0, ntypes)
+ *   lj_table dev, ntypes x ntypes x 2 doubles = (sigma_ab, eps_ab), symmetric (Eq. 5 filled by the
+ *            caller, reading C-16); ntypes <= 64
+ *   box      host, 3 doubles, must equal the build box (else DIMOS_ESTALE)
+ *   params   host
+ *   F        dev, N x 3, overwritten: F_i = sum_j f_ij (plus the exclusion-correction forces)
+ *   E        dev, 4 doubles, overwritten: {total, lj, coul_pair, coul_excl_corr}
+ *   virial   dev, 9 doubles row-major, overwritten: W_ab = sum_pairs d_a f_ij,b with
+ *            d = r_i - r_j (minimum image), including exclusion-correction pairs; may be NULL
+ * Does not synchronise. */
+DIMOS_API int dimos_nonbonded(dimos_ctx* ctx, const dimos_nl* nl, const void* pos, const void* charge,
+                              const int32_t* type, const double* lj_table, int32_t ntypes, const double* box,
+                              const dimos_nb_params* params, void* F, double* E, double* virial, void* stream);
+
+/* dimos_nonbonded_host -- the same call with HOST arrays (pinned memory recommended): copies
+ * pos/charge/type/lj_table to the device, runs dimos_nonbonded, copies F, E[4] and virial[9]
+ * back and synchronises the stream before returning.  Staging buffers live in the list. */
+DIMOS_API int dimos_nonbonded_host(dimos_ctx* ctx, dimos_nl* nl, const void* pos_host, const void* charge_host,
+                                   const int32_t* type_host, const double* lj_table_host, int32_t ntypes,
+                                   const double* box, const dimos_nb_params* params, void* F_host,
+                                   double* E_host, double* virial_host, void* stream);
+
+/* dimos_nl_export_pairs -- the neighbour set the list represents, for parity checks and for
+ * consumers that want a plain edge list.
+ * Writes every unordered pair (i < j, original atom indices) that is not excluded and has
+ * minimum-image r < r_cut + skin at the build positions, in unspecified order (reading C-6).
+ *   pairs         dev, cap x 2 int32; may be NULL when cap == 0 (count only)
+ *   n_pairs_host  host, receives the number of pairs in the list; if it exceeds cap only the first
+ *                 cap pairs found were written and the call returns DIMOS_EOVERFLOW.
+ * Synchronises the stream. */
+DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
+                                    int64_t* n_pairs_host, void* stream);
+
+/* Sizes of the list (host call, no device work). */
+DIMOS_API int dimos_nl_stats(const dimos_nl* nl, dimos_nl_stats_t* out);
+
+/* Number of kernels of this library launched through ctx since dimos_create (host counter). */
+DIMOS_API int64_t dimos_launch_count(const dimos_ctx* ctx);
+
+/* Peak-rate probe used by bench.py's roofline: runs an FFMA-only microkernel on the context's
+ * device for about `ms_target` milliseconds and returns the measured FP32 rate in *tflops_host
+ * (2 flops per FMA).  Synchronises. */
+DIMOS_API int dimos_probe_fp32_peak(dimos_ctx* ctx, double ms_target, double* tflops_host, void* stream);
+
+DIMOS_API const char* dimos_status_string(int status);
+DIMOS_API const char* dimos_last_error(const dimos_ctx* ctx);
+DIMOS_API const char* dimos_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DIMOS_H_ */

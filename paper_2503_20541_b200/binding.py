@@ -1,0 +1,326 @@
+"""Thin Python binding of libdimos_b200 (include/dimos.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; this module converts torch
+tensors to raw pointers, hands the library torch's caching allocator and the current stream, and
+turns status codes into exceptions.  There is no CPU fallback: if the shared library cannot be
+loaded (or built with nvcc), importing the compute entry points fails loudly.
+
+The three entry points keep the C names: `dimos_nl_build`, `dimos_nl_needs_rebuild`,
+`dimos_nonbonded` (PAPER.md:173-185 NeighborHandling / get_neighborlist).
+"""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import os
+
+import torch
+
+from . import build_ext
+
+DIMOS_F32, DIMOS_F64, DIMOS_MIXED = 0, 1, 2
+DIMOS_RF, DIMOS_EWALD_REAL = 0, 1
+UNIT = 8
+_PRECISIONS = {"f32": DIMOS_F32, "f64": DIMOS_F64, "mixed": DIMOS_MIXED}
+_METHODS = {"rf": DIMOS_RF, "ewald": DIMOS_EWALD_REAL}
+
+EXPORTED_SYMBOLS = (
+    "dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
+    "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats", "dimos_launch_count",
+    "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
+)
+
+
+class DimosError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{message} (status {status})")
+        self.status = status
+
+
+class _Allocator(ctypes.Structure):
+    _fields_ = [("alloc", ctypes.c_void_p), ("free_", ctypes.c_void_p), ("user", ctypes.c_void_p)]
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("r_cut", ctypes.c_double), ("eps_rf", ctypes.c_double), ("alpha", ctypes.c_double),
+                ("coulomb_const", ctypes.c_double), ("method", ctypes.c_int32)]
+
+
+class _Stats(ctypes.Structure):
+    _fields_ = [("n_atoms", ctypes.c_int64), ("n_units", ctypes.c_int64), ("n_slots", ctypes.c_int64),
+                ("n_entries", ctypes.c_int64), ("n_entries_padded", ctypes.c_int64), ("n_pair_slots", ctypes.c_int64),
+                ("list_bytes", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("n_cells", ctypes.c_int32 * 3),
+                ("pbc_mode", ctypes.c_int32), ("row_capacity", ctypes.c_int32), ("n_rebuild_grow", ctypes.c_int32)]
+
+
+_ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_void_p)
+_FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+
+_lib_handle = None
+
+
+def library_path() -> str:
+    return build_ext.OUT
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libdimos_b200.so, building it in-tree with nvcc if it is missing or stale."""
+    global _lib_handle
+    if _lib_handle is not None:
+        return _lib_handle
+    path = build_ext.OUT
+    if not os.path.exists(path) or build_ext._stale():
+        try:
+            build_ext.build()
+        except Exception as exc:  # no silent fallback: the product IS the CUDA library
+            if not os.path.exists(path):
+                raise RuntimeError(f"libdimos_b200.so is missing and could not be built: {exc}") from exc
+    lib = ctypes.CDLL(path)
+    vp, i64, i32, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+    lib.dimos_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, ctypes.c_int, ctypes.POINTER(_Allocator)]
+    lib.dimos_destroy.argtypes = [vp]
+    lib.dimos_nl_build.argtypes = [vp, vp, i64, ctypes.POINTER(dbl), dbl, dbl, vp, i64, vp, vp, ctypes.POINTER(vp)]
+    lib.dimos_nl_destroy.argtypes = [vp, vp]
+    lib.dimos_nl_needs_rebuild.argtypes = [vp, vp, vp, i64, dbl, vp, ctypes.POINTER(i32), vp]
+    lib.dimos_nonbonded.argtypes = [vp, vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), ctypes.POINTER(_Params), vp, vp, vp, vp]
+    lib.dimos_nonbonded_host.argtypes = [vp, vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), ctypes.POINTER(_Params), vp, vp, vp, vp]
+    lib.dimos_nl_export_pairs.argtypes = [vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+    lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
+    lib.dimos_launch_count.argtypes = [vp]
+    lib.dimos_launch_count.restype = i64
+    lib.dimos_probe_fp32_peak.argtypes = [vp, dbl, ctypes.POINTER(dbl), vp]
+    lib.dimos_status_string.argtypes = [ctypes.c_int]
+    lib.dimos_status_string.restype = ctypes.c_char_p
+    lib.dimos_last_error.argtypes = [vp]
+    lib.dimos_last_error.restype = ctypes.c_char_p
+    lib.dimos_version.restype = ctypes.c_char_p
+    for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
+                 "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
+                 "dimos_probe_fp32_peak"):
+        getattr(lib, name).restype = ctypes.c_int
+    _lib_handle = lib
+    return lib
+
+
+def _stream_ptr() -> int:
+    return int(torch.cuda.current_stream().cuda_stream)
+
+
+def _box3(box):
+    vals = [float(b) for b in (box.tolist() if hasattr(box, "tolist") else box)]
+    if len(vals) != 3:
+        raise ValueError("box must have 3 entries")
+    return (ctypes.c_double * 3)(*vals)
+
+
+@dataclasses.dataclass
+class NeighborList:
+    handle: ctypes.c_void_p
+    ctx: "Context"
+    pos_at_build: torch.Tensor
+    box: tuple
+    r_cut: float
+    skin: float
+
+    def stats(self) -> dict:
+        return self.ctx.nl_stats(self)
+
+
+class Context:
+    """One library context: device + precision + torch-backed allocator."""
+
+    def __init__(self, device: int = 0, precision: str = "f32", torch_allocator: bool = True):
+        if not torch.cuda.is_available():
+            raise RuntimeError("dimos_b200 needs a CUDA device: there is no CPU fallback")
+        self.lib = load_library()
+        self.device = int(device)
+        self.precision = precision
+        self.real = torch.float64 if precision == "f64" else torch.float32
+        self._blocks: dict[int, torch.Tensor] = {}
+        self._alloc_struct = None
+        if torch_allocator:
+            dev = torch.device("cuda", self.device)
+
+            def _alloc(nbytes, _stream, _user):
+                try:
+                    t = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+                except Exception:
+                    return None
+                self._blocks[t.data_ptr()] = t
+                return t.data_ptr()
+
+            def _free(ptr, _user):
+                self._blocks.pop(int(ptr), None)
+
+            self._alloc_cb = _ALLOC_FN(_alloc)
+            self._free_cb = _FREE_FN(_free)
+            self._alloc_struct = _Allocator(ctypes.cast(self._alloc_cb, ctypes.c_void_p),
+                                            ctypes.cast(self._free_cb, ctypes.c_void_p), None)
+        h = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_create(ctypes.byref(h), self.device, _PRECISIONS[precision],
+                                       ctypes.byref(self._alloc_struct) if self._alloc_struct else None)
+        if rc != 0:
+            raise DimosError(rc, self.lib.dimos_status_string(rc).decode())
+        self.handle = h
+        self._flag = torch.zeros(1, dtype=torch.int32, device=torch.device("cuda", self.device))
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            msg = self.lib.dimos_last_error(self.handle).decode() or self.lib.dimos_status_string(rc).decode()
+            raise DimosError(rc, msg)
+
+    def _dev(self, t: torch.Tensor, dtype, shape_last=None) -> torch.Tensor:
+        if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+            raise ValueError(f"expected a contiguous CUDA tensor of dtype {dtype}, got {t.dtype} on {t.device}")
+        if shape_last is not None and (t.dim() != 2 or t.shape[1] != shape_last):
+            raise ValueError(f"expected shape (N, {shape_last})")
+        return t
+
+    def close(self):
+        if getattr(self, "handle", None):
+            torch.cuda.synchronize(self.device)
+            self.lib.dimos_destroy(self.handle)
+            self.handle = None
+            self._blocks.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C-ABI calls -------------------------------------------------------------------------
+    def nl_build(self, pos, box, r_cut, skin, excl_pairs=None, pos_at_build=None, nl: NeighborList | None = None):
+        """dimos_nl_build: returns a NeighborList (rebuilt in place when `nl` is given)."""
+        pos = self._dev(pos, self.real, 3)
+        n = pos.shape[0]
+        if pos_at_build is None:
+            pos_at_build = nl.pos_at_build if nl is not None and nl.pos_at_build.shape == pos.shape else torch.empty_like(pos)
+        self._dev(pos_at_build, self.real, 3)
+        n_excl = 0
+        excl_ptr = None
+        if excl_pairs is not None and excl_pairs.numel() > 0:
+            excl_pairs = self._dev(excl_pairs, torch.int32, 2)
+            n_excl = excl_pairs.shape[0]
+            excl_ptr = excl_pairs.data_ptr()
+        h = ctypes.c_void_p(nl.handle.value if nl is not None else None)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_build(self.handle, pos.data_ptr(), n, _box3(box), float(r_cut), float(skin), excl_ptr,
+                                         n_excl, pos_at_build.data_ptr(), _stream_ptr(), ctypes.byref(h))
+        self._check(rc)
+        boxt = tuple(float(b) for b in (box.tolist() if hasattr(box, "tolist") else box))
+        if nl is not None:
+            nl.handle, nl.pos_at_build, nl.box, nl.r_cut, nl.skin = h, pos_at_build, boxt, float(r_cut), float(skin)
+            return nl
+        return NeighborList(h, self, pos_at_build, boxt, float(r_cut), float(skin))
+
+    def nl_needs_rebuild(self, pos, pos_at_build, skin, sync: bool = True):
+        """dimos_nl_needs_rebuild: bool when sync=True, else the device flag tensor (no host sync)."""
+        pos = self._dev(pos, self.real, 3)
+        ref = self._dev(pos_at_build, self.real, 3)
+        host = ctypes.c_int32(0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_needs_rebuild(self.handle, pos.data_ptr(), ref.data_ptr(), pos.shape[0], float(skin),
+                                                 self._flag.data_ptr(), ctypes.byref(host) if sync else None, _stream_ptr())
+        self._check(rc)
+        return bool(host.value) if sync else self._flag
+
+    def _params(self, nl, method, eps_rf, alpha, coulomb_const):
+        return _Params(float(nl.r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method] if isinstance(method, str) else int(method))
+
+    def nonbonded(self, nl: NeighborList, pos, charge, type_, lj_table, *, method="rf", eps_rf=78.5, alpha=3.12,
+                  coulomb_const=138.935456, F=None, E=None, virial=None):
+        """dimos_nonbonded: returns (F (N,3) real, E (4,) float64, virial (3,3) float64) device tensors."""
+        pos = self._dev(pos, self.real, 3)
+        n = pos.shape[0]
+        charge = self._dev(charge, self.real)
+        type_ = self._dev(type_, torch.int32)
+        lj_table = self._dev(lj_table, torch.float64)
+        nt = lj_table.shape[0]
+        if lj_table.shape != (nt, nt, 2) or charge.numel() != n or type_.numel() != n:
+            raise ValueError("shape mismatch")
+        dev = pos.device
+        F = torch.empty_like(pos) if F is None else self._dev(F, self.real, 3)
+        E = torch.empty(4, dtype=torch.float64, device=dev) if E is None else self._dev(E, torch.float64)
+        virial = torch.empty(3, 3, dtype=torch.float64, device=dev) if virial is None else self._dev(virial, torch.float64)
+        prm = self._params(nl, method, eps_rf, alpha, coulomb_const)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nonbonded(self.handle, nl.handle, pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
+                                          lj_table.data_ptr(), nt, _box3(nl.box), ctypes.byref(prm), F.data_ptr(),
+                                          E.data_ptr(), virial.data_ptr(), _stream_ptr())
+        self._check(rc)
+        return F, E, virial
+
+    def nonbonded_host(self, nl: NeighborList, pos, charge, type_, lj_table, F, E, virial, *, method="rf", eps_rf=78.5,
+                       alpha=3.12, coulomb_const=138.935456):
+        """dimos_nonbonded_host: all arrays are HOST tensors (pinned recommended); synchronises."""
+        for t in (pos, charge, type_, lj_table, F, E, virial):
+            if t.is_cuda or not t.is_contiguous():
+                raise ValueError("nonbonded_host takes contiguous host tensors")
+        prm = self._params(nl, method, eps_rf, alpha, coulomb_const)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nonbonded_host(self.handle, nl.handle, pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
+                                               lj_table.data_ptr(), lj_table.shape[0], _box3(nl.box), ctypes.byref(prm),
+                                               F.data_ptr(), E.data_ptr(), virial.data_ptr(), _stream_ptr())
+        self._check(rc)
+        return F, E, virial
+
+    def nl_export_pairs(self, nl: NeighborList) -> torch.Tensor:
+        """dimos_nl_export_pairs: (n,2) int32 device tensor of pairs i<j, order unspecified."""
+        n = ctypes.c_int64(0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_export_pairs(self.handle, nl.handle, None, 0, ctypes.byref(n), _stream_ptr())
+        self._check(rc)
+        out = torch.empty((max(n.value, 1), 2), dtype=torch.int32, device=torch.device("cuda", self.device))
+        got = ctypes.c_int64(0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_export_pairs(self.handle, nl.handle, out.data_ptr(), out.shape[0], ctypes.byref(got), _stream_ptr())
+        self._check(rc)
+        return out[: got.value]
+
+    def nl_stats(self, nl: NeighborList) -> dict:
+        st = _Stats()
+        rc = self.lib.dimos_nl_stats(nl.handle, ctypes.byref(st))
+        self._check(rc)
+        d = {name: getattr(st, name) for name, _ in _Stats._fields_ if name != "n_cells"}
+        d["n_cells"] = tuple(st.n_cells)
+        return d
+
+    def launch_count(self) -> int:
+        return int(self.lib.dimos_launch_count(self.handle))
+
+    def probe_fp32_peak(self, ms_target: float = 3.0) -> float:
+        out = ctypes.c_double(0.0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_probe_fp32_peak(self.handle, float(ms_target), ctypes.byref(out), _stream_ptr())
+        self._check(rc)
+        return float(out.value)
+
+
+# -- module-level functions with the C names -------------------------------------------------------
+def dimos_nl_build(ctx: Context, pos, box, r_cut, skin, excl_pairs=None, pos_at_build=None, nl=None) -> NeighborList:
+    return ctx.nl_build(pos, box, r_cut, skin, excl_pairs, pos_at_build, nl)
+
+
+def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = True):
+    return ctx.nl_needs_rebuild(pos, pos_at_build, skin, sync)
+
+
+def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
+    return ctx.nonbonded(nl, pos, charge, type_, lj_table, **kw)
+
+
+def dimos_nl_export_pairs(ctx: Context, nl: NeighborList) -> torch.Tensor:
+    return ctx.nl_export_pairs(nl)
+
+
+def lj_table_from_types(sigma, epsilon) -> torch.Tensor:
+    """Host-side fill of the (sigma_ab, eps_ab) table by Lorentz-Berthelot, Eq. (5) PAPER.md:195."""
+    s = torch.as_tensor(sigma, dtype=torch.float64)
+    e = torch.as_tensor(epsilon, dtype=torch.float64)
+    table = torch.empty(s.numel(), s.numel(), 2, dtype=torch.float64)
+    table[:, :, 0] = 0.5 * (s[:, None] + s[None, :])
+    table[:, :, 1] = torch.sqrt(e[:, None] * e[None, :])
+    return table

@@ -1,0 +1,140 @@
+// common.cuh -- internal declarations shared by the translation units of libdimos_b200.
+// Product code: shares nothing with oracle/ (see DESIGN.md).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/dimos.h"
+
+namespace dimos {
+
+constexpr int UNIT = DIMOS_UNIT;  // atoms per i-cluster
+constexpr int KD_MAX = 4096;      // max atoms per cell the in-cell sorter handles
+constexpr int MAX_EXCL_PER_ATOM = 32;
+constexpr int MAX_TYPES = 64;
+constexpr int SELF_CODE = 13;  // stencil code of offset (0,0,0): (dx+1)*9+(dy+1)*3+(dz+1)
+
+// device error flag bits (NL::d_flags[0])
+enum : int {
+    FLAG_ROW_OVERFLOW = 1,     // a unit row needed more than row_cap entries
+    FLAG_MASKED_OVERFLOW = 2,  // more masked entries than m_res in one unit
+    FLAG_NONFINITE = 4,        // non-finite coordinate
+    FLAG_CELL_OVERFLOW = 8,    // more than KD_MAX atoms in one cell
+    FLAG_EXCL_OVERFLOW = 16,   // more than MAX_EXCL_PER_ATOM partners for one atom
+    FLAG_EXCL_RANGE = 32       // exclusion index out of range / not i<j
+};
+
+template <typename real> struct vec4;
+template <> struct vec4<float> { using type = float4; };
+template <> struct vec4<double> { using type = double4; };
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+};
+
+struct Ctx {
+    int device = 0;
+    int precision = DIMOS_F32;
+    bool has_alloc = false;
+    dimos_allocator alloc{};
+    std::string err;
+    int64_t launches = 0;
+    int sm_count = 148;
+    int* h_pinned = nullptr;        // 64 ints pinned scratch for read-backs
+    unsigned long long* d_rebuild_state = nullptr;  // {max bits, ticket}
+    std::vector<struct NL*> lists;
+};
+
+// geometry of the cell grid / list, passed by value to kernels
+struct Grid {
+    int n[3];          // cells per axis
+    int pbc_mode;      // 0: image from cell offsets (all n >= 3), 1: per-pair minimum image
+    double L[3];       // box
+    double h[3];       // cell edge = L / n
+    int64_t ncells;
+};
+
+struct NL {
+    Ctx* ctx = nullptr;
+    int64_t N = 0;
+    double box[3] = {0, 0, 0};
+    double r_cut = 0, skin = 0, r_nl = 0;
+    Grid grid{};
+    int64_t n_units = 0, n_slots = 0;
+    int row_cap = 0;  // entries per unit row (multiple of 32), includes m_res
+    int m_res = 128;  // reserved masked-entry region at the front of each row (multiple of 32)
+    int n_grow = 0;
+    int64_t n_entries = 0, n_entries_padded = 0;
+    int64_t n_excl = 0;
+    int max_cell_count = 0;
+
+    // build-time device arrays
+    DevBuf cell_count, cell_start, unit_start, scan_tmp;  // int[ncells+1] each
+    DevBuf atom_cell, atom_rank, cell_atoms;              // int[N]
+    DevBuf perm;       // int[n_slots]: original atom index, or ~src for padding slots
+    DevBuf inv_perm;   // int[N]: slot of each original atom
+    DevBuf ref;        // double[3*n_slots]: origin subtracted from the raw coordinate
+    DevBuf xyz_build;  // real4[n_slots]: cell-relative coordinates at build time
+    DevBuf bb_lo, bb_hi;  // real4[n_units] unit bounding boxes (cell-relative)
+    DevBuf unit_cell;  // int[n_units]
+    DevBuf excl_start, excl_adj;  // CSR over both directions: int[N+1], int[2*n_excl]
+    DevBuf excl_pairs;            // int2[n_excl] copy (Ewald exclusion correction)
+    DevBuf jslot;      // int[n_units*row_cap]
+    DevBuf meta;       // uint16[n_units*row_cap]: mask | code<<8
+    DevBuf row_info;   // int2[n_units]: {masked chunks, unmasked entries}
+    DevBuf flags;      // int[8]: [0] error flags, [1] max cell count, [2..3] entry counters (u64), [4..5] padded
+    // per-step device arrays
+    DevBuf xyzq;       // real4[n_slots]
+    DevBuf stype;      // int[n_slots]
+    DevBuf Facc;       // real4[n_slots] j-side force accumulators (atomics)
+    DevBuf Fown;       // real4[n_slots] i-side forces (plain stores)
+    DevBuf lj;         // real2[nt*nt] (c6,c12) + int[nt] row-active flags after it
+    DevBuf partials;   // double[9 * n_partial_blocks]
+    DevBuf accum;      // double[16] + unsigned ticket
+    // host-call staging (dimos_nonbonded_host)
+    DevBuf st_pos, st_charge, st_type, st_lj, st_F, st_EW;
+    DevBuf export_count;  // unsigned long long[1]
+};
+
+// ---- helpers implemented in api.cu ------------------------------------------------------------
+int set_error(Ctx* ctx, int status, const std::string& msg);
+int ensure(Ctx* ctx, DevBuf& b, size_t bytes, cudaStream_t s);
+void release(Ctx* ctx, DevBuf& b);
+
+#define DIMOS_CUDA_TRY(ctx, call)                                                                   \
+    do {                                                                                            \
+        cudaError_t e_ = (call);                                                                    \
+        if (e_ != cudaSuccess)                                                                      \
+            return ::dimos::set_error((ctx), DIMOS_ECUDA,                                           \
+                                      std::string(#call) + ": " + cudaGetErrorString(e_));          \
+    } while (0)
+
+#define DIMOS_LAUNCH_CHECK(ctx, name)                                                               \
+    do {                                                                                            \
+        (ctx)->launches++;                                                                          \
+        cudaError_t e_ = cudaGetLastError();                                                        \
+        if (e_ != cudaSuccess)                                                                      \
+            return ::dimos::set_error((ctx), DIMOS_ECUDA,                                           \
+                                      std::string("launch ") + name + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+// ---- entry points implemented per translation unit ---------------------------------------------
+int nl_build_impl(Ctx* ctx, NL* nl, const void* pos, const int32_t* excl_pairs, int64_t n_excl,
+                  void* pos_at_build, cudaStream_t s);
+int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, cudaStream_t s);
+int needs_rebuild_impl(Ctx* ctx, const void* pos, const void* ref, int64_t N, double skin, int32_t* flag_dev,
+                       cudaStream_t s);
+int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const int32_t* type,
+                   const double* lj_table, int32_t ntypes, const dimos_nb_params* prm, void* F, double* E,
+                   double* virial, cudaStream_t s);
+int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s);
+
+// stencil code <-> offset
+__host__ __device__ inline int stencil_code(int dx, int dy, int dz) { return (dx + 1) * 9 + (dy + 1) * 3 + (dz + 1); }
+
+}  // namespace dimos

@@ -1,0 +1,1029 @@
+// nl_build.cu -- neighbour-list construction.
+//
+//   A1  cell binning by counting sort: bin_atoms (histogram) -> block-scan exclusive prefix sum ->
+//       scatter; then, per cell, a k-d bisection in shared memory orders the cell's atoms so that
+//       every 8 consecutive atoms form a spatially compact "unit" (i-cluster).
+//   A2  cluster-pair list: one warp per unit gathers, from the (de-duplicated) 27-cell stencil,
+//       first the units whose bounding box is within r_nl of its own, then the individual j-atoms
+//       of those units that have at least one unit atom within r_nl.  Every unordered atom pair is
+//       owned by exactly one unit (circular half-ordering of unit indices; triangular mask inside a
+//       unit).  Entries carry an 8-bit mask (exclusions, intra-unit half, padding) and a stencil
+//       code that selects the periodic image; entries whose mask is not all-ones are stored in a
+//       reserved region in front of the row so the force kernel runs a mask-free loop over the rest.
+//
+// All coordinates used here are cell-relative (x - cell origin - wrap*L, formed in fp64 and rounded
+// once), so fp32 distance tests across the periodic seam keep ~1e-7 nm absolute accuracy at any L.
+#include <math.h>
+
+#include <algorithm>
+
+#include "common.cuh"
+
+namespace dimos {
+
+// ------------------------------------------------------------------------------------------------
+// small device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned ordered_u32(float f)
+{
+    unsigned u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float4 make4(float x, float y, float z, float w) { return make_float4(x, y, z, w); }
+__device__ __forceinline__ double4 make4(double x, double y, double z, double w) { return make_double4(x, y, z, w); }
+
+__device__ __forceinline__ float rint_r(float x) { return rintf(x); }
+__device__ __forceinline__ double rint_r(double x) { return rint(x); }
+
+// ------------------------------------------------------------------------------------------------
+// A1a: cell index of every atom + histogram ("each atom is assigned to one of the cells")
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void bin_atoms_kernel(const real* __restrict__ pos, int64_t N, Grid g, int* __restrict__ cell_count,
+                                 int* __restrict__ atom_cell, int* __restrict__ atom_rank,
+                                 real* __restrict__ pos_at_build, int* __restrict__ flags)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int c[3];
+    bool bad = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        real xr = pos[3 * i + a];
+        pos_at_build[3 * i + a] = xr;
+        double x = (double)xr;
+        if (!isfinite(x)) { bad = true; x = 0.0; }
+        double f = x / g.L[a];
+        f -= floor(f);  // fractional coordinate in [0,1)
+        int ci = (int)(f * g.n[a]);
+        ci = ci < 0 ? 0 : (ci >= g.n[a] ? g.n[a] - 1 : ci);  // reading C-18
+        c[a] = ci;
+    }
+    if (bad) atomicOr(&flags[0], FLAG_NONFINITE);
+    int cell = (c[0] * g.n[1] + c[1]) * g.n[2] + c[2];
+    atom_cell[i] = cell;
+    atom_rank[i] = atomicAdd(&cell_count[cell], 1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// generic exclusive prefix sum of int32 (block scan, three phases); out has n+1 elements
+// ------------------------------------------------------------------------------------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 4;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total, int* warp_sums)
+{
+    // inclusive warp scan
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_sums[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        int s = lane < (SCAN_THREADS / 32) ? warp_sums[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += y;
+        }
+        if (lane < (SCAN_THREADS / 32)) warp_sums[lane] = s;  // inclusive warp totals
+    }
+    __syncthreads();
+    int base = w > 0 ? warp_sums[w - 1] : 0;
+    *total = warp_sums[SCAN_THREADS / 32 - 1];
+    __syncthreads();
+    return base + x - v;
+}
+
+__global__ void scan_reduce_kernel(const int* __restrict__ in, int64_t n, int* __restrict__ block_sums)
+{
+    __shared__ int warp_sums[SCAN_THREADS / 32];
+    int64_t base = (int64_t)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k)
+        if (base + k < n) s += in[base + k];
+    int total;
+    block_exclusive_scan(s, &total, warp_sums);
+    if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+}
+
+__global__ void scan_block_sums_kernel(int* __restrict__ block_sums, int nb)
+{
+    __shared__ int warp_sums[SCAN_THREADS / 32];
+    __shared__ int carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int t0 = 0; t0 < nb; t0 += SCAN_THREADS) {
+        int idx = t0 + threadIdx.x;
+        int v = idx < nb ? block_sums[idx] : 0;
+        int total;
+        int ex = block_exclusive_scan(v, &total, warp_sums);
+        int carry = carry_s;
+        if (idx < nb) block_sums[idx] = ex + carry;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) block_sums[nb] = carry_s;  // grand total
+}
+
+__global__ void scan_apply_kernel(const int* __restrict__ in, int64_t n, const int* __restrict__ block_sums,
+                                  int nb, int* __restrict__ out)
+{
+    __shared__ int warp_sums[SCAN_THREADS / 32];
+    int64_t base = (int64_t)blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS];
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        v[k] = (base + k < n) ? in[base + k] : 0;
+        s += v[k];
+    }
+    int total;
+    int ex = block_exclusive_scan(s, &total, warp_sums) + block_sums[blockIdx.x];
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        if (base + k < n) out[base + k] = ex;
+        ex += v[k];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) out[n] = block_sums[nb];
+}
+
+static int exclusive_scan(Ctx* ctx, const int* in, int* out, int64_t n, int* tmp, cudaStream_t s)
+{
+    int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
+    if (nb < 1) nb = 1;
+    scan_reduce_kernel<<<nb, SCAN_THREADS, 0, s>>>(in, n, tmp);
+    DIMOS_LAUNCH_CHECK(ctx, "scan_reduce");
+    scan_block_sums_kernel<<<1, SCAN_THREADS, 0, s>>>(tmp, nb);
+    DIMOS_LAUNCH_CHECK(ctx, "scan_block_sums");
+    scan_apply_kernel<<<nb, SCAN_THREADS, 0, s>>>(in, n, tmp, nb, out);
+    DIMOS_LAUNCH_CHECK(ctx, "scan_apply");
+    return DIMOS_OK;
+}
+static size_t scan_tmp_ints(int64_t n) { return (size_t)((n + SCAN_TILE - 1) / SCAN_TILE) + 2; }
+
+// units per cell = ceil(count / UNIT); also records the maximum cell population
+__global__ void cell_units_kernel(const int* __restrict__ cell_count, int64_t ncells, int* __restrict__ unit_count,
+                                  int* __restrict__ flags)
+{
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int n = c < ncells ? cell_count[c] : 0;
+    if (c < ncells) unit_count[c] = (n + UNIT - 1) / UNIT;
+    int m = n;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(&flags[1], m);
+}
+
+// A1c: scatter atoms into cell order (counting sort; order inside a cell is fixed later by the k-d sort)
+__global__ void scatter_atoms_kernel(int64_t N, const int* __restrict__ atom_cell, const int* __restrict__ atom_rank,
+                                     const int* __restrict__ cell_start, int* __restrict__ cell_atoms)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    cell_atoms[cell_start[atom_cell[i]] + atom_rank[i]] = (int)i;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A1d: per-cell k-d bisection -> compact units of 8 atoms
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bitonic_sort_u64(unsigned long long* K, int npad)
+{
+    for (int k = 2; k <= npad; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < npad; t += blockDim.x) {
+                int ixj = t ^ j;
+                if (ixj > t) {
+                    unsigned long long a = K[t], b = K[ixj];
+                    bool asc = (t & k) == 0;
+                    if ((a > b) == asc) { K[t] = b; K[ixj] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+constexpr int KD_SEGS = KD_MAX / UNIT;  // 512
+
+template <typename real>
+__global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const int* __restrict__ cell_start,
+                                  const int* __restrict__ unit_start, const int* __restrict__ cell_atoms,
+                                  int* __restrict__ perm, int* __restrict__ inv_perm, double* __restrict__ ref,
+                                  typename vec4<real>::type* __restrict__ xyz_build,
+                                  typename vec4<real>::type* __restrict__ bb_lo,
+                                  typename vec4<real>::type* __restrict__ bb_hi, int* __restrict__ unit_cell,
+                                  int npad_max)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int cell = blockIdx.x;
+    const int a0 = cell_start[cell];
+    const int n = cell_start[cell + 1] - a0;
+    if (n == 0) return;
+    int npad = 32;
+    while (npad < n) npad <<= 1;
+
+    unsigned long long* K = reinterpret_cast<unsigned long long*>(smem_raw);
+    real* X = reinterpret_cast<real*>(K + npad_max);
+    real* Y = X + npad_max;
+    real* Z = Y + npad_max;
+    int* ID = reinterpret_cast<int*>(Z + npad_max);
+    int* segS = ID + npad_max;
+    int* segN = segS + KD_SEGS;
+    int* segS2 = segN + KD_SEGS;
+    int* segN2 = segS2 + KD_SEGS;
+    int* segAxis = segN2 + KD_SEGS;
+    int* bbmin = segAxis + KD_SEGS;  // [3][KD_SEGS]
+    int* bbmax = bbmin + 3 * KD_SEGS;
+    unsigned short* SEG = reinterpret_cast<unsigned short*>(bbmax + 3 * KD_SEGS);
+    __shared__ int any_big;
+
+    // canonical order: by original atom index (makes the result independent of the binning atomics)
+    for (int p = threadIdx.x; p < npad; p += blockDim.x)
+        K[p] = p < n ? (((unsigned long long)(unsigned)cell_atoms[a0 + p]) << 12) : ~0ull;
+    __syncthreads();
+    bitonic_sort_u64(K, npad);
+
+    const int cz = cell % g.n[2];
+    const int cy = (cell / g.n[2]) % g.n[1];
+    const int cx = cell / (g.n[2] * g.n[1]);
+    const double org[3] = {cx * g.h[0], cy * g.h[1], cz * g.h[2]};
+
+    for (int p = threadIdx.x; p < n; p += blockDim.x) {
+        int id = (int)(K[p] >> 12);
+        ID[p] = id;
+        double r[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            double x = (double)pos[3 * (int64_t)id + a];
+            if (!isfinite(x)) x = 0.0;
+            double k = floor(x / g.L[a]);
+            r[a] = x - (org[a] + k * g.L[a]);
+        }
+        X[p] = (real)r[0];
+        Y[p] = (real)r[1];
+        Z[p] = (real)r[2];
+        SEG[p] = 0;
+    }
+    __syncthreads();
+    for (int p = threadIdx.x; p < npad; p += blockDim.x) K[p] = p < n ? (unsigned long long)p : ~0ull;
+    if (threadIdx.x == 0) { segS[0] = 0; segN[0] = n; }
+    __syncthreads();
+
+    int nseg = 1;
+    int *cS = segS, *cN = segN, *nS = segS2, *nN = segN2;
+    for (int level = 0; level < 10; ++level) {
+        if (threadIdx.x == 0) any_big = 0;
+        __syncthreads();
+        for (int s = threadIdx.x; s < nseg; s += blockDim.x) {
+            if (cN[s] > UNIT) any_big = 1;
+            bbmin[s] = bbmin[KD_SEGS + s] = bbmin[2 * KD_SEGS + s] = 0x7fffffff;
+            bbmax[s] = bbmax[KD_SEGS + s] = bbmax[2 * KD_SEGS + s] = (int)0x80000000;
+        }
+        __syncthreads();
+        if (!any_big) break;
+        // bounding box of every segment that will be split (ordered-int atomics in shared memory)
+        for (int p = threadIdx.x; p < n; p += blockDim.x) {
+            int s = SEG[p];
+            if (cN[s] > UNIT) {
+                int lid = (int)(K[p] & 0xFFF);
+                int ox = (int)(ordered_u32((float)X[lid]) ^ 0x80000000u);
+                int oy = (int)(ordered_u32((float)Y[lid]) ^ 0x80000000u);
+                int oz = (int)(ordered_u32((float)Z[lid]) ^ 0x80000000u);
+                atomicMin(&bbmin[s], ox); atomicMax(&bbmax[s], ox);
+                atomicMin(&bbmin[KD_SEGS + s], oy); atomicMax(&bbmax[KD_SEGS + s], oy);
+                atomicMin(&bbmin[2 * KD_SEGS + s], oz); atomicMax(&bbmax[2 * KD_SEGS + s], oz);
+            }
+        }
+        __syncthreads();
+        for (int s = threadIdx.x; s < nseg; s += blockDim.x) {
+            int ax = 0;
+            if (cN[s] > UNIT) {
+                float ext[3];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    unsigned lo = (unsigned)bbmin[a * KD_SEGS + s] ^ 0x80000000u;
+                    unsigned hi = (unsigned)bbmax[a * KD_SEGS + s] ^ 0x80000000u;
+                    // undo ordered_u32
+                    float flo = __uint_as_float((lo & 0x80000000u) ? (lo & 0x7fffffffu) : ~lo);
+                    float fhi = __uint_as_float((hi & 0x80000000u) ? (hi & 0x7fffffffu) : ~hi);
+                    ext[a] = fhi - flo;
+                }
+                if (ext[1] > ext[ax]) ax = 1;
+                if (ext[2] > ext[ax]) ax = 2;
+            }
+            segAxis[s] = ax;
+        }
+        __syncthreads();
+        for (int p = threadIdx.x; p < n; p += blockDim.x) {
+            int s = SEG[p];
+            int lid = (int)(K[p] & 0xFFF);
+            unsigned c;
+            if (cN[s] > UNIT) {
+                int ax = segAxis[s];
+                float v = ax == 0 ? (float)X[lid] : (ax == 1 ? (float)Y[lid] : (float)Z[lid]);
+                c = ordered_u32(v);
+            } else {
+                c = (unsigned)(p - cS[s]);
+            }
+            K[p] = ((unsigned long long)s << 44) | ((unsigned long long)c << 12) | (unsigned long long)lid;
+        }
+        __syncthreads();
+        bitonic_sort_u64(K, npad);
+        // split every big segment: the left child takes a multiple of UNIT atoms
+        for (int s = threadIdx.x; s < nseg; s += blockDim.x) {
+            int cnt = cN[s], st = cS[s];
+            if (cnt > UNIT) {
+                int u = (cnt + UNIT - 1) / UNIT;
+                int nl = UNIT * ((u + 1) / 2);
+                nS[2 * s] = st; nN[2 * s] = nl;
+                nS[2 * s + 1] = st + nl; nN[2 * s + 1] = cnt - nl;
+            } else {
+                nS[2 * s] = st; nN[2 * s] = cnt;
+                nS[2 * s + 1] = st + cnt; nN[2 * s + 1] = 0;
+            }
+        }
+        __syncthreads();
+        for (int p = threadIdx.x; p < n; p += blockDim.x) {
+            int s = SEG[p];
+            int child = 2 * s;
+            if (cN[s] > UNIT && p >= nS[2 * s + 1]) child = 2 * s + 1;
+            SEG[p] = (unsigned short)child;
+        }
+        __syncthreads();
+        int* t;
+        t = cS; cS = nS; nS = t;
+        t = cN; cN = nN; nN = t;
+        nseg *= 2;
+    }
+
+    // write the cell's atoms in their final order; position p -> slot u0*UNIT + p
+    const int u0 = unit_start[cell];
+    const int nu = (n + UNIT - 1) / UNIT;
+    using real4 = typename vec4<real>::type;
+    for (int p = threadIdx.x; p < nu * UNIT; p += blockDim.x) {
+        int q = p < n ? p : n - 1;  // padding slots mirror the cell's last atom
+        int lid = (int)(K[q] & 0xFFF);
+        int id = ID[lid];
+        int64_t slot = (int64_t)u0 * UNIT + p;
+        perm[slot] = p < n ? id : ~id;
+        if (p < n) inv_perm[id] = (int)slot;
+        xyz_build[slot] = make4(X[lid], Y[lid], Z[lid], (real)0);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            double x = (double)pos[3 * (int64_t)id + a];
+            if (!isfinite(x)) x = 0.0;
+            double k = floor(x / g.L[a]);
+            ref[3 * slot + a] = org[a] + k * g.L[a];
+        }
+    }
+    for (int u = threadIdx.x; u < nu; u += blockDim.x) {
+        real lo[3] = {(real)1e30, (real)1e30, (real)1e30}, hi[3] = {(real)-1e30, (real)-1e30, (real)-1e30};
+        for (int k = 0; k < UNIT; ++k) {
+            int p = u * UNIT + k;
+            if (p >= n) break;
+            int lid = (int)(K[p] & 0xFFF);
+            real v[3] = {X[lid], Y[lid], Z[lid]};
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { lo[a] = v[a] < lo[a] ? v[a] : lo[a]; hi[a] = v[a] > hi[a] ? v[a] : hi[a]; }
+        }
+        bb_lo[u0 + u] = make4(lo[0], lo[1], lo[2], (real)0);
+        bb_hi[u0 + u] = make4(hi[0], hi[1], hi[2], (real)0);
+        unit_cell[u0 + u] = cell;
+    }
+}
+
+static size_t kd_smem_bytes(int npad_max, size_t real_size)
+{
+    return (size_t)npad_max * (8 + 3 * real_size + 4 + 2) + (size_t)KD_SEGS * 4 * (5 + 6) + 64;
+}
+
+// ------------------------------------------------------------------------------------------------
+// exclusion adjacency (CSR over both directions)
+// ------------------------------------------------------------------------------------------------
+__global__ void excl_degree_kernel(const int2* __restrict__ pairs, int64_t n_excl, int64_t N, int* __restrict__ deg,
+                                   int* __restrict__ flags)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_excl) return;
+    int2 p = pairs[k];
+    if (p.x < 0 || p.y < 0 || p.x >= N || p.y >= N || p.x >= p.y) { atomicOr(&flags[0], FLAG_EXCL_RANGE); return; }
+    int a = atomicAdd(&deg[p.x], 1);
+    int b = atomicAdd(&deg[p.y], 1);
+    if (a >= MAX_EXCL_PER_ATOM || b >= MAX_EXCL_PER_ATOM) atomicOr(&flags[0], FLAG_EXCL_OVERFLOW);
+}
+__global__ void excl_fill_kernel(const int2* __restrict__ pairs, int64_t n_excl, int64_t N,
+                                 const int* __restrict__ start, int* __restrict__ cursor, int* __restrict__ adj)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_excl) return;
+    int2 p = pairs[k];
+    if (p.x < 0 || p.y < 0 || p.x >= N || p.y >= N || p.x >= p.y) return;
+    adj[start[p.x] + atomicAdd(&cursor[p.x], 1)] = p.y;
+    adj[start[p.y] + atomicAdd(&cursor[p.y], 1)] = p.x;
+}
+__global__ void zero_int_kernel(int* __restrict__ p, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A2: list build, one warp per unit
+// ------------------------------------------------------------------------------------------------
+constexpr int BL_WARPS = 4;
+constexpr int CAND_MAX = 256;  // candidate units buffered per warp before the atom-level pass
+constexpr int EX_MAX = UNIT * MAX_EXCL_PER_ATOM;
+
+template <typename real>
+struct BuildParams {
+    using real4 = typename vec4<real>::type;
+    Grid g;
+    int64_t n_units;
+    int row_cap, m_res;
+    real rnl2;
+    real L[3], h[3];
+    const int* unit_start;
+    const int* unit_cell;
+    const int* perm;
+    const int* inv_perm;
+    const real4* xyz;
+    const real4* bb_lo;
+    const real4* bb_hi;
+    const int* excl_start;
+    const int* excl_adj;
+    int* jslot;
+    unsigned short* meta;
+    int2* row_info;
+    int* flags;
+};
+
+// does unit U own the pairs between U and V (U != V)?  Circular half-ordering: balanced rows.
+__device__ __forceinline__ bool owns(int64_t U, int64_t V, int64_t n_units)
+{
+    int64_t d = V - U;
+    if (d < 0) d += n_units;
+    if (2 * d < n_units) return true;
+    if (2 * d == n_units) return U < V;
+    return false;
+}
+
+template <typename real, int PBC>
+__device__ __forceinline__ real axis_gap(real lo1, real hi1, real lo2, real hi2, real L)
+{
+    real g = fmax((real)0, fmax(lo1 - hi2, lo2 - hi1));
+    if (PBC == 1) {
+        real g1 = fmax((real)0, fmax(lo1 - (hi2 + L), (lo2 + L) - hi1));
+        real g2 = fmax((real)0, fmax(lo1 - (hi2 - L), (lo2 - L) - hi1));
+        g = fmin(g, fmin(g1, g2));
+    }
+    return g;
+}
+
+template <typename real, int PBC>
+__global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<real> P)
+{
+    using real4 = typename vec4<real>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    const int wib = threadIdx.x >> 5;
+    const int64_t U = (int64_t)blockIdx.x * BL_WARPS + wib;
+    if (U >= P.n_units) return;  // no block-wide barriers below
+    const unsigned FULL = 0xffffffffu;
+    const unsigned lt_mask = (1u << lane) - 1u;
+
+    // per-warp shared-memory carve-up
+    const size_t per_warp = (size_t)CAND_MAX * 4 + CAND_MAX + (size_t)P.m_res * 4 + (size_t)P.m_res * 2 +
+                            (size_t)EX_MAX * 4 + EX_MAX;
+    unsigned char* base = smem_raw + (size_t)wib * ((per_warp + 15) & ~(size_t)15);
+    int* cand_unit = reinterpret_cast<int*>(base);
+    int* st_j = cand_unit + CAND_MAX;
+    int* ex_slot = st_j + P.m_res;
+    unsigned short* st_meta = reinterpret_cast<unsigned short*>(ex_slot + EX_MAX);
+    unsigned char* cand_code = reinterpret_cast<unsigned char*>(st_meta + P.m_res);
+    unsigned char* ex_i = cand_code + CAND_MAX;
+
+    // ---- the unit's own atoms, broadcast to every lane ----
+    real xi[UNIT], yi[UNIT], zi[UNIT];
+    int my_perm = -1;
+    real4 mine = make4((real)0, (real)0, (real)0, (real)0);
+    if (lane < UNIT) { mine = P.xyz[U * UNIT + lane]; my_perm = P.perm[U * UNIT + lane]; }
+#pragma unroll
+    for (int i = 0; i < UNIT; ++i) {
+        xi[i] = __shfl_sync(FULL, mine.x, i);
+        yi[i] = __shfl_sync(FULL, mine.y, i);
+        zi[i] = __shfl_sync(FULL, mine.z, i);
+    }
+    const unsigned valid_i = __ballot_sync(FULL, lane < UNIT && my_perm >= 0) & 0xFFu;
+    const bool unit_full = valid_i == 0xFFu;
+    const real4 ulo = P.bb_lo[U], uhi = P.bb_hi[U];
+
+    // ---- exclusion partners of the unit's atoms, as (slot, i) pairs in shared memory ----
+    int deg = 0, es = 0;
+    if (lane < UNIT && my_perm >= 0) { es = P.excl_start[my_perm]; deg = min(P.excl_start[my_perm + 1] - es, MAX_EXCL_PER_ATOM); }
+    int off_ex = deg;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(FULL, off_ex, o);
+        if (lane >= o) off_ex += y;
+    }
+    const int n_ex = __shfl_sync(FULL, off_ex, 31);
+    off_ex -= deg;
+    int ex_lo = 0x7fffffff, ex_hi = -1;
+    for (int k = 0; k < deg; ++k) {
+        int s = P.inv_perm[P.excl_adj[es + k]];
+        ex_slot[off_ex + k] = s;
+        ex_i[off_ex + k] = (unsigned char)lane;
+        ex_lo = min(ex_lo, s);
+        ex_hi = max(ex_hi, s);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ex_lo = min(ex_lo, __shfl_xor_sync(FULL, ex_lo, o));
+        ex_hi = max(ex_hi, __shfl_xor_sync(FULL, ex_hi, o));
+    }
+    __syncwarp();
+
+    const int64_t row = U * (int64_t)P.row_cap;
+    int nm = 0;  // masked entries staged
+    int nu = 0;  // unmasked entries written (or needed, once overflowing)
+    const int nu_cap = P.row_cap - P.m_res;
+
+    // append one warp-wide batch of entries
+    auto append = [&](bool accept, unsigned mask, int j, int code) {
+        const bool is_masked = accept && (mask != (unit_full ? 0xFFu : valid_i) || !unit_full);
+        const bool is_plain = accept && !is_masked;
+        unsigned bm = __ballot_sync(FULL, is_masked);
+        unsigned bp = __ballot_sync(FULL, is_plain);
+        if (is_masked) {
+            int pos = nm + __popc(bm & lt_mask);
+            if (pos < P.m_res) { st_j[pos] = j; st_meta[pos] = (unsigned short)(mask | (code << 8)); }
+        }
+        if (is_plain) {
+            int pos = nu + __popc(bp & lt_mask);
+            if (pos < nu_cap) {
+                P.jslot[row + P.m_res + pos] = j;
+                P.meta[row + P.m_res + pos] = (unsigned short)(0xFFu | (code << 8));
+            }
+        }
+        nm += __popc(bm);
+        nu += __popc(bp);
+    };
+    // Partial units (fewer than UNIT real atoms, one per cell) keep every entry in the row's plain
+    // region with mask = valid_i: the force kernel runs them through its masked path.
+    auto append_any = [&](bool accept, unsigned mask, int j, int code) {
+        if (unit_full) { append(accept, mask, j, code); return; }
+        unsigned bp = __ballot_sync(FULL, accept);
+        if (accept) {
+            int pos = nu + __popc(bp & lt_mask);
+            if (pos < nu_cap) {
+                P.jslot[row + P.m_res + pos] = j;
+                P.meta[row + P.m_res + pos] = (unsigned short)(mask | (code << 8));
+            }
+        }
+        nu += __popc(bp);
+    };
+
+    auto excl_bits = [&](int slot) -> unsigned {
+        unsigned ex = 0;
+        if (slot >= ex_lo && slot <= ex_hi)
+            for (int k = 0; k < n_ex; ++k)
+                if (ex_slot[k] == slot) ex |= 1u << ex_i[k];
+        return ex;
+    };
+
+    // ---- own-unit entries: the i < j half ----
+    {
+        bool acc = lane < UNIT && my_perm >= 0;
+        int slot = (int)(U * UNIT + lane);
+        unsigned mask = 0;
+        if (acc) {
+            mask = ((1u << lane) - 1u) & valid_i & ~excl_bits(slot);
+            acc = mask != 0;
+        }
+        append_any(acc, mask, slot, SELF_CODE);
+    }
+
+    // ---- stencil: unique neighbour cells per axis (reading C-18) ----
+    const int cell = P.unit_cell[U];
+    const int ccz = cell % P.g.n[2];
+    const int ccy = (cell / P.g.n[2]) % P.g.n[1];
+    const int ccx = cell / (P.g.n[2] * P.g.n[1]);
+    const int cc[3] = {ccx, ccy, ccz};
+    int sc[3][3], sd[3][3], sn[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int n = P.g.n[a];
+        if (n == 1) { sn[a] = 1; sc[a][0] = cc[a]; sd[a][0] = 0; }
+        else if (n == 2) { sn[a] = 2; sc[a][0] = cc[a]; sd[a][0] = 0; sc[a][1] = 1 - cc[a]; sd[a][1] = 1 - 2 * cc[a]; }
+        else {
+            sn[a] = 3;
+            for (int k = 0; k < 3; ++k) { int d = k - 1; sd[a][k] = d; sc[a][k] = (cc[a] + d + n) % n; }
+        }
+    }
+
+    int ncand = 0;
+    // atom-level pass over the buffered candidate units
+    auto flush = [&]() {
+        const int T = ncand * UNIT;
+        for (int t0 = 0; t0 < T; t0 += 32) {
+            const int t = t0 + lane;
+            bool acc = false;
+            unsigned mask = 0;
+            int slot = 0, code = SELF_CODE;
+            if (t < T) {
+                const int v = cand_unit[t >> 3];
+                code = cand_code[t >> 3];
+                slot = v * UNIT + (t & 7);
+                if (P.perm[slot] >= 0) {
+                    real4 pj = P.xyz[slot];
+                    const int dx = code / 9 - 1, dy = (code / 3) % 3 - 1, dz = code % 3 - 1;
+                    const real px = pj.x + (real)dx * P.h[0], py = pj.y + (real)dy * P.h[1], pz = pj.z + (real)dz * P.h[2];
+                    unsigned bits = 0;
+#pragma unroll
+                    for (int i = 0; i < UNIT; ++i) {
+                        real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
+                        if (PBC == 1) {
+                            ddx -= P.L[0] * rint_r(ddx / P.L[0]);
+                            ddy -= P.L[1] * rint_r(ddy / P.L[1]);
+                            ddz -= P.L[2] * rint_r(ddz / P.L[2]);
+                        }
+                        real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                        bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
+                    }
+                    mask = valid_i & ~excl_bits(slot);
+                    acc = (bits & mask) != 0;
+                }
+            }
+            append_any(acc, mask, slot, code);
+        }
+        ncand = 0;
+    };
+
+    for (int ix = 0; ix < sn[0]; ++ix)
+        for (int iy = 0; iy < sn[1]; ++iy)
+            for (int iz = 0; iz < sn[2]; ++iz) {
+                const int c2 = (sc[0][ix] * P.g.n[1] + sc[1][iy]) * P.g.n[2] + sc[2][iz];
+                const int code = stencil_code(sd[0][ix], sd[1][iy], sd[2][iz]);
+                const real ox = (real)sd[0][ix] * P.h[0], oy = (real)sd[1][iy] * P.h[1], oz = (real)sd[2][iz] * P.h[2];
+                const int us = P.unit_start[c2], ue = P.unit_start[c2 + 1];
+                for (int v0 = us; v0 < ue; v0 += 32) {
+                    if (ncand + 32 > CAND_MAX) flush();
+                    const int v = v0 + lane;
+                    bool acc = false;
+                    if (v < ue && v != U && owns(U, v, P.n_units)) {
+                        real4 lo = P.bb_lo[v], hi = P.bb_hi[v];
+                        real gx = axis_gap<real, PBC>(ulo.x, uhi.x, lo.x + ox, hi.x + ox, P.L[0]);
+                        real gy = axis_gap<real, PBC>(ulo.y, uhi.y, lo.y + oy, hi.y + oy, P.L[1]);
+                        real gz = axis_gap<real, PBC>(ulo.z, uhi.z, lo.z + oz, hi.z + oz, P.L[2]);
+                        acc = gx * gx + gy * gy + gz * gz < P.rnl2;
+                    }
+                    unsigned b = __ballot_sync(FULL, acc);
+                    if (acc) {
+                        int pos = ncand + __popc(b & lt_mask);
+                        cand_unit[pos] = v;
+                        cand_code[pos] = (unsigned char)code;
+                    }
+                    ncand += __popc(b);
+                    __syncwarp();
+                }
+            }
+    flush();
+    __syncwarp();
+
+    // ---- finish the row ----
+    if (nm > P.m_res) {
+        if (lane == 0) { atomicOr(&P.flags[0], FLAG_MASKED_OVERFLOW); atomicMax(&P.flags[7], nm); }
+        nm = P.m_res;
+    }
+    const int nu_pad = (nu + 31) & ~31;
+    if (nu_pad > nu_cap) {
+        if (lane == 0) { atomicOr(&P.flags[0], FLAG_ROW_OVERFLOW); atomicMax(&P.flags[6], nu_pad); }
+        nu = 0;  // the row is unusable; the host grows row_cap and rebuilds
+    }
+    const int mc = (nm + 31) >> 5;
+    const int self = (int)(U * UNIT);
+    const unsigned short pad_meta = (unsigned short)(SELF_CODE << 8);  // mask 0
+    for (int k = lane; k < mc * 32; k += 32) {
+        int64_t e = row + P.m_res - mc * 32 + k;
+        P.jslot[e] = k < nm ? st_j[k] : self;
+        P.meta[e] = k < nm ? st_meta[k] : pad_meta;
+    }
+    {
+        const int nu_ok = min(nu, nu_cap);
+        const int pad_to = min((nu_ok + 31) & ~31, nu_cap);
+        for (int k = nu_ok + lane; k < pad_to; k += 32) {
+            P.jslot[row + P.m_res + k] = self;
+            P.meta[row + P.m_res + k] = pad_meta;
+        }
+    }
+    if (lane == 0) {
+        P.row_info[U] = make_int2(mc | (unit_full ? 0 : 0x10000), nu);
+        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[2]), (unsigned long long)(nm + nu));
+        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[4]), (unsigned long long)(mc * 32 + ((nu + 31) & ~31)));
+    }
+}
+
+static size_t build_smem_bytes(int m_res)
+{
+    size_t per_warp = (size_t)CAND_MAX * 4 + CAND_MAX + (size_t)m_res * 4 + (size_t)m_res * 2 + (size_t)EX_MAX * 4 + EX_MAX;
+    per_warp = (per_warp + 15) & ~(size_t)15;
+    return per_warp * BL_WARPS;
+}
+
+// ------------------------------------------------------------------------------------------------
+// export: expand the list to atom pairs at the build positions
+// ------------------------------------------------------------------------------------------------
+template <typename real, int PBC>
+__global__ __launch_bounds__(128) void export_pairs_kernel(BuildParams<real> P, int2* __restrict__ pairs, int64_t cap,
+                                                           unsigned long long* __restrict__ counter)
+{
+    using real4 = typename vec4<real>::type;
+    const int lane = threadIdx.x & 31;
+    const int64_t U = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (U >= P.n_units) return;
+    const unsigned FULL = 0xffffffffu;
+    real xi[UNIT], yi[UNIT], zi[UNIT];
+    int pi[UNIT];
+    int my_perm = -1;
+    real4 mine = make4((real)0, (real)0, (real)0, (real)0);
+    if (lane < UNIT) { mine = P.xyz[U * UNIT + lane]; my_perm = P.perm[U * UNIT + lane]; }
+#pragma unroll
+    for (int i = 0; i < UNIT; ++i) {
+        xi[i] = __shfl_sync(FULL, mine.x, i);
+        yi[i] = __shfl_sync(FULL, mine.y, i);
+        zi[i] = __shfl_sync(FULL, mine.z, i);
+        pi[i] = __shfl_sync(FULL, my_perm, i);
+    }
+    const int2 ri = P.row_info[U];
+    const int mc = ri.x & 0xFFFF, nu = ri.y;
+    const int64_t row = U * (int64_t)P.row_cap + P.m_res;
+    const int nch = (nu + 31) >> 5;
+    for (int c = -mc; c < nch; ++c) {
+        const int64_t e = row + (int64_t)c * 32 + lane;
+        const int j = P.jslot[e];
+        const unsigned m = P.meta[e];
+        const unsigned mask = m & 0xFFu;
+        const int code = (int)(m >> 8);
+        real4 pj = P.xyz[j];
+        const int pj_orig = P.perm[j];
+        const int dx = code / 9 - 1, dy = (code / 3) % 3 - 1, dz = code % 3 - 1;
+        const real px = pj.x + (real)dx * P.h[0], py = pj.y + (real)dy * P.h[1], pz = pj.z + (real)dz * P.h[2];
+        unsigned bits = 0;
+#pragma unroll
+        for (int i = 0; i < UNIT; ++i) {
+            real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
+            if (PBC == 1) {
+                ddx -= P.L[0] * rint_r(ddx / P.L[0]);
+                ddy -= P.L[1] * rint_r(ddy / P.L[1]);
+                ddz -= P.L[2] * rint_r(ddz / P.L[2]);
+            }
+            real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+            bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
+        }
+        bits &= mask;
+        int cnt = __popc(bits);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += y;
+        }
+        int total = __shfl_sync(FULL, incl, 31);
+        unsigned long long basep = 0;
+        if (lane == 0 && total > 0) basep = atomicAdd(counter, (unsigned long long)total);
+        basep = __shfl_sync(FULL, basep, 0);
+        unsigned long long w = basep + (unsigned long long)(incl - cnt);
+#pragma unroll
+        for (int i = 0; i < UNIT; ++i) {
+            if (bits & (1u << i)) {
+                if ((int64_t)w < cap) {
+                    int a = pi[i], b = pj_orig;
+                    pairs[w] = a < b ? make_int2(a, b) : make_int2(b, a);
+                }
+                ++w;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host orchestration
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+static BuildParams<real> make_build_params(const NL* nl)
+{
+    using real4 = typename vec4<real>::type;
+    BuildParams<real> P;
+    P.g = nl->grid;
+    P.n_units = nl->n_units;
+    P.row_cap = nl->row_cap;
+    P.m_res = nl->m_res;
+    P.rnl2 = (real)nl->r_nl * (real)nl->r_nl;
+    for (int a = 0; a < 3; ++a) { P.L[a] = (real)nl->grid.L[a]; P.h[a] = (real)nl->grid.h[a]; }
+    P.unit_start = (const int*)nl->unit_start.p;
+    P.unit_cell = (const int*)nl->unit_cell.p;
+    P.perm = (const int*)nl->perm.p;
+    P.inv_perm = (const int*)nl->inv_perm.p;
+    P.xyz = (const real4*)nl->xyz_build.p;
+    P.bb_lo = (const real4*)nl->bb_lo.p;
+    P.bb_hi = (const real4*)nl->bb_hi.p;
+    P.excl_start = (const int*)nl->excl_start.p;
+    P.excl_adj = (const int*)nl->excl_adj.p;
+    P.jslot = (int*)nl->jslot.p;
+    P.meta = (unsigned short*)nl->meta.p;
+    P.row_info = (int2*)nl->row_info.p;
+    P.flags = (int*)nl->flags.p;
+    return P;
+}
+
+template <typename real>
+static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl_pairs, int64_t n_excl,
+                          real* pos_at_build, cudaStream_t s)
+{
+    using real4 = typename vec4<real>::type;
+    const int64_t N = nl->N;
+    const Grid& g = nl->grid;
+    const int64_t ncells = g.ncells;
+    int rc;
+    // ---- workspace that depends only on N / ncells ----
+    if ((rc = ensure(ctx, nl->cell_count, (ncells + 1) * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->cell_start, (ncells + 1) * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->unit_start, (ncells + 1) * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->scan_tmp, (scan_tmp_ints(std::max(ncells, N) + 1) + (size_t)ncells + 1 + (size_t)N + 1) * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->atom_cell, N * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->atom_rank, N * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->cell_atoms, N * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->inv_perm, N * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->flags, 16 * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->excl_start, (N + 1) * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->excl_adj, (size_t)std::max<int64_t>(2 * n_excl, 1) * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->excl_pairs, (size_t)std::max<int64_t>(n_excl, 1) * sizeof(int2), s))) return rc;
+    if ((rc = ensure(ctx, nl->export_count, 8, s))) return rc;
+    int* flags = (int*)nl->flags.p;
+    int* scan_tmp = (int*)nl->scan_tmp.p;
+    int* unit_count = scan_tmp + scan_tmp_ints(std::max(ncells, N) + 1);  // int[ncells+1]
+    int* excl_deg = unit_count + ncells + 1;                               // int[N+1]
+    const int T = 256;
+
+    zero_int_kernel<<<1, 32, 0, s>>>(flags, 16);
+    DIMOS_LAUNCH_CHECK(ctx, "zero_flags");
+    zero_int_kernel<<<(unsigned)((ncells + 1 + T - 1) / T), T, 0, s>>>((int*)nl->cell_count.p, ncells + 1);
+    DIMOS_LAUNCH_CHECK(ctx, "zero_cells");
+    bin_atoms_kernel<real><<<(unsigned)((N + T - 1) / T), T, 0, s>>>(pos, N, g, (int*)nl->cell_count.p,
+                                                                      (int*)nl->atom_cell.p, (int*)nl->atom_rank.p,
+                                                                      pos_at_build, flags);
+    DIMOS_LAUNCH_CHECK(ctx, "bin_atoms");
+    cell_units_kernel<<<(unsigned)((ncells + T - 1) / T), T, 0, s>>>((const int*)nl->cell_count.p, ncells, unit_count, flags);
+    DIMOS_LAUNCH_CHECK(ctx, "cell_units");
+    if ((rc = exclusive_scan(ctx, (const int*)nl->cell_count.p, (int*)nl->cell_start.p, ncells, scan_tmp, s))) return rc;
+    if ((rc = exclusive_scan(ctx, unit_count, (int*)nl->unit_start.p, ncells, scan_tmp, s))) return rc;
+    scatter_atoms_kernel<<<(unsigned)((N + T - 1) / T), T, 0, s>>>(N, (const int*)nl->atom_cell.p, (const int*)nl->atom_rank.p,
+                                                                   (const int*)nl->cell_start.p, (int*)nl->cell_atoms.p);
+    DIMOS_LAUNCH_CHECK(ctx, "scatter_atoms");
+
+    // exclusion CSR
+    nl->n_excl = n_excl;
+    zero_int_kernel<<<(unsigned)((N + 1 + T - 1) / T), T, 0, s>>>(excl_deg, N + 1);
+    DIMOS_LAUNCH_CHECK(ctx, "zero_deg");
+    if (n_excl > 0) {
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->excl_pairs.p, excl_pairs, n_excl * sizeof(int2), cudaMemcpyDeviceToDevice, s));
+        excl_degree_kernel<<<(unsigned)((n_excl + T - 1) / T), T, 0, s>>>((const int2*)nl->excl_pairs.p, n_excl, N, excl_deg, flags);
+        DIMOS_LAUNCH_CHECK(ctx, "excl_degree");
+    }
+    if ((rc = exclusive_scan(ctx, excl_deg, (int*)nl->excl_start.p, N, scan_tmp, s))) return rc;
+    if (n_excl > 0) {
+        zero_int_kernel<<<(unsigned)((N + 1 + T - 1) / T), T, 0, s>>>(excl_deg, N + 1);
+        DIMOS_LAUNCH_CHECK(ctx, "zero_cursor");
+        excl_fill_kernel<<<(unsigned)((n_excl + T - 1) / T), T, 0, s>>>((const int2*)nl->excl_pairs.p, n_excl, N,
+                                                                        (const int*)nl->excl_start.p, excl_deg, (int*)nl->excl_adj.p);
+        DIMOS_LAUNCH_CHECK(ctx, "excl_fill");
+    }
+
+    // ---- read back: number of units, max cell population, early error flags (sync #1) ----
+    int* h = ctx->h_pinned;
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h, flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h + 2, (int*)nl->unit_start.p + ncells, sizeof(int), cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    if (h[0] & FLAG_NONFINITE) return set_error(ctx, DIMOS_EINVAL, "non-finite coordinate in pos");
+    if (h[0] & FLAG_EXCL_RANGE) return set_error(ctx, DIMOS_EINVAL, "excl_pairs row out of range or not i<j");
+    if (h[0] & FLAG_EXCL_OVERFLOW) return set_error(ctx, DIMOS_EINVAL, "an atom has more than 32 exclusion partners");
+    nl->max_cell_count = h[1];
+    if (h[1] > KD_MAX) return set_error(ctx, DIMOS_EOVERFLOW, "more than 4096 atoms in one cell (r_cut+skin too large for this density)");
+    nl->n_units = h[2];
+    nl->n_slots = nl->n_units * UNIT;
+    const int64_t nun = nl->n_units, nsl = nl->n_slots;
+
+    if ((rc = ensure(ctx, nl->perm, nsl * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->ref, nsl * 3 * sizeof(double), s))) return rc;
+    if ((rc = ensure(ctx, nl->xyz_build, nsl * sizeof(real4), s))) return rc;
+    if ((rc = ensure(ctx, nl->bb_lo, nun * sizeof(real4), s))) return rc;
+    if ((rc = ensure(ctx, nl->bb_hi, nun * sizeof(real4), s))) return rc;
+    if ((rc = ensure(ctx, nl->unit_cell, nun * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->row_info, nun * sizeof(int2), s))) return rc;
+
+    int npad_max = 32;
+    while (npad_max < nl->max_cell_count) npad_max <<= 1;
+    const size_t kd_smem = kd_smem_bytes(npad_max, sizeof(real));
+    DIMOS_CUDA_TRY(ctx, cudaFuncSetAttribute(kd_cluster_kernel<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kd_smem));
+    kd_cluster_kernel<real><<<(unsigned)ncells, 256, kd_smem, s>>>(
+        pos, g, (const int*)nl->cell_start.p, (const int*)nl->unit_start.p, (const int*)nl->cell_atoms.p, (int*)nl->perm.p,
+        (int*)nl->inv_perm.p, (double*)nl->ref.p, (real4*)nl->xyz_build.p, (real4*)nl->bb_lo.p, (real4*)nl->bb_hi.p,
+        (int*)nl->unit_cell.p, npad_max);
+    DIMOS_LAUNCH_CHECK(ctx, "kd_cluster");
+
+    // ---- row capacity estimate (grown on overflow) ----
+    if (nl->row_cap == 0) {
+        const double vol = g.L[0] * g.L[1] * g.L[2];
+        const double dens = (double)N / vol;
+        const double ext = 0.75 * cbrt((double)UNIT / dens);
+        const double rr = nl->r_nl + ext;
+        double est = 0.5 * dens * (4.0 / 3.0) * M_PI * rr * rr * rr * 1.3 + 64;
+        if (est > (double)N + 32) est = (double)N + 32;
+        nl->row_cap = nl->m_res + (((int)est + 31) & ~31);
+    }
+    for (int attempt = 0; attempt < 6; ++attempt) {
+        if ((rc = ensure(ctx, nl->jslot, (size_t)nun * nl->row_cap * sizeof(int), s))) return rc;
+        if ((rc = ensure(ctx, nl->meta, (size_t)nun * nl->row_cap * sizeof(unsigned short), s))) return rc;
+        zero_int_kernel<<<1, 32, 0, s>>>(flags + 2, 8);
+        DIMOS_LAUNCH_CHECK(ctx, "zero_counters");
+        BuildParams<real> P = make_build_params<real>(nl);
+        const size_t smem = build_smem_bytes(nl->m_res);
+        const unsigned nb = (unsigned)((nun + BL_WARPS - 1) / BL_WARPS);
+        if (g.pbc_mode == 0) {
+            DIMOS_CUDA_TRY(ctx, cudaFuncSetAttribute(build_list_kernel<real, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            build_list_kernel<real, 0><<<nb, BL_WARPS * 32, smem, s>>>(P);
+        } else {
+            DIMOS_CUDA_TRY(ctx, cudaFuncSetAttribute(build_list_kernel<real, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            build_list_kernel<real, 1><<<nb, BL_WARPS * 32, smem, s>>>(P);
+        }
+        DIMOS_LAUNCH_CHECK(ctx, "build_list");
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h, flags, 8 * sizeof(int), cudaMemcpyDeviceToHost, s));
+        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));  // sync #2
+        if (!(h[0] & (FLAG_ROW_OVERFLOW | FLAG_MASKED_OVERFLOW))) {
+            unsigned long long ne, np;
+            memcpy(&ne, h + 2, 8);
+            memcpy(&np, h + 4, 8);
+            nl->n_entries = (int64_t)ne;
+            nl->n_entries_padded = (int64_t)np;
+            return DIMOS_OK;
+        }
+        nl->n_grow++;
+        if (h[0] & FLAG_MASKED_OVERFLOW) {
+            int need = (h[7] + 31) & ~31;
+            if (need > 4096) return set_error(ctx, DIMOS_EOVERFLOW, "too many masked entries per unit");
+            nl->row_cap += need - nl->m_res;
+            nl->m_res = need;
+        }
+        if (h[0] & FLAG_ROW_OVERFLOW) nl->row_cap = nl->m_res + (((int)(h[6] * 1.15) + 63) & ~31);
+        zero_int_kernel<<<1, 32, 0, s>>>(flags, 1);
+        DIMOS_LAUNCH_CHECK(ctx, "zero_flags");
+        zero_int_kernel<<<1, 32, 0, s>>>(flags + 6, 2);
+        DIMOS_LAUNCH_CHECK(ctx, "zero_flags");
+    }
+    return set_error(ctx, DIMOS_EOVERFLOW, "neighbour-list row capacity still exceeded after 6 growth attempts");
+}
+
+int nl_build_impl(Ctx* ctx, NL* nl, const void* pos, const int32_t* excl_pairs, int64_t n_excl, void* pos_at_build,
+                  cudaStream_t s)
+{
+    if (ctx->precision == DIMOS_F64)
+        return nl_build_typed<double>(ctx, nl, (const double*)pos, excl_pairs, n_excl, (double*)pos_at_build, s);
+    return nl_build_typed<float>(ctx, nl, (const float*)pos, excl_pairs, n_excl, (float*)pos_at_build, s);
+}
+
+template <typename real>
+static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, cudaStream_t s)
+{
+    BuildParams<real> P = make_build_params<real>(nl);
+    unsigned long long* counter = (unsigned long long*)nl->export_count.p;
+    zero_int_kernel<<<1, 32, 0, s>>>((int*)counter, 2);
+    DIMOS_LAUNCH_CHECK(ctx, "zero_counter");
+    const unsigned nb = (unsigned)((nl->n_units + 3) / 4);
+    if (nl->grid.pbc_mode == 0)
+        export_pairs_kernel<real, 0><<<nb, 128, 0, s>>>(P, (int2*)pairs, pairs ? cap : 0, counter);
+    else
+        export_pairs_kernel<real, 1><<<nb, 128, 0, s>>>(P, (int2*)pairs, pairs ? cap : 0, counter);
+    DIMOS_LAUNCH_CHECK(ctx, "export_pairs");
+    unsigned long long* h = reinterpret_cast<unsigned long long*>(ctx->h_pinned + 16);
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h, counter, 8, cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    *n_pairs_host = (int64_t)*h;
+    if ((int64_t)*h > cap && pairs) return set_error(ctx, DIMOS_EOVERFLOW, "pairs buffer too small");
+    return DIMOS_OK;
+}
+
+int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, cudaStream_t s)
+{
+    if (ctx->precision == DIMOS_F64) return nl_export_typed<double>(ctx, nl, pairs, cap, n_pairs_host, s);
+    return nl_export_typed<float>(ctx, nl, pairs, cap, n_pairs_host, s);
+}
+
+}  // namespace dimos

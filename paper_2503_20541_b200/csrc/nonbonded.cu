@@ -1,0 +1,635 @@
+// nonbonded.cu -- per-step kernels.
+//
+//   A3  needs_rebuild: warp-reduced max of |pos - pos_at_build|^2.
+//   gather: current positions -> cell-relative sorted float4 (x,y,z,q), LJ type, zeroed j-side force
+//           accumulators; block 0 also converts the (sigma, eps) table to (c6, c12).
+//   A4  pair_force: one warp per unit of 8 i-atoms held in registers; every lane owns one j-atom of
+//       a 32-wide chunk of the unit's list, evaluates it against the 8 i-atoms (LJ Eq. 4 + reaction
+//       field Eq. 8, or + Ewald direct space Eq. 10), accumulates F_i in registers over the whole
+//       row and F_j over the 8 slots, then issues ONE vector reduction (red.global.add.v4.f32) per
+//       j-atom.  F_i is reduced across the warp once per unit by recursive halving shuffles.
+//       Energy and virial are per-lane partial sums, reduced per warp, per block and finally in
+//       fp64 (A6).  The virial uses W = sum_i x_i (x) F_i^unit + sum_entries x_j' (x) F_j^entry in
+//       unit-local coordinates, so it costs 6 FMA per entry instead of 6 per pair.
+//   A5  excl_correction: Ewald erf correction over the static exclusion list.
+//   A6  finalize: F[orig] = F_own + F_acc, fp64 reduction of block partials, E[4], W[9].
+#include <math.h>
+
+#include "common.cuh"
+
+namespace dimos {
+
+__device__ __forceinline__ float4 mk4(float x, float y, float z, float w) { return make_float4(x, y, z, w); }
+__device__ __forceinline__ double4 mk4(double x, double y, double z, double w) { return make_double4(x, y, z, w); }
+
+// rsqrt: one MUFU.RSQ in fp32 (2^-22.9 max relative error); IEEE-quality in fp64
+__device__ __forceinline__ float rsqrt_r(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ double rsqrt_r(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ float rintr(float x) { return rintf(x); }
+__device__ __forceinline__ double rintr(double x) { return rint(x); }
+__device__ __forceinline__ float erfc_r(float x) { return erfcf(x); }
+__device__ __forceinline__ double erfc_r(double x) { return erfc(x); }
+__device__ __forceinline__ float erf_r(float x) { return erff(x); }
+__device__ __forceinline__ double erf_r(double x) { return erf(x); }
+__device__ __forceinline__ float exp_r(float x) { return expf(x); }
+__device__ __forceinline__ double exp_r(double x) { return exp(x); }
+
+// one vector reduction per j-atom (REDG.E.ADD.F32x4 on sm_100a); fp64 falls back to three scalar REDs
+__device__ __forceinline__ void red_add_xyz(float4* p, float x, float y, float z)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(x), "f"(y), "f"(z), "f"(0.0f) : "memory");
+}
+__device__ __forceinline__ void red_add_xyz(double4* p, double x, double y, double z)
+{
+    atomicAdd(&p->x, x);
+    atomicAdd(&p->y, y);
+    atomicAdd(&p->z, z);
+}
+
+// ------------------------------------------------------------------------------------------------
+// A3: rebuild trigger
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void needs_rebuild_kernel(const real* __restrict__ pos, const real* __restrict__ ref, int64_t N, real thr2,
+                                     unsigned long long* __restrict__ state, int* __restrict__ flag)
+{
+    real m = 0;
+    const int64_t n3 = 3 * N;
+    // each thread handles whole atoms; consecutive threads read consecutive atoms (12-byte stride, coalesced)
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        real dx = pos[3 * i] - ref[3 * i];
+        real dy = pos[3 * i + 1] - ref[3 * i + 1];
+        real dz = pos[3 * i + 2] - ref[3 * i + 2];
+        real d2 = dx * dx + dy * dy + dz * dz;
+        m = d2 > m ? d2 : m;
+        if (!(d2 == d2)) m = (real)INFINITY;  // NaN -> force a rebuild
+    }
+    (void)n3;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        real y = __shfl_xor_sync(0xffffffffu, m, o);
+        m = y > m ? y : m;
+    }
+    __shared__ real wmax[32];
+    __shared__ bool last;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) wmax[w] = m;
+    __syncthreads();
+    if (w == 0) {
+        m = lane < (blockDim.x >> 5) ? wmax[lane] : (real)0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            real y = __shfl_xor_sync(0xffffffffu, m, o);
+            m = y > m ? y : m;
+        }
+        if (lane == 0) {
+            // non-negative doubles order like their bit patterns
+            atomicMax(&state[0], (unsigned long long)__double_as_longlong((double)m));
+            __threadfence();
+            unsigned long long t = atomicAdd(&state[1], 1ull);
+            last = (t == (unsigned long long)gridDim.x - 1);
+        }
+    }
+    __syncthreads();
+    if (last && threadIdx.x == 0) {
+        __threadfence();
+        unsigned long long bits = atomicExch(&state[0], 0ull);
+        state[1] = 0ull;
+        double mx = __longlong_as_double((long long)bits);
+        *flag = mx > (double)thr2 ? 1 : 0;
+    }
+}
+
+int needs_rebuild_impl(Ctx* ctx, const void* pos, const void* ref, int64_t N, double skin, int32_t* flag_dev, cudaStream_t s)
+{
+    int blocks = (int)((N + 255) / 256);
+    int maxb = ctx->sm_count * 8;
+    if (blocks > maxb) blocks = maxb;
+    if (blocks < 1) blocks = 1;
+    if (ctx->precision == DIMOS_F64) {
+        double h = 0.5 * skin;
+        needs_rebuild_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos, (const double*)ref, N, h * h, ctx->d_rebuild_state, flag_dev);
+    } else {
+        float h = 0.5f * (float)skin;
+        needs_rebuild_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos, (const float*)ref, N, h * h, ctx->d_rebuild_state, flag_dev);
+    }
+    DIMOS_LAUNCH_CHECK(ctx, "needs_rebuild");
+    return DIMOS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// gather: caller-order inputs -> sorted, cell-relative device arrays
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void gather_kernel(const real* __restrict__ pos, const real* __restrict__ charge, const int* __restrict__ type,
+                              const int* __restrict__ perm, const double* __restrict__ ref, int64_t n_slots,
+                              typename vec4<real>::type* __restrict__ xyzq, int* __restrict__ stype,
+                              typename vec4<real>::type* __restrict__ Facc, const double* __restrict__ lj_table, int nt,
+                              real* __restrict__ lj_out, int* __restrict__ row_active, double* __restrict__ accum)
+{
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n_slots) {
+        int o = perm[s];
+        const bool pad = o < 0;
+        if (pad) o = ~o;
+        const double x = (double)pos[3 * (int64_t)o] - ref[3 * s];
+        const double y = (double)pos[3 * (int64_t)o + 1] - ref[3 * s + 1];
+        const double z = (double)pos[3 * (int64_t)o + 2] - ref[3 * s + 2];
+        xyzq[s] = mk4((real)x, (real)y, (real)z, pad ? (real)0 : charge[o]);
+        stype[s] = type[o];
+        Facc[s] = mk4((real)0, (real)0, (real)0, (real)0);
+    }
+    if (blockIdx.x == 0) {
+        // (sigma, eps) -> c6 = 4 eps sigma^6, c12 = 4 eps sigma^12  (Eq. 4)
+        for (int k = threadIdx.x; k < nt * nt; k += blockDim.x) {
+            double sg = lj_table[2 * k], ep = lj_table[2 * k + 1];
+            double s2 = sg * sg, s6 = s2 * s2 * s2;
+            lj_out[2 * k] = (real)(4.0 * ep * s6);
+            lj_out[2 * k + 1] = (real)(4.0 * ep * s6 * s6);
+        }
+        for (int t = threadIdx.x; t < nt; t += blockDim.x) {
+            int act = 0;
+            for (int u = 0; u < nt; ++u)
+                if (lj_table[2 * (t * nt + u) + 1] != 0.0 && lj_table[2 * (t * nt + u)] != 0.0) act = 1;
+            row_active[t] = act;
+        }
+        if (threadIdx.x < 16) accum[threadIdx.x] = 0.0;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A4: pair-force kernel
+// ------------------------------------------------------------------------------------------------
+constexpr int PF_WARPS = 8;
+constexpr int N_PART = 9;  // E_lj, E_coul, Wxx, Wxy, Wxz, Wyy, Wyz, Wzz, E_excl
+
+template <typename real>
+struct ForceParams {
+    using real4 = typename vec4<real>::type;
+    int64_t n_units;
+    int row_cap, m_res, nt;
+    const real4* xyzq;
+    const int* stype;
+    const int* jslot;
+    const unsigned short* meta;
+    const int2* row_info;
+    const real* lj;          // (c6, c12) per type pair
+    const int* row_active;   // per type: any non-zero LJ partner
+    real4* Facc;
+    real4* Fown;
+    double* partials;        // [gridDim.x][N_PART]
+    real rc2, ke, krf, crf, alpha, two_a_sqrtpi;
+    real L[3], invL[3], h[3];
+};
+
+// reduce-scatter of 8 values over the 32 lanes: on return lane l holds, in v[0], the warp-wide sum of
+// element ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1)   (9 shuffles instead of 40)
+template <typename T>
+__device__ __forceinline__ T reduce8_scatter(T (&v)[8], int lane)
+{
+    const unsigned FULL = 0xffffffffu;
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+    T a[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        T send = b4 ? v[k] : v[k + 4];
+        T keep = b4 ? v[k + 4] : v[k];
+        a[k] = keep + __shfl_xor_sync(FULL, send, 16);
+    }
+    T b[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        T send = b3 ? a[k] : a[k + 2];
+        T keep = b3 ? a[k + 2] : a[k];
+        b[k] = keep + __shfl_xor_sync(FULL, send, 8);
+    }
+    T send = b2 ? b[0] : b[1];
+    T keep = b2 ? b[1] : b[0];
+    T c = keep + __shfl_xor_sync(FULL, send, 4);
+    c += __shfl_xor_sync(FULL, c, 2);
+    c += __shfl_xor_sync(FULL, c, 1);
+    return c;
+}
+
+template <typename real, typename acc_t, int METHOD, int PBC>
+__global__ __launch_bounds__(PF_WARPS * 32, 2) void pair_force_kernel(ForceParams<real> P)
+{
+    using real4 = typename vec4<real>::type;
+    __shared__ real lj_s[MAX_TYPES * MAX_TYPES * 2 > 2048 ? 2048 : MAX_TYPES * MAX_TYPES * 2];
+    __shared__ real4 off_s[27];
+    __shared__ double part_s[PF_WARPS][N_PART];
+    extern __shared__ __align__(16) unsigned char dyn_smem[];
+    real* ljt = (P.nt * P.nt * 2 <= 2048) ? lj_s : reinterpret_cast<real*>(dyn_smem);
+
+    for (int k = threadIdx.x; k < P.nt * P.nt * 2; k += blockDim.x) ljt[k] = P.lj[k];
+    if (threadIdx.x < 27) {
+        const int c = threadIdx.x;
+        off_s[c] = mk4((real)(c / 9 - 1) * P.h[0], (real)((c / 3) % 3 - 1) * P.h[1], (real)(c % 3 - 1) * P.h[2], (real)0);
+    }
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const int wib = threadIdx.x >> 5;
+    const int64_t U = (int64_t)blockIdx.x * PF_WARPS + wib;
+
+    acc_t e_lj = 0, e_c = 0;
+    acc_t w[6] = {0, 0, 0, 0, 0, 0};
+
+    if (U < P.n_units) {
+        // ---- the unit's 8 i-atoms in registers (uniform across the warp) ----
+        real xi[UNIT], yi[UNIT], zi[UNIT], qi[UNIT];
+        int ti[UNIT];
+        real fix[UNIT], fiy[UNIT], fiz[UNIT];
+#pragma unroll
+        for (int i = 0; i < UNIT; ++i) {
+            const real4 v = P.xyzq[U * UNIT + i];
+            xi[i] = v.x; yi[i] = v.y; zi[i] = v.z;
+            qi[i] = v.w * P.ke;  // k_e folded into the i-side charge
+            const int t = P.stype[U * UNIT + i];
+            ti[i] = P.row_active[t] ? t * P.nt : -1;
+            fix[i] = fiy[i] = fiz[i] = 0;
+        }
+        const int2 ri = P.row_info[U];
+        const int mc = ri.x & 0xFFFF;
+        const bool unit_full = (ri.x & 0x10000) == 0;
+        const int nu = ri.y;
+        const int nch = (nu + 31) >> 5;
+        const int64_t row = U * (int64_t)P.row_cap + P.m_res;
+
+        for (int c = -mc; c < nch; ++c) {
+            const int64_t e = row + (int64_t)c * 32 + lane;
+            const int j = P.jslot[e];
+            const unsigned m = P.meta[e];
+            const real4 pj = P.xyzq[j];
+            const int tj = P.stype[j];
+            const real4 off = off_s[m >> 8];
+            const real xj = pj.x + off.x, yj = pj.y + off.y, zj = pj.z + off.z;
+            const real qj = pj.w;
+            const unsigned mask = m & 0xFFu;
+            real fjx = 0, fjy = 0, fjz = 0;
+            const bool plain = unit_full && c >= 0 && (c * 32 + 32 <= nu);  // warp-uniform: no mask needed
+
+            auto slot = [&](const int i, const bool use_mask) {
+                real dx = xi[i] - xj, dy = yi[i] - yj, dz = zi[i] - zj;
+                if (PBC == 1) {
+                    dx -= P.L[0] * rintr(dx * P.invL[0]);
+                    dy -= P.L[1] * rintr(dy * P.invL[1]);
+                    dz -= P.L[2] * rintr(dz * P.invL[2]);
+                }
+                const real r2 = dx * dx + dy * dy + dz * dz;
+                bool in = r2 < P.rc2;
+                if (use_mask) in = in && ((mask >> i) & 1u);
+                const real rinv = in ? rsqrt_r(r2) : (real)0;
+                const real qq = in ? qi[i] * qj : (real)0;
+                const real rinv2 = rinv * rinv;
+                real fr2;  // force * r^2 (scalar), so that f_ij = fr2 * rinv2 * d
+                real elj = 0;
+                if (ti[i] >= 0) {  // warp-uniform: this i-atom has LJ partners
+                    const real rinv6 = rinv2 * rinv2 * rinv2;
+                    const real c6 = ljt[2 * (ti[i] + tj)], c12 = ljt[2 * (ti[i] + tj) + 1];
+                    const real t1 = c12 * rinv6;
+                    const real u = t1 - c6;
+                    elj = u * rinv6;                      // 4 eps [(s/r)^12 - (s/r)^6]
+                    fr2 = (real)6 * ((u + t1) * rinv6);   // 24 eps [2 (s/r)^12 - (s/r)^6]
+                } else {
+                    fr2 = 0;
+                }
+                real ec;
+                if (METHOD == DIMOS_RF) {
+                    const real a = P.krf * r2;
+                    ec = qq * (rinv + a - P.crf);                 // Eq. 8
+                    fr2 += qq * (rinv - (real)2 * a);             // r^2 * k_e qq (1/r^3 - 2 k_rf)
+                } else {
+                    const real r = r2 * rinv;
+                    const real ar = P.alpha * r;
+                    const real erfc_ar = erfc_r(ar);
+                    const real ex = exp_r(-ar * ar);
+                    ec = qq * rinv * erfc_ar;                     // Eq. 10, n = 0
+                    fr2 += qq * (rinv * erfc_ar + P.two_a_sqrtpi * ex);
+                }
+                const real fs = fr2 * rinv2;
+                fix[i] += fs * dx; fiy[i] += fs * dy; fiz[i] += fs * dz;
+                fjx -= fs * dx; fjy -= fs * dy; fjz -= fs * dz;
+                e_lj += (acc_t)elj;
+                e_c += (acc_t)ec;
+                if (PBC == 1) {  // the image can differ per pair: direct per-pair virial
+                    const real fx = fs * dx, fy = fs * dy, fz = fs * dz;
+                    w[0] += (acc_t)(dx * fx); w[1] += (acc_t)(dx * fy); w[2] += (acc_t)(dx * fz);
+                    w[3] += (acc_t)(dy * fy); w[4] += (acc_t)(dy * fz); w[5] += (acc_t)(dz * fz);
+                }
+            };
+            if (plain) {
+#pragma unroll
+                for (int i = 0; i < UNIT; ++i) slot(i, false);
+            } else {
+#pragma unroll
+                for (int i = 0; i < UNIT; ++i) slot(i, true);
+            }
+            if (PBC == 0) {  // x_j' (x) F_j^entry, unit-local coordinates
+                w[0] += (acc_t)(xj * fjx); w[1] += (acc_t)(xj * fjy); w[2] += (acc_t)(xj * fjz);
+                w[3] += (acc_t)(yj * fjy); w[4] += (acc_t)(yj * fjz); w[5] += (acc_t)(zj * fjz);
+            }
+            if (mask) red_add_xyz(&P.Facc[j], fjx, fjy, fjz);
+        }
+
+        // ---- F_i: reduce over the warp once per unit; lanes 0,4,..,28 end up holding one i-atom each ----
+        const real rx = reduce8_scatter(fix, lane);
+        const real ry = reduce8_scatter(fiy, lane);
+        const real rz = reduce8_scatter(fiz, lane);
+        const int ii = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+        if ((lane & 3) == 0) {
+            P.Fown[U * UNIT + ii] = mk4(rx, ry, rz, (real)0);
+            if (PBC == 0) {  // x_i (x) F_i^unit
+                const real4 v = P.xyzq[U * UNIT + ii];
+                w[0] += (acc_t)(v.x * rx); w[1] += (acc_t)(v.x * ry); w[2] += (acc_t)(v.x * rz);
+                w[3] += (acc_t)(v.y * ry); w[4] += (acc_t)(v.y * rz); w[5] += (acc_t)(v.z * rz);
+            }
+        }
+    }
+
+    // ---- energy / virial: warp -> block -> one fp64 partial row per block ----
+    double red[8] = {(double)e_lj, (double)e_c, (double)w[0], (double)w[1], (double)w[2], (double)w[3], (double)w[4], (double)w[5]};
+    const double tot = reduce8_scatter(red, lane);
+    const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+    if ((lane & 3) == 0) part_s[wib][idx] = tot;
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        double sum = 0;
+#pragma unroll
+        for (int k = 0; k < PF_WARPS; ++k) sum += part_s[k][threadIdx.x];
+        P.partials[(int64_t)blockIdx.x * N_PART + threadIdx.x] = sum;
+    }
+    if (threadIdx.x == 8) P.partials[(int64_t)blockIdx.x * N_PART + 8] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A5: Ewald exclusion correction  -k_e q_i q_j erf(alpha r)/r over all excluded pairs (reading C-15)
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void excl_correction_kernel(const int2* __restrict__ pairs, int64_t n_excl, const int* __restrict__ inv_perm,
+                                       const typename vec4<real>::type* __restrict__ xyzq, const double* __restrict__ ref,
+                                       typename vec4<real>::type* __restrict__ Facc, double* __restrict__ partials,
+                                       real ke, real alpha, real two_a_sqrtpi, double Lx, double Ly, double Lz)
+{
+    using real4 = typename vec4<real>::type;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double e = 0, w[6] = {0, 0, 0, 0, 0, 0};
+    if (k < n_excl) {
+        const int2 p = pairs[k];
+        const int si = inv_perm[p.x], sj = inv_perm[p.y];
+        const real4 a = xyzq[si], b = xyzq[sj];
+        // raw-coordinate difference formed in fp64 from cell-relative parts, then nearest image (C-3)
+        double ddx = ((double)a.x - (double)b.x) + (ref[3 * (int64_t)si] - ref[3 * (int64_t)sj]);
+        double ddy = ((double)a.y - (double)b.y) + (ref[3 * (int64_t)si + 1] - ref[3 * (int64_t)sj + 1]);
+        double ddz = ((double)a.z - (double)b.z) + (ref[3 * (int64_t)si + 2] - ref[3 * (int64_t)sj + 2]);
+        ddx -= Lx * rint(ddx / Lx);
+        ddy -= Ly * rint(ddy / Ly);
+        ddz -= Lz * rint(ddz / Lz);
+        const real dx = (real)ddx, dy = (real)ddy, dz = (real)ddz;
+        const real r2 = dx * dx + dy * dy + dz * dz;
+        const real rinv = (real)1 / sqrt(r2);
+        const real r = r2 * rinv;
+        const real qq = ke * a.w * b.w;
+        const real erf_ar = erf_r(alpha * r);
+        const real ex = exp_r(-(alpha * r) * (alpha * r));
+        const real ee = -qq * erf_ar * rinv;
+        const real fs = qq * (two_a_sqrtpi * ex - erf_ar * rinv) * rinv * rinv;
+        const real fx = fs * dx, fy = fs * dy, fz = fs * dz;
+        red_add_xyz(&Facc[si], fx, fy, fz);
+        red_add_xyz(&Facc[sj], -fx, -fy, -fz);
+        e = (double)ee;
+        w[0] = (double)(dx * fx); w[1] = (double)(dx * fy); w[2] = (double)(dx * fz);
+        w[3] = (double)(dy * fy); w[4] = (double)(dy * fz); w[5] = (double)(dz * fz);
+    }
+    // block reduction of 7 values
+    __shared__ double sh[8][7];
+    double v[7] = {e, w[0], w[1], w[2], w[3], w[4], w[5]};
+#pragma unroll
+    for (int q = 0; q < 7; ++q)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    if (lane == 0)
+        for (int q = 0; q < 7; ++q) sh[wi][q] = v[q];
+    __syncthreads();
+    if (threadIdx.x < N_PART) {
+        double sum = 0;
+        int q = -1;
+        if (threadIdx.x == 8) q = 0;                       // E_excl
+        else if (threadIdx.x >= 2) q = threadIdx.x - 1;    // W components
+        if (q >= 0)
+            for (int ww = 0; ww < (int)(blockDim.x >> 5); ++ww) sum += sh[ww][q];
+        partials[(int64_t)blockIdx.x * N_PART + threadIdx.x] = sum;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A6: finalize
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void finalize_kernel(const int* __restrict__ perm, int64_t n_slots,
+                                const typename vec4<real>::type* __restrict__ Fown,
+                                const typename vec4<real>::type* __restrict__ Facc, real* __restrict__ F,
+                                const double* __restrict__ partials, int64_t n_part_rows, double* __restrict__ accum,
+                                double* __restrict__ E, double* __restrict__ W)
+{
+    using real4 = typename vec4<real>::type;
+    for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s < n_slots; s += (int64_t)gridDim.x * blockDim.x) {
+        const int o = perm[s];
+        if (o >= 0) {
+            const real4 a = Fown[s], b = Facc[s];
+            F[3 * (int64_t)o] = a.x + b.x;
+            F[3 * (int64_t)o + 1] = a.y + b.y;
+            F[3 * (int64_t)o + 2] = a.z + b.z;
+        }
+    }
+    // fp64 reduction of the block partials: thread t of every block sums a strided share of column t%9
+    __shared__ double sh[256];
+    __shared__ bool last;
+    {
+        const int col = threadIdx.x % N_PART;
+        const int lanes_per_col = blockDim.x / N_PART;  // 28 for 256 threads
+        const int sub = threadIdx.x / N_PART;
+        double sum = 0;
+        if (sub < lanes_per_col)
+            for (int64_t r = (int64_t)blockIdx.x * lanes_per_col + sub; r < n_part_rows; r += (int64_t)gridDim.x * lanes_per_col)
+                sum += partials[r * N_PART + col];
+        sh[threadIdx.x] = sub < lanes_per_col ? sum : 0.0;
+        __syncthreads();
+        if (threadIdx.x < N_PART) {
+            double t = 0;
+            for (int k = 0; k < lanes_per_col; ++k) t += sh[k * N_PART + threadIdx.x];
+            atomicAdd(&accum[threadIdx.x], t);
+        }
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long* ticket = reinterpret_cast<unsigned long long*>(accum + 15);
+            unsigned long long t = atomicAdd(ticket, 1ull);
+            last = (t == (unsigned long long)gridDim.x - 1);
+        }
+        __syncthreads();
+        if (last && threadIdx.x == 0) {
+            __threadfence();
+            volatile double* a = accum;
+            const double elj = a[0], ec = a[1], eex = a[8];
+            E[1] = elj; E[2] = ec; E[3] = eex; E[0] = elj + ec + eex;
+            if (W) {
+                W[0] = a[2]; W[1] = a[3]; W[2] = a[4];
+                W[3] = a[3]; W[4] = a[5]; W[5] = a[6];
+                W[6] = a[4]; W[7] = a[6]; W[8] = a[7];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// FP32 peak probe (roofline denominator for bench.py)
+// ------------------------------------------------------------------------------------------------
+__global__ void fma_probe_kernel(float* out, int iters, float a, float b)
+{
+    float r[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) r[k] = threadIdx.x * 0.001f + k;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) r[k] = fmaf(r[k], a, b);
+    }
+    float s = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += r[k];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s)
+{
+    const int blocks = ctx->sm_count * 8, thr = 256;
+    float* out = nullptr;
+    DIMOS_CUDA_TRY(ctx, cudaMalloc(&out, (size_t)blocks * thr * sizeof(float)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    int iters = 2000;
+    double best = 0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, s);
+        fma_probe_kernel<<<blocks, thr, 0, s>>>(out, iters, 1.0001f, 0.5f);
+        ctx->launches++;
+        cudaEventRecord(e1, s);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(out); return set_error(ctx, DIMOS_ECUDA, cudaGetErrorString(e)); }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        double tf = 2.0 * 16.0 * iters * (double)blocks * thr / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+        if (rep == 0 && ms > 0) {  // scale the loop to the requested duration
+            double want = ms_target > 0 ? ms_target : 2.0;
+            double f = want / ms;
+            iters = (int)(iters * (f < 0.1 ? 0.1 : (f > 50 ? 50 : f)));
+            if (iters < 100) iters = 100;
+        }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    *tflops = best;
+    return DIMOS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host orchestration of one force call
+// ------------------------------------------------------------------------------------------------
+template <typename real, typename acc_t>
+static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P, int method, unsigned nb, size_t dyn, cudaStream_t s)
+{
+    const int pbc = nl->grid.pbc_mode;
+#define DIMOS_PF(M, B)                                                                                            \
+    do {                                                                                                          \
+        if (dyn) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
+        pair_force_kernel<real, acc_t, M, B><<<nb, PF_WARPS * 32, dyn, s>>>(P);                                   \
+    } while (0)
+    if (method == DIMOS_RF) { if (pbc == 0) DIMOS_PF(DIMOS_RF, 0); else DIMOS_PF(DIMOS_RF, 1); }
+    else { if (pbc == 0) DIMOS_PF(DIMOS_EWALD_REAL, 0); else DIMOS_PF(DIMOS_EWALD_REAL, 1); }
+#undef DIMOS_PF
+    DIMOS_LAUNCH_CHECK(ctx, "pair_force");
+    return DIMOS_OK;
+}
+
+template <typename real>
+static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge, const int32_t* type,
+                           const double* lj_table, int32_t nt, const dimos_nb_params* prm, real* F, double* E,
+                           double* W, cudaStream_t s)
+{
+    using real4 = typename vec4<real>::type;
+    int rc;
+    const int64_t nsl = nl->n_slots, nun = nl->n_units;
+    const unsigned nb_force = (unsigned)((nun + PF_WARPS - 1) / PF_WARPS);
+    const bool ewald = prm->method == DIMOS_EWALD_REAL;
+    const unsigned nb_excl = ewald && nl->n_excl > 0 ? (unsigned)((nl->n_excl + 255) / 256) : 0;
+    if ((rc = ensure(ctx, nl->xyzq, nsl * sizeof(real4), s))) return rc;
+    if ((rc = ensure(ctx, nl->stype, nsl * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->Facc, nsl * sizeof(real4), s))) return rc;
+    if ((rc = ensure(ctx, nl->Fown, nsl * sizeof(real4), s))) return rc;
+    if ((rc = ensure(ctx, nl->lj, (size_t)MAX_TYPES * MAX_TYPES * 2 * sizeof(double) + MAX_TYPES * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->partials, ((size_t)nb_force + (size_t)((nl->n_excl + 255) / 256) + 1) * N_PART * sizeof(double), s))) return rc;
+    if ((rc = ensure(ctx, nl->accum, 16 * sizeof(double), s))) return rc;
+    real* lj_dev = (real*)nl->lj.p;
+    int* row_active = (int*)((char*)nl->lj.p + (size_t)MAX_TYPES * MAX_TYPES * 2 * sizeof(double));
+
+    const int T = 256;
+    gather_kernel<real><<<(unsigned)((nsl + T - 1) / T), T, 0, s>>>(pos, charge, type, (const int*)nl->perm.p, (const double*)nl->ref.p,
+                                                                    nsl, (real4*)nl->xyzq.p, (int*)nl->stype.p, (real4*)nl->Facc.p,
+                                                                    lj_table, nt, lj_dev, row_active, (double*)nl->accum.p);
+    DIMOS_LAUNCH_CHECK(ctx, "gather");
+
+    ForceParams<real> P;
+    P.n_units = nun; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;
+    P.xyzq = (const real4*)nl->xyzq.p; P.stype = (const int*)nl->stype.p;
+    P.jslot = (const int*)nl->jslot.p; P.meta = (const unsigned short*)nl->meta.p; P.row_info = (const int2*)nl->row_info.p;
+    P.lj = lj_dev; P.row_active = row_active;
+    P.Facc = (real4*)nl->Facc.p; P.Fown = (real4*)nl->Fown.p; P.partials = (double*)nl->partials.p;
+    const double rc_ = prm->r_cut;
+    P.rc2 = (real)rc_ * (real)rc_;
+    P.ke = (real)prm->coulomb_const;
+    P.krf = (real)((prm->eps_rf - 1.0) / ((2.0 * prm->eps_rf + 1.0) * rc_ * rc_ * rc_));  // Eq. 8 constants, reading C-1
+    P.crf = (real)(3.0 * prm->eps_rf / ((2.0 * prm->eps_rf + 1.0) * rc_));
+    P.alpha = (real)prm->alpha;
+    P.two_a_sqrtpi = (real)(2.0 * prm->alpha / sqrt(M_PI));
+    for (int a = 0; a < 3; ++a) { P.L[a] = (real)nl->grid.L[a]; P.invL[a] = (real)(1.0 / nl->grid.L[a]); P.h[a] = (real)nl->grid.h[a]; }
+    const size_t dyn = (nt * nt * 2 > 2048) ? (size_t)nt * nt * 2 * sizeof(real) : 0;
+    if (ctx->precision == DIMOS_MIXED) { if ((rc = launch_pair_force<real, double>(ctx, nl, P, prm->method, nb_force, dyn, s))) return rc; }
+    else { if ((rc = launch_pair_force<real, real>(ctx, nl, P, prm->method, nb_force, dyn, s))) return rc; }
+
+    if (nb_excl) {
+        excl_correction_kernel<real><<<nb_excl, 256, 0, s>>>((const int2*)nl->excl_pairs.p, nl->n_excl, (const int*)nl->inv_perm.p,
+                                                              (const real4*)nl->xyzq.p, (const double*)nl->ref.p, (real4*)nl->Facc.p,
+                                                              (double*)nl->partials.p + (size_t)nb_force * N_PART, P.ke, P.alpha,
+                                                              P.two_a_sqrtpi, nl->grid.L[0], nl->grid.L[1], nl->grid.L[2]);
+        DIMOS_LAUNCH_CHECK(ctx, "excl_correction");
+    }
+    int fb = (int)((nsl + T - 1) / T);
+    const int maxfb = ctx->sm_count * 8;
+    if (fb > maxfb) fb = maxfb;
+    if (fb < 1) fb = 1;
+    finalize_kernel<real><<<fb, T, 0, s>>>((const int*)nl->perm.p, nsl, (const real4*)nl->Fown.p, (const real4*)nl->Facc.p, F,
+                                           (const double*)nl->partials.p, (int64_t)nb_force + nb_excl, (double*)nl->accum.p, E, W);
+    DIMOS_LAUNCH_CHECK(ctx, "finalize");
+    return DIMOS_OK;
+}
+
+int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const int32_t* type, const double* lj_table,
+                   int32_t ntypes, const dimos_nb_params* prm, void* F, double* E, double* virial, cudaStream_t s)
+{
+    if (ctx->precision == DIMOS_F64)
+        return nonbonded_typed<double>(ctx, nl, (const double*)pos, (const double*)charge, type, lj_table, ntypes, prm,
+                                       (double*)F, E, virial, s);
+    return nonbonded_typed<float>(ctx, nl, (const float*)pos, (const float*)charge, type, lj_table, ntypes, prm, (float*)F, E,
+                                  virial, s);
+}
+
+}  // namespace dimos
