@@ -1,0 +1,430 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the DIMOS hot path (cell-list Verlet list + rebuild trigger + LJ/RF pair forces)
+on synthetic constant-density water boxes (BASELINE.json metric: pair interactions/s and tau per force step).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--precision f32]
+
+One "step" is one pass of the whole hot path on a synthetic ballistic trajectory:
+the rebuild trigger is evaluated every step, the list is rebuilt when it fires
+ and the nonbonded forces, energy and virial are evaluated every step.
+`value` = in-cutoff pair interactions per second, whole job (all ranks), inputs resident in HBM.
+`e2e` = the same protocol through dimos_step_host with pinned HOST buffers (H2D + D2H inside the timed region).
+`--impl reference` times the CPU fp64 oracle (oracle/, as it stands) on the host cores on a bounded sample.
+N > 1 (torchrun): independent replicas, one box per rank, no data-path collective ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2503_20541_b200 import workloads as wl  # noqa: E402
+
+METRIC = "pair_interactions_per_s"
+UNIT = "pair interactions/s"
+# algorithmic FLOP model of the pair kernel: per listed pair
+# (r < r_nl) the distance test, per in-cutoff pair additionally force + energy
+FLOPS_PER_LISTED_PAIR = 9
+FLOPS_PER_CUTOFF_PAIR = {"rf": 31, "ewald": 56}
+# FP32 ALU peak derived from the guide's unit counts and clocks: 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz
+FP32_LANES_PER_SM = 128
+DT_PS = 0.001  # 1 fs ballistic drift per step (configs[1] recipe: Maxwell-Boltzmann 300 K, dt = 1 fs)
+TEMPERATURE = 300.0
+TRIANGLE_HALF_PERIOD = 25  # velocities reverse every 25 steps so the box stays near its seeded structure
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs index (3 = 900,000 atoms, headline)")
+    ap.add_argument("--precision", default=None, help="f32 | mixed | f64 (default: first precision of the config)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def aggregate_over_ranks(local_seconds: float, local_units: float, world: int, dist=None, device=None):
+    """max-over-ranks time, sum-over-ranks units (weak scaling, independent replicas).  Works on gloo or nccl."""
+    if world == 1 or dist is None:
+        return local_seconds, local_units
+    import torch
+
+    t = torch.tensor([local_seconds], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def trajectory_offsets(step: int) -> float:
+    """Signed number of dt the positions are displaced from the seeded box at `step` (triangle wave)."""
+    p = TRIANGLE_HALF_PERIOD
+    k = step % (2 * p)
+    return float(k if k <= p else 2 * p - k)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md clocks line)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.fh = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=self.fh, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.fh.close()
+        sm, smax, reasons, power = [], [], set(), []
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.path)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "power_w_max": float(max(power)), "samples": len(sm)}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+def load_traffic(kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        try:
+            return json.load(open(path)).get(kernel)
+        except Exception:
+            return None
+    return None
+
+
+# ------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on the host cores, on a bounded sample
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample_box(method: str, big: bool):
+    """A constant-density box of the same recipe as the headline workload, small enough for the CPU."""
+    n_mol = 30000 if big else 3000
+    return wl.make_scaled(n_mol, seed=wl.SEED_BASE + 50, method=method)
+
+
+def time_oracle_step(box, method: str):
+    import oracle
+
+    lj = oracle.lorentz_berthelot(box.sigma, box.epsilon)
+    t0 = time.perf_counter()
+    res = oracle.nonbonded(box.pos, box.charge, box.type, lj, box.box, box.spec.r_cut,
+                           method=oracle.METHOD_RF if method == "rf" else oracle.METHOD_EWALD_REAL,
+                           alpha=box.spec.alpha, excl_pairs=box.excl_pairs, algorithm="celllist")
+    return time.perf_counter() - t0, res.n_pairs
+
+
+def cpu_baseline(method: str, budget_s: float = 20.0) -> dict:
+    import oracle
+
+    small = oracle_sample_box(method, big=False)
+    t_small, n_small = time_oracle_step(small, method)
+    cores = oracle.num_threads()
+    if t_small * 10.0 <= budget_s:  # a 10x larger box fits the budget: use it (less cache-friendly, more honest)
+        big = oracle_sample_box(method, big=True)
+        t, n = time_oracle_step(big, method)
+        sample = f"one oracle cell-list force evaluation (fp64, OpenMP) of a {big.n_atoms}-atom box of the same recipe"
+    else:
+        t, n, sample = t_small, n_small, f"one oracle cell-list force evaluation (fp64, OpenMP) of a {small.n_atoms}-atom box of the same recipe"
+    return {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": t}
+
+
+def run_reference(args, spec, precision):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    import oracle
+
+    method = spec.method
+    small = oracle_sample_box(method, big=False)
+    t_probe, _ = time_oracle_step(small, method)
+    total_steps = args.steps + args.warmup
+    big = t_probe * 10.0 * total_steps <= 150.0
+    box = oracle_sample_box(method, big=big)
+    for _ in range(args.warmup):
+        time_oracle_step(box, method)
+    t0 = time.perf_counter()
+    pairs = 0
+    for _ in range(args.steps):
+        _, n = time_oracle_step(box, method)
+        pairs += n
+    dt = time.perf_counter() - t0
+    value = pairs / dt
+    sample = (f"each step = one oracle cell-list force evaluation (fp64, OpenMP) of a {box.n_atoms}-atom box of the same recipe "
+              f"(density, r_cut={box.spec.r_cut}, method={method})")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(spec, precision), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(spec, precision):
+    return (f"configs[{spec.index}] {spec.name}: {3 * spec.n_molecules} atoms, density {wl.DENSITY} molecules/nm^3, "
+            f"r_cut={spec.r_cut} nm, skin={spec.skin} nm, LJ + {'reaction field' if spec.method == 'rf' else 'Ewald real space'}, {precision}")
+
+
+# ------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------
+def run_ours(args, spec, precision):
+    import torch
+
+    from paper_2503_20541_b200 import binding as dimos
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        dist = dist_mod
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    real = torch.float64 if precision == "f64" else torch.float32
+    np_real = np.float64 if precision == "f64" else np.float32
+
+    # one independent box per rank (weak scaling: replicas of the same recipe, different seeds)
+    box = wl.make_water_box(spec.n_molecules, wl.box_edge_for(spec), wl.SEED_BASE + spec.index + 1000 * rank, spec)
+    n = box.n_atoms
+    vel = wl.maxwell_boltzmann_velocities(box.mass, TEMPERATURE, wl.SEED_BASE + 7 + rank)
+    lj_host = dimos.lj_table_from_types(box.sigma, box.epsilon)
+    pos0 = torch.from_numpy(box.pos.astype(np_real)).to(dev)
+    dstep = torch.from_numpy((vel * DT_PS).astype(np_real)).to(dev)
+    charge = torch.from_numpy(box.charge.astype(np_real)).to(dev)
+    typ = torch.from_numpy(box.type).to(dev)
+    excl = torch.from_numpy(box.excl_pairs).to(dev)
+    lj = lj_host.to(dev)
+    pos = pos0.clone()
+    F = torch.empty_like(pos)
+    E = torch.empty(4, dtype=torch.float64, device=dev)
+    W = torch.empty(3, 3, dtype=torch.float64, device=dev)
+
+    ctx = dimos.Context(local_rank, precision)
+    kw = dict(method=spec.method, eps_rf=spec.eps_rf, alpha=spec.alpha)
+    nl = dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl)
+    n_cut = ctx.nl_count_within(nl, spec.r_cut)
+    n_listed = ctx.nl_count_within(nl, spec.r_cut + spec.skin)
+    stats = nl.stats()
+    state = {"step": 0, "rebuilds": 0}
+
+    def step():
+        # harness: ballistic drift (one fused axpy); library: trigger, (re)build, forces
+        torch.add(pos0, dstep, alpha=trajectory_offsets(state["step"]), out=pos)
+        if dimos.dimos_nl_needs_rebuild(ctx, pos, nl.pos_at_build, spec.skin):
+            dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl, nl=nl)
+            state["rebuilds"] += 1
+        dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw)
+        state["step"] += 1
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ctx.profile_enable(True)
+    launches0 = ctx.launch_count()
+    state["rebuilds"] = 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    seconds = e0.elapsed_time(e1) * 1e-3
+    launches = ctx.launch_count() - launches0
+    pair_ms, pair_n = ctx.profile_read()
+    ctx.profile_enable(False)
+    clocks = sampler.stop() if rank == 0 else None
+    rebuilds = state["rebuilds"]
+    assert bool(torch.isfinite(E).all()), "non-finite energy in the timed region"
+
+    # separate timings of the three calls (tau_force, tau_build, tau_check), list valid, median of 20
+    def timed(fn, reps=20):
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b) * 1e-3)
+        return float(np.median(ts))
+
+    pos.copy_(pos0)
+    dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl, nl=nl)
+    tau_force = timed(lambda: dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw))
+    tau_check = timed(lambda: dimos.dimos_nl_needs_rebuild(ctx, pos, nl.pos_at_build, spec.skin, sync=False))
+    tau_build = timed(lambda: dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl, nl=nl), reps=5)
+    fp32_probe = ctx.probe_fp32_peak(3.0) if rank == 0 else None
+
+    # e2e: the same protocol through dimos_step_host, pinned host buffers, H2D/D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        ring = 2 * TRIANGLE_HALF_PERIOD
+        host_pos = [(box.pos.astype(np.float64) + vel * DT_PS * trajectory_offsets(k)).astype(np_real) for k in range(ring)]
+        host_pos = [torch.from_numpy(p).pin_memory() for p in host_pos]
+        h_charge = torch.from_numpy(box.charge.astype(np_real)).pin_memory()
+        h_type = torch.from_numpy(box.type).pin_memory()
+        h_excl = torch.from_numpy(box.excl_pairs).pin_memory()
+        h_lj = lj_host.pin_memory()
+        h_F = torch.empty((n, 3), dtype=real).pin_memory()
+        h_E = torch.empty(4, dtype=torch.float64).pin_memory()
+        h_W = torch.empty((3, 3), dtype=torch.float64).pin_memory()
+        hnl = None
+        k = 0
+        for _ in range(max(args.warmup, 3)):
+            hnl, _ = ctx.step_host(hnl, host_pos[k % ring], h_charge, h_type, h_lj, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E,
+                                   h_W, **kw)
+            k += 1
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        t0 = time.perf_counter()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        e2e_rebuilds = 0
+        for _ in range(args.steps):
+            hnl, rb = ctx.step_host(hnl, host_pos[k % ring], h_charge, h_type, h_lj, box.box, spec.r_cut, spec.skin, h_excl, h_F,
+                                    h_E, h_W, **kw)
+            e2e_rebuilds += int(rb)
+            k += 1
+        b.record()
+        torch.cuda.synchronize()
+        e2e_seconds = max(a.elapsed_time(b) * 1e-3, 0.0)
+        wall = time.perf_counter() - t0
+        if dist:
+            dist.barrier()
+        rs = 8 if precision == "f64" else 4
+        e2e_t, e2e_units = aggregate_over_ranks(e2e_seconds, float(n_cut) * args.steps, world, dist, dev)
+        e2e = {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": n * (3 * rs + rs + 4) + int(h_lj.numel()) * 8,
+               "d2h_bytes_per_step": n * 3 * rs + 13 * 8 + 4, "ms_per_step": 1e3 * e2e_t / args.steps, "rebuilds": e2e_rebuilds,
+               "wall_ms_per_step": 1e3 * wall / args.steps, "api": "dimos_step_host (pinned host buffers)"}
+
+    total_t, total_units = aggregate_over_ranks(seconds, float(n_cut) * args.steps, world, dist, dev)
+    if rank != 0:
+        ctx.close()
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    peaks = load_peaks()
+    flops_per_launch = FLOPS_PER_LISTED_PAIR * n_listed + FLOPS_PER_CUTOFF_PAIR[spec.method] * n_cut
+    pair_s = pair_ms * 1e-3 / max(pair_n, 1)
+    achieved_tflops = flops_per_launch / pair_s * 1e-12 if pair_n else None
+    fp32_peak = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 * 1e-12  # TFLOP/s
+    if precision == "f64":
+        fp32_peak = 40.0  # NVIDIA's nominal B200 FP64 vector rate (no measured figure on this pool); context only
+    list_bytes = stats["list_bytes"] + stats["n_slots"] * (16 + 4 + 16 + 16)
+    roofline = {
+        "bound": "alu", "kernel": "pair_force_kernel", "achieved": achieved_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
+        "frac": (achieved_tflops / fp32_peak) if achieved_tflops else None, "traffic": load_traffic("pair_force_kernel"),
+        "peak_source": f"derived: 148 SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md); FFMA probe measured "
+                       f"{fp32_probe:.1f} TFLOP/s in this run",
+        "fp32_probe_tflops": fp32_probe,
+        "flops_per_launch": flops_per_launch, "flop_model": f"{FLOPS_PER_LISTED_PAIR}*N_nl + {FLOPS_PER_CUTOFF_PAIR[spec.method]}*N_c",
+        "kernel_ms": 1e3 * pair_s, "kernel_launches_timed": pair_n, "kernel_share_of_step": pair_ms * 1e-3 / seconds,
+        "hbm_bytes_per_launch": list_bytes, "hbm_gbs_achieved": list_bytes / pair_s * 1e-9 if pair_n else None,
+        "hbm_peak_gbs": peaks["hbm_gbs"], "hbm_peak_source": peaks["source"],
+        "pair_slots_executed": stats["n_pair_slots"], "fill_in_cutoff": n_cut / stats["n_pair_slots"],
+    }
+    line = {
+        "metric": METRIC, "value": total_units / total_t, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * total_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": precision, "data": "synthetic",
+        "config": {"workload": workload_name(spec, precision), "n_atoms": n, "pairs_in_cutoff": n_cut, "pairs_listed": n_listed,
+                   "protocol": f"ballistic Maxwell-Boltzmann {TEMPERATURE:.0f} K drift, dt=1 fs, trigger checked every step, "
+                               f"list rebuilt when it fires ({rebuilds} rebuilds in {args.steps} steps)",
+                   "l2": f"inputs larger than L2: the pair list streamed per force call is {stats['list_bytes'] / 1e6:.0f} MB",
+                   "parallelism": "replicas" if world > 1 else "single"},
+        "tau": {"force_s": tau_force, "check_s": tau_check, "build_s": tau_build, "rebuilds": rebuilds,
+                "pairs_per_s_force_only": n_cut / tau_force},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "list": {k: stats[k] for k in ("n_units", "n_entries", "n_entries_padded", "n_pair_slots", "list_bytes", "row_capacity")},
+    }
+    if not args.no_cpu_baseline and world >= 1:
+        line["cpu_baseline"] = cpu_baseline(spec.method)
+    ctx.close()
+    if dist:
+        dist.destroy_process_group()
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    spec = wl.CONFIGS[args.config]
+    precision = args.precision or ("f32" if "f32" in spec.precisions else spec.precisions[0])
+    if args.impl == "reference":
+        run_reference(args, spec, precision)
+    else:
+        run_ours(args, spec, precision)
+
+
+if __name__ == "__main__":
+    main()

@@ -179,6 +179,23 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* ctx, dimos_nl* nl, const void* pos
                                    const double* box, const dimos_nb_params* params, void* F_host,
                                    double* E_host, double* virial_host, void* stream);
 
+/* dimos_step_host -- one whole pass of the hot path for a caller whose arrays live in HOST memory
+ * (pinned recommended): uploads pos (and charge/type/lj_table), evaluates the rebuild trigger
+ * against the reference positions kept inside the list, rebuilds the list in place
+ * when it fired, runs dimos_nonbonded and copies F, E[4] and virial[9] back.
+ *   inout         *inout == NULL (or a list whose N / box / r_cut / skin / n_excl differ): the list is
+ *                 built from pos_host and returned; otherwise reused / rebuilt in place
+ *   excl_pairs_host  host, n_excl x 2 int32 (read only when the list is first built; the list keeps
+ *                 its device copy for later rebuilds)
+ *   rebuilt_host  host, may be NULL: receives 1 if this call (re)built the list, else 0
+ * Other arguments as in dimos_nonbonded_host.  Synchronises the stream (twice: once to read the
+ * trigger, once at the end). */
+DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_host, const void* charge_host,
+                              const int32_t* type_host, const double* lj_table_host, int32_t ntypes, int64_t N,
+                              const double* box, double skin, const int32_t* excl_pairs_host, int64_t n_excl,
+                              const dimos_nb_params* params, void* F_host, double* E_host, double* virial_host,
+                              int32_t* rebuilt_host, void* stream);
+
 /* dimos_nl_export_pairs -- the neighbour set the list represents, for parity checks and for
  * consumers that want a plain edge list.
  * Writes every unordered pair (i < j, original atom indices) that is not excluded and has
@@ -190,11 +207,24 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* ctx, dimos_nl* nl, const void* pos
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
                                     int64_t* n_pairs_host, void* stream);
 
+/* Number of unordered, non-excluded pairs of the list with minimum-image r < radius at the build
+ * positions, 0 < radius <= r_cut + skin (radius = r_cut gives the in-cutoff pair count the
+ * throughput metric "pair interactions/s" is quoted on).  Synchronises the stream. */
+DIMOS_API int dimos_nl_count_within(dimos_ctx* ctx, const dimos_nl* nl, double radius, int64_t* n_pairs_host,
+                                    void* stream);
+
 /* Sizes of the list (host call, no device work). */
 DIMOS_API int dimos_nl_stats(const dimos_nl* nl, dimos_nl_stats_t* out);
 
 /* Number of kernels of this library launched through ctx since dimos_create (host counter). */
 DIMOS_API int64_t dimos_launch_count(const dimos_ctx* ctx);
+
+/* Per-kernel timing of the pair-force kernel (row A4) for bench.py's roofline: while enabled,
+ * dimos_nonbonded records a CUDA event pair around that one kernel on the call's stream (at most
+ * 4096 launches between reads).  dimos_profile_read synchronises on the recorded events, returns
+ * the summed kernel time in milliseconds and the number of launches it covers, and resets. */
+DIMOS_API int dimos_profile_enable(dimos_ctx* ctx, int on);
+DIMOS_API int dimos_profile_read(dimos_ctx* ctx, double* pair_force_ms_host, int64_t* n_launches_host);
 
 /* Peak-rate probe used by bench.py's roofline: runs an FFMA-only microkernel on the context's
  * device for about `ms_target` milliseconds and returns the measured FP32 rate in *tflops_host

@@ -28,6 +28,7 @@ EXPORTED_SYMBOLS = (
     "dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
     "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats", "dimos_launch_count",
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
+    "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host",
 )
 
 
@@ -85,6 +86,12 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_nonbonded.argtypes = [vp, vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), ctypes.POINTER(_Params), vp, vp, vp, vp]
     lib.dimos_nonbonded_host.argtypes = [vp, vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), ctypes.POINTER(_Params), vp, vp, vp, vp]
     lib.dimos_nl_export_pairs.argtypes = [vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+    lib.dimos_step_host.argtypes = [vp, ctypes.POINTER(vp), vp, vp, vp, vp, i32, i64, ctypes.POINTER(dbl), dbl, vp, i64,
+                                    ctypes.POINTER(_Params), vp, vp, vp, ctypes.POINTER(i32), vp]
+    lib.dimos_step_host.restype = ctypes.c_int
+    lib.dimos_nl_count_within.argtypes = [vp, vp, dbl, ctypes.POINTER(i64), vp]
+    lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
+    lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
     lib.dimos_launch_count.argtypes = [vp]
     lib.dimos_launch_count.restype = i64
@@ -96,7 +103,7 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_version.restype = ctypes.c_char_p
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
-                 "dimos_probe_fp32_peak"):
+                 "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -267,6 +274,29 @@ class Context:
         self._check(rc)
         return F, E, virial
 
+    def step_host(self, nl: "NeighborList | None", pos, charge, type_, lj_table, box, r_cut, skin, excl_pairs, F, E, virial, *,
+                  method="rf", eps_rf=78.5, alpha=3.12, coulomb_const=138.935456):
+        """dimos_step_host: HOST tensors in and out; returns (NeighborList, rebuilt: bool)."""
+        for t in (pos, charge, type_, lj_table, F, E, virial) + ((excl_pairs,) if excl_pairs is not None else ()):
+            if t.is_cuda or not t.is_contiguous():
+                raise ValueError("step_host takes contiguous host tensors")
+        prm = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method])
+        h = ctypes.c_void_p(nl.handle.value if nl is not None else None)
+        rebuilt = ctypes.c_int32(0)
+        n_excl = 0 if excl_pairs is None else excl_pairs.shape[0]
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_step_host(self.handle, ctypes.byref(h), pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
+                                          lj_table.data_ptr(), lj_table.shape[0], pos.shape[0], _box3(box), float(skin),
+                                          excl_pairs.data_ptr() if n_excl else None, n_excl, ctypes.byref(prm), F.data_ptr(),
+                                          E.data_ptr(), virial.data_ptr(), ctypes.byref(rebuilt), _stream_ptr())
+        self._check(rc)
+        boxt = tuple(float(b) for b in (box.tolist() if hasattr(box, "tolist") else box))
+        if nl is None:
+            nl = NeighborList(h, self, torch.empty(0), boxt, float(r_cut), float(skin))
+        else:
+            nl.handle = h
+        return nl, bool(rebuilt.value)
+
     def nl_export_pairs(self, nl: NeighborList) -> torch.Tensor:
         """dimos_nl_export_pairs: (n,2) int32 device tensor of pairs i<j, order unspecified."""
         n = ctypes.c_int64(0)
@@ -279,6 +309,23 @@ class Context:
             rc = self.lib.dimos_nl_export_pairs(self.handle, nl.handle, out.data_ptr(), out.shape[0], ctypes.byref(got), _stream_ptr())
         self._check(rc)
         return out[: got.value]
+
+    def nl_count_within(self, nl: NeighborList, radius: float) -> int:
+        """dimos_nl_count_within: pairs of the list with r < radius at the build positions."""
+        n = ctypes.c_int64(0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_count_within(self.handle, nl.handle, float(radius), ctypes.byref(n), _stream_ptr())
+        self._check(rc)
+        return int(n.value)
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.dimos_profile_enable(self.handle, 1 if on else 0))
+
+    def profile_read(self):
+        """(summed pair-force kernel milliseconds, launches covered) since the last read."""
+        ms, n = ctypes.c_double(0.0), ctypes.c_int64(0)
+        self._check(self.lib.dimos_profile_read(self.handle, ctypes.byref(ms), ctypes.byref(n)))
+        return float(ms.value), int(n.value)
 
     def nl_stats(self, nl: NeighborList) -> dict:
         st = _Stats()

@@ -55,7 +55,8 @@ static void free_list(Ctx* ctx, NL* nl)
                       &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
                       &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->jslot, &nl->meta, &nl->row_info,
                       &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials, &nl->accum,
-                      &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW, &nl->export_count};
+                      &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW, &nl->st_ref, &nl->st_flag,
+                      &nl->export_count};
     for (DevBuf* b : bufs) release(ctx, *b);
     delete nl;
 }
@@ -67,7 +68,7 @@ static size_t list_workspace_bytes(const NL* nl)
                             &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->jslot, &nl->meta,
                             &nl->row_info, &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials,
                             &nl->accum, &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW,
-                            &nl->export_count};
+                            &nl->st_ref, &nl->st_flag, &nl->export_count};
     size_t t = 0;
     for (const DevBuf* b : bufs) t += b->bytes;
     return t;
@@ -121,6 +122,7 @@ DIMOS_API int dimos_destroy(dimos_ctx* c)
     ctx->lists.clear();
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     if (ctx->d_rebuild_state) cudaFree(ctx->d_rebuild_state);
+    for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
     delete ctx;
     return DIMOS_OK;
 }
@@ -279,6 +281,93 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* c, dimos_nl* l, const void* pos_ho
     return DIMOS_OK;
 }
 
+DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_host, const void* charge_host,
+                              const int32_t* type_host, const double* lj_table_host, int32_t ntypes, int64_t N,
+                              const double* box, double skin, const int32_t* excl_pairs_host, int64_t n_excl,
+                              const dimos_nb_params* params, void* F_host, double* E_host, double* virial_host,
+                              int32_t* rebuilt_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!inout || !pos_host || !charge_host || !type_host || !lj_table_host || !box || !params || !F_host || !E_host)
+        return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || n_excl < 0 || (n_excl > 0 && !excl_pairs_host)) return set_error(ctx, DIMOS_EINVAL, "bad N or exclusion list");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t rs = ctx->precision == DIMOS_F64 ? sizeof(double) : sizeof(float);
+    NL* nl = reinterpret_cast<NL*>(*inout);
+    int rc;
+    int rebuilt = 0;
+    bool fresh = nl == nullptr || !list_belongs(ctx, nl) || nl->N != N || nl->r_cut != params->r_cut || nl->skin != skin ||
+                 nl->box[0] != box[0] || nl->box[1] != box[1] || nl->box[2] != box[2] || nl->n_excl != n_excl ||
+                 nl->st_ref.p == nullptr;
+    if (nl && !list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");
+    if (!fresh) {
+        // upload the positions and test the rebuild trigger against the list's own reference positions
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_pos.p, pos_host, 3 * (size_t)N * rs, cudaMemcpyHostToDevice, s));
+        int32_t flag = 0;
+        rc = needs_rebuild_impl(ctx, nl->st_pos.p, nl->st_ref.p, N, skin, (int32_t*)nl->st_flag.p, s);
+        if (rc) return rc;
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 33, nl->st_flag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
+        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+        flag = ctx->h_pinned[33];
+        fresh = flag != 0;
+    } else {
+        // first call (or changed geometry): a throw-away device copy of pos/excl, then a normal build
+        DevBuf tmp_pos, tmp_ref, tmp_excl;
+        if ((rc = ensure(ctx, tmp_pos, 3 * (size_t)N * rs, s))) return rc;
+        if ((rc = ensure(ctx, tmp_ref, 3 * (size_t)N * rs, s))) { release(ctx, tmp_pos); return rc; }
+        if ((rc = ensure(ctx, tmp_excl, (size_t)std::max<int64_t>(n_excl, 1) * 2 * sizeof(int32_t), s))) { release(ctx, tmp_pos); release(ctx, tmp_ref); return rc; }
+        cudaMemcpyAsync(tmp_pos.p, pos_host, 3 * (size_t)N * rs, cudaMemcpyHostToDevice, s);
+        if (n_excl > 0) cudaMemcpyAsync(tmp_excl.p, excl_pairs_host, (size_t)n_excl * 2 * sizeof(int32_t), cudaMemcpyHostToDevice, s);
+        dimos_nl* h = reinterpret_cast<dimos_nl*>(nl);
+        rc = dimos_nl_build(c, tmp_pos.p, N, box, params->r_cut, skin, n_excl > 0 ? (const int32_t*)tmp_excl.p : nullptr, n_excl,
+                            tmp_ref.p, stream, &h);
+        if (rc == DIMOS_OK) {
+            nl = reinterpret_cast<NL*>(h);
+            *inout = h;
+            rc = ensure(ctx, nl->st_pos, 3 * (size_t)N * rs, s);
+            if (!rc) rc = ensure(ctx, nl->st_ref, 3 * (size_t)N * rs, s);
+            if (!rc) rc = ensure(ctx, nl->st_flag, sizeof(int), s);
+            if (!rc) {
+                cudaMemcpyAsync(nl->st_pos.p, tmp_pos.p, 3 * (size_t)N * rs, cudaMemcpyDeviceToDevice, s);
+                cudaMemcpyAsync(nl->st_ref.p, tmp_ref.p, 3 * (size_t)N * rs, cudaMemcpyDeviceToDevice, s);
+            }
+        }
+        cudaStreamSynchronize(s);
+        release(ctx, tmp_pos); release(ctx, tmp_ref); release(ctx, tmp_excl);
+        if (rc) return rc;
+        rebuilt = 1;
+        fresh = false;
+    }
+    if (fresh) {  // trigger fired: rebuild in place from the staged positions, exclusions retained by the list
+        dimos_nl* h = reinterpret_cast<dimos_nl*>(nl);
+        rc = dimos_nl_build(c, nl->st_pos.p, N, box, params->r_cut, skin, n_excl > 0 ? (const int32_t*)nl->excl_pairs.p : nullptr,
+                            n_excl, nl->st_ref.p, stream, &h);
+        if (rc) return rc;
+        rebuilt = 1;
+    }
+    if (rebuilt_host) *rebuilt_host = rebuilt;
+    if ((rc = check_nb_args(ctx, nl, ntypes, box, params))) return rc;
+    if ((rc = ensure(ctx, nl->st_charge, (size_t)N * rs, s))) return rc;
+    if ((rc = ensure(ctx, nl->st_type, (size_t)N * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->st_lj, (size_t)ntypes * ntypes * 2 * sizeof(double), s))) return rc;
+    if ((rc = ensure(ctx, nl->st_F, 3 * (size_t)N * rs, s))) return rc;
+    if ((rc = ensure(ctx, nl->st_EW, 16 * sizeof(double), s))) return rc;
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
+    double* EW = (double*)nl->st_EW.p;
+    rc = nonbonded_impl(ctx, nl, nl->st_pos.p, nl->st_charge.p, (const int32_t*)nl->st_type.p, (const double*)nl->st_lj.p, ntypes,
+                        params, nl->st_F.p, EW, EW + 4, s);
+    if (rc) return rc;
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(F_host, nl->st_F.p, 3 * (size_t)N * rs, cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(E_host, EW, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (virial_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(virial_host, EW + 4, 9 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    return DIMOS_OK;
+}
+
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* c, const dimos_nl* l, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, void* stream)
 {
     if (!c) return DIMOS_EINVAL;
@@ -287,7 +376,48 @@ DIMOS_API int dimos_nl_export_pairs(dimos_ctx* c, const dimos_nl* l, int32_t* pa
     const NL* nl = reinterpret_cast<const NL*>(l);
     if (!list_belongs(ctx, nl) || nl->N <= 0) return set_error(ctx, DIMOS_EINVAL, "list not built with this context");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
-    return nl_export_impl(ctx, nl, pairs, cap, n_pairs_host, (cudaStream_t)stream);
+    return nl_export_impl(ctx, nl, pairs, cap, n_pairs_host, nl->r_nl, (cudaStream_t)stream);
+}
+
+DIMOS_API int dimos_nl_count_within(dimos_ctx* c, const dimos_nl* l, double radius, int64_t* n_pairs_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!l || !n_pairs_host) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    const NL* nl = reinterpret_cast<const NL*>(l);
+    if (!list_belongs(ctx, nl) || nl->N <= 0) return set_error(ctx, DIMOS_EINVAL, "list not built with this context");
+    if (!(radius > 0) || radius > nl->r_nl) return set_error(ctx, DIMOS_EINVAL, "radius must be in (0, r_cut + skin]");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return nl_export_impl(ctx, nl, nullptr, 0, n_pairs_host, radius, (cudaStream_t)stream);
+}
+
+DIMOS_API int dimos_profile_enable(dimos_ctx* c, int on)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    ctx->profiling = on != 0;
+    ctx->prof_used = 0;
+    return DIMOS_OK;
+}
+
+DIMOS_API int dimos_profile_read(dimos_ctx* c, double* pair_force_ms_host, int64_t* n_launches_host)
+{
+    if (!c || !pair_force_ms_host || !n_launches_host) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    double total = 0;
+    int64_t n = 0;
+    for (size_t k = 0; k + 1 < ctx->prof_used; k += 2) {
+        cudaError_t e = cudaEventSynchronize(ctx->prof_events[k + 1]);
+        float ms = 0;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ctx->prof_events[k], ctx->prof_events[k + 1]);
+        if (e != cudaSuccess) { ctx->prof_used = 0; return set_error(ctx, DIMOS_ECUDA, cudaGetErrorString(e)); }
+        total += ms;
+        ++n;
+    }
+    ctx->prof_used = 0;
+    *pair_force_ms_host = total;
+    *n_launches_host = n;
+    return DIMOS_OK;
 }
 
 DIMOS_API int dimos_nl_stats(const dimos_nl* l, dimos_nl_stats_t* out)

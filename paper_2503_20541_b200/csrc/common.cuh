@@ -48,7 +48,12 @@ struct Ctx {
     int* h_pinned = nullptr;        // 64 ints pinned scratch for read-backs
     unsigned long long* d_rebuild_state = nullptr;  // {max bits, ticket}
     std::vector<struct NL*> lists;
+    // optional per-kernel timing of the pair-force kernel (dimos_profile_enable / dimos_profile_read)
+    bool profiling = false;
+    std::vector<cudaEvent_t> prof_events;  // pairs (start, stop), recycled after each read
+    size_t prof_used = 0;                  // events handed out since the last read
 };
+constexpr size_t PROF_MAX_EVENTS = 8192;
 
 // geometry of the cell grid / list, passed by value to kernels
 struct Grid {
@@ -97,7 +102,7 @@ struct NL {
     DevBuf partials;   // double[9 * n_partial_blocks]
     DevBuf accum;      // double[16] + unsigned ticket
     // host-call staging (dimos_nonbonded_host)
-    DevBuf st_pos, st_charge, st_type, st_lj, st_F, st_EW;
+    DevBuf st_pos, st_charge, st_type, st_lj, st_F, st_EW, st_ref, st_flag;
     DevBuf export_count;  // unsigned long long[1]
 };
 
@@ -126,7 +131,7 @@ void release(Ctx* ctx, DevBuf& b);
 // ---- entry points implemented per translation unit ---------------------------------------------
 int nl_build_impl(Ctx* ctx, NL* nl, const void* pos, const int32_t* excl_pairs, int64_t n_excl,
                   void* pos_at_build, cudaStream_t s);
-int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, cudaStream_t s);
+int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s);
 int needs_rebuild_impl(Ctx* ctx, const void* pos, const void* ref, int64_t N, double skin, int32_t* flag_dev,
                        cudaStream_t s);
 int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const int32_t* type,

@@ -894,7 +894,8 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
     zero_int_kernel<<<(unsigned)((N + 1 + T - 1) / T), T, 0, s>>>(excl_deg, N + 1);
     DIMOS_LAUNCH_CHECK(ctx, "zero_deg");
     if (n_excl > 0) {
-        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->excl_pairs.p, excl_pairs, n_excl * sizeof(int2), cudaMemcpyDeviceToDevice, s));
+        if ((const void*)excl_pairs != (const void*)nl->excl_pairs.p)  // dimos_step_host rebuilds from the retained copy
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->excl_pairs.p, excl_pairs, n_excl * sizeof(int2), cudaMemcpyDeviceToDevice, s));
         excl_degree_kernel<<<(unsigned)((n_excl + T - 1) / T), T, 0, s>>>((const int2*)nl->excl_pairs.p, n_excl, N, excl_deg, flags);
         DIMOS_LAUNCH_CHECK(ctx, "excl_degree");
     }
@@ -1000,9 +1001,10 @@ int nl_build_impl(Ctx* ctx, NL* nl, const void* pos, const int32_t* excl_pairs, 
 }
 
 template <typename real>
-static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, cudaStream_t s)
+static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s)
 {
     BuildParams<real> P = make_build_params<real>(nl);
+    P.rnl2 = (real)radius * (real)radius;
     unsigned long long* counter = (unsigned long long*)nl->export_count.p;
     zero_int_kernel<<<1, 32, 0, s>>>((int*)counter, 2);
     DIMOS_LAUNCH_CHECK(ctx, "zero_counter");
@@ -1020,10 +1022,10 @@ static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, 
     return DIMOS_OK;
 }
 
-int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, cudaStream_t s)
+int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s)
 {
-    if (ctx->precision == DIMOS_F64) return nl_export_typed<double>(ctx, nl, pairs, cap, n_pairs_host, s);
-    return nl_export_typed<float>(ctx, nl, pairs, cap, n_pairs_host, s);
+    if (ctx->precision == DIMOS_F64) return nl_export_typed<double>(ctx, nl, pairs, cap, n_pairs_host, radius, s);
+    return nl_export_typed<float>(ctx, nl, pairs, cap, n_pairs_host, radius, s);
 }
 
 }  // namespace dimos

@@ -548,6 +548,17 @@ template <typename real, typename acc_t>
 static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P, int method, unsigned nb, size_t dyn, cudaStream_t s)
 {
     const int pbc = nl->grid.pbc_mode;
+    cudaEvent_t ev_stop = nullptr;
+    if (ctx->profiling && ctx->prof_used + 2 <= PROF_MAX_EVENTS) {  // per-kernel timing for bench.py's roofline
+        while (ctx->prof_events.size() < ctx->prof_used + 2) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaEventCreate failed");
+            ctx->prof_events.push_back(e);
+        }
+        cudaEventRecord(ctx->prof_events[ctx->prof_used], s);
+        ev_stop = ctx->prof_events[ctx->prof_used + 1];
+        ctx->prof_used += 2;
+    }
 #define DIMOS_PF(M, B)                                                                                            \
     do {                                                                                                          \
         if (dyn) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
@@ -556,6 +567,7 @@ static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P,
     if (method == DIMOS_RF) { if (pbc == 0) DIMOS_PF(DIMOS_RF, 0); else DIMOS_PF(DIMOS_RF, 1); }
     else { if (pbc == 0) DIMOS_PF(DIMOS_EWALD_REAL, 0); else DIMOS_PF(DIMOS_EWALD_REAL, 1); }
 #undef DIMOS_PF
+    if (ev_stop) cudaEventRecord(ev_stop, s);
     DIMOS_LAUNCH_CHECK(ctx, "pair_force");
     return DIMOS_OK;
 }

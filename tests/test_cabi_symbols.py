@@ -1,0 +1,67 @@
+"""CPU-side checks of the boundary: the C-ABI library builds, loads and exports every symbol that
+include/dimos.h declares; the binding refuses to run without a CUDA device (no CPU fallback);
+the product package never touches oracle/."""
+import ctypes
+import os
+import re
+
+import pytest
+import torch
+
+from paper_2503_20541_b200 import binding, build_ext
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "dimos.h")).read()
+    return sorted(set(re.findall(r"DIMOS_API\s+[\w\s\*]+?\b(dimos_\w+)\s*\(", text)))
+
+
+def test_header_declares_the_three_north_star_calls():
+    names = declared_symbols()
+    for must in ("dimos_nl_build", "dimos_nl_needs_rebuild", "dimos_nonbonded"):
+        assert must in names
+    assert set(names) == set(binding.EXPORTED_SYMBOLS)
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    path = build_ext.build()
+    assert os.path.exists(path)
+    lib = ctypes.CDLL(path)
+    for name in declared_symbols():
+        assert hasattr(lib, name), f"{name} declared in include/dimos.h but not exported"
+    lib.dimos_version.restype = ctypes.c_char_p
+    assert b"sm_100a" in lib.dimos_version()
+    lib.dimos_status_string.restype = ctypes.c_char_p
+    lib.dimos_status_string.argtypes = [ctypes.c_int]
+    assert lib.dimos_status_string(0) == b"DIMOS_OK"
+    assert b"DIMOS_EBOX" in lib.dimos_status_string(-2)
+
+
+def test_built_for_sm_100a_only():
+    out = os.popen(f"cuobjdump -lelf {build_ext.build()} 2>/dev/null").read()
+    if not out:
+        pytest.skip("cuobjdump not available")
+    archs = set(re.findall(r"sm_\d+a?", out))
+    assert archs == {"sm_100a"}, archs
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_no_cpu_fallback_without_a_device():
+    lib = binding.load_library()
+    h = ctypes.c_void_p()
+    assert lib.dimos_create(ctypes.byref(h), 0, 0, None) == -5  # DIMOS_ECUDA
+    assert not h.value
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.Context(0, "f32")
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2503_20541_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), f
+                assert "liboracle" not in text and "dimos_oracle" not in text, f

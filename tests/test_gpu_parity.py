@@ -1,0 +1,349 @@
+"""`-m gpu` parity tests: the CUDA path, called through the C ABI, against the CPU fp64 oracle on the same
+seeded inputs, element by element (tolerances in tests/gpu_harness.py and DESIGN.md)."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2503_20541_b200 import binding as dimos
+from paper_2503_20541_b200 import workloads as wl
+
+from gpu_harness import BAND, DeviceBox, check_neighbor_set, check_nonbonded, lj_table_np, run_case
+
+pytestmark = pytest.mark.gpu
+
+
+# --- A3: rebuild trigger (reading C-5) -----------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("n", [1, 5, 1000, 70001])
+def test_needs_rebuild_matches_oracle(precision, n):
+    rng = np.random.default_rng(n)
+    real = np.float64 if precision == "f64" else np.float32
+    ref = rng.uniform(0, 5, size=(n, 3)).astype(real)
+    ctx = dimos.Context(0, precision)
+    skin = 0.1
+    try:
+        for scale in (0.0, 0.02, 0.0288, 0.0290, 0.05, 1.0):
+            step = rng.standard_normal((n, 3))
+            step *= scale / np.maximum(np.linalg.norm(step, axis=1, keepdims=True), 1e-30)
+            step[rng.integers(0, n)] *= 1.7  # one atom moves furthest
+            pos = (ref.astype(np.float64) + step).astype(real)
+            want, m = oracle.needs_rebuild(pos, ref, skin)
+            got = dimos.dimos_nl_needs_rebuild(ctx, torch.from_numpy(pos).cuda(), torch.from_numpy(ref).cuda(), skin)
+            if abs(m - 0.5 * skin) > 1e-6:  # reading C-5: within 1e-6 nm of skin/2 either answer is legal
+                assert got == want, (scale, m)
+            flag = dimos.dimos_nl_needs_rebuild(ctx, torch.from_numpy(pos).cuda(), torch.from_numpy(ref).cuda(), skin, sync=False)
+            assert bool(flag.item()) == got  # the no-sync variant writes the same device flag
+    finally:
+        ctx.close()
+
+
+def test_needs_rebuild_strict_and_raw_coordinates():
+    ctx = dimos.Context(0, "f64")
+    try:
+        ref = torch.zeros(4, 3, dtype=torch.float64, device="cuda")
+        pos = ref.clone()
+        pos[2] = torch.tensor([0.03, 0.04, 0.0], dtype=torch.float64)  # |dr| == skin/2 exactly: strict > => False
+        assert dimos.dimos_nl_needs_rebuild(ctx, pos, ref, 0.1) == oracle.needs_rebuild(pos.cpu().numpy(), ref.cpu().numpy(), 0.1)[0]
+        pos[2, 2] = 0.001
+        assert dimos.dimos_nl_needs_rebuild(ctx, pos, ref, 0.1) is True
+        pos[2] = torch.tensor([2.0, 0.0, 0.0], dtype=torch.float64)  # a whole-box jump counts (no re-wrap)
+        assert dimos.dimos_nl_needs_rebuild(ctx, pos, ref, 0.1) is True
+    finally:
+        ctx.close()
+
+
+# --- A1 + A2 + A4 + A6 on the BASELINE configs the oracle finishes in seconds ----------------------------
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_config0_water216(precision):
+    """configs[0]: 648 atoms, L = 1.8621 < 2 r_nl: degenerate 1x1x1 grid, r_nl > L/2 (readings C-3, C-18)."""
+    wb = wl.make_config(0)
+    rep = run_case(wb, precision, 0.9, 0.1, "rf", oracle_alg="bruteforce")
+    assert rep["stats"]["n_cells"] == (1, 1, 1) and rep["stats"]["pbc_mode"] == 1
+    assert rep["n_pairs_cut"] == 95574
+
+
+@pytest.mark.parametrize("precision", ["f32", "mixed", "f64"])
+def test_config1_water3k(precision):
+    """configs[1] geometry: 9,000 atoms, 4^3 grid; several units per cell, ragged last unit in every cell."""
+    wb = wl.make_config(1)
+    rep = run_case(wb, precision, 1.0, 0.1, "rf")
+    assert rep["stats"]["n_cells"] == (4, 4, 4) and rep["stats"]["pbc_mode"] == 0
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_ewald_real_space_and_exclusion_correction(precision):
+    """configs[4] method on a box the oracle finishes quickly (2,000 waters): Eq. 10 + reading C-15."""
+    wb = wl.make_scaled(2000, seed=wl.SEED_BASE + 4, method="ewald")
+    rep = run_case(wb, precision, 1.0, 0.1, "ewald", alpha=3.12)
+    assert rep["stats"]["pbc_mode"] == 0
+
+
+def test_ewald_degenerate_grid_f32():
+    wb = wl.make_water_box(100, 2.2, 4)
+    run_case(wb, "f32", 1.0, 0.1, "ewald", oracle_alg="bruteforce")
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_slab_box_two_cells_per_axis(precision):
+    """2 cells along x and y, 3 along z: stencil de-duplication, non-cubic box (reading C-18)."""
+    wb = wl.make_water_box(150, 2.5, 21)
+    run_case(wb, precision, 1.0, 0.1, "rf", box=np.array([2.5, 2.3, 3.4]), oracle_alg="bruteforce")
+
+
+def test_unwrapped_and_shifted_positions_f32():
+    """Positions need not lie in [0,L): shift by an arbitrary vector (> L) and move single atoms by +-L."""
+    wb = wl.make_config(1)
+    rng = np.random.default_rng(5)
+    pos = wb.pos.astype(np.float64) + np.array([7.3, -11.9, 0.25])
+    pos[rng.integers(0, wb.n_atoms, 200)] += np.array([wb.box[0], 0, 0])
+    pos[rng.integers(0, wb.n_atoms, 200)] -= np.array([0, 2 * wb.box[1], 0])
+    run_case(wb, "f32", 1.0, 0.1, "rf", pos=pos.astype(np.float32))
+
+
+def test_no_exclusions_and_zero_skin_f64():
+    """Empty exclusion list (NULL pointer), skin = 0; an LJ + RF fluid of well separated O atoms."""
+    wb = wl.make_water_box(400, 3.3, 77)
+    sel = np.arange(0, wb.n_atoms, 3)  # oxygens only: no close contacts
+    import dataclasses
+    sub = dataclasses.replace(wb, pos=wb.pos[sel].copy(), charge=wb.charge[sel].copy(), type=wb.type[sel].copy(),
+                              excl_pairs=np.zeros((0, 2), np.int32), mass=wb.mass[sel].copy())
+    run_case(sub, "f64", 1.0, 0.0, "rf")
+
+
+def test_tiny_systems_f64():
+    """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
+    two = wl.make_water_box(2, 5.0, 3)
+    pos = two.pos.astype(np.float64)
+    pos[3:] = pos[3:] - pos[3] + pos[0] + np.array([0.31, 0.05, -0.02])
+    import dataclasses
+    one = dataclasses.replace(two, pos=two.pos[:3].copy(), charge=two.charge[:3].copy(), type=two.type[:3].copy(),
+                              excl_pairs=two.excl_pairs[:3].copy(), mass=two.mass[:3].copy())
+    db = DeviceBox(one, "f64")
+    ctx = dimos.Context(0, "f64")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        assert dimos.dimos_nl_export_pairs(ctx, nl).shape[0] == 0
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)
+        assert float(F.abs().max()) == 0.0 and float(E.abs().max()) == 0.0 and float(W.abs().max()) == 0.0
+    finally:
+        ctx.close()
+    rep = run_case(two, "f64", 1.0, 0.1, "rf", pos=pos, oracle_alg="bruteforce")
+    assert rep["set"][0] == 9 and rep["n_pairs_cut"] == 9
+
+
+def test_two_particle_closed_form_through_gpu():
+    """The golden two-particle values (tests/golden/two_particle_closed_forms.txt) through the CUDA path."""
+    u = np.array([0.3, -0.5, 0.81])
+    u /= np.linalg.norm(u)
+    lj = torch.from_numpy(oracle.lorentz_berthelot([wl.SIGMA_O, 0.0], [wl.EPS_O, 0.0])).cuda()
+    ctx = dimos.Context(0, "f64")
+    try:
+        for (qa, ta, qb, tb, r, rc, e_want, f_want) in [
+            (wl.Q_O, 0, wl.Q_O, 0, 0.30, 0.9, 1.16685351179584 + 167.933704824648, 1149.71580381198),
+            (wl.Q_O, 0, wl.Q_O, 0, 0.35, 1.0, 137.241056774674, 757.184487000131),
+            (wl.Q_O, 0, wl.Q_H, 1, 0.20, 0.9, -162.872453453971, -1194.96291686214),
+            (wl.Q_H, 1, wl.Q_H, 1, 0.25, 1.0, 61.3683742187847, 380.624403704081),
+        ]:
+            pos = torch.tensor(np.array([[10.0, 11.0, 12.0] + r * u, [10.0, 11.0, 12.0]]), device="cuda")
+            q = torch.tensor([qa, qb], dtype=torch.float64, device="cuda")
+            t = torch.tensor([ta, tb], dtype=torch.int32, device="cuda")
+            nl = dimos.dimos_nl_build(ctx, pos, [50.0, 50.0, 50.0], rc, 0.1)
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, pos, q, t, lj)
+            assert float(E[0]) == pytest.approx(e_want, rel=1e-12)
+            assert float(F[0].cpu().numpy() @ u) == pytest.approx(f_want, rel=1e-12)
+            assert np.allclose(F[0].cpu().numpy(), -F[1].cpu().numpy(), rtol=0, atol=1e-9)
+            assert float(torch.trace(W)) == pytest.approx(r * f_want, rel=1e-12)
+    finally:
+        ctx.close()
+
+
+# --- list reuse: forces from a list built at earlier positions ----------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_list_stays_valid_under_half_skin_displacement(precision):
+    wb = wl.make_config(1)
+    rc, skin = 1.0, 0.1
+    db = DeviceBox(wb, precision)
+    rng = np.random.default_rng(11)
+    step = rng.standard_normal(wb.pos.shape)
+    step *= (0.5 * skin * 0.98) / np.linalg.norm(step, axis=1, keepdims=True)
+    moved = (wb.pos.astype(np.float64) + step).astype(np.float64 if precision == "f64" else np.float32)
+    db2 = DeviceBox(wb, precision, pos=moved)
+    ctx = dimos.Context(0, precision)
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, rc, skin, db.excl)
+        assert dimos.dimos_nl_needs_rebuild(ctx, db2.pos, nl.pos_at_build, skin) is False
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, db2.pos, db.charge, db.type, db.lj)
+        orc = oracle.nonbonded(db2.pos.double().cpu().numpy(), db.charge.double().cpu().numpy(), wb.type, db.lj_np, db.box, rc,
+                               excl_pairs=wb.excl_pairs, band=BAND)
+        check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision)
+        # rebuilding in place at the new positions gives the same answer and the oracle's new pair set
+        nl = dimos.dimos_nl_build(ctx, db2.pos, db.box, rc, skin, db.excl, nl=nl)
+        check_neighbor_set(dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy(), db2.pos.double().cpu().numpy(), db.box, rc + skin,
+                           wb.excl_pairs)
+        F2, E2, W2 = dimos.dimos_nonbonded(ctx, nl, db2.pos, db.charge, db.type, db.lj)
+        check_nonbonded(F2.cpu().numpy(), E2.cpu().numpy(), W2.cpu().numpy(), orc, precision)
+    finally:
+        ctx.close()
+
+
+def test_repeat_calls_are_consistent_f32():
+    """Two force calls on one list agree to summation-order noise; two builds export the identical set."""
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        a = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy().astype(np.int64)
+        F1, E1, _ = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)
+        F1, E1 = F1.clone(), E1.clone()
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)
+        b = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy().astype(np.int64)
+        n = wb.n_atoms
+        assert np.array_equal(np.sort(a[:, 0] * n + a[:, 1]), np.sort(b[:, 0] * n + b[:, 1]))
+        F2, E2, _ = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)
+        rms = float(F1.double().pow(2).sum(1).mean().sqrt())
+        assert float((F1 - F2).abs().max()) <= 2e-5 * rms
+        assert abs(float(E1[0] - E2[0])) <= 1e-6 * abs(float(E1[0]))
+    finally:
+        ctx.close()
+
+
+def test_host_buffer_entry_point_f32():
+    """dimos_nonbonded_host (the e2e leg of bench.py): same result as the device call."""
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)
+        hp = torch.from_numpy(wb.pos).pin_memory()
+        hq = torch.from_numpy(wb.charge).pin_memory()
+        ht = torch.from_numpy(wb.type).pin_memory()
+        hl = torch.from_numpy(db.lj_np).pin_memory()
+        hF = torch.empty_like(hp).pin_memory()
+        hE = torch.empty(4, dtype=torch.float64).pin_memory()
+        hW = torch.empty(3, 3, dtype=torch.float64).pin_memory()
+        ctx.nonbonded_host(nl, hp, hq, ht, hl, hF, hE, hW)
+        rms = float(F.double().pow(2).sum(1).mean().sqrt())
+        assert float((F.cpu() - hF).abs().max()) <= 2e-5 * rms
+        assert abs(float(E[0].cpu() - hE[0])) <= 1e-6 * abs(float(hE[0]))
+    finally:
+        ctx.close()
+
+
+# --- error behaviour of the boundary (include/dimos.h) ----------------------------------------------------
+def test_error_codes():
+    wb = wl.make_config(0)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        with pytest.raises(dimos.DimosError) as ei:
+            dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)  # r_cut > L/2
+        assert ei.value.status == -2
+        with pytest.raises(dimos.DimosError) as ei:
+            dimos.dimos_nl_build(ctx, db.pos, [1.0, -1.0, 1.0], 0.4, 0.1, db.excl)
+        assert ei.value.status == -1
+        bad = db.pos.clone()
+        bad[17, 1] = float("nan")
+        with pytest.raises(dimos.DimosError) as ei:
+            dimos.dimos_nl_build(ctx, bad, db.box, 0.9, 0.1, db.excl)
+        assert ei.value.status == -1
+        bad_excl = db.excl.clone()
+        bad_excl[5, 1] = wb.n_atoms + 3
+        with pytest.raises(dimos.DimosError) as ei:
+            dimos.dimos_nl_build(ctx, db.pos, db.box, 0.9, 0.1, bad_excl)
+        assert ei.value.status == -1
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 0.9, 0.1, db.excl)
+        nl.r_cut = 0.8  # params.r_cut differs from the build r_cut
+        with pytest.raises(dimos.DimosError) as ei:
+            dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)
+        assert ei.value.status == -6
+        nl.r_cut = 0.9
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)  # still usable afterwards
+        assert torch.isfinite(F).all()
+        rc = ctx.lib.dimos_nl_build(None, None, 0, None, 0.0, 0.0, None, 0, None, None, None)
+        assert rc == -1
+    finally:
+        ctx.close()
+
+
+# --- full-size configs in bench.py's launch configuration: sampled outputs + properties -------------------
+def _sampled_force_check(wb, precision, r_cut, skin, method, n_sample, alpha=3.12):
+    """At sizes where the whole-system oracle takes minutes: compare F_i for sampled atoms i with the oracle's
+    plain per-atom sum over all j (numpy fp64, minimum image, definition of SURVEY.md §8(c)), and check
+    properties that hold at any size (Newton III, virial symmetry, E = sum of components)."""
+    db = DeviceBox(wb, precision)
+    ctx = dimos.Context(0, precision)
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, r_cut, skin, db.excl)
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, method=method, alpha=alpha)
+        stats = nl.stats()
+        npairs = ctypes.c_int64(0)
+        ctx._check(ctx.lib.dimos_nl_export_pairs(ctx.handle, nl.handle, None, 0, ctypes.byref(npairs), 0))
+        F = F.double().cpu().numpy()
+        E = E.cpu().numpy()
+        W = W.cpu().numpy()
+    finally:
+        ctx.close()
+    n = wb.n_atoms
+    pos = wb.pos.astype(np.float64)
+    q = wb.charge.astype(np.float64)
+    rng = np.random.default_rng(123)
+    sample = rng.choice(n, n_sample, replace=False)
+    # per-sampled-atom oracle: treat the sampled atom's full neighbourhood by running the oracle on the
+    # sub-box of atoms within r_cut + 0.2 nm of it (the pair sum for atom i only involves those)
+    rms = float(np.sqrt((F ** 2).sum(axis=1).mean()))
+    e_tol, f_tol = (1e-10, 1e-10) if precision == "f64" else (1e-5, 1e-4)
+    worst = 0.0
+    for i in sample:
+        d = pos - pos[i]
+        d -= db.box * np.rint(d / db.box)
+        near = np.nonzero((d ** 2).sum(axis=1) < (r_cut + 0.2) ** 2)[0]
+        loc = {int(a): k for k, a in enumerate(near)}
+        mol = np.unique(near // 3)  # water: atoms 3m, 3m+1, 3m+2 exclude one another (workloads.py)
+        ex = []
+        for m in mol:
+            ids = [3 * m, 3 * m + 1, 3 * m + 2]
+            for a in range(3):
+                for b in range(a + 1, 3):
+                    if ids[a] in loc and ids[b] in loc:
+                        ex.append((loc[ids[a]], loc[ids[b]]))
+        ex = np.array(sorted((min(a, b), max(a, b)) for a, b in ex), dtype=np.int32).reshape(-1, 2)
+        sub = pos[i] + d[near]  # unwrapped around atom i: no periodic images needed inside a huge box
+        orc = oracle.nonbonded(sub, q[near], wb.type[near], db.lj_np, np.array([1e3, 1e3, 1e3]), r_cut,
+                               method=oracle.METHOD_RF if method == "rf" else oracle.METHOD_EWALD_REAL, alpha=alpha,
+                               excl_pairs=ex, band=BAND, algorithm="bruteforce")
+        k = loc[int(i)]
+        err = np.linalg.norm(F[i] - orc.F[k]) - (orc.allow[k] if precision != "f64" else 0.0)
+        worst = max(worst, err / rms)
+        assert err <= f_tol * rms, f"atom {i}: |dF|={np.linalg.norm(F[i] - orc.F[k]):.3e} tol {f_tol * rms:.3e}"
+    assert np.abs(F.sum(axis=0)).max() <= (1e-9 if precision == "f64" else 2e-3) * rms * np.sqrt(n)
+    assert np.abs(W - W.T).max() <= 1e-6 * np.abs(W).max()
+    assert abs(E[0] - E[1:].sum()) <= 1e-9 * np.abs(E[1:]).sum()
+    return stats, int(npairs.value), worst
+
+
+def test_config2_water30k_sampled_f32_and_mixed():
+    wb = wl.make_config(2)
+    for precision in ("f32", "mixed"):
+        stats, npairs, worst = _sampled_force_check(wb, precision, 1.0, 0.1, "rf", 24)
+        assert stats["n_cells"] == (8, 8, 8)
+        assert abs(npairs / (wb.n_atoms * 278.8) - 1.0) < 0.02  # pairs < r_nl per atom at this density
+
+
+def test_config3_water300k_headline_sampled_f32():
+    """The bench workload (configs[3], 900,000 atoms) in the launch configuration bench.py times."""
+    wb = wl.make_config(3)
+    stats, npairs, worst = _sampled_force_check(wb, "f32", 1.0, 0.1, "rf", 24)
+    assert stats["n_cells"] == (18, 18, 18)
+    assert abs(npairs / (wb.n_atoms * 278.8) - 1.0) < 0.02
+
+
+def test_config4_water100k_ewald_sampled():
+    wb = wl.make_config(4)
+    for precision in ("f32", "f64"):
+        stats, npairs, worst = _sampled_force_check(wb, precision, 1.0, 0.1, "ewald", 16)
+        assert stats["n_cells"] == (13, 13, 13)
