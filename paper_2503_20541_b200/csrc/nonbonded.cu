@@ -30,6 +30,12 @@ __device__ __forceinline__ float rsqrt_r(float x)
     return y;
 }
 __device__ __forceinline__ double rsqrt_r(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
+// accumulate a*b into an accumulator that may be wider than the operands (DIMOS_MIXED: fp64 from the first add)
+__device__ __forceinline__ float fma_acc(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_acc(float a, float b, double c) { return c + (double)(a * b); }
+__device__ __forceinline__ double fma_acc(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float rintr(float x) { return rintf(x); }
 __device__ __forceinline__ double rintr(double x) { return rint(x); }
 __device__ __forceinline__ float erfc_r(float x) { return erfcf(x); }
@@ -145,12 +151,15 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
         Facc[s] = mk4((real)0, (real)0, (real)0, (real)0);
     }
     if (blockIdx.x == 0) {
-        // (sigma, eps) -> c6 = 4 eps sigma^6, c12 = 4 eps sigma^12  (Eq. 4)
+        // (sigma, eps) -> c6 = 4 eps sigma^6, c12 = 4 eps sigma^12, 6 c6, 12 c12  (Eq. 4)
         for (int k = threadIdx.x; k < nt * nt; k += blockDim.x) {
             double sg = lj_table[2 * k], ep = lj_table[2 * k + 1];
             double s2 = sg * sg, s6 = s2 * s2 * s2;
-            lj_out[2 * k] = (real)(4.0 * ep * s6);
-            lj_out[2 * k + 1] = (real)(4.0 * ep * s6 * s6);
+            const double c6 = 4.0 * ep * s6, c12 = 4.0 * ep * s6 * s6;
+            lj_out[4 * k] = (real)c6;
+            lj_out[4 * k + 1] = (real)c12;
+            lj_out[4 * k + 2] = (real)(6.0 * c6);    // pre-scaled for the force: 24 eps [2 (s/r)^12 - (s/r)^6]
+            lj_out[4 * k + 3] = (real)(12.0 * c12);
         }
         for (int t = threadIdx.x; t < nt; t += blockDim.x) {
             int act = 0;
@@ -178,12 +187,13 @@ struct ForceParams {
     const int* jslot;
     const unsigned short* meta;
     const int2* row_info;
-    const real* lj;          // (c6, c12) per type pair
+    const typename vec4<real>::type* lj4;  // (c6, c12, 6 c6, 12 c12) per type pair
+    unsigned long long* unit_counter;      // dynamic unit scheduling (zeroed by gather_kernel)
     const int* row_active;   // per type: any non-zero LJ partner
     real4* Facc;
     real4* Fown;
     double* partials;        // [gridDim.x][N_PART]
-    real rc2, ke, krf, crf, alpha, two_a_sqrtpi;
+    real rc2, ke, krf, m2krf, crf, alpha, two_a_sqrtpi;
     real L[3], invL[3], h[3];
 };
 
@@ -216,31 +226,85 @@ __device__ __forceinline__ T reduce8_scatter(T (&v)[8], int lane)
     return c;
 }
 
+// One pair slot (i-atom i of the unit  x  the lane's j-atom).  LJ: this i-atom has LJ partners
+// (warp-uniform).  MASKED: honour the entry's i-mask bit.  All arithmetic is written as explicit
+// FMAs so that one slot is ~24 (no LJ) / ~32 (LJ) issued instructions.
+#define DIMOS_SLOT(i, LJ, MASKED)                                                                    \
+    do {                                                                                             \
+        const real dx = xi[i] - xj, dy = yi[i] - yj, dz = zi[i] - zj;                                \
+        real ddx = dx, ddy = dy, ddz = dz;                                                           \
+        if (PBC == 1) {                                                                              \
+            ddx -= P.L[0] * rintr(ddx * P.invL[0]);                                                  \
+            ddy -= P.L[1] * rintr(ddy * P.invL[1]);                                                  \
+            ddz -= P.L[2] * rintr(ddz * P.invL[2]);                                                  \
+        }                                                                                            \
+        const real r2 = fma_r(ddz, ddz, fma_r(ddy, ddy, ddx * ddx));                                 \
+        bool in = r2 < P.rc2;                                                                        \
+        if (MASKED) in = in && ((mask >> i) & 1u);                                                   \
+        real rinv = rsqrt_r(r2);                                                                     \
+        if (LJ || MASKED || METHOD != DIMOS_RF) rinv = in ? rinv : (real)0;                          \
+        const real qq = in ? qi[i] * qj : (real)0;                                                   \
+        const real rinv2 = rinv * rinv;                                                              \
+        real fr2;                                                                                    \
+        if (METHOD == DIMOS_RF) {                                                                    \
+            const real t = fma_r(P.krf, r2, rinv);              /* 1/r + k_rf r^2 */                 \
+            e_c = fma_acc(qq, t - P.crf, e_c);                  /* Eq. 8 */                          \
+            fr2 = qq * fma_r(P.m2krf, r2, rinv);                /* r^2 k_e qq (1/r^3 - 2 k_rf) */    \
+        } else {                                                                                     \
+            const real r = r2 * rinv;                                                                \
+            const real ar = P.alpha * r;                                                             \
+            const real erfc_ar = erfc_r(ar);                                                         \
+            const real ex = exp_r(-ar * ar);                                                         \
+            const real qr = qq * rinv;                                                               \
+            e_c = fma_acc(qr, erfc_ar, e_c);                    /* Eq. 10, n = 0 */                  \
+            fr2 = fma_r(qq * P.two_a_sqrtpi, ex, qr * erfc_ar);                                      \
+        }                                                                                            \
+        if (LJ) {                                                                                    \
+            const real4 cc = ljt[ti[i] + tj];                   /* c6, c12, 6 c6, 12 c12 */          \
+            const real rinv6 = rinv2 * rinv2 * rinv2;                                                \
+            e_lj = fma_acc(fma_r(cc.y, rinv6, -cc.x), rinv6, e_lj);   /* Eq. 4 */                    \
+            fr2 = fma_r(fma_r(cc.w, rinv6, -cc.z), rinv6, fr2);                                      \
+        }                                                                                            \
+        const real fs = fr2 * rinv2;                                                                 \
+        fix[i] = fma_r(fs, ddx, fix[i]); fiy[i] = fma_r(fs, ddy, fiy[i]); fiz[i] = fma_r(fs, ddz, fiz[i]); \
+        fjx = fma_r(-fs, ddx, fjx); fjy = fma_r(-fs, ddy, fjy); fjz = fma_r(-fs, ddz, fjz);          \
+        if (PBC == 1) { /* the image can differ per pair: direct per-pair virial */                  \
+            const real fx = fs * ddx, fy = fs * ddy, fz = fs * ddz;                                  \
+            w[0] += (acc_t)(ddx * fx); w[1] += (acc_t)(ddx * fy); w[2] += (acc_t)(ddx * fz);         \
+            w[3] += (acc_t)(ddy * fy); w[4] += (acc_t)(ddy * fz); w[5] += (acc_t)(ddz * fz);         \
+        }                                                                                            \
+    } while (0)
+
 template <typename real, typename acc_t, int METHOD, int PBC>
-__global__ __launch_bounds__(PF_WARPS * 32, 2) void pair_force_kernel(ForceParams<real> P)
+__global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair_force_kernel(ForceParams<real> P)
 {
     using real4 = typename vec4<real>::type;
-    __shared__ real lj_s[MAX_TYPES * MAX_TYPES * 2 > 2048 ? 2048 : MAX_TYPES * MAX_TYPES * 2];
     __shared__ real4 off_s[27];
-    __shared__ double part_s[PF_WARPS][N_PART];
     extern __shared__ __align__(16) unsigned char dyn_smem[];
-    real* ljt = (P.nt * P.nt * 2 <= 2048) ? lj_s : reinterpret_cast<real*>(dyn_smem);
+    real4* ljt = reinterpret_cast<real4*>(dyn_smem);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
 
-    for (int k = threadIdx.x; k < P.nt * P.nt * 2; k += blockDim.x) ljt[k] = P.lj[k];
+    for (int k = threadIdx.x; k < P.nt * P.nt; k += blockDim.x) ljt[k] = P.lj4[k];
     if (threadIdx.x < 27) {
         const int c = threadIdx.x;
         off_s[c] = mk4((real)(c / 9 - 1) * P.h[0], (real)((c / 3) % 3 - 1) * P.h[1], (real)(c % 3 - 1) * P.h[2], (real)0);
     }
-    __syncthreads();
+    __syncthreads();  // the only CTA-wide barrier: warps are independent from here on
 
+    const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
-    const int64_t U = (int64_t)blockIdx.x * PF_WARPS + wib;
+    const int comp = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);  // reduce8_scatter's element of this lane
+    double acc_d = 0.0;  // running fp64 total of component `comp` over all units of this warp
 
-    acc_t e_lj = 0, e_c = 0;
-    acc_t w[6] = {0, 0, 0, 0, 0, 0};
+    // dynamic unit scheduling: every warp draws unit indices from one global counter, so no warp
+    // waits for another (rows differ in length) and the tail is at most one unit long
+    long long U = 0, U_next = 0;
+    if (lane == 0) U = (long long)atomicAdd(P.unit_counter, 1ull);
+    U = __shfl_sync(FULL, U, 0);
 
-    if (U < P.n_units) {
+    while (U < P.n_units) {
+        if (lane == 0) U_next = (long long)atomicAdd(P.unit_counter, 1ull);  // in flight while this unit is processed
+
         // ---- the unit's 8 i-atoms in registers (uniform across the warp) ----
         real xi[UNIT], yi[UNIT], zi[UNIT], qi[UNIT];
         int ti[UNIT];
@@ -258,81 +322,53 @@ __global__ __launch_bounds__(PF_WARPS * 32, 2) void pair_force_kernel(ForceParam
         const int mc = ri.x & 0xFFFF;
         const bool unit_full = (ri.x & 0x10000) == 0;
         const int nu = ri.y;
-        const int nch = (nu + 31) >> 5;
-        const int64_t row = U * (int64_t)P.row_cap + P.m_res;
+        const int total = mc + ((nu + 31) >> 5);
+        acc_t e_lj = 0, e_c = 0;
+        acc_t w[6] = {0, 0, 0, 0, 0, 0};
 
-        for (int c = -mc; c < nch; ++c) {
-            const int64_t e = row + (int64_t)c * 32 + lane;
-            const int j = P.jslot[e];
-            const unsigned m = P.meta[e];
-            const real4 pj = P.xyzq[j];
-            const int tj = P.stype[j];
+        // software pipeline: (jslot, meta) two chunks ahead, (xyzq, stype) one chunk ahead
+        int64_t e = U * (int64_t)P.row_cap + P.m_res - (int64_t)mc * 32 + lane;
+        int jn = 0, jn2 = 0, tjn = 0;
+        unsigned mn = 0, mn2 = 0;
+        real4 pjn = mk4((real)0, (real)0, (real)0, (real)0);
+        if (total > 0) { jn = P.jslot[e]; mn = P.meta[e]; }
+        if (total > 1) { jn2 = P.jslot[e + 32]; mn2 = P.meta[e + 32]; }
+        if (total > 0) { pjn = P.xyzq[jn]; tjn = P.stype[jn]; }
+
+        for (int c = 0; c < total; ++c) {
+            const int j = jn;
+            const unsigned m = mn;
+            const real4 pj = pjn;
+            const int tj = tjn;
+            jn = jn2; mn = mn2;
+            if (c + 1 < total) { pjn = P.xyzq[jn]; tjn = P.stype[jn]; }
+            if (c + 2 < total) { jn2 = P.jslot[e + 64]; mn2 = P.meta[e + 64]; }
+            e += 32;
+
             const real4 off = off_s[m >> 8];
             const real xj = pj.x + off.x, yj = pj.y + off.y, zj = pj.z + off.z;
             const real qj = pj.w;
             const unsigned mask = m & 0xFFu;
             real fjx = 0, fjy = 0, fjz = 0;
-            const bool plain = unit_full && c >= 0 && (c * 32 + 32 <= nu);  // warp-uniform: no mask needed
+            const int cc_ = c - mc;
+            const bool plain = unit_full && cc_ >= 0 && (cc_ * 32 + 32 <= nu);  // warp-uniform: no mask needed
 
-            auto slot = [&](const int i, const bool use_mask) {
-                real dx = xi[i] - xj, dy = yi[i] - yj, dz = zi[i] - zj;
-                if (PBC == 1) {
-                    dx -= P.L[0] * rintr(dx * P.invL[0]);
-                    dy -= P.L[1] * rintr(dy * P.invL[1]);
-                    dz -= P.L[2] * rintr(dz * P.invL[2]);
-                }
-                const real r2 = dx * dx + dy * dy + dz * dz;
-                bool in = r2 < P.rc2;
-                if (use_mask) in = in && ((mask >> i) & 1u);
-                const real rinv = in ? rsqrt_r(r2) : (real)0;
-                const real qq = in ? qi[i] * qj : (real)0;
-                const real rinv2 = rinv * rinv;
-                real fr2;  // force * r^2 (scalar), so that f_ij = fr2 * rinv2 * d
-                real elj = 0;
-                if (ti[i] >= 0) {  // warp-uniform: this i-atom has LJ partners
-                    const real rinv6 = rinv2 * rinv2 * rinv2;
-                    const real c6 = ljt[2 * (ti[i] + tj)], c12 = ljt[2 * (ti[i] + tj) + 1];
-                    const real t1 = c12 * rinv6;
-                    const real u = t1 - c6;
-                    elj = u * rinv6;                      // 4 eps [(s/r)^12 - (s/r)^6]
-                    fr2 = (real)6 * ((u + t1) * rinv6);   // 24 eps [2 (s/r)^12 - (s/r)^6]
-                } else {
-                    fr2 = 0;
-                }
-                real ec;
-                if (METHOD == DIMOS_RF) {
-                    const real a = P.krf * r2;
-                    ec = qq * (rinv + a - P.crf);                 // Eq. 8
-                    fr2 += qq * (rinv - (real)2 * a);             // r^2 * k_e qq (1/r^3 - 2 k_rf)
-                } else {
-                    const real r = r2 * rinv;
-                    const real ar = P.alpha * r;
-                    const real erfc_ar = erfc_r(ar);
-                    const real ex = exp_r(-ar * ar);
-                    ec = qq * rinv * erfc_ar;                     // Eq. 10, n = 0
-                    fr2 += qq * (rinv * erfc_ar + P.two_a_sqrtpi * ex);
-                }
-                const real fs = fr2 * rinv2;
-                fix[i] += fs * dx; fiy[i] += fs * dy; fiz[i] += fs * dz;
-                fjx -= fs * dx; fjy -= fs * dy; fjz -= fs * dz;
-                e_lj += (acc_t)elj;
-                e_c += (acc_t)ec;
-                if (PBC == 1) {  // the image can differ per pair: direct per-pair virial
-                    const real fx = fs * dx, fy = fs * dy, fz = fs * dz;
-                    w[0] += (acc_t)(dx * fx); w[1] += (acc_t)(dx * fy); w[2] += (acc_t)(dx * fz);
-                    w[3] += (acc_t)(dy * fy); w[4] += (acc_t)(dy * fz); w[5] += (acc_t)(dz * fz);
-                }
-            };
             if (plain) {
 #pragma unroll
-                for (int i = 0; i < UNIT; ++i) slot(i, false);
+                for (int i = 0; i < UNIT; ++i) {
+                    if (ti[i] >= 0) DIMOS_SLOT(i, true, false);
+                    else DIMOS_SLOT(i, false, false);
+                }
             } else {
 #pragma unroll
-                for (int i = 0; i < UNIT; ++i) slot(i, true);
+                for (int i = 0; i < UNIT; ++i) {
+                    if (ti[i] >= 0) DIMOS_SLOT(i, true, true);
+                    else DIMOS_SLOT(i, false, true);
+                }
             }
             if (PBC == 0) {  // x_j' (x) F_j^entry, unit-local coordinates
-                w[0] += (acc_t)(xj * fjx); w[1] += (acc_t)(xj * fjy); w[2] += (acc_t)(xj * fjz);
-                w[3] += (acc_t)(yj * fjy); w[4] += (acc_t)(yj * fjz); w[5] += (acc_t)(zj * fjz);
+                w[0] = fma_acc(xj, fjx, w[0]); w[1] = fma_acc(xj, fjy, w[1]); w[2] = fma_acc(xj, fjz, w[2]);
+                w[3] = fma_acc(yj, fjy, w[3]); w[4] = fma_acc(yj, fjz, w[4]); w[5] = fma_acc(zj, fjz, w[5]);
             }
             if (mask) red_add_xyz(&P.Facc[j], fjx, fjy, fjz);
         }
@@ -341,31 +377,27 @@ __global__ __launch_bounds__(PF_WARPS * 32, 2) void pair_force_kernel(ForceParam
         const real rx = reduce8_scatter(fix, lane);
         const real ry = reduce8_scatter(fiy, lane);
         const real rz = reduce8_scatter(fiz, lane);
-        const int ii = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
         if ((lane & 3) == 0) {
-            P.Fown[U * UNIT + ii] = mk4(rx, ry, rz, (real)0);
+            P.Fown[U * UNIT + comp] = mk4(rx, ry, rz, (real)0);
             if (PBC == 0) {  // x_i (x) F_i^unit
-                const real4 v = P.xyzq[U * UNIT + ii];
+                const real4 v = P.xyzq[U * UNIT + comp];
                 w[0] += (acc_t)(v.x * rx); w[1] += (acc_t)(v.x * ry); w[2] += (acc_t)(v.x * rz);
                 w[3] += (acc_t)(v.y * ry); w[4] += (acc_t)(v.y * rz); w[5] += (acc_t)(v.z * rz);
             }
         }
+        // ---- energy / virial of this unit: lane partials -> fp64 warp totals, kept per warp ----
+        double red[8] = {(double)e_lj, (double)e_c, (double)w[0], (double)w[1], (double)w[2], (double)w[3], (double)w[4], (double)w[5]};
+        acc_d += reduce8_scatter(red, lane);
+
+        U = __shfl_sync(FULL, U_next, 0);
     }
 
-    // ---- energy / virial: warp -> block -> one fp64 partial row per block ----
-    double red[8] = {(double)e_lj, (double)e_c, (double)w[0], (double)w[1], (double)w[2], (double)w[3], (double)w[4], (double)w[5]};
-    const double tot = reduce8_scatter(red, lane);
-    const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
-    if ((lane & 3) == 0) part_s[wib][idx] = tot;
-    __syncthreads();
-    if (threadIdx.x < 8) {
-        double sum = 0;
-#pragma unroll
-        for (int k = 0; k < PF_WARPS; ++k) sum += part_s[k][threadIdx.x];
-        P.partials[(int64_t)blockIdx.x * N_PART + threadIdx.x] = sum;
-    }
-    if (threadIdx.x == 8) P.partials[(int64_t)blockIdx.x * N_PART + 8] = 0.0;
+    // one fp64 partial row per warp; the final reduction is finalize_kernel's (A6)
+    const int64_t prow = ((int64_t)blockIdx.x * PF_WARPS + wib) * N_PART;
+    if ((lane & 3) == 0) P.partials[prow + comp] = acc_d;
+    if (lane == 1) P.partials[prow + 8] = 0.0;
 }
+#undef DIMOS_SLOT
 
 // ------------------------------------------------------------------------------------------------
 // A5: Ewald exclusion correction  -k_e q_i q_j erf(alpha r)/r over all excluded pairs (reading C-15)
@@ -561,7 +593,7 @@ static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P,
     }
 #define DIMOS_PF(M, B)                                                                                            \
     do {                                                                                                          \
-        if (dyn) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
+        if (dyn > 48 * 1024) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
         pair_force_kernel<real, acc_t, M, B><<<nb, PF_WARPS * 32, dyn, s>>>(P);                                   \
     } while (0)
     if (method == DIMOS_RF) { if (pbc == 0) DIMOS_PF(DIMOS_RF, 0); else DIMOS_PF(DIMOS_RF, 1); }
@@ -580,18 +612,22 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     using real4 = typename vec4<real>::type;
     int rc;
     const int64_t nsl = nl->n_slots, nun = nl->n_units;
-    const unsigned nb_force = (unsigned)((nun + PF_WARPS - 1) / PF_WARPS);
+    // persistent-style grid: at most 2 resident CTAs per SM (fp32; 1 for fp64), warps draw units dynamically
+    const unsigned nb_full = (unsigned)((nun + PF_WARPS - 1) / PF_WARPS);
+    const unsigned nb_res = (unsigned)ctx->sm_count * (sizeof(real) == 4 ? 2u : 1u);
+    const unsigned nb_force = nb_full < nb_res ? nb_full : nb_res;
+    const size_t n_force_rows = (size_t)nb_force * PF_WARPS;  // one fp64 partial row per warp
     const bool ewald = prm->method == DIMOS_EWALD_REAL;
     const unsigned nb_excl = ewald && nl->n_excl > 0 ? (unsigned)((nl->n_excl + 255) / 256) : 0;
     if ((rc = ensure(ctx, nl->xyzq, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->stype, nsl * sizeof(int), s))) return rc;
     if ((rc = ensure(ctx, nl->Facc, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->Fown, nsl * sizeof(real4), s))) return rc;
-    if ((rc = ensure(ctx, nl->lj, (size_t)MAX_TYPES * MAX_TYPES * 2 * sizeof(double) + MAX_TYPES * sizeof(int), s))) return rc;
-    if ((rc = ensure(ctx, nl->partials, ((size_t)nb_force + (size_t)((nl->n_excl + 255) / 256) + 1) * N_PART * sizeof(double), s))) return rc;
+    if ((rc = ensure(ctx, nl->lj, (size_t)MAX_TYPES * MAX_TYPES * 4 * sizeof(double) + MAX_TYPES * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->partials, (n_force_rows + (size_t)((nl->n_excl + 255) / 256) + 1) * N_PART * sizeof(double), s))) return rc;
     if ((rc = ensure(ctx, nl->accum, 16 * sizeof(double), s))) return rc;
     real* lj_dev = (real*)nl->lj.p;
-    int* row_active = (int*)((char*)nl->lj.p + (size_t)MAX_TYPES * MAX_TYPES * 2 * sizeof(double));
+    int* row_active = (int*)((char*)nl->lj.p + (size_t)MAX_TYPES * MAX_TYPES * 4 * sizeof(double));
 
     const int T = 256;
     gather_kernel<real><<<(unsigned)((nsl + T - 1) / T), T, 0, s>>>(pos, charge, type, (const int*)nl->perm.p, (const double*)nl->ref.p,
@@ -603,24 +639,26 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     P.n_units = nun; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;
     P.xyzq = (const real4*)nl->xyzq.p; P.stype = (const int*)nl->stype.p;
     P.jslot = (const int*)nl->jslot.p; P.meta = (const unsigned short*)nl->meta.p; P.row_info = (const int2*)nl->row_info.p;
-    P.lj = lj_dev; P.row_active = row_active;
+    P.lj4 = (const real4*)lj_dev; P.row_active = row_active;
+    P.unit_counter = reinterpret_cast<unsigned long long*>((double*)nl->accum.p + 14);
     P.Facc = (real4*)nl->Facc.p; P.Fown = (real4*)nl->Fown.p; P.partials = (double*)nl->partials.p;
     const double rc_ = prm->r_cut;
     P.rc2 = (real)rc_ * (real)rc_;
     P.ke = (real)prm->coulomb_const;
     P.krf = (real)((prm->eps_rf - 1.0) / ((2.0 * prm->eps_rf + 1.0) * rc_ * rc_ * rc_));  // Eq. 8 constants, reading C-1
+    P.m2krf = (real)-2 * P.krf;
     P.crf = (real)(3.0 * prm->eps_rf / ((2.0 * prm->eps_rf + 1.0) * rc_));
     P.alpha = (real)prm->alpha;
     P.two_a_sqrtpi = (real)(2.0 * prm->alpha / sqrt(M_PI));
     for (int a = 0; a < 3; ++a) { P.L[a] = (real)nl->grid.L[a]; P.invL[a] = (real)(1.0 / nl->grid.L[a]); P.h[a] = (real)nl->grid.h[a]; }
-    const size_t dyn = (nt * nt * 2 > 2048) ? (size_t)nt * nt * 2 * sizeof(real) : 0;
+    const size_t dyn = (size_t)nt * nt * sizeof(real4);
     if (ctx->precision == DIMOS_MIXED) { if ((rc = launch_pair_force<real, double>(ctx, nl, P, prm->method, nb_force, dyn, s))) return rc; }
     else { if ((rc = launch_pair_force<real, real>(ctx, nl, P, prm->method, nb_force, dyn, s))) return rc; }
 
     if (nb_excl) {
         excl_correction_kernel<real><<<nb_excl, 256, 0, s>>>((const int2*)nl->excl_pairs.p, nl->n_excl, (const int*)nl->inv_perm.p,
                                                               (const real4*)nl->xyzq.p, (const double*)nl->ref.p, (real4*)nl->Facc.p,
-                                                              (double*)nl->partials.p + (size_t)nb_force * N_PART, P.ke, P.alpha,
+                                                              (double*)nl->partials.p + n_force_rows * N_PART, P.ke, P.alpha,
                                                               P.two_a_sqrtpi, nl->grid.L[0], nl->grid.L[1], nl->grid.L[2]);
         DIMOS_LAUNCH_CHECK(ctx, "excl_correction");
     }
@@ -629,7 +667,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     if (fb > maxfb) fb = maxfb;
     if (fb < 1) fb = 1;
     finalize_kernel<real><<<fb, T, 0, s>>>((const int*)nl->perm.p, nsl, (const real4*)nl->Fown.p, (const real4*)nl->Facc.p, F,
-                                           (const double*)nl->partials.p, (int64_t)nb_force + nb_excl, (double*)nl->accum.p, E, W);
+                                           (const double*)nl->partials.p, (int64_t)n_force_rows + nb_excl, (double*)nl->accum.p, E, W);
     DIMOS_LAUNCH_CHECK(ctx, "finalize");
     return DIMOS_OK;
 }
