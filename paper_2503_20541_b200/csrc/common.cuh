@@ -16,6 +16,7 @@ constexpr int UNIT = DIMOS_UNIT;  // atoms per i-cluster
 constexpr int KD_MAX = 4096;      // max atoms per cell the in-cell sorter handles
 constexpr int MAX_EXCL_PER_ATOM = 32;
 constexpr int MAX_TYPES = 64;
+constexpr int LIST_SLACK = 1024;  // entries readable past the last row (the force kernels prefetch two chunks ahead unguarded)
 constexpr int SELF_CODE = 13;  // stencil code of offset (0,0,0): (dx+1)*9+(dy+1)*3+(dz+1)
 
 // device error flag bits (NL::d_flags[0])
@@ -74,6 +75,7 @@ struct NL {
     int row_cap = 0;  // entries per unit row (multiple of 32), includes m_res
     int m_res = 128;  // reserved masked-entry region at the front of each row (multiple of 32)
     int n_grow = 0;
+    bool rows_sorted = false;  // plain entries partitioned LJ-active-j first (done lazily by the first force call after a build)
     int64_t n_entries = 0, n_entries_padded = 0;
     int64_t n_excl = 0;
     int max_cell_count = 0;

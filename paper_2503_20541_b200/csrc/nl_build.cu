@@ -951,8 +951,8 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
         nl->row_cap = nl->m_res + (((int)est + 31) & ~31);
     }
     for (int attempt = 0; attempt < 6; ++attempt) {
-        if ((rc = ensure(ctx, nl->jslot, (size_t)nun * nl->row_cap * sizeof(int), s))) return rc;
-        if ((rc = ensure(ctx, nl->meta, (size_t)nun * nl->row_cap * sizeof(unsigned short), s))) return rc;
+        if ((rc = ensure(ctx, nl->jslot, ((size_t)nun * nl->row_cap + LIST_SLACK) * sizeof(int), s))) return rc;
+        if ((rc = ensure(ctx, nl->meta, ((size_t)nun * nl->row_cap + LIST_SLACK) * sizeof(unsigned short), s))) return rc;
         zero_int_kernel<<<1, 32, 0, s>>>(flags + 2, 8);
         DIMOS_LAUNCH_CHECK(ctx, "zero_counters");
         BuildParams<real> P = make_build_params<real>(nl);
@@ -974,6 +974,7 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
             memcpy(&np, h + 4, 8);
             nl->n_entries = (int64_t)ne;
             nl->n_entries_padded = (int64_t)np;
+            nl->rows_sorted = false;  // the next force call re-partitions the rows by LJ activity
             return DIMOS_OK;
         }
         nl->n_grow++;

@@ -14,13 +14,14 @@
 //   A5  excl_correction: Ewald erf correction over the static exclusion list.
 //   A6  finalize: F[orig] = F_own + F_acc, fp64 reduction of block partials, E[4], W[9].
 #include <math.h>
+#include <stdlib.h>
 
-#include "common.cuh"
+#include <string>
+#include <type_traits>
+
+#include "pair_common.cuh"
 
 namespace dimos {
-
-__device__ __forceinline__ float4 mk4(float x, float y, float z, float w) { return make_float4(x, y, z, w); }
-__device__ __forceinline__ double4 mk4(double x, double y, double z, double w) { return make_double4(x, y, z, w); }
 
 // rsqrt: one MUFU.RSQ in fp32 (2^-22.9 max relative error); IEEE-quality in fp64
 __device__ __forceinline__ float rsqrt_r(float x)
@@ -44,18 +45,6 @@ __device__ __forceinline__ float erf_r(float x) { return erff(x); }
 __device__ __forceinline__ double erf_r(double x) { return erf(x); }
 __device__ __forceinline__ float exp_r(float x) { return expf(x); }
 __device__ __forceinline__ double exp_r(double x) { return exp(x); }
-
-// one vector reduction per j-atom (REDG.E.ADD.F32x4 on sm_100a); fp64 falls back to three scalar REDs
-__device__ __forceinline__ void red_add_xyz(float4* p, float x, float y, float z)
-{
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(x), "f"(y), "f"(z), "f"(0.0f) : "memory");
-}
-__device__ __forceinline__ void red_add_xyz(double4* p, double x, double y, double z)
-{
-    atomicAdd(&p->x, x);
-    atomicAdd(&p->y, y);
-    atomicAdd(&p->z, z);
-}
 
 // ------------------------------------------------------------------------------------------------
 // A3: rebuild trigger
@@ -138,6 +127,15 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
                               typename vec4<real>::type* __restrict__ Facc, const double* __restrict__ lj_table, int nt,
                               real* __restrict__ lj_out, int* __restrict__ row_active, double* __restrict__ accum)
 {
+    // per type: does it have any non-zero LJ partner?  (every block recomputes the tiny table: no inter-block order)
+    __shared__ int act_sh[MAX_TYPES];
+    for (int t = threadIdx.x; t < nt; t += blockDim.x) {
+        int act = 0;
+        for (int u = 0; u < nt; ++u)
+            if (lj_table[2 * (t * nt + u) + 1] != 0.0 && lj_table[2 * (t * nt + u)] != 0.0) act = 1;
+        act_sh[t] = act;
+    }
+    __syncthreads();
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s < n_slots) {
         int o = perm[s];
@@ -147,7 +145,8 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
         const double y = (double)pos[3 * (int64_t)o + 1] - ref[3 * s + 1];
         const double z = (double)pos[3 * (int64_t)o + 2] - ref[3 * s + 2];
         xyzq[s] = mk4((real)x, (real)y, (real)z, pad ? (real)0 : charge[o]);
-        stype[s] = type[o];
+        const int t = type[o];
+        stype[s] = t | (act_sh[t] ? STYPE_ACTIVE : 0);  // bit 30: the atom has LJ partners
         Facc[s] = mk4((real)0, (real)0, (real)0, (real)0);
     }
     if (blockIdx.x == 0) {
@@ -161,12 +160,7 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
             lj_out[4 * k + 2] = (real)(6.0 * c6);    // pre-scaled for the force: 24 eps [2 (s/r)^12 - (s/r)^6]
             lj_out[4 * k + 3] = (real)(12.0 * c12);
         }
-        for (int t = threadIdx.x; t < nt; t += blockDim.x) {
-            int act = 0;
-            for (int u = 0; u < nt; ++u)
-                if (lj_table[2 * (t * nt + u) + 1] != 0.0 && lj_table[2 * (t * nt + u)] != 0.0) act = 1;
-            row_active[t] = act;
-        }
+        for (int t = threadIdx.x; t < nt; t += blockDim.x) row_active[t] = act_sh[t];
         if (threadIdx.x < 16) accum[threadIdx.x] = 0.0;
     }
 }
@@ -174,58 +168,6 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
 // ------------------------------------------------------------------------------------------------
 // A4: pair-force kernel
 // ------------------------------------------------------------------------------------------------
-constexpr int PF_WARPS = 8;
-constexpr int N_PART = 9;  // E_lj, E_coul, Wxx, Wxy, Wxz, Wyy, Wyz, Wzz, E_excl
-
-template <typename real>
-struct ForceParams {
-    using real4 = typename vec4<real>::type;
-    int64_t n_units;
-    int row_cap, m_res, nt;
-    const real4* xyzq;
-    const int* stype;
-    const int* jslot;
-    const unsigned short* meta;
-    const int2* row_info;
-    const typename vec4<real>::type* lj4;  // (c6, c12, 6 c6, 12 c12) per type pair
-    unsigned long long* unit_counter;      // dynamic unit scheduling (zeroed by gather_kernel)
-    const int* row_active;   // per type: any non-zero LJ partner
-    real4* Facc;
-    real4* Fown;
-    double* partials;        // [gridDim.x][N_PART]
-    real rc2, ke, krf, m2krf, crf, alpha, two_a_sqrtpi;
-    real L[3], invL[3], h[3];
-};
-
-// reduce-scatter of 8 values over the 32 lanes: on return lane l holds, in v[0], the warp-wide sum of
-// element ((l>>4)&1)*4 + ((l>>3)&1)*2 + ((l>>2)&1)   (9 shuffles instead of 40)
-template <typename T>
-__device__ __forceinline__ T reduce8_scatter(T (&v)[8], int lane)
-{
-    const unsigned FULL = 0xffffffffu;
-    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
-    T a[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        T send = b4 ? v[k] : v[k + 4];
-        T keep = b4 ? v[k + 4] : v[k];
-        a[k] = keep + __shfl_xor_sync(FULL, send, 16);
-    }
-    T b[2];
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-        T send = b3 ? a[k] : a[k + 2];
-        T keep = b3 ? a[k + 2] : a[k];
-        b[k] = keep + __shfl_xor_sync(FULL, send, 8);
-    }
-    T send = b2 ? b[0] : b[1];
-    T keep = b2 ? b[1] : b[0];
-    T c = keep + __shfl_xor_sync(FULL, send, 4);
-    c += __shfl_xor_sync(FULL, c, 2);
-    c += __shfl_xor_sync(FULL, c, 1);
-    return c;
-}
-
 // One pair slot (i-atom i of the unit  x  the lane's j-atom).  LJ: this i-atom has LJ partners
 // (warp-uniform).  MASKED: honour the entry's i-mask bit.  All arithmetic is written as explicit
 // FMAs so that one slot is ~24 (no LJ) / ~32 (LJ) issued instructions.
@@ -314,7 +256,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const real4 v = P.xyzq[U * UNIT + i];
             xi[i] = v.x; yi[i] = v.y; zi[i] = v.z;
             qi[i] = v.w * P.ke;  // k_e folded into the i-side charge
-            const int t = P.stype[U * UNIT + i];
+            const int t = P.stype[U * UNIT + i] & STYPE_MASK;
             ti[i] = P.row_active[t] ? t * P.nt : -1;
             fix[i] = fiy[i] = fiz[i] = 0;
         }
@@ -333,7 +275,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
         real4 pjn = mk4((real)0, (real)0, (real)0, (real)0);
         if (total > 0) { jn = P.jslot[e]; mn = P.meta[e]; }
         if (total > 1) { jn2 = P.jslot[e + 32]; mn2 = P.meta[e + 32]; }
-        if (total > 0) { pjn = P.xyzq[jn]; tjn = P.stype[jn]; }
+        if (total > 0) { pjn = P.xyzq[jn]; tjn = P.stype[jn] & STYPE_MASK; }
 
         for (int c = 0; c < total; ++c) {
             const int j = jn;
@@ -341,7 +283,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const real4 pj = pjn;
             const int tj = tjn;
             jn = jn2; mn = mn2;
-            if (c + 1 < total) { pjn = P.xyzq[jn]; tjn = P.stype[jn]; }
+            if (c + 1 < total) { pjn = P.xyzq[jn]; tjn = P.stype[jn] & STYPE_MASK; }
             if (c + 2 < total) { jn2 = P.jslot[e + 64]; mn2 = P.meta[e + 64]; }
             e += 32;
 
@@ -576,6 +518,14 @@ int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s)
 // ------------------------------------------------------------------------------------------------
 // host orchestration of one force call
 // ------------------------------------------------------------------------------------------------
+// packed-FP32 kernel (pair_f32x2.cu): fp32 accumulation, image shift from the stencil code, reaction field;
+// DIMOS_PAIR_KERNEL=generic disables it (A/B timing)
+static bool use_f32x2(const Ctx* ctx, const NL* nl, int method)
+{
+    static const bool enabled = [] { const char* e = getenv("DIMOS_PAIR_KERNEL"); return !(e && std::string(e) == "generic"); }();
+    return enabled && ctx->precision == DIMOS_F32 && nl->grid.pbc_mode == 0 && method == DIMOS_RF;
+}
+
 template <typename real, typename acc_t>
 static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P, int method, unsigned nb, size_t dyn, cudaStream_t s)
 {
@@ -596,7 +546,12 @@ static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P,
         if (dyn > 48 * 1024) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
         pair_force_kernel<real, acc_t, M, B><<<nb, PF_WARPS * 32, dyn, s>>>(P);                                   \
     } while (0)
-    if (method == DIMOS_RF) { if (pbc == 0) DIMOS_PF(DIMOS_RF, 0); else DIMOS_PF(DIMOS_RF, 1); }
+    bool done = false;
+    if constexpr (std::is_same<real, float>::value && std::is_same<acc_t, float>::value) {
+        if (use_f32x2(ctx, nl, method)) done = launch_pair_force_f32x2(P, method, nb, dyn, s);
+    }
+    if (done) {}
+    else if (method == DIMOS_RF) { if (pbc == 0) DIMOS_PF(DIMOS_RF, 0); else DIMOS_PF(DIMOS_RF, 1); }
     else { if (pbc == 0) DIMOS_PF(DIMOS_EWALD_REAL, 0); else DIMOS_PF(DIMOS_EWALD_REAL, 1); }
 #undef DIMOS_PF
     if (ev_stop) cudaEventRecord(ev_stop, s);
@@ -613,10 +568,12 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     int rc;
     const int64_t nsl = nl->n_slots, nun = nl->n_units;
     // persistent-style grid: at most 2 resident CTAs per SM (fp32; 1 for fp64), warps draw units dynamically
-    const unsigned nb_full = (unsigned)((nun + PF_WARPS - 1) / PF_WARPS);
-    const unsigned nb_res = (unsigned)ctx->sm_count * (sizeof(real) == 4 ? 2u : 1u);
+    const bool fx = sizeof(real) == 4 && use_f32x2(ctx, nl, prm->method);
+    const int wpb = fx ? FX_WARPS : PF_WARPS;  // warps per CTA
+    const unsigned nb_full = (unsigned)((nun + wpb - 1) / wpb);
+    const unsigned nb_res = (unsigned)ctx->sm_count * (fx ? (unsigned)FX_CTAS_PER_SM : (sizeof(real) == 4 ? 2u : 1u));
     const unsigned nb_force = nb_full < nb_res ? nb_full : nb_res;
-    const size_t n_force_rows = (size_t)nb_force * PF_WARPS;  // one fp64 partial row per warp
+    const size_t n_force_rows = (size_t)nb_force * wpb;  // one fp64 partial row per warp
     const bool ewald = prm->method == DIMOS_EWALD_REAL;
     const unsigned nb_excl = ewald && nl->n_excl > 0 ? (unsigned)((nl->n_excl + 255) / 256) : 0;
     if ((rc = ensure(ctx, nl->xyzq, nsl * sizeof(real4), s))) return rc;
@@ -634,9 +591,15 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
                                                                     nsl, (real4*)nl->xyzq.p, (int*)nl->stype.p, (real4*)nl->Facc.p,
                                                                     lj_table, nt, lj_dev, row_active, (double*)nl->accum.p);
     DIMOS_LAUNCH_CHECK(ctx, "gather");
+    if (!nl->rows_sorted) {  // once per build: partition every row's mask-free entries, LJ-active j-atoms first
+        launch_reorder_rows((int*)nl->jslot.p, (unsigned short*)nl->meta.p, (const int2*)nl->row_info.p, (const int*)nl->stype.p,
+                            nun, nl->row_cap, nl->m_res, s);
+        DIMOS_LAUNCH_CHECK(ctx, "reorder_rows");
+        nl->rows_sorted = true;
+    }
 
     ForceParams<real> P;
-    P.n_units = nun; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;
+    P.n_units = nun; P.n_slots = nsl; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;
     P.xyzq = (const real4*)nl->xyzq.p; P.stype = (const int*)nl->stype.p;
     P.jslot = (const int*)nl->jslot.p; P.meta = (const unsigned short*)nl->meta.p; P.row_info = (const int2*)nl->row_info.p;
     P.lj4 = (const real4*)lj_dev; P.row_active = row_active;
