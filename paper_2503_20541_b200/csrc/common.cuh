@@ -73,7 +73,7 @@ struct NL {
     Grid grid{};
     int64_t n_units = 0, n_slots = 0;
     int row_cap = 0;  // entries per unit row (multiple of 32), includes m_res
-    int m_res = 128;  // reserved masked-entry region at the front of each row (multiple of 32)
+    int m_res = 128;  // max masked entries per row staged by the builder (multiple of 32); rows start m_res entries into their slab
     int n_grow = 0;
     bool rows_sorted = false;  // plain entries partitioned LJ-active-j first (done lazily by the first force call after a build)
     int64_t n_entries = 0, n_entries_padded = 0;
@@ -93,7 +93,7 @@ struct NL {
     DevBuf excl_pairs;            // int2[n_excl] copy (Ewald exclusion correction)
     DevBuf jslot;      // int[n_units*row_cap]
     DevBuf meta;       // uint16[n_units*row_cap]: mask | code<<8
-    DevBuf row_info;   // int2[n_units]: {masked chunks, unmasked entries}
+    DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, leading mask-free chunks}
     DevBuf flags;      // int[8]: [0] error flags, [1] max cell count, [2..3] entry counters (u64), [4..5] padded
     // per-step device arrays
     DevBuf xyzq;       // real4[n_slots]

@@ -703,31 +703,26 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         if (lane == 0) { atomicOr(&P.flags[0], FLAG_MASKED_OVERFLOW); atomicMax(&P.flags[7], nm); }
         nm = P.m_res;
     }
-    const int nu_pad = (nu + 31) & ~31;
-    if (nu_pad > nu_cap) {
-        if (lane == 0) { atomicOr(&P.flags[0], FLAG_ROW_OVERFLOW); atomicMax(&P.flags[6], nu_pad); }
+    // Row layout: the mask-free entries first (the leading nu/32 full chunks are the force kernels' mask-free
+    // chunks), then the masked entries, then padding up to a multiple of 32: one chunk sequence, no hole.
+    int n_pad = (nu + nm + 31) & ~31;
+    if (n_pad > nu_cap) {
+        if (lane == 0) { atomicOr(&P.flags[0], FLAG_ROW_OVERFLOW); atomicMax(&P.flags[6], n_pad); }
         nu = 0;  // the row is unusable; the host grows row_cap and rebuilds
+        nm = 0;
+        n_pad = 0;
     }
-    const int mc = (nm + 31) >> 5;
     const int self = (int)(U * UNIT);
     const unsigned short pad_meta = (unsigned short)(SELF_CODE << 8);  // mask 0
-    for (int k = lane; k < mc * 32; k += 32) {
-        int64_t e = row + P.m_res - mc * 32 + k;
+    for (int k = lane; k < n_pad - nu; k += 32) {
+        const int64_t e = row + P.m_res + nu + k;
         P.jslot[e] = k < nm ? st_j[k] : self;
         P.meta[e] = k < nm ? st_meta[k] : pad_meta;
     }
-    {
-        const int nu_ok = min(nu, nu_cap);
-        const int pad_to = min((nu_ok + 31) & ~31, nu_cap);
-        for (int k = nu_ok + lane; k < pad_to; k += 32) {
-            P.jslot[row + P.m_res + k] = self;
-            P.meta[row + P.m_res + k] = pad_meta;
-        }
-    }
     if (lane == 0) {
-        P.row_info[U] = make_int2(mc | (unit_full ? 0 : 0x10000), nu);
+        P.row_info[U] = make_int2((n_pad >> 5) | (unit_full ? 0 : 0x10000), unit_full ? (nu >> 5) : 0);
         atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[2]), (unsigned long long)(nm + nu));
-        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[4]), (unsigned long long)(mc * 32 + ((nu + 31) & ~31)));
+        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[4]), (unsigned long long)n_pad);
     }
 }
 
@@ -763,10 +758,9 @@ __global__ __launch_bounds__(128) void export_pairs_kernel(BuildParams<real> P, 
         pi[i] = __shfl_sync(FULL, my_perm, i);
     }
     const int2 ri = P.row_info[U];
-    const int mc = ri.x & 0xFFFF, nu = ri.y;
+    const int nch = ri.x & 0xFFFF;  // chunks in the row (mask-free chunks first, then masked entries and padding)
     const int64_t row = U * (int64_t)P.row_cap + P.m_res;
-    const int nch = (nu + 31) >> 5;
-    for (int c = -mc; c < nch; ++c) {
+    for (int c = 0; c < nch; ++c) {
         const int64_t e = row + (int64_t)c * 32 + lane;
         const int j = P.jslot[e];
         const unsigned m = P.meta[e];

@@ -261,15 +261,13 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             fix[i] = fiy[i] = fiz[i] = 0;
         }
         const int2 ri = P.row_info[U];
-        const int mc = ri.x & 0xFFFF;
-        const bool unit_full = (ri.x & 0x10000) == 0;
-        const int nu = ri.y;
-        const int total = mc + ((nu + 31) >> 5);
+        const int total = ri.x & 0xFFFF;  // chunks in the row
+        const int n_plain = ri.y;         // leading chunks that need no mask
         acc_t e_lj = 0, e_c = 0;
         acc_t w[6] = {0, 0, 0, 0, 0, 0};
 
         // software pipeline: (jslot, meta) two chunks ahead, (xyzq, stype) one chunk ahead
-        int64_t e = U * (int64_t)P.row_cap + P.m_res - (int64_t)mc * 32 + lane;
+        int64_t e = U * (int64_t)P.row_cap + P.m_res + lane;
         int jn = 0, jn2 = 0, tjn = 0;
         unsigned mn = 0, mn2 = 0;
         real4 pjn = mk4((real)0, (real)0, (real)0, (real)0);
@@ -292,8 +290,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const real qj = pj.w;
             const unsigned mask = m & 0xFFu;
             real fjx = 0, fjy = 0, fjz = 0;
-            const int cc_ = c - mc;
-            const bool plain = unit_full && cc_ >= 0 && (cc_ * 32 + 32 <= nu);  // warp-uniform: no mask needed
+            const bool plain = c < n_plain;  // warp-uniform: no mask needed
 
             if (plain) {
 #pragma unroll

@@ -29,8 +29,6 @@ __device__ __forceinline__ float rsqrt_f(float x)
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-constexpr int PF_AHEAD = 8;  // chunks of list stream kept in flight towards L2 ahead of the register pipeline
 
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }
@@ -179,15 +177,12 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         if (lane == 0) U_next = (long long)atomicAdd(P.unit_counter, 1ull);  // in flight while this unit is processed
 
         const int2 ri = P.row_info[U];
-        const int mc = ri.x & 0xFFFF;
-        const bool unit_full = (ri.x & 0x10000) == 0;
-        const int nu = ri.y;
-        const int total = mc + ((nu + 31) >> 5);
-        const int c_plain = mc;                                   // first mask-free chunk
-        const unsigned n_plain = unit_full ? (unsigned)(nu >> 5) : 0u;  // number of mask-free chunks
+        const int total = ri.x & 0xFFFF;        // chunks in the row
+        const int c_plain = 0;                  // the mask-free chunks come first ...
+        const unsigned n_plain = (unsigned)ri.y;  // ... this many of them
 
         // pipeline prologue: indices of chunks 0 and 1, coordinates of chunk 0
-        const int64_t e0 = U * (int64_t)P.row_cap + P.m_res - (int64_t)mc * 32 + lane;
+        const int64_t e0 = U * (int64_t)P.row_cap + P.m_res + lane;
         const int* jp = P.jslot + e0;
         const unsigned short* mp = P.meta + e0;
         int j0 = jp[0], j1 = jp[32], j2 = jp[64];
@@ -279,8 +274,8 @@ __global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(int* __rest
     int* sj = reinterpret_cast<int*>(ro_smem) + (size_t)wib * cap;
     unsigned short* sm = reinterpret_cast<unsigned short*>(reinterpret_cast<int*>(ro_smem) + (size_t)RO_WARPS * cap) + (size_t)wib * cap;
     const int2 ri = row_info[U];
-    if (ri.x & 0x10000) return;  // partial unit: every chunk takes the masked path
-    const int nu = ri.y < cap ? ri.y : cap;
+    const int nu = ri.y * 32 < cap ? ri.y * 32 : cap;  // entries of the mask-free chunks (0 for a partial unit)
+    if (nu == 0) return;
     const int64_t base = U * (int64_t)row_cap + m_res;
     const unsigned FULL = 0xffffffffu, lt = (1u << lane) - 1u;
     int n_act = 0;
