@@ -10,7 +10,7 @@ import oracle
 from paper_2503_20541_b200 import binding as dimos
 from paper_2503_20541_b200 import workloads as wl
 
-from gpu_harness import BAND, DeviceBox, check_neighbor_set, check_nonbonded, lj_table_np, run_case
+from gpu_harness import BAND, METHOD, DeviceBox, check_neighbor_set, check_nonbonded, lj_table_np, run_case
 
 pytestmark = pytest.mark.gpu
 
@@ -207,6 +207,29 @@ def test_repeat_calls_are_consistent_f32():
         rms = float(F1.double().pow(2).sum(1).mean().sqrt())
         assert float((F1 - F2).abs().max()) <= 2e-5 * rms
         assert abs(float(E1[0] - E2[0])) <= 1e-6 * abs(float(E1[0]))
+    finally:
+        ctx.close()
+
+
+def test_lj_table_change_after_row_reorder_f32():
+    """The first force call after a build partitions every row by the LJ activity of the j-atoms (an optimisation of
+    the packed-FP32 kernel).  A later call with a table in which the OTHER type carries LJ (stale order, every
+    i-atom pair LJ-active on the hydrogen side) must still match the oracle: the kernel decides per chunk."""
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        pos64 = db.pos.double().cpu().numpy()
+        q64 = db.charge.double().cpu().numpy()
+        for sigma, eps in ((wb.sigma, wb.epsilon), ([0.0, 0.12], [0.0, 0.25]), ([0.30, 0.10], [0.5, 0.2])):
+            lj_np = oracle.lorentz_berthelot(np.asarray(sigma, dtype=np.float64), np.asarray(eps, dtype=np.float64))
+            lj = torch.from_numpy(lj_np).to(db.pos.device).contiguous()
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, lj)
+            torch.cuda.synchronize()
+            orc = oracle.nonbonded(pos64, q64, wb.type, lj_np, db.box, 1.0, method=METHOD["rf"], eps_rf=78.5,
+                                   excl_pairs=wb.excl_pairs, band=BAND, algorithm="celllist")
+            check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, "f32")
     finally:
         ctx.close()
 
