@@ -53,6 +53,7 @@ def parse_args():
     ap.add_argument("--precision", default=None, help="f32 | mixed | f64 (default: first precision of the config)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-scan", action="store_true", help="skip the tau-versus-N scan over smaller boxes of the same recipe")
     return ap.parse_args()
 
 
@@ -219,6 +220,40 @@ def run_reference(args, spec, precision):
     print(json.dumps(line), flush=True)
 
 
+def tau_vs_n(ctx, dimos, dev, spec, precision, timed, tau_force_main, tau_build_main, n_main, n_cut_main):
+    """tau (s per force call) and pair interactions/s versus N on constant-density boxes of the same recipe
+    (the shape of the paper's scaling study); the last row is the headline workload itself."""
+    import torch
+
+    rows = []
+    for n_mol in (216, 3000, 30000, 100000):
+        if 3 * n_mol >= n_main:
+            continue
+        b = wl.make_scaled(n_mol, seed=wl.SEED_BASE + 200 + n_mol % 97, r_cut=spec.r_cut, skin=spec.skin, method=spec.method)
+        if spec.r_cut > 0.5 * float(min(b.box)):
+            continue  # the minimum-image requirement r_c <= L/2 (reading C-3) rules this size out
+        pos = torch.from_numpy(b.pos.astype(np.float32)).to(dev)
+        charge = torch.from_numpy(b.charge.astype(np.float32)).to(dev)
+        typ = torch.from_numpy(b.type).to(dev)
+        excl = torch.from_numpy(b.excl_pairs).to(dev)
+        lj = dimos.lj_table_from_types(b.sigma, b.epsilon).to(dev)
+        kw = dict(method=spec.method, eps_rf=spec.eps_rf, alpha=spec.alpha)
+        nl = dimos.dimos_nl_build(ctx, pos, b.box, spec.r_cut, spec.skin, excl)
+        n_cut = ctx.nl_count_within(nl, spec.r_cut)
+        F = torch.empty_like(pos)
+        E = torch.empty(4, dtype=torch.float64, device=dev)
+        W = torch.empty(3, 3, dtype=torch.float64, device=dev)
+        for _ in range(3):
+            dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw)
+        t_f = timed(lambda: dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw), reps=20)
+        t_b = timed(lambda: dimos.dimos_nl_build(ctx, pos, b.box, spec.r_cut, spec.skin, excl, nl=nl), reps=5)
+        rows.append({"n_atoms": int(b.n_atoms), "tau_force_s": t_f, "tau_build_s": t_b, "pairs_in_cutoff": int(n_cut),
+                     "pairs_per_s_force_only": n_cut / t_f})
+    rows.append({"n_atoms": int(n_main), "tau_force_s": tau_force_main, "tau_build_s": tau_build_main,
+                 "pairs_in_cutoff": int(n_cut_main), "pairs_per_s_force_only": n_cut_main / tau_force_main})
+    return rows
+
+
 def workload_name(spec, precision):
     return (f"configs[{spec.index}] {spec.name}: {3 * spec.n_molecules} atoms, density {wl.DENSITY} molecules/nm^3, "
             f"r_cut={spec.r_cut} nm, skin={spec.skin} nm, LJ + {'reaction field' if spec.method == 'rf' else 'Ewald real space'}, {precision}")
@@ -383,7 +418,7 @@ def run_ours(args, spec, precision):
         fp32_peak = 40.0  # NVIDIA's nominal B200 FP64 vector rate (no measured figure on this pool); context only
     list_bytes = stats["list_bytes"] + stats["n_slots"] * (16 + 4 + 16 + 16)
     roofline = {
-        "bound": "alu", "kernel": "pair_force_kernel", "achieved": achieved_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
+        "bound": "alu", "kernel": "pair_force_f32x2_kernel" if (precision == "f32" and spec.method == "rf") else "pair_force_kernel", "achieved": achieved_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
         "frac": (achieved_tflops / fp32_peak) if achieved_tflops else None, "traffic": load_traffic("pair_force_kernel"),
         "peak_source": f"derived: 148 SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md); FFMA probe measured "
                        f"{fp32_probe:.1f} TFLOP/s in this run",
@@ -408,6 +443,8 @@ def run_ours(args, spec, precision):
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
         "list": {k: stats[k] for k in ("n_units", "n_entries", "n_entries_padded", "n_pair_slots", "list_bytes", "row_capacity")},
     }
+    if not args.no_scan and world == 1 and precision != "f64":
+        line["tau_vs_n"] = tau_vs_n(ctx, dimos, dev, spec, precision, timed, tau_force, tau_build, n, n_cut)
     if not args.no_cpu_baseline and world >= 1:
         line["cpu_baseline"] = cpu_baseline(spec.method)
     ctx.close()
