@@ -515,12 +515,12 @@ int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s)
 // ------------------------------------------------------------------------------------------------
 // host orchestration of one force call
 // ------------------------------------------------------------------------------------------------
-// packed-FP32 kernel (pair_f32x2.cu): fp32 accumulation, image shift from the stencil code, reaction field;
+// packed-FP32 kernel (pair_f32x2.cu): fp32 accumulation, image shift from the stencil code;
 // DIMOS_PAIR_KERNEL=generic disables it (A/B timing)
 static bool use_f32x2(const Ctx* ctx, const NL* nl, int method)
 {
     static const bool enabled = [] { const char* e = getenv("DIMOS_PAIR_KERNEL"); return !(e && std::string(e) == "generic"); }();
-    return enabled && ctx->precision == DIMOS_F32 && nl->grid.pbc_mode == 0 && method == DIMOS_RF;
+    return enabled && ctx->precision == DIMOS_F32 && nl->grid.pbc_mode == 0 && (method == DIMOS_RF || method == DIMOS_EWALD_REAL);
 }
 
 template <typename real, typename acc_t>

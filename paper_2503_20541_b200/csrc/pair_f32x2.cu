@@ -7,8 +7,9 @@
 // profiles/r1_b_pair_force_ncu.md), so MUFU.RSQ, the cutoff FSETP/FSEL, loads and loop bookkeeping ride in the
 // freed slots and the kernel is bound by the FMA pipe instead of by instruction issue.
 //
-// Covers: fp32 positions, fp32 accumulation (DIMOS_F32), image shift from the stencil code (pbc_mode 0).
-// Everything else (fp64, mixed, per-pair minimum image) stays on the generic kernel.
+// Covers: fp32 positions, fp32 accumulation (DIMOS_F32), image shift from the stencil code (pbc_mode 0), reaction
+// field (Eq. 8) and Ewald real space (Eq. 10).  Everything else (fp64, mixed, per-pair minimum image) stays on the
+// generic kernel.
 //
 // LJ is evaluated only in chunks in which at least one j-atom has LJ partners (warp vote) and, there, only for
 // i-atom pairs with an LJ-active member; rows are reordered LJ-active-j-first after a build (reorder_rows_kernel
@@ -40,13 +41,43 @@ struct UnitRegs {
 };
 
 struct Consts {
-    float rc2, krf, m2krf, mcrf;
+    float rc2, krf, m2krf, mcrf;   // reaction field
+    float alpha, two_a_sqrtpi;     // Ewald real space
 };
+
+__device__ __forceinline__ float rcp_f(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float ex2_f(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// erfc(x) and exp(-x^2) for two values, x >= 0: erfc(x) = t (a1 + t (a2 + t (a3 + t (a4 + t a5)))) exp(-x^2),
+// t = 1 / (1 + p x)  (Abramowitz & Stegun 7.1.26, |error| <= 1.5e-7 absolute), with MUFU.RCP / MUFU.EX2 for the
+// reciprocal and the exponential and packed FMAs for the rest.
+__device__ __forceinline__ void erfc_exp2(float2 x, float2& erfc_x, float2& exp_mx2)
+{
+    const float2 den = __ffma2_rn(bc(0.3275911f), x, bc(1.0f));
+    const float2 t = f2(rcp_f(den.x), rcp_f(den.y));
+    const float2 y = __fmul2_rn(__fmul2_rn(x, x), bc(-1.4426950408889634f));  // -x^2 log2(e)
+    exp_mx2 = f2(ex2_f(y.x), ex2_f(y.y));
+    float2 pl = __ffma2_rn(bc(1.061405429f), t, bc(-1.453152027f));
+    pl = __ffma2_rn(pl, t, bc(1.421413741f));
+    pl = __ffma2_rn(pl, t, bc(-0.284496736f));
+    pl = __ffma2_rn(pl, t, bc(0.254829592f));
+    erfc_x = __fmul2_rn(__fmul2_rn(pl, t), exp_mx2);
+}
 
 // One chunk: the lane's j-atom against the 8 i-atoms, two i-atoms per packed instruction.
 //   MASKED: honour the entry's i-mask (exclusions, intra-unit half, padding); LJ: evaluate Eq. 4 for the
 //   i-pairs flagged in lj_pairs.  Returns F_j = -sum_i fs_i * d_i.
-template <bool MASKED, bool LJ>
+template <int METHOD, bool MASKED, bool LJ>
 __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const float4* __restrict__ ljt, const int* __restrict__ ti, float nxj,
                                            float nyj, float nzj, float qj, int tj, unsigned mask, unsigned lj_pairs,
                                            float& sx, float& sy, float& sz)
@@ -75,13 +106,26 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
         float2 qq = __fmul2_rn(u.q[p], qj2);
         qq.x = in_a ? qq.x : 0.f;
         qq.y = in_b ? qq.y : 0.f;
-        // reaction field, Eq. 8 (reading C-1): e = qq (1/r + k_rf r^2 - c_rf);  f/r = qq (1/r^3 - 2 k_rf)
-        float2 t = __ffma2_rn(krf2, r2, rinv);
-        t = __fadd2_rn(t, mcrf2);
-        u.e_c = __ffma2_rn(qq, t, u.e_c);
         const float2 rinvsq = __fmul2_rn(rinv, rinv);
-        const float2 g = __ffma2_rn(rinvsq, rinv, m2krf2);
-        float2 fs = __fmul2_rn(qq, g);
+        float2 fs;
+        if (METHOD == DIMOS_RF) {
+            // reaction field, Eq. 8 (reading C-1): e = qq (1/r + k_rf r^2 - c_rf);  f/r = qq (1/r^3 - 2 k_rf)
+            float2 t = __ffma2_rn(krf2, r2, rinv);
+            t = __fadd2_rn(t, mcrf2);
+            u.e_c = __ffma2_rn(qq, t, u.e_c);
+            const float2 g = __ffma2_rn(rinvsq, rinv, m2krf2);
+            fs = __fmul2_rn(qq, g);
+        } else {
+            // Ewald real space, Eq. 10 with n = 0 (readings C-14): e = qq erfc(a r)/r;
+            // f/r = qq [erfc(a r)/r + (2a/sqrt(pi)) exp(-a^2 r^2)] / r^2
+            const float2 ar = __fmul2_rn(__fmul2_rn(r2, rinv), bc(k.alpha));
+            float2 erfc_ar, ex;
+            erfc_exp2(ar, erfc_ar, ex);
+            const float2 qr = __fmul2_rn(qq, rinv);
+            u.e_c = __ffma2_rn(qr, erfc_ar, u.e_c);
+            const float2 g = __ffma2_rn(__fmul2_rn(qq, bc(k.two_a_sqrtpi)), ex, __fmul2_rn(qr, erfc_ar));
+            fs = __fmul2_rn(g, rinvsq);
+        }
         if (LJ) {
             if (lj_pairs & (1u << p)) {  // warp-uniform
                 const float4 ca = ljt[ti[2 * p] + (tj & STYPE_MASK)], cb = ljt[ti[2 * p + 1] + (tj & STYPE_MASK)];  // c6, c12, 6 c6, 12 c12
@@ -130,11 +174,11 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
         float sx, sy, sz;                                                                                        \
         if ((unsigned)((C) - c_plain) < n_plain) { /* warp-uniform: full chunk of a full unit, all masks 0xFF */ \
             if (lj_pairs != 0u && __any_sync(FULL, (TJ & STYPE_ACTIVE) != 0))                                    \
-                chunk_body<false, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, lj_pairs, sx, sy, sz);  \
+                chunk_body<METHOD, false, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, lj_pairs, sx, sy, sz);  \
             else                                                                                                 \
-                chunk_body<false, false>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, 0u, sx, sy, sz);       \
+                chunk_body<METHOD, false, false>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, 0u, sx, sy, sz);       \
         } else {                                                                                                 \
-            chunk_body<true, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, mk & 0xFFu, lj_pairs, sx, sy, sz);  \
+            chunk_body<METHOD, true, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, mk & 0xFFu, lj_pairs, sx, sy, sz);  \
         }                                                                                                        \
         /* virial: x_j' (x) F_j in unit-local coordinates, x_j' = -nxj */                                        \
         w[0] = fmaf(-nxj, sx, w[0]); w[1] = fmaf(-nxj, sy, w[1]); w[2] = fmaf(-nxj, sz, w[2]);                   \
@@ -168,6 +212,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     double acc_d = 0.0;  // running fp64 total of component `comp` over all units of this warp
     Consts k;
     k.rc2 = P.rc2; k.krf = P.krf; k.m2krf = P.m2krf; k.mcrf = -P.crf;
+    k.alpha = P.alpha; k.two_a_sqrtpi = P.two_a_sqrtpi;
 
     long long U = 0, U_next = 0;
     if (lane == 0) U = (long long)atomicAdd(P.unit_counter, 1ull);
@@ -325,10 +370,17 @@ void launch_reorder_rows(int* jslot, unsigned short* meta, const int2* row_info,
 
 bool launch_pair_force_f32x2(const ForceParams<float>& P, int method, unsigned nb, size_t dyn, cudaStream_t s)
 {
-    if (method != DIMOS_RF) return false;
-    if (dyn > 48 * 1024)
-        cudaFuncSetAttribute(pair_force_f32x2_kernel<DIMOS_RF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-    pair_force_f32x2_kernel<DIMOS_RF><<<nb, FX_WARPS * 32, dyn, s>>>(P);
+    if (method == DIMOS_RF) {
+        if (dyn > 48 * 1024)
+            cudaFuncSetAttribute(pair_force_f32x2_kernel<DIMOS_RF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        pair_force_f32x2_kernel<DIMOS_RF><<<nb, FX_WARPS * 32, dyn, s>>>(P);
+    } else if (method == DIMOS_EWALD_REAL) {
+        if (dyn > 48 * 1024)
+            cudaFuncSetAttribute(pair_force_f32x2_kernel<DIMOS_EWALD_REAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+        pair_force_f32x2_kernel<DIMOS_EWALD_REAL><<<nb, FX_WARPS * 32, dyn, s>>>(P);
+    } else {
+        return false;
+    }
     return true;
 }
 
