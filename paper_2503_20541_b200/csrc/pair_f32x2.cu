@@ -13,7 +13,7 @@
 //
 // LJ is evaluated only in chunks in which at least one j-atom has LJ partners (warp vote) and, there, only for
 // i-atom pairs with an LJ-active member; rows are reordered LJ-active-j-first after a build (reorder_rows_kernel
-// in nonbonded.cu), which is an optimisation only: correctness never depends on the order.
+// below), which is an optimisation only: correctness never depends on the order.
 #include <math.h>
 
 #include "pair_common.cuh"
