@@ -330,8 +330,8 @@ __global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(int* __rest
         if (k < nu) {
             const int j = jslot[base + k];
             sj[k] = j;
-            sm[k] = meta[base + k];
             act = (stype[j] & STYPE_ACTIVE) != 0;
+            sm[k] = (unsigned short)(meta[base + k] | (act ? 0x8000u : 0u));  // bit 15 is free: remember the flag
         }
         n_act += __popc(__ballot_sync(FULL, act));
     }
@@ -341,16 +341,18 @@ __global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(int* __rest
         const int k = k0 + lane;
         bool act = false, ina = false;
         int j = 0;
+        unsigned short m = 0;
         if (k < nu) {
             j = sj[k];
-            act = (stype[j] & STYPE_ACTIVE) != 0;
+            m = sm[k];
+            act = (m & 0x8000u) != 0;
             ina = !act;
         }
         const unsigned ba = __ballot_sync(FULL, act), bi = __ballot_sync(FULL, ina);
         if (k < nu) {
             const int pos = act ? pa + __popc(ba & lt) : pi + __popc(bi & lt);
             jslot[base + pos] = j;
-            meta[base + pos] = sm[k];
+            meta[base + pos] = (unsigned short)(m & 0x7FFFu);
         }
         pa += __popc(ba);
         pi += __popc(bi);
