@@ -298,6 +298,7 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
     NL* nl = reinterpret_cast<NL*>(*inout);
     int rc;
     int rebuilt = 0;
+    bool static_uploaded = false;
     bool fresh = nl == nullptr || !list_belongs(ctx, nl) || nl->N != N || nl->r_cut != params->r_cut || nl->skin != skin ||
                  nl->box[0] != box[0] || nl->box[1] != box[1] || nl->box[2] != box[2] || nl->n_excl != n_excl ||
                  nl->st_ref.p == nullptr;
@@ -309,6 +310,14 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
         rc = needs_rebuild_impl(ctx, nl->st_pos.p, nl->st_ref.p, N, skin, (int32_t*)nl->st_flag.p, s);
         if (rc) return rc;
         DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 33, nl->st_flag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
+        // the other per-step inputs go up while the host waits for the flag
+        if (nl->st_charge.p && nl->st_type.p && nl->st_lj.p && nl->st_charge.bytes >= (size_t)N * rs &&
+            nl->st_type.bytes >= (size_t)N * sizeof(int) && nl->st_lj.bytes >= (size_t)ntypes * ntypes * 2 * sizeof(double)) {
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
+            static_uploaded = true;
+        }
         DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
         flag = ctx->h_pinned[33];
         fresh = flag != 0;
@@ -354,9 +363,11 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
     if ((rc = ensure(ctx, nl->st_lj, (size_t)ntypes * ntypes * 2 * sizeof(double), s))) return rc;
     if ((rc = ensure(ctx, nl->st_F, 3 * (size_t)N * rs, s))) return rc;
     if ((rc = ensure(ctx, nl->st_EW, 16 * sizeof(double), s))) return rc;
-    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
-    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
-    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
+    if (!static_uploaded) {
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
+    }
     double* EW = (double*)nl->st_EW.p;
     rc = nonbonded_impl(ctx, nl, nl->st_pos.p, nl->st_charge.p, (const int32_t*)nl->st_type.p, (const double*)nl->st_lj.p, ntypes,
                         params, nl->st_F.p, EW, EW + 4, s);
