@@ -190,13 +190,11 @@ template <int METHOD>
 __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x2_kernel(ForceParams<float> P)
 {
     __shared__ float4 off_s[27];
-    __shared__ int act_s[MAX_TYPES];
     __shared__ int ti_s[FX_WARPS][UNIT];  // type * nt of the warp's current i-atoms
     extern __shared__ __align__(16) unsigned char dyn_smem[];
     float4* ljt = reinterpret_cast<float4*>(dyn_smem);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
 
     for (int t = threadIdx.x; t < P.nt * P.nt; t += blockDim.x) ljt[t] = P.lj4[t];
-    for (int t = threadIdx.x; t < P.nt; t += blockDim.x) act_s[t] = P.row_active[t];
     if (threadIdx.x < 27) {  // NEGATED image offsets: the kernel works with -x_j
         const int c = threadIdx.x;
         off_s[c] = make_float4(-(float)(c / 9 - 1) * P.h[0], -(float)((c / 3) % 3 - 1) * P.h[1], -(float)(c % 3 - 1) * P.h[2], 0.f);
