@@ -113,6 +113,42 @@ def test_no_exclusions_and_zero_skin_f64():
     run_case(sub, "f64", 1.0, 0.0, "rf")
 
 
+def _mixture_box(n_side, edge, seed):
+    """A non-water workload for the same path: point particles of three LJ types (one without LJ) with random
+    charges (neutral in total) on a jittered lattice with vacancies, and a random exclusion list between lattice
+    neighbours.  Units then mix types freely, some atoms have no exclusions and rows differ widely in length."""
+    import dataclasses
+
+    rng = np.random.default_rng(seed)
+    a = edge / n_side
+    sites = np.stack(np.meshgrid(*[np.arange(n_side)] * 3, indexing="ij"), axis=-1).reshape(-1, 3)
+    keep = rng.random(sites.shape[0]) > 0.15
+    sites = sites[keep]
+    n = sites.shape[0]
+    pos = ((sites + 0.5) * a + rng.uniform(-0.06, 0.06, size=(n, 3))) % edge
+    pos = pos.astype(np.float32)
+    charge = rng.choice(np.array([-0.6, -0.2, 0.0, 0.3, 0.5]), size=n)
+    charge -= charge.mean()
+    typ = rng.integers(0, 3, size=n).astype(np.int32)
+    cand = np.arange(0, n - 1, dtype=np.int32)
+    pick = cand[rng.random(cand.size) < 0.3]
+    excl = np.stack([pick, pick + 1], axis=1).astype(np.int32)
+    base = wl.make_water_box(2, 5.0, 3)
+    box = np.array([np.float32(edge)] * 3, dtype=np.float64)
+    return dataclasses.replace(base, box=box, pos=pos, charge=charge.astype(np.float32), type=typ,
+                               sigma=np.array([0.28, 0.22, 0.0]), epsilon=np.array([0.6, 0.3, 0.0]), excl_pairs=excl,
+                               mass=np.ones(n))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,method", [("f32", "rf"), ("f32", "ewald"), ("mixed", "rf"), ("f64", "ewald")])
+def test_three_type_mixture_with_vacancies(precision, method):
+    """Generality of the list and of both pair kernels beyond water: see _mixture_box."""
+    wb = _mixture_box(16, 4.6, 2024)
+    rep = run_case(wb, precision, 1.0, 0.1, method)
+    assert rep["stats"]["pbc_mode"] == 0  # 4 cells per axis: the packed-FP32 kernel for f32, the generic one otherwise
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)
