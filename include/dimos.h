@@ -86,6 +86,9 @@ typedef struct {
     double alpha;         /* Ewald splitting parameter, nm^-1 (DIMOS_EWALD_REAL) */
     double coulomb_const; /* k_e = 1/(4 pi eps0), kJ mol^-1 nm e^-2 (138.935456, reading C-2) */
     int32_t method;       /* dimos_method */
+    double r_switch;      /* LJ switching distance r_s of Eq. 6: for r_s < r < r_c the LJ term is
+                           * multiplied by S(x) = 1 - 6x^5 + 15x^4 - 10x^3, x = (r - r_s)/(r_c - r_s); Coulomb terms are
+                           * not switched.  <= 0 or >= r_cut: plain truncation at r_cut (reading C-8).  NaN: EINVAL */
 } dimos_nb_params;
 
 typedef struct {

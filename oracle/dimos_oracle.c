@@ -22,6 +22,7 @@
  *   cell list, cells >= r_nl, neighbouring cells .......... PAPER.md:177
  *   Lennard-Jones 12-6, Eq. (4) ........................... PAPER.md:189-191
  *   Lorentz-Berthelot combining rules, Eq. (5) ............ PAPER.md:193-196
+ *   LJ switching function S(x), Eq. (6) (optional, r_switch) PAPER.md:198-202
  *   Coulomb, Eq. (7) ...................................... PAPER.md:204-206
  *   reaction field, Eq. (8) with k_RFA, c_RFA ............. PAPER.md:208-213
  *   Ewald direct-space term, Eq. (10), n = 0 image only ... PAPER.md:215-223
@@ -64,6 +65,7 @@ typedef struct {
     double alpha;
     double coulomb_const; /* k_e = 1/(4 pi eps0) in kJ mol^-1 nm e^-2 */
     int32_t method;
+    double r_switch;      /* LJ switching distance r_s of Eq. 6; <= 0 or >= r_cut: plain truncation */
 } orc_params;
 
 int orc_num_threads(void)
@@ -114,6 +116,16 @@ static void pair_terms(double r2, double qq, double sigma, double eps, const orc
     double ke_qq = p->coulomb_const * qq;
     *e_lj = 4.0 * eps * (sr12 - sr6);
     double f = 24.0 * eps * (2.0 * sr12 - sr6) / r2;
+    if (p->r_switch > 0.0 && p->r_switch < p->r_cut && r > p->r_switch) {
+        /* Eq. 6: U_LJ -> S(x) U_LJ, x = (r - r_s)/(r_c - r_s), S = 1 - 6x^5 + 15x^4 - 10x^3;
+         * -d(S U)/dr = S (-U') - S'(x) U / (r_c - r_s), S'(x) = -30x^4 + 60x^3 - 30x^2 */
+        double w = p->r_cut - p->r_switch;
+        double x = (r - p->r_switch) / w;
+        double S = 1.0 - 6.0 * x * x * x * x * x + 15.0 * x * x * x * x - 10.0 * x * x * x;
+        double dS = -30.0 * x * x * x * x + 60.0 * x * x * x - 30.0 * x * x;
+        f = S * f - dS / w * (*e_lj) / r;
+        *e_lj = S * (*e_lj);
+    }
     if (p->method == ORC_METHOD_RF) {
         double k_rf, c_rf;
         rf_constants(p, &k_rf, &c_rf);

@@ -23,6 +23,7 @@ class _Params(ctypes.Structure):
         ("alpha", ctypes.c_double),
         ("coulomb_const", ctypes.c_double),
         ("method", ctypes.c_int32),
+        ("r_switch", ctypes.c_double),
     ]
 
 
@@ -94,15 +95,16 @@ class NonbondedResult:
 
 
 def nonbonded(pos, charge, type_, lj_table, box, r_cut, *, method=METHOD_RF, eps_rf=78.5, alpha=3.12,
-              coulomb_const=138.935456, excl_pairs=None, band=0.0, algorithm="celllist") -> NonbondedResult:
-    """Forces, energy components and virial for one configuration.  algorithm: 'bruteforce' | 'celllist'."""
+              coulomb_const=138.935456, excl_pairs=None, band=0.0, algorithm="celllist", r_switch=0.0) -> NonbondedResult:
+    """Forces, energy components and virial for one configuration.  algorithm: 'bruteforce' | 'celllist'.
+    r_switch: LJ switching distance r_s of Eq. 6; 0 = plain truncation at r_cut."""
     lib = _load()
     pos, charge, type_, box = _d(pos), _d(charge), _i(type_), _d(box)
     lj_table = _d(lj_table)
     n = pos.shape[0]
     nt = lj_table.shape[0]
     excl = _i(excl_pairs if excl_pairs is not None else np.zeros((0, 2), np.int32)).reshape(-1, 2)
-    params = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), int(method))
+    params = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), int(method), float(r_switch))
     F = np.zeros((n, 3), dtype=np.float64)
     E = np.zeros(4, dtype=np.float64)
     W = np.zeros(9, dtype=np.float64)

@@ -44,7 +44,7 @@ class _Allocator(ctypes.Structure):
 
 class _Params(ctypes.Structure):
     _fields_ = [("r_cut", ctypes.c_double), ("eps_rf", ctypes.c_double), ("alpha", ctypes.c_double),
-                ("coulomb_const", ctypes.c_double), ("method", ctypes.c_int32)]
+                ("coulomb_const", ctypes.c_double), ("method", ctypes.c_int32), ("r_switch", ctypes.c_double)]
 
 
 class _Stats(ctypes.Structure):
@@ -234,11 +234,12 @@ class Context:
         self._check(rc)
         return bool(host.value) if sync else self._flag
 
-    def _params(self, nl, method, eps_rf, alpha, coulomb_const):
-        return _Params(float(nl.r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method] if isinstance(method, str) else int(method))
+    def _params(self, nl, method, eps_rf, alpha, coulomb_const, r_switch=0.0):
+        return _Params(float(nl.r_cut), float(eps_rf), float(alpha), float(coulomb_const),
+                       _METHODS[method] if isinstance(method, str) else int(method), float(r_switch))
 
     def nonbonded(self, nl: NeighborList, pos, charge, type_, lj_table, *, method="rf", eps_rf=78.5, alpha=3.12,
-                  coulomb_const=138.935456, F=None, E=None, virial=None):
+                  coulomb_const=138.935456, r_switch=0.0, F=None, E=None, virial=None):
         """dimos_nonbonded: returns (F (N,3) real, E (4,) float64, virial (3,3) float64) device tensors."""
         pos = self._dev(pos, self.real, 3)
         n = pos.shape[0]
@@ -252,7 +253,7 @@ class Context:
         F = torch.empty_like(pos) if F is None else self._dev(F, self.real, 3)
         E = torch.empty(4, dtype=torch.float64, device=dev) if E is None else self._dev(E, torch.float64)
         virial = torch.empty(3, 3, dtype=torch.float64, device=dev) if virial is None else self._dev(virial, torch.float64)
-        prm = self._params(nl, method, eps_rf, alpha, coulomb_const)
+        prm = self._params(nl, method, eps_rf, alpha, coulomb_const, r_switch)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_nonbonded(self.handle, nl.handle, pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
                                           lj_table.data_ptr(), nt, _box3(nl.box), ctypes.byref(prm), F.data_ptr(),
@@ -261,12 +262,12 @@ class Context:
         return F, E, virial
 
     def nonbonded_host(self, nl: NeighborList, pos, charge, type_, lj_table, F, E, virial, *, method="rf", eps_rf=78.5,
-                       alpha=3.12, coulomb_const=138.935456):
+                       alpha=3.12, coulomb_const=138.935456, r_switch=0.0):
         """dimos_nonbonded_host: all arrays are HOST tensors (pinned recommended); synchronises."""
         for t in (pos, charge, type_, lj_table, F, E, virial):
             if t.is_cuda or not t.is_contiguous():
                 raise ValueError("nonbonded_host takes contiguous host tensors")
-        prm = self._params(nl, method, eps_rf, alpha, coulomb_const)
+        prm = self._params(nl, method, eps_rf, alpha, coulomb_const, r_switch)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_nonbonded_host(self.handle, nl.handle, pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
                                                lj_table.data_ptr(), lj_table.shape[0], _box3(nl.box), ctypes.byref(prm),
@@ -275,12 +276,12 @@ class Context:
         return F, E, virial
 
     def step_host(self, nl: "NeighborList | None", pos, charge, type_, lj_table, box, r_cut, skin, excl_pairs, F, E, virial, *,
-                  method="rf", eps_rf=78.5, alpha=3.12, coulomb_const=138.935456):
+                  method="rf", eps_rf=78.5, alpha=3.12, coulomb_const=138.935456, r_switch=0.0):
         """dimos_step_host: HOST tensors in and out; returns (NeighborList, rebuilt: bool)."""
         for t in (pos, charge, type_, lj_table, F, E, virial) + ((excl_pairs,) if excl_pairs is not None else ()):
             if t.is_cuda or not t.is_contiguous():
                 raise ValueError("step_host takes contiguous host tensors")
-        prm = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method])
+        prm = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method], float(r_switch))
         h = ctypes.c_void_p(nl.handle.value if nl is not None else None)
         rebuilt = ctypes.c_int32(0)
         n_excl = 0 if excl_pairs is None else excl_pairs.shape[0]

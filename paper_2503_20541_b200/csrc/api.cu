@@ -226,6 +226,7 @@ static int check_nb_args(Ctx* ctx, const NL* nl, int32_t ntypes, const double* b
     if (box[0] != nl->box[0] || box[1] != nl->box[1] || box[2] != nl->box[2]) return set_error(ctx, DIMOS_ESTALE, "box differs from the build box");
     if (p->r_cut != nl->r_cut) return set_error(ctx, DIMOS_ESTALE, "r_cut differs from the build r_cut");
     if (!(p->coulomb_const >= 0) || !isfinite(p->coulomb_const)) return set_error(ctx, DIMOS_EINVAL, "bad coulomb_const");
+    if (p->r_switch != p->r_switch) return set_error(ctx, DIMOS_EINVAL, "r_switch is NaN");
     if (p->method == DIMOS_RF && !(2.0 * p->eps_rf + 1.0 != 0.0)) return set_error(ctx, DIMOS_EINVAL, "bad eps_rf");
     if (p->method == DIMOS_EWALD_REAL && !(p->alpha > 0)) return set_error(ctx, DIMOS_EINVAL, "alpha must be > 0");
     return DIMOS_OK;

@@ -204,8 +204,21 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
         if (LJ) {                                                                                    \
             const real4 cc = ljt[ti[i] + tj];                   /* c6, c12, 6 c6, 12 c12 */          \
             const real rinv6 = rinv2 * rinv2 * rinv2;                                                \
-            e_lj = fma_acc(fma_r(cc.y, rinv6, -cc.x), rinv6, e_lj);   /* Eq. 4 */                    \
-            fr2 = fma_r(fma_r(cc.w, rinv6, -cc.z), rinv6, fr2);                                      \
+            real elj = fma_r(cc.y, rinv6, -cc.x) * rinv6;       /* Eq. 4 */                          \
+            real flj = fma_r(cc.w, rinv6, -cc.z) * rinv6;       /* r (-dU/dr) */                     \
+            if (P.sw_on) {                                      /* Eq. 6: U -> S(x) U */             \
+                const real r_ = r2 * rinv;                                                           \
+                const real x_ = (r_ - P.rs) * P.inv_sw;                                              \
+                if (x_ > (real)0) {                                                                  \
+                    const real x2_ = x_ * x_, xm_ = x_ - (real)1;                                    \
+                    const real S_ = fma_r(fma_r(fma_r((real)-6, x_, (real)15), x_, (real)-10), x2_ * x_, (real)1); \
+                    const real dS_ = (real)-30 * x2_ * xm_ * xm_ * P.inv_sw;                         \
+                    flj = S_ * flj - dS_ * elj * r_;                                                 \
+                    elj = S_ * elj;                                                                  \
+                }                                                                                    \
+            }                                                                                        \
+            e_lj = e_lj + (acc_t)elj;                                                                \
+            fr2 += flj;                                                                              \
         }                                                                                            \
         const real fs = fr2 * rinv2;                                                                 \
         fix[i] = fma_r(fs, ddx, fix[i]); fiy[i] = fma_r(fs, ddy, fiy[i]); fiz[i] = fma_r(fs, ddz, fiz[i]); \
@@ -608,6 +621,9 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     P.krf = (real)((prm->eps_rf - 1.0) / ((2.0 * prm->eps_rf + 1.0) * rc_ * rc_ * rc_));  // Eq. 8 constants, reading C-1
     P.m2krf = (real)-2 * P.krf;
     P.crf = (real)(3.0 * prm->eps_rf / ((2.0 * prm->eps_rf + 1.0) * rc_));
+    P.sw_on = (prm->r_switch > 0.0 && prm->r_switch < rc_) ? 1 : 0;  // Eq. 6; otherwise plain truncation (reading C-8)
+    P.rs = (real)prm->r_switch;
+    P.inv_sw = P.sw_on ? (real)(1.0 / (rc_ - prm->r_switch)) : (real)0;
     P.alpha = (real)prm->alpha;
     P.two_a_sqrtpi = (real)(2.0 * prm->alpha / sqrt(M_PI));
     for (int a = 0; a < 3; ++a) { P.L[a] = (real)nl->grid.L[a]; P.invL[a] = (real)(1.0 / nl->grid.L[a]); P.h[a] = (real)nl->grid.h[a]; }

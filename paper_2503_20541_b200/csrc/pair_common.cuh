@@ -45,6 +45,8 @@ struct ForceParams {
     real4* Fown;
     double* partials;        // [gridDim.x][N_PART]
     real rc2, ke, krf, m2krf, crf, alpha, two_a_sqrtpi;
+    real rs, inv_sw;  // LJ switch (Eq. 6): r_s and 1/(r_c - r_s)
+    int sw_on;
     real L[3], invL[3], h[3];
 };
 

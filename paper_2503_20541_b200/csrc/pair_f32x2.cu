@@ -43,6 +43,7 @@ struct UnitRegs {
 struct Consts {
     float rc2, krf, m2krf, mcrf;   // reaction field
     float alpha, two_a_sqrtpi;     // Ewald real space
+    float rs, inv_sw;              // LJ switch, Eq. 6: r_s and 1/(r_c - r_s)
 };
 
 __device__ __forceinline__ float rcp_f(float x)
@@ -77,7 +78,7 @@ __device__ __forceinline__ void erfc_exp2(float2 x, float2& erfc_x, float2& exp_
 // One chunk: the lane's j-atom against the 8 i-atoms, two i-atoms per packed instruction.
 //   MASKED: honour the entry's i-mask (exclusions, intra-unit half, padding); LJ: evaluate Eq. 4 for the
 //   i-pairs flagged in lj_pairs.  Returns F_j = -sum_i fs_i * d_i.
-template <int METHOD, bool MASKED, bool LJ>
+template <int METHOD, bool SW, bool MASKED, bool LJ>
 __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const float4* __restrict__ ljt, const int* __restrict__ ti, float nxj,
                                            float nyj, float nzj, float qj, int tj, unsigned mask, unsigned lj_pairs,
                                            float& sx, float& sy, float& sz)
@@ -133,9 +134,29 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
                 rinv6.x = in_a ? rinv6.x : 0.f;
                 rinv6.y = in_b ? rinv6.y : 0.f;
                 const float2 e6 = __ffma2_rn(f2(ca.y, cb.y), rinv6, f2(-ca.x, -cb.x));   // c12 r^-6 - c6
-                u.e_lj = __ffma2_rn(e6, rinv6, u.e_lj);                                   // Eq. 4
                 const float2 p6 = __ffma2_rn(f2(ca.w, cb.w), rinv6, f2(-ca.z, -cb.z));   // 12 c12 r^-6 - 6 c6
-                fs = __ffma2_rn(__fmul2_rn(p6, rinv6), rinvsq, fs);
+                if (!SW) {
+                    u.e_lj = __ffma2_rn(e6, rinv6, u.e_lj);                               // Eq. 4
+                    fs = __ffma2_rn(__fmul2_rn(p6, rinv6), rinvsq, fs);
+                } else {
+                    // Eq. 6: U_LJ -> S(x) U_LJ, x = (r - r_s)/(r_c - r_s) clamped at 0 (S(0) = 1, S'(0) = 0);
+                    // r F = S (r F_LJ) - r S'(x)/(r_c - r_s) U_LJ
+                    float2 elj = __fmul2_rn(e6, rinv6);
+                    float2 flj = __fmul2_rn(p6, rinv6);
+                    const float2 r = __fmul2_rn(r2, rinv);
+                    float2 x = __fmul2_rn(__fadd2_rn(r, bc(-k.rs)), bc(k.inv_sw));
+                    x = f2(fmaxf(x.x, 0.f), fmaxf(x.y, 0.f));
+                    const float2 x2 = __fmul2_rn(x, x);
+                    float2 S = __ffma2_rn(bc(-6.f), x, bc(15.f));
+                    S = __ffma2_rn(S, x, bc(-10.f));
+                    S = __ffma2_rn(S, __fmul2_rn(x2, x), bc(1.f));
+                    const float2 xd = __fmul2_rn(x, __fadd2_rn(x, bc(-1.f)));             // x (x - 1)
+                    const float2 dS = __fmul2_rn(__fmul2_rn(xd, xd), bc(-30.f * k.inv_sw)); // S'(x)/(r_c - r_s)
+                    flj = __ffma2_rn(S, flj, __fmul2_rn(__fmul2_rn(dS, elj), f2(-r.x, -r.y)));
+                    elj = __fmul2_rn(S, elj);
+                    u.e_lj = __fadd2_rn(u.e_lj, elj);
+                    fs = __ffma2_rn(flj, rinvsq, fs);
+                }
             }
         }
         u.fx[p] = __ffma2_rn(fs, dx, u.fx[p]);
@@ -174,11 +195,11 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
         float sx, sy, sz;                                                                                        \
         if ((unsigned)((C) - c_plain) < n_plain) { /* warp-uniform: full chunk of a full unit, all masks 0xFF */ \
             if (lj_pairs != 0u && __any_sync(FULL, (TJ & STYPE_ACTIVE) != 0))                                    \
-                chunk_body<METHOD, false, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, lj_pairs, sx, sy, sz);  \
+                chunk_body<METHOD, SW, false, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, lj_pairs, sx, sy, sz);  \
             else                                                                                                 \
-                chunk_body<METHOD, false, false>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, 0u, sx, sy, sz);       \
+                chunk_body<METHOD, SW, false, false>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, 0u, sx, sy, sz);       \
         } else {                                                                                                 \
-            chunk_body<METHOD, true, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, mk & 0xFFu, lj_pairs, sx, sy, sz);  \
+            chunk_body<METHOD, SW, true, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, mk & 0xFFu, lj_pairs, sx, sy, sz);  \
         }                                                                                                        \
         /* virial: x_j' (x) F_j in unit-local coordinates, x_j' = -nxj */                                        \
         w[0] = fmaf(-nxj, sx, w[0]); w[1] = fmaf(-nxj, sy, w[1]); w[2] = fmaf(-nxj, sz, w[2]);                   \
@@ -186,7 +207,7 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
         red_add_xyz(P.Facc + jc, sx, sy, sz);                                                                    \
     } while (0)
 
-template <int METHOD>
+template <int METHOD, bool SW>
 __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x2_kernel(ForceParams<float> P)
 {
     __shared__ float4 off_s[27];
@@ -211,6 +232,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     Consts k;
     k.rc2 = P.rc2; k.krf = P.krf; k.m2krf = P.m2krf; k.mcrf = -P.crf;
     k.alpha = P.alpha; k.two_a_sqrtpi = P.two_a_sqrtpi;
+    k.rs = P.rs; k.inv_sw = P.inv_sw;
 
     long long U = 0, U_next = 0;
     if (lane == 0) U = (long long)atomicAdd(P.unit_counter, 1ull);
@@ -368,16 +390,22 @@ void launch_reorder_rows(int* jslot, unsigned short* meta, const int2* row_info,
     reorder_rows_kernel<<<nb, RO_WARPS * 32, smem, s>>>(jslot, meta, row_info, stype, n_units, row_cap, m_res);
 }
 
+template <int METHOD, bool SW>
+static void launch_one(const ForceParams<float>& P, unsigned nb, size_t dyn, cudaStream_t s)
+{
+    if (dyn > 48 * 1024)
+        cudaFuncSetAttribute(pair_force_f32x2_kernel<METHOD, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    pair_force_f32x2_kernel<METHOD, SW><<<nb, FX_WARPS * 32, dyn, s>>>(P);
+}
+
 bool launch_pair_force_f32x2(const ForceParams<float>& P, int method, unsigned nb, size_t dyn, cudaStream_t s)
 {
     if (method == DIMOS_RF) {
-        if (dyn > 48 * 1024)
-            cudaFuncSetAttribute(pair_force_f32x2_kernel<DIMOS_RF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-        pair_force_f32x2_kernel<DIMOS_RF><<<nb, FX_WARPS * 32, dyn, s>>>(P);
+        if (P.sw_on) launch_one<DIMOS_RF, true>(P, nb, dyn, s);
+        else launch_one<DIMOS_RF, false>(P, nb, dyn, s);
     } else if (method == DIMOS_EWALD_REAL) {
-        if (dyn > 48 * 1024)
-            cudaFuncSetAttribute(pair_force_f32x2_kernel<DIMOS_EWALD_REAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-        pair_force_f32x2_kernel<DIMOS_EWALD_REAL><<<nb, FX_WARPS * 32, dyn, s>>>(P);
+        if (P.sw_on) launch_one<DIMOS_EWALD_REAL, true>(P, nb, dyn, s);
+        else launch_one<DIMOS_EWALD_REAL, false>(P, nb, dyn, s);
     } else {
         return false;
     }

@@ -149,6 +149,35 @@ def test_three_type_mixture_with_vacancies(precision, method):
     assert rep["stats"]["pbc_mode"] == 0  # 4 cells per axis: the packed-FP32 kernel for f32, the generic one otherwise
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,method", [("f32", "rf"), ("f32", "ewald"), ("mixed", "rf"), ("f64", "rf")])
+def test_lj_switching_function(precision, method):
+    """LJ switching function S(x) of Eq. 6 between r_s = 0.8 nm and r_c = 1.0 nm: water (LJ on O
+    only) and the three-type mixture, on the packed-FP32 kernel (f32) and on the generic one (mixed, f64)."""
+    rep_w = run_case(wl.make_config(1), precision, 1.0, 0.1, method, r_switch=0.8, check_set=False)
+    rep_m = run_case(_mixture_box(16, 4.6, 99), precision, 1.0, 0.1, method, r_switch=0.75, check_set=False)
+    assert rep_w["n_pairs_cut"] > 0 and rep_m["n_pairs_cut"] > 0
+
+
+def test_lj_switch_outside_range_is_plain_truncation_f32():
+    """r_switch <= 0 or >= r_cut means no switching (include/dimos.h); NaN is rejected."""
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        ref = [t.clone() for t in dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)]
+        for rs in (-1.0, 1.0, 2.5):
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, r_switch=rs)
+            assert abs(float(E[1] - ref[1][1])) <= 1e-9 * abs(float(ref[1][1]))
+        Fs, Es, _ = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, r_switch=0.8)
+        assert float(Es[1]) != float(ref[1][1]) and abs(float(Es[2] - ref[1][2])) <= 1e-9 * abs(float(ref[1][2]))
+        with pytest.raises(Exception):
+            dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, r_switch=float("nan"))
+    finally:
+        ctx.close()
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)

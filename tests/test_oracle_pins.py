@@ -348,3 +348,56 @@ def test_verlet_list_validity_invariant():
     now = oracle.neighbor_pairs(pos1, wb.box, rc, wb.excl_pairs, "bruteforce")
     now_key = set((now[:, 0].astype(np.int64) * n + now[:, 1]).tolist())
     assert now_key <= listed_key
+
+
+# --- LJ switching function, Eq. (6) ---------------------------------------------------------
+def test_lj_switch_special_values():
+    """S(x) = 1 - 6x^5 + 15x^4 - 10x^3 with x = (r - r_s)/(r_c - r_s): S = 1 below r_s, S(1/2) = 1/2 exactly with
+    S'(1/2) = -15/8, S(1) = S'(1) = 0.  Checked against the plain potential, which the closed forms above pin."""
+    rs, rc = 0.8, 1.0
+    for r in (0.35, 0.6, 0.7999):  # below r_s: identical to the unswitched potential
+        a, fa = two_particles("O", "O", r, rc, r_switch=rs)
+        b, fb = two_particles("O", "O", r, rc)
+        assert a.E[1] == b.E[1] and fa == fb
+    plain, f_plain = two_particles("O", "O", 0.9, rc)
+    sw, f_sw = two_particles("O", "O", 0.9, rc, r_switch=rs)
+    assert sw.E[1] == pytest.approx(0.5 * plain.E[1], rel=1e-14)
+    assert sw.E[2] == plain.E[2]  # Coulomb untouched
+    # the neutral LJ-only pair isolates the LJ force: F = S F_LJ - S'(x)/(r_c - r_s) U_LJ = F_LJ/2 + (15/8)/0.2 U_LJ
+    z_plain, fz_plain = _lj_only_pair(0.9, rc, 0.0)
+    z_sw, fz_sw = _lj_only_pair(0.9, rc, rs)
+    assert fz_sw == pytest.approx(0.5 * fz_plain + (15.0 / 8.0) / (rc - rs) * z_plain.E[1], rel=1e-13)
+    assert f_sw - f_plain == pytest.approx(fz_sw - fz_plain, rel=1e-9)  # and the charged pair differs by the same amount
+    # at the cutoff both the energy and the force vanish like (1 - x)^3 and (1 - x)^2
+    near, f_near = _lj_only_pair(rc - 1e-7, rc, rs)
+    assert abs(near.E[1]) < 1e-18 and abs(f_near) < 1e-12
+
+
+def _lj_only_pair(r, r_cut, r_switch):
+    u = np.array([0.6, 0.0, 0.8])
+    pos = np.array([[10.0, 11.0, 12.0] + r * u, [10.0, 11.0, 12.0]])
+    res = oracle.nonbonded(pos, [0.0, 0.0], [0, 0], lj_table(), BIGBOX, r_cut, algorithm="bruteforce", r_switch=r_switch)
+    return res, float(res.F[0] @ u)
+
+
+def test_lj_switch_forces_are_minus_gradient_and_continuous():
+    """Finite-difference gradient through the whole switching interval, and continuity of U and F at r_s."""
+    rs, rc = 0.75, 1.0
+    h = 1e-6
+    for r in np.linspace(0.70, 0.999, 14):
+        e = lambda rr: _lj_only_pair(rr, rc, rs)[0].E[1]
+        f = _lj_only_pair(r, rc, rs)[1]
+        assert f == pytest.approx(-(e(r + h) - e(r - h)) / (2 * h), rel=5e-6, abs=1e-9)
+    lo, f_lo = _lj_only_pair(rs - 1e-9, rc, rs)
+    hi, f_hi = _lj_only_pair(rs + 1e-9, rc, rs)
+    assert hi.E[1] == pytest.approx(lo.E[1], rel=1e-7) and f_hi == pytest.approx(f_lo, rel=1e-6)
+
+
+def test_lj_switch_many_body_cell_list_equals_bruteforce():
+    wb = small_box()
+    lj = lj_table()
+    a = oracle.nonbonded(wb.pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs, algorithm="bruteforce", r_switch=0.8)
+    b = oracle.nonbonded(wb.pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs, algorithm="celllist", r_switch=0.8)
+    c = oracle.nonbonded(wb.pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs, algorithm="celllist")
+    assert np.abs(a.F - b.F).max() < 1e-9 and a.E[1] == pytest.approx(b.E[1], rel=1e-13)
+    assert a.E[1] != c.E[1] and a.E[2] == pytest.approx(c.E[2], rel=1e-13)
