@@ -338,6 +338,41 @@ static void add_exclusion_correction(int64_t N, const double* pos, const double*
     E[3] = e_sum;
 }
 
+/* 1-4 exceptions ("scale the strength of the non-bonded interactions by some common factor", or an
+ * individual factor per pair; "handled explicitly by the non-bonded interaction method").  Reading C-21 (the paper
+ * gives no formula): every exception pair is also an excluded pair, so the sums above skip it; it contributes
+ *   U = s_lj * 4 eps [(s/r)^12 - (s/r)^6]  (Eq. 4)  +  s_c * k_e q_i q_j / r  (Eq. 7)
+ * at its minimum-image distance, without cutoff, switch, reaction field or Ewald modification.
+ *   exc_pairs n_exc x 2 (i<j), exc_scale n_exc x 2 = (s_c, s_lj).  Adds into F, W, E[0], E[1] (LJ), E[2] (Coulomb). */
+int orc_add_exceptions(int64_t N, const double* pos, const double* charge, const int32_t* type, const double* lj_table,
+                       int32_t ntypes, const double* box, double coulomb_const, const int32_t* exc_pairs,
+                       const double* exc_scale, int64_t n_exc, double* F, double* E, double* W)
+{
+    (void)N;
+    for (int64_t k = 0; k < n_exc; ++k) {
+        int64_t i = exc_pairs[2 * k], j = exc_pairs[2 * k + 1];
+        double d[3];
+        for (int a = 0; a < 3; ++a) d[a] = min_image(pos[3 * i + a] - pos[3 * j + a], box[a]);
+        double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+        double r = sqrt(r2);
+        const double* sp = &lj_table[((int64_t)type[i] * ntypes + type[j]) * 2];
+        double sr = sp[0] / r, sr2 = sr * sr, sr6 = sr2 * sr2 * sr2, sr12 = sr6 * sr6;
+        double s_c = exc_scale[2 * k], s_lj = exc_scale[2 * k + 1];
+        double e_lj = s_lj * 4.0 * sp[1] * (sr12 - sr6);
+        double e_c = s_c * coulomb_const * charge[i] * charge[j] / r;
+        double f_over_r = s_lj * 24.0 * sp[1] * (2.0 * sr12 - sr6) / r2 + e_c / r2;
+        E[1] += e_lj;
+        E[2] += e_c;
+        E[0] += e_lj + e_c;
+        for (int a = 0; a < 3; ++a) {
+            F[3 * i + a] += f_over_r * d[a];
+            F[3 * j + a] -= f_over_r * d[a];
+            for (int b = 0; b < 3; ++b) W[3 * a + b] += d[a] * (f_over_r * d[b]);
+        }
+    }
+    return 0;
+}
+
 /* O(N^2) brute force: THE definition.
  *   pos N x 3, charge N, type N, lj_table ntypes x ntypes x 2 = (sigma_ab, eps_ab), box[3],
  *   excl_pairs n_excl x 2 (i<j, unique).

@@ -47,6 +47,8 @@ def _load():
             fn = getattr(lib, name)
             fn.argtypes = [i64, dp, dp, ctypes.c_double, ip, i64, ip, i64]
             fn.restype = i64
+        lib.orc_add_exceptions.argtypes = [i64, dp, dp, ip, dp, ctypes.c_int32, dp, ctypes.c_double, ip, dp, i64, dp, dp, dp]
+        lib.orc_add_exceptions.restype = ctypes.c_int
         lib.orc_needs_rebuild.argtypes = [i64, dp, dp, ctypes.c_double, dp]
         lib.orc_needs_rebuild.restype = ctypes.c_int
         lib.orc_lorentz_berthelot.argtypes = [dp, dp, ctypes.c_int32, dp]
@@ -95,9 +97,12 @@ class NonbondedResult:
 
 
 def nonbonded(pos, charge, type_, lj_table, box, r_cut, *, method=METHOD_RF, eps_rf=78.5, alpha=3.12,
-              coulomb_const=138.935456, excl_pairs=None, band=0.0, algorithm="celllist", r_switch=0.0) -> NonbondedResult:
+              coulomb_const=138.935456, excl_pairs=None, band=0.0, algorithm="celllist", r_switch=0.0,
+              exceptions=None) -> NonbondedResult:
     """Forces, energy components and virial for one configuration.  algorithm: 'bruteforce' | 'celllist'.
-    r_switch: LJ switching distance r_s of Eq. 6; 0 = plain truncation at r_cut."""
+    r_switch: LJ switching distance r_s of Eq. 6; 0 = plain truncation at r_cut.
+    exceptions: (pairs (n,2) int32 i<j, scale (n,2) float64 = (coulomb scale, LJ scale)) of 1-4 exceptions (PAPER.md:243,
+    reading C-21); every exception pair must also be listed in excl_pairs."""
     lib = _load()
     pos, charge, type_, box = _d(pos), _d(charge), _i(type_), _d(box)
     lj_table = _d(lj_table)
@@ -116,6 +121,16 @@ def nonbonded(pos, charge, type_, lj_table, box, r_cut, *, method=METHOD_RF, eps
             _dp(allow) if allow is not None else None, ctypes.byref(npairs))
     if rc != 0:
         raise MemoryError(f"oracle nonbonded failed rc={rc}")
+    if exceptions is not None:
+        ep = _i(exceptions[0]).reshape(-1, 2)
+        es = _d(exceptions[1]).reshape(-1, 2)
+        if ep.shape[0] != es.shape[0]:
+            raise ValueError("exceptions: pairs and scales differ in length")
+        have = set(map(tuple, excl.tolist()))
+        if any(tuple(p) not in have for p in ep.tolist()):
+            raise ValueError("every exception pair must also be an excluded pair")
+        lib.orc_add_exceptions(n, _dp(pos), _dp(charge), _ip(type_), _dp(lj_table), nt, _dp(box), float(coulomb_const),
+                               _ip(ep), _dp(es), ep.shape[0], _dp(F), _dp(E), _dp(W))
     return NonbondedResult(F, E, W.reshape(3, 3), int(npairs.value), allow)
 
 

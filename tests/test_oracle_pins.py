@@ -401,3 +401,63 @@ def test_lj_switch_many_body_cell_list_equals_bruteforce():
     c = oracle.nonbonded(wb.pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs, algorithm="celllist")
     assert np.abs(a.F - b.F).max() < 1e-9 and a.E[1] == pytest.approx(b.E[1], rel=1e-13)
     assert a.E[1] != c.E[1] and a.E[2] == pytest.approx(c.E[2], rel=1e-13)
+
+
+# --- 1-4 exceptions (reading C-21) -----------------------------------------------------------------
+def _exception_pair(kind_a, kind_b, r, s_c, s_lj, method=oracle.METHOD_RF):
+    u = np.array([0.48, -0.6, 0.64])
+    pos = np.array([[10.0, 11.0, 12.0] + r * u, [10.0, 11.0, 12.0]])
+    pair = np.array([[0, 1]], dtype=np.int32)
+    res = oracle.nonbonded(pos, [Q[kind_a], Q[kind_b]], [TYPE[kind_a], TYPE[kind_b]], lj_table(), BIGBOX, 1.0, method=method,
+                           excl_pairs=pair, exceptions=(pair, np.array([[s_c, s_lj]])), algorithm="bruteforce")
+    return res, float(res.F[0] @ u)
+
+
+def test_exception_is_scaled_bare_lj_plus_bare_coulomb():
+    """An exception pair contributes s_lj U_LJ (Eq. 4) + s_c k_e q q / r (Eq. 7) and nothing else.  The LJ part is
+    checked against the pinned pair potential; the bare Coulomb part through erfc + erf = 1: the Ewald real-space term
+    of the free pair minus the exclusion correction of the excluded pair IS k_e q q / r (and likewise the forces)."""
+    r = 0.31
+    free, f_free = two_particles("O", "O", r, 1.0)                                    # LJ + RF, pinned above
+    ew, f_ew = two_particles("O", "O", r, 1.0, method=oracle.METHOD_EWALD_REAL)       # LJ + erfc/r
+    corr, f_corr = two_particles("O", "O", r, 1.0, method=oracle.METHOD_EWALD_REAL, excluded=True)  # -erf/r
+    bare_e, bare_f = ew.E[2] - corr.E[3], (f_ew - f_corr)                              # includes the LJ force once
+    lj_e = free.E[1]
+    z, f_lj = _lj_only_pair(r, 1.0, 0.0)
+    for s_c, s_lj in ((1.0, 1.0), (0.5, 0.5), (0.8333, 0.5), (0.0, 1.0), (1.0, 0.0)):
+        res, f = _exception_pair("O", "O", r, s_c, s_lj)
+        assert res.E[1] == pytest.approx(s_lj * lj_e, rel=1e-11, abs=1e-15)  # r is rebuilt from rounded coordinates
+        assert res.E[2] == pytest.approx(s_c * bare_e, rel=1e-12, abs=1e-12)
+        assert res.E[3] == 0.0 and res.E[0] == pytest.approx(res.E[1] + res.E[2], rel=1e-15)
+        assert f == pytest.approx(s_lj * f_lj + s_c * (bare_f - f_lj), rel=1e-11, abs=1e-9)
+    # under Ewald the pair is still an excluded pair: its -erf correction stays, the exception is added on top
+    res, _ = _exception_pair("O", "H", 0.2, 0.5, 0.0, method=oracle.METHOD_EWALD_REAL)
+    only_corr, _ = two_particles("O", "H", 0.2, 1.0, method=oracle.METHOD_EWALD_REAL, excluded=True)
+    assert res.E[3] == pytest.approx(only_corr.E[3], rel=1e-12) and res.E[2] != 0.0
+
+
+def test_exception_forces_are_minus_gradient_and_newton():
+    wb = small_box(m=20, edge=2.3, seed=8)
+    pos = wb.pos.astype(np.float64)
+    exc = wb.excl_pairs[::3].copy()  # a third of the intramolecular pairs become scaled exceptions
+    scale = np.tile(np.array([[0.8333, 0.5]]), (exc.shape[0], 1))
+    lj = oracle.lorentz_berthelot([wl.SIGMA_O, 0.1], [wl.EPS_O, 0.2])  # LJ on H too, so the LJ scale acts on O-H pairs
+
+    def en(p):
+        return oracle.nonbonded(p, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs, exceptions=(exc, scale),
+                                algorithm="bruteforce")
+
+    res = en(pos)
+    base = oracle.nonbonded(pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs, algorithm="bruteforce")
+    assert res.E[0] != base.E[0]
+    assert np.abs(res.F.sum(axis=0)).max() < 1e-9 and np.abs(res.W - res.W.T).max() < 1e-9
+    h = 1e-6
+    for i in (int(exc[0, 0]), int(exc[1, 1]), int(exc[-1, 0])):
+        for a in range(3):
+            p, m = pos.copy(), pos.copy()
+            p[i, a] += h
+            m[i, a] -= h
+            assert res.F[i, a] == pytest.approx(-(en(p).E[0] - en(m).E[0]) / (2 * h), rel=2e-6, abs=2e-4)
+    with pytest.raises(ValueError):  # an exception must also be an exclusion
+        oracle.nonbonded(pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs[1:],
+                         exceptions=(wb.excl_pairs[:1], np.array([[1.0, 1.0]])), algorithm="bruteforce")
