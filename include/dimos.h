@@ -210,6 +210,20 @@ DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
                                     int64_t* n_pairs_host, void* stream);
 
+/* dimos_nl_set_exceptions -- PAPER.md:243 ("1-4 exceptions ... scale the strength of the non-bonded interactions by
+ * some common factor", or an individual factor per pair; "handled explicitly by the non-bonded interaction method").
+ * Reading C-21 (the paper gives no formula): every exception pair must ALSO be one of the excluded pairs the list was
+ * built with, so the pair sums skip it (under DIMOS_EWALD_REAL it keeps the exclusion correction); dimos_nonbonded
+ * then adds, for every exception, s_lj * U_LJ(r) (Eq. 4) + s_c * k_e q_i q_j / r (Eq. 7) at the minimum-image distance,
+ * without cutoff, switch, reaction-field or Ewald modification, and the matching forces and virial.  The LJ part goes
+ * into E[1], the Coulomb part into E[2].
+ *   pairs   dev, n_exc x 2 int32, (i, j) with i < j, original atom indices; read (copied into the list)
+ *   scale   dev, n_exc x 2 double, (s_c, s_lj) per pair; read (copied)
+ *   n_exc   >= 0; 0 removes the exceptions.  The copy belongs to the list and survives rebuilds in place.
+ * Not checked: that the pairs are excluded pairs (the caller's precondition). */
+DIMOS_API int dimos_nl_set_exceptions(dimos_ctx* ctx, dimos_nl* nl, const int32_t* pairs, const double* scale,
+                                      int64_t n_exc, void* stream);
+
 /* Number of unordered, non-excluded pairs of the list with minimum-image r < radius at the build
  * positions, 0 < radius <= r_cut + skin (radius = r_cut gives the in-cutoff pair count the
  * throughput metric "pair interactions/s" is quoted on).  Synchronises the stream. */

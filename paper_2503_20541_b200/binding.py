@@ -28,7 +28,7 @@ EXPORTED_SYMBOLS = (
     "dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
     "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats", "dimos_launch_count",
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
-    "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host",
+    "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
 )
 
 
@@ -90,6 +90,7 @@ def load_library() -> ctypes.CDLL:
                                     ctypes.POINTER(_Params), vp, vp, vp, ctypes.POINTER(i32), vp]
     lib.dimos_step_host.restype = ctypes.c_int
     lib.dimos_nl_count_within.argtypes = [vp, vp, dbl, ctypes.POINTER(i64), vp]
+    lib.dimos_nl_set_exceptions.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -103,7 +104,8 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_version.restype = ctypes.c_char_p
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
-                 "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read"):
+                 "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
+                 "dimos_nl_set_exceptions"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -298,6 +300,22 @@ class Context:
             nl.handle = h
         return nl, bool(rebuilt.value)
 
+    def nl_set_exceptions(self, nl: NeighborList, pairs, scale):
+        """dimos_nl_set_exceptions: pairs (n,2) int32 i<j, scale (n,2) float64 = (Coulomb scale, LJ scale); None clears."""
+        if pairs is None or len(pairs) == 0:
+            with torch.cuda.device(self.device):
+                rc = self.lib.dimos_nl_set_exceptions(self.handle, nl.handle, None, None, 0, _stream_ptr())
+            self._check(rc)
+            return
+        pairs = self._dev(pairs, torch.int32, 2)
+        scale = self._dev(scale, torch.float64, 2)
+        if pairs.shape[0] != scale.shape[0]:
+            raise ValueError("exceptions: pairs and scales differ in length")
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_set_exceptions(self.handle, nl.handle, pairs.data_ptr(), scale.data_ptr(), pairs.shape[0],
+                                                  _stream_ptr())
+        self._check(rc)
+
     def nl_export_pairs(self, nl: NeighborList) -> torch.Tensor:
         """dimos_nl_export_pairs: (n,2) int32 device tensor of pairs i<j, order unspecified."""
         n = ctypes.c_int64(0)
@@ -358,6 +376,10 @@ def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = T
 
 def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
     return ctx.nonbonded(nl, pos, charge, type_, lj_table, **kw)
+
+
+def dimos_nl_set_exceptions(ctx: Context, nl: NeighborList, pairs, scale):
+    return ctx.nl_set_exceptions(nl, pairs, scale)
 
 
 def dimos_nl_export_pairs(ctx: Context, nl: NeighborList) -> torch.Tensor:

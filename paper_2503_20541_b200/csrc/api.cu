@@ -53,7 +53,7 @@ static void free_list(Ctx* ctx, NL* nl)
 {
     DevBuf* bufs[] = {&nl->cell_count, &nl->cell_start, &nl->unit_start, &nl->scan_tmp, &nl->atom_cell, &nl->atom_rank,
                       &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
-                      &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->jslot, &nl->meta, &nl->row_info,
+                      &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->jslot, &nl->meta, &nl->row_info,
                       &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials, &nl->accum,
                       &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW, &nl->st_ref, &nl->st_flag,
                       &nl->export_count};
@@ -65,7 +65,7 @@ static size_t list_workspace_bytes(const NL* nl)
 {
     const DevBuf* bufs[] = {&nl->cell_count, &nl->cell_start, &nl->unit_start, &nl->scan_tmp, &nl->atom_cell, &nl->atom_rank,
                             &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
-                            &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->jslot, &nl->meta,
+                            &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->jslot, &nl->meta,
                             &nl->row_info, &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials,
                             &nl->accum, &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW,
                             &nl->st_ref, &nl->st_flag, &nl->export_count};
@@ -401,6 +401,28 @@ DIMOS_API int dimos_nl_count_within(dimos_ctx* c, const dimos_nl* l, double radi
     if (!(radius > 0) || radius > nl->r_nl) return set_error(ctx, DIMOS_EINVAL, "radius must be in (0, r_cut + skin]");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
     return nl_export_impl(ctx, nl, nullptr, 0, n_pairs_host, radius, (cudaStream_t)stream);
+}
+
+DIMOS_API int dimos_nl_set_exceptions(dimos_ctx* c, dimos_nl* l, const int32_t* pairs, const double* scale, int64_t n_exc,
+                                      void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!l) return set_error(ctx, DIMOS_EINVAL, "NULL list");
+    NL* nl = reinterpret_cast<NL*>(l);
+    if (!list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");
+    if (n_exc < 0 || (n_exc > 0 && (!pairs || !scale))) return set_error(ctx, DIMOS_EINVAL, "bad exception list");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    nl->n_exc = 0;
+    if (n_exc == 0) return DIMOS_OK;
+    int rc;
+    if ((rc = ensure(ctx, nl->exc_pairs, (size_t)n_exc * 2 * sizeof(int32_t), s))) return rc;
+    if ((rc = ensure(ctx, nl->exc_scale, (size_t)n_exc * 2 * sizeof(double), s))) return rc;
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->exc_pairs.p, pairs, (size_t)n_exc * 2 * sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->exc_scale.p, scale, (size_t)n_exc * 2 * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    nl->n_exc = n_exc;
+    return DIMOS_OK;
 }
 
 DIMOS_API int dimos_profile_enable(dimos_ctx* c, int on)

@@ -91,6 +91,8 @@ struct NL {
     DevBuf unit_cell;  // int[n_units]
     DevBuf excl_start, excl_adj;  // CSR over both directions: int[N+1], int[2*n_excl]
     DevBuf excl_pairs;            // int2[n_excl] copy (Ewald exclusion correction)
+    DevBuf exc_pairs, exc_scale;  // 1-4 exceptions: int2[n_exc], double2[n_exc] = (Coulomb scale, LJ scale); survive rebuilds
+    int64_t n_exc = 0;
     DevBuf jslot;      // int[n_units*row_cap]
     DevBuf meta;       // uint16[n_units*row_cap]: mask | code<<8
     DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, leading mask-free chunks}

@@ -413,6 +413,68 @@ __global__ void excl_correction_kernel(const int2* __restrict__ pairs, int64_t n
 }
 
 // ------------------------------------------------------------------------------------------------
+// 1-4 exceptions (reading C-21): s_lj U_LJ (Eq. 4) + s_c k_e q_i q_j / r (Eq. 7) over a static pair list
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void exceptions_kernel(const int2* __restrict__ pairs, const double2* __restrict__ scale, int64_t n_exc,
+                                  const int* __restrict__ inv_perm, const typename vec4<real>::type* __restrict__ xyzq,
+                                  const int* __restrict__ stype, const double* __restrict__ ref,
+                                  const double* __restrict__ lj_table, int nt,
+                                  typename vec4<real>::type* __restrict__ Facc, double* __restrict__ partials, real ke,
+                                  double Lx, double Ly, double Lz)
+{
+    using real4 = typename vec4<real>::type;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // E_lj, E_coul, Wxx, Wxy, Wxz, Wyy, Wyz, Wzz
+    if (k < n_exc) {
+        const int2 p = pairs[k];
+        const double2 sc = scale[k];
+        const int si = inv_perm[p.x], sj = inv_perm[p.y];
+        const real4 a = xyzq[si], b = xyzq[sj];
+        // raw-coordinate difference formed in fp64 from cell-relative parts, then nearest image (C-3)
+        double ddx = ((double)a.x - (double)b.x) + (ref[3 * (int64_t)si] - ref[3 * (int64_t)sj]);
+        double ddy = ((double)a.y - (double)b.y) + (ref[3 * (int64_t)si + 1] - ref[3 * (int64_t)sj + 1]);
+        double ddz = ((double)a.z - (double)b.z) + (ref[3 * (int64_t)si + 2] - ref[3 * (int64_t)sj + 2]);
+        ddx -= Lx * rint(ddx / Lx);
+        ddy -= Ly * rint(ddy / Ly);
+        ddz -= Lz * rint(ddz / Lz);
+        const real dx = (real)ddx, dy = (real)ddy, dz = (real)ddz;
+        const real r2 = dx * dx + dy * dy + dz * dz;
+        const real rinv = (real)1 / sqrt(r2);
+        const real rinv2 = rinv * rinv;
+        const int ti = stype[si] & STYPE_MASK, tj = stype[sj] & STYPE_MASK;
+        const double sg = lj_table[2 * (ti * nt + tj)], ep = lj_table[2 * (ti * nt + tj) + 1];
+        const double s2 = sg * sg, s6 = s2 * s2 * s2;
+        const real c6 = (real)(4.0 * ep * s6), c12 = (real)(4.0 * ep * s6 * s6);
+        const real rinv6 = rinv2 * rinv2 * rinv2;
+        const real e_lj = (real)sc.y * (c12 * rinv6 - c6) * rinv6;
+        const real e_c = (real)sc.x * ke * a.w * b.w * rinv;
+        const real fs = ((real)sc.y * ((real)12 * c12 * rinv6 - (real)6 * c6) * rinv6 + e_c) * rinv2;
+        const real fx = fs * dx, fy = fs * dy, fz = fs * dz;
+        red_add_xyz(&Facc[si], fx, fy, fz);
+        red_add_xyz(&Facc[sj], -fx, -fy, -fz);
+        v[0] = (double)e_lj; v[1] = (double)e_c;
+        v[2] = (double)(dx * fx); v[3] = (double)(dx * fy); v[4] = (double)(dx * fz);
+        v[5] = (double)(dy * fy); v[6] = (double)(dy * fz); v[7] = (double)(dz * fz);
+    }
+    __shared__ double sh[8][8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    if (lane == 0)
+        for (int q = 0; q < 8; ++q) sh[wi][q] = v[q];
+    __syncthreads();
+    if (threadIdx.x < N_PART) {  // columns: E_lj, E_coul, W (6), E_excl
+        double sum = 0;
+        if (threadIdx.x < 8)
+            for (int ww = 0; ww < (int)(blockDim.x >> 5); ++ww) sum += sh[ww][threadIdx.x];
+        partials[(int64_t)blockIdx.x * N_PART + threadIdx.x] = sum;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // A6: finalize
 // ------------------------------------------------------------------------------------------------
 template <typename real>
@@ -591,7 +653,8 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     if ((rc = ensure(ctx, nl->Facc, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->Fown, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->lj, (size_t)MAX_TYPES * MAX_TYPES * 4 * sizeof(double) + MAX_TYPES * sizeof(int), s))) return rc;
-    if ((rc = ensure(ctx, nl->partials, (n_force_rows + (size_t)((nl->n_excl + 255) / 256) + 1) * N_PART * sizeof(double), s))) return rc;
+    const unsigned nb_exc = nl->n_exc > 0 ? (unsigned)((nl->n_exc + 255) / 256) : 0;
+    if ((rc = ensure(ctx, nl->partials, (n_force_rows + (size_t)((nl->n_excl + 255) / 256) + nb_exc + 1) * N_PART * sizeof(double), s))) return rc;
     if ((rc = ensure(ctx, nl->accum, 16 * sizeof(double), s))) return rc;
     real* lj_dev = (real*)nl->lj.p;
     int* row_active = (int*)((char*)nl->lj.p + (size_t)MAX_TYPES * MAX_TYPES * 4 * sizeof(double));
@@ -638,12 +701,20 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
                                                               P.two_a_sqrtpi, nl->grid.L[0], nl->grid.L[1], nl->grid.L[2]);
         DIMOS_LAUNCH_CHECK(ctx, "excl_correction");
     }
+    if (nb_exc) {
+        exceptions_kernel<real><<<nb_exc, 256, 0, s>>>((const int2*)nl->exc_pairs.p, (const double2*)nl->exc_scale.p, nl->n_exc,
+                                                        (const int*)nl->inv_perm.p, (const real4*)nl->xyzq.p, (const int*)nl->stype.p,
+                                                        (const double*)nl->ref.p, lj_table, nt, (real4*)nl->Facc.p,
+                                                        (double*)nl->partials.p + (n_force_rows + nb_excl) * N_PART, P.ke,
+                                                        nl->grid.L[0], nl->grid.L[1], nl->grid.L[2]);
+        DIMOS_LAUNCH_CHECK(ctx, "exceptions");
+    }
     int fb = (int)((nsl + T - 1) / T);
     const int maxfb = ctx->sm_count * 8;
     if (fb > maxfb) fb = maxfb;
     if (fb < 1) fb = 1;
     finalize_kernel<real><<<fb, T, 0, s>>>((const int*)nl->perm.p, nsl, (const real4*)nl->Fown.p, (const real4*)nl->Facc.p, F,
-                                           (const double*)nl->partials.p, (int64_t)n_force_rows + nb_excl, (double*)nl->accum.p, E, W);
+                                           (const double*)nl->partials.p, (int64_t)n_force_rows + nb_excl + nb_exc, (double*)nl->accum.p, E, W);
     DIMOS_LAUNCH_CHECK(ctx, "finalize");
     return DIMOS_OK;
 }

@@ -92,7 +92,7 @@ def check_nonbonded(F, E, W, orc, precision, use_allow=True):
 
 
 def run_case(wb, precision, r_cut, skin, method, box=None, pos=None, eps_rf=78.5, alpha=3.12, oracle_alg="celllist",
-             check_set=True, r_switch=0.0):
+             check_set=True, r_switch=0.0, exceptions=None):
     """Build + export + nonbonded on the GPU, compare all of it with the oracle.  Returns a small report."""
     db = DeviceBox(wb, precision, box=box, pos=pos)
     ctx = dimos.Context(0, precision)
@@ -104,12 +104,15 @@ def run_case(wb, precision, r_cut, skin, method, box=None, pos=None, eps_rf=78.5
         if check_set:
             gp = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy()
             rep["set"] = check_neighbor_set(gp, pos64, db.box, r_cut + skin, wb.excl_pairs)
+        if exceptions is not None:
+            dimos.dimos_nl_set_exceptions(ctx, nl, torch.from_numpy(np.ascontiguousarray(exceptions[0], dtype=np.int32)).to(db.pos.device),
+                                          torch.from_numpy(np.ascontiguousarray(exceptions[1], dtype=np.float64)).to(db.pos.device))
         F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, method=method, eps_rf=eps_rf, alpha=alpha,
                                         r_switch=r_switch)
         torch.cuda.synchronize()
         orc = oracle.nonbonded(pos64, db.charge.double().cpu().numpy(), wb.type, db.lj_np, db.box, r_cut, method=METHOD[method],
                                eps_rf=eps_rf, alpha=alpha, excl_pairs=wb.excl_pairs, band=BAND, algorithm=oracle_alg,
-                               r_switch=r_switch)
+                               r_switch=r_switch, exceptions=exceptions)
         rep.update(check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision))
         rep["n_pairs_cut"] = orc.n_pairs
         return rep

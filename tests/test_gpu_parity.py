@@ -178,6 +178,46 @@ def test_lj_switch_outside_range_is_plain_truncation_f32():
         ctx.close()
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,method", [("f32", "rf"), ("f32", "ewald"), ("mixed", "rf"), ("f64", "ewald")])
+def test_one_four_exceptions(precision, method):
+    """1-4 exceptions (reading C-21): a third of the excluded pairs of a water box (LJ on H too, so
+    that the LJ scale acts) and of the three-type mixture add back scaled bare LJ + Coulomb."""
+    import dataclasses
+
+    wb = dataclasses.replace(wl.make_config(1), sigma=np.array([wl.SIGMA_O, 0.1]), epsilon=np.array([wl.EPS_O, 0.2]))
+    exc = wb.excl_pairs[::3].copy()
+    scale = np.tile(np.array([[0.8333, 0.5]]), (exc.shape[0], 1))
+    scale[::2, 1] = 0.25  # individual factors
+    plain = run_case(wb, precision, 1.0, 0.1, method, check_set=False)
+    rep = run_case(wb, precision, 1.0, 0.1, method, check_set=False, exceptions=(exc, scale))
+    assert rep["n_pairs_cut"] == plain["n_pairs_cut"]
+    mix = _mixture_box(16, 4.6, 7)
+    exc_m = mix.excl_pairs[1::2].copy()
+    run_case(mix, precision, 1.0, 0.1, method, check_set=False, exceptions=(exc_m, np.full((exc_m.shape[0], 2), 0.5)))
+
+
+def test_exceptions_survive_rebuild_and_can_be_cleared_f32():
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        E0 = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)[1].clone()
+        exc = db.excl[::3].contiguous()
+        sc = torch.full((exc.shape[0], 2), 0.5, dtype=torch.float64, device=exc.device)
+        dimos.dimos_nl_set_exceptions(ctx, nl, exc, sc)
+        E1 = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)[1].clone()
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)  # rebuild in place keeps them
+        E2 = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)[1].clone()
+        dimos.dimos_nl_set_exceptions(ctx, nl, None, None)
+        E3 = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)[1].clone()
+        assert abs(float(E1[2] - E0[2])) > 1.0  # intramolecular Coulomb added back at half strength: large
+        assert abs(float(E2[0] - E1[0])) <= 1e-6 * abs(float(E1[0])) and abs(float(E3[0] - E0[0])) <= 1e-6 * abs(float(E0[0]))
+    finally:
+        ctx.close()
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)
