@@ -461,3 +461,41 @@ def test_exception_forces_are_minus_gradient_and_newton():
     with pytest.raises(ValueError):  # an exception must also be an exclusion
         oracle.nonbonded(pos, wb.charge, wb.type, lj, wb.box, 1.0, excl_pairs=wb.excl_pairs[1:],
                          exceptions=(wb.excl_pairs[:1], np.array([[1.0, 1.0]])), algorithm="bruteforce")
+
+
+# --- velocity Verlet, steps 1, 2, 5 of PAPER.md:281-292 -----------------------------------------------------------
+def _vv_run(x, v, force_fn, inv_m, dt, n):
+    f = force_fn(x)
+    for _ in range(n):
+        x, v = oracle.vv_kick_drift(x, v, f, inv_m, dt)
+        f = force_fn(x)
+        v = oracle.vv_kick(v, f, inv_m, dt)
+    return x, v
+
+
+def test_velocity_verlet_is_exact_for_a_constant_force():
+    """x(t) = x0 + v0 t + F t^2 / (2 m), v(t) = v0 + F t / m: velocity Verlet reproduces it exactly; the units need no
+    conversion factor (kJ mol^-1 nm^-1 / amu = nm ps^-2)."""
+    x0 = np.array([[0.1, -0.2, 0.3], [1.0, 2.0, 3.0]])
+    v0 = np.array([[0.5, 0.0, -1.0], [0.0, 0.25, 0.0]])
+    F = np.array([[10.0, -4.0, 2.5], [-3.0, 0.0, 8.0]])
+    m = np.array([15.9994, 1.008])
+    dt, n = 0.002, 50
+    x, v = _vv_run(x0, v0, lambda _x: F, 1.0 / m, dt, n)
+    t = n * dt
+    assert np.allclose(x, x0 + v0 * t + 0.5 * F / m[:, None] * t * t, rtol=0, atol=1e-13)
+    assert np.allclose(v, v0 + F / m[:, None] * t, rtol=0, atol=1e-13)
+
+
+def test_velocity_verlet_harmonic_oscillator_closed_form_and_reversibility():
+    """For F = -k x velocity Verlet is the exact flow of a shadow oscillator: x_n = x_0 cos(n phi) with
+    cos(phi) = 1 - (omega dt)^2 / 2 (v_0 = 0).  Negating the velocities retraces the trajectory."""
+    k, m, dt, n = 300.0, 2.0, 0.004, 137
+    w2 = k / m
+    x0 = np.array([[0.7, 0.0, 0.0]])
+    v0 = np.zeros((1, 3))
+    x, v = _vv_run(x0, v0, lambda xx: -k * xx, np.array([1.0 / m]), dt, n)
+    phi = np.arccos(1.0 - 0.5 * w2 * dt * dt)
+    assert x[0, 0] == pytest.approx(0.7 * np.cos(n * phi), abs=1e-12)
+    xb, vb = _vv_run(x, -v, lambda xx: -k * xx, np.array([1.0 / m]), dt, n)
+    assert np.allclose(xb, x0, atol=1e-12) and np.allclose(vb, -v0, atol=1e-12)
