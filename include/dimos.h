@@ -210,6 +210,21 @@ DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
                                     int64_t* n_pairs_host, void* stream);
 
+/* dimos_vv_kick_drift / dimos_vv_kick -- velocity Verlet, PAPER.md:281-292 (steps 1 + 2, and step 5; constraints and
+ * thermostats, steps 3, 6, 7, are not built).  Units nm, ps, amu, kJ mol^-1 nm^-1: a = F / m needs no conversion factor.
+ *   kick_drift:  v <- v + (dt/2) F / m;  x <- x + dt v      (in place)
+ *   kick:        v <- v + (dt/2) F / m                      (in place, with the forces at the new positions)
+ *   pos, vel, F   dev, N x 3, float or double per the context precision
+ *   inv_mass      dev, N, same type: 1 / m_i
+ *   pos_at_build, skin, flag_dev, flag_host (kick_drift only; pos_at_build and flag_dev both NULL to skip): the rebuild
+ *                 trigger of dimos_nl_needs_rebuild evaluated on the NEW positions in the same pass.
+ *                 A non-NULL flag_host synchronises the stream. */
+DIMOS_API int dimos_vv_kick_drift(dimos_ctx* ctx, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N,
+                                  double dt, const void* pos_at_build, double skin, int32_t* flag_dev, int32_t* flag_host,
+                                  void* stream);
+DIMOS_API int dimos_vv_kick(dimos_ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
+                            void* stream);
+
 /* dimos_nl_set_exceptions -- PAPER.md:243 ("1-4 exceptions ... scale the strength of the non-bonded interactions by
  * some common factor", or an individual factor per pair; "handled explicitly by the non-bonded interaction method").
  * Reading C-21 (the paper gives no formula): every exception pair must ALSO be one of the excluded pairs the list was

@@ -29,6 +29,7 @@ EXPORTED_SYMBOLS = (
     "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats", "dimos_launch_count",
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
+    "dimos_vv_kick_drift", "dimos_vv_kick",
 )
 
 
@@ -91,6 +92,8 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_step_host.restype = ctypes.c_int
     lib.dimos_nl_count_within.argtypes = [vp, vp, dbl, ctypes.POINTER(i64), vp]
     lib.dimos_nl_set_exceptions.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.dimos_vv_kick_drift.argtypes = [vp, vp, vp, vp, vp, i64, dbl, vp, dbl, vp, ctypes.POINTER(i32), vp]
+    lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -105,7 +108,7 @@ def load_library() -> ctypes.CDLL:
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
-                 "dimos_nl_set_exceptions"):
+                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -300,6 +303,37 @@ class Context:
             nl.handle = h
         return nl, bool(rebuilt.value)
 
+    def vv_kick_drift(self, pos, vel, F, inv_mass, dt, pos_at_build=None, skin=0.0, sync=True):
+        """dimos_vv_kick_drift: velocity-Verlet steps 1 + 2 in place; with pos_at_build also the rebuild flag (bool when
+        sync, else the device flag tensor)."""
+        pos = self._dev(pos, self.real, 3)
+        vel = self._dev(vel, self.real, 3)
+        F = self._dev(F, self.real, 3)
+        inv_mass = self._dev(inv_mass, self.real)
+        host = ctypes.c_int32(0)
+        trig = pos_at_build is not None
+        if trig:
+            pos_at_build = self._dev(pos_at_build, self.real, 3)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_vv_kick_drift(self.handle, pos.data_ptr(), vel.data_ptr(), F.data_ptr(), inv_mass.data_ptr(),
+                                              pos.shape[0], float(dt), pos_at_build.data_ptr() if trig else None, float(skin),
+                                              self._flag.data_ptr() if trig else None,
+                                              ctypes.byref(host) if (trig and sync) else None, _stream_ptr())
+        self._check(rc)
+        if not trig:
+            return None
+        return bool(host.value) if sync else self._flag
+
+    def vv_kick(self, vel, F, inv_mass, dt):
+        """dimos_vv_kick: velocity-Verlet step 5 in place."""
+        vel = self._dev(vel, self.real, 3)
+        F = self._dev(F, self.real, 3)
+        inv_mass = self._dev(inv_mass, self.real)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_vv_kick(self.handle, vel.data_ptr(), F.data_ptr(), inv_mass.data_ptr(), vel.shape[0], float(dt),
+                                        _stream_ptr())
+        self._check(rc)
+
     def nl_set_exceptions(self, nl: NeighborList, pairs, scale):
         """dimos_nl_set_exceptions: pairs (n,2) int32 i<j, scale (n,2) float64 = (Coulomb scale, LJ scale); None clears."""
         if pairs is None or len(pairs) == 0:
@@ -376,6 +410,14 @@ def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = T
 
 def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
     return ctx.nonbonded(nl, pos, charge, type_, lj_table, **kw)
+
+
+def dimos_vv_kick_drift(ctx: Context, pos, vel, F, inv_mass, dt, **kw):
+    return ctx.vv_kick_drift(pos, vel, F, inv_mass, dt, **kw)
+
+
+def dimos_vv_kick(ctx: Context, vel, F, inv_mass, dt):
+    return ctx.vv_kick(vel, F, inv_mass, dt)
 
 
 def dimos_nl_set_exceptions(ctx: Context, nl: NeighborList, pairs, scale):

@@ -217,6 +217,37 @@ DIMOS_API int dimos_nl_needs_rebuild(dimos_ctx* c, const void* pos, const void* 
     return DIMOS_OK;
 }
 
+DIMOS_API int dimos_vv_kick_drift(dimos_ctx* c, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
+                                  const void* pos_at_build, double skin, int32_t* flag_dev, int32_t* flag_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!pos || !vel || !F || !inv_mass) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || !(dt == dt) || !(skin >= 0)) return set_error(ctx, DIMOS_EINVAL, "bad N, dt or skin");
+    if ((pos_at_build != nullptr) != (flag_dev != nullptr)) return set_error(ctx, DIMOS_EINVAL, "pos_at_build and flag_dev go together");
+    if (flag_host && !flag_dev) return set_error(ctx, DIMOS_EINVAL, "flag_host needs flag_dev");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = vv_kick_drift_impl(ctx, pos, vel, F, inv_mass, N, dt, pos_at_build, skin, flag_dev, s);
+    if (rc) return rc;
+    if (flag_host) {
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 32, flag_dev, sizeof(int), cudaMemcpyDeviceToHost, s));
+        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+        *flag_host = ctx->h_pinned[32];
+    }
+    return DIMOS_OK;
+}
+
+DIMOS_API int dimos_vv_kick(dimos_ctx* c, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!vel || !F || !inv_mass) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || !(dt == dt)) return set_error(ctx, DIMOS_EINVAL, "bad N or dt");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return vv_kick_impl(ctx, vel, F, inv_mass, N, dt, (cudaStream_t)stream);
+}
+
 static int check_nb_args(Ctx* ctx, const NL* nl, int32_t ntypes, const double* box, const dimos_nb_params* p)
 {
     if (!list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");

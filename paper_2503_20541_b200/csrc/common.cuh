@@ -142,6 +142,9 @@ int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const 
                    const double* lj_table, int32_t ntypes, const dimos_nb_params* prm, void* F, double* E,
                    double* virial, cudaStream_t s);
 int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s);
+int vv_kick_drift_impl(Ctx* ctx, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
+                       const void* pos_at_build, double skin, int32_t* flag_dev, cudaStream_t s);
+int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, cudaStream_t s);
 
 // stencil code <-> offset
 __host__ __device__ inline int stencil_code(int dx, int dy, int dz) { return (dx + 1) * 9 + (dy + 1) * 3 + (dz + 1); }

@@ -20,6 +20,7 @@
 #include <type_traits>
 
 #include "pair_common.cuh"
+#include "trigger.cuh"
 
 namespace dimos {
 
@@ -65,39 +66,7 @@ __global__ void needs_rebuild_kernel(const real* __restrict__ pos, const real* _
         if (!(d2 == d2)) m = (real)INFINITY;  // NaN -> force a rebuild
     }
     (void)n3;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        real y = __shfl_xor_sync(0xffffffffu, m, o);
-        m = y > m ? y : m;
-    }
-    __shared__ real wmax[32];
-    __shared__ bool last;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (lane == 0) wmax[w] = m;
-    __syncthreads();
-    if (w == 0) {
-        m = lane < (blockDim.x >> 5) ? wmax[lane] : (real)0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            real y = __shfl_xor_sync(0xffffffffu, m, o);
-            m = y > m ? y : m;
-        }
-        if (lane == 0) {
-            // non-negative doubles order like their bit patterns
-            atomicMax(&state[0], (unsigned long long)__double_as_longlong((double)m));
-            __threadfence();
-            unsigned long long t = atomicAdd(&state[1], 1ull);
-            last = (t == (unsigned long long)gridDim.x - 1);
-        }
-    }
-    __syncthreads();
-    if (last && threadIdx.x == 0) {
-        __threadfence();
-        unsigned long long bits = atomicExch(&state[0], 0ull);
-        state[1] = 0ull;
-        double mx = __longlong_as_double((long long)bits);
-        *flag = mx > (double)thr2 ? 1 : 0;
-    }
+    trigger_reduce_and_flag<real>(m, thr2, state, flag);
 }
 
 int needs_rebuild_impl(Ctx* ctx, const void* pos, const void* ref, int64_t N, double skin, int32_t* flag_dev, cudaStream_t s)
