@@ -166,7 +166,8 @@ DIMOS_API int dimos_nl_needs_rebuild(dimos_ctx* ctx, const void* pos, const void
  *   box      host, 3 doubles, must equal the build box (else DIMOS_ESTALE)
  *   params   host
  *   F        dev, N x 3, overwritten: F_i = sum_j f_ij (plus the exclusion-correction forces)
- *   E        dev, 4 doubles, overwritten: {total, lj, coul_pair, coul_excl_corr}
+ *   E        dev, 4 doubles, overwritten: {total, lj, coul_pair, coul_excl_corr}; the 1-4 exceptions set with
+ *            dimos_nl_set_exceptions add their LJ part to lj and their Coulomb part to coul_pair
  *   virial   dev, 9 doubles row-major, overwritten: W_ab = sum_pairs d_a f_ij,b with
  *            d = r_i - r_j (minimum image), including exclusion-correction pairs; may be NULL
  * Does not synchronise. */

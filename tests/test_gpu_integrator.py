@@ -78,7 +78,8 @@ def test_md_loop_through_the_library_f32():
             dimos.dimos_vv_kick(ctx, vel, F, inv_m, 0.004)
         p1 = (vel.double() / inv_m.double()[:, None]).sum(0)
         assert rebuilds >= 1
-        assert float((p1 - p0).abs().max()) < 1e-2 * float((vel.double() / inv_m.double()[:, None]).abs().sum(0).max()) * 1e-2
+        scale = float((vel.double() / inv_m.double()[:, None]).abs().sum(0).max())  # sum of |p_i| per axis
+        assert float((p1 - p0).abs().max()) < 1e-4 * scale  # pair forces are antisymmetric: total momentum is conserved
         assert bool(torch.isfinite(E).all())
     finally:
         ctx.close()
