@@ -240,6 +240,17 @@ DIMOS_API int dimos_vv_kick(dimos_ctx* ctx, void* vel, const void* F, const void
 DIMOS_API int dimos_nl_set_exceptions(dimos_ctx* ctx, dimos_nl* nl, const int32_t* pairs, const double* scale,
                                       int64_t n_exc, void* stream);
 
+/* dimos_nl_export_edges -- the neighbour list as an edge list with distance vectors and periodic shifts, the form a
+ * machine-learned interatomic potential consumes (PAPER.md:179-185 get_neighborlist, 251).  Like dimos_nl_export_pairs,
+ * but only the pairs with minimum-image r < radius (0 < radius <= r_cut + skin) at the build positions, and per pair k
+ *   pairs[k] = (a, b), a < b, original atom indices          dev, cap x 2 int32
+ *   dvec[k]  = r_a - r_b - shift[k] * box (minimum image)    dev, cap x 3, float or double per the precision; may be NULL
+ *   shift[k] = nearbyint((r_a - r_b) / box) per axis         dev, cap x 3 int32; may be NULL
+ * in unspecified order (the three arrays share it).  n_pairs_host receives the number of edges; if it exceeds cap only
+ * the first cap were written and the call returns DIMOS_EOVERFLOW.  Synchronises the stream. */
+DIMOS_API int dimos_nl_export_edges(dimos_ctx* ctx, const dimos_nl* nl, double radius, int32_t* pairs, void* dvec,
+                                    int32_t* shift, int64_t cap, int64_t* n_pairs_host, void* stream);
+
 /* Number of unordered, non-excluded pairs of the list with minimum-image r < radius at the build
  * positions, 0 < radius <= r_cut + skin (radius = r_cut gives the in-cutoff pair count the
  * throughput metric "pair interactions/s" is quoted on).  Synchronises the stream. */

@@ -157,3 +157,13 @@ def needs_rebuild(pos, pos_at_build, skin):
     m = ctypes.c_double(0.0)
     flag = _load().orc_needs_rebuild(pos.shape[0], _dp(pos), _dp(ref), float(skin), ctypes.byref(m))
     return bool(flag), float(m.value)
+
+
+def edge_vectors(pos, box, pairs):
+    """Distance vectors and periodic shifts of an edge list (minimum image, reading C-3): for every
+    pair (a, b): shift = nearbyint((r_a - r_b) / L) per axis and d = r_a - r_b - shift * L.  numpy fp64."""
+    pos, box = _d(pos), _d(box)
+    pairs = np.asarray(pairs, dtype=np.int64).reshape(-1, 2)
+    diff = pos[pairs[:, 0]] - pos[pairs[:, 1]]
+    shift = np.rint(diff / box)
+    return diff - shift * box, shift.astype(np.int64)

@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = (
     "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats", "dimos_launch_count",
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
-    "dimos_vv_kick_drift", "dimos_vv_kick",
+    "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges",
 )
 
 
@@ -94,6 +94,7 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_nl_set_exceptions.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.dimos_vv_kick_drift.argtypes = [vp, vp, vp, vp, vp, i64, dbl, vp, dbl, vp, ctypes.POINTER(i32), vp]
     lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
+    lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -108,7 +109,7 @@ def load_library() -> ctypes.CDLL:
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
-                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick"):
+                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -363,6 +364,21 @@ class Context:
         self._check(rc)
         return out[: got.value]
 
+    def nl_export_edges(self, nl: NeighborList, radius: float):
+        """dimos_nl_export_edges: (pairs (n,2) int32 a<b, dvec (n,3) real = r_a - r_b - shift*box, shift (n,3) int32) of the
+        pairs with minimum-image r < radius at the build positions; device tensors, order unspecified."""
+        n = self.nl_count_within(nl, radius)
+        dev = torch.device("cuda", self.device)
+        pairs = torch.empty((max(n, 1), 2), dtype=torch.int32, device=dev)
+        dvec = torch.empty((max(n, 1), 3), dtype=self.real, device=dev)
+        shift = torch.empty((max(n, 1), 3), dtype=torch.int32, device=dev)
+        got = ctypes.c_int64(0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_export_edges(self.handle, nl.handle, float(radius), pairs.data_ptr(), dvec.data_ptr(),
+                                                shift.data_ptr(), pairs.shape[0], ctypes.byref(got), _stream_ptr())
+        self._check(rc)
+        return pairs[: got.value], dvec[: got.value], shift[: got.value]
+
     def nl_count_within(self, nl: NeighborList, radius: float) -> int:
         """dimos_nl_count_within: pairs of the list with r < radius at the build positions."""
         n = ctypes.c_int64(0)
@@ -422,6 +438,10 @@ def dimos_vv_kick(ctx: Context, vel, F, inv_mass, dt):
 
 def dimos_nl_set_exceptions(ctx: Context, nl: NeighborList, pairs, scale):
     return ctx.nl_set_exceptions(nl, pairs, scale)
+
+
+def dimos_nl_export_edges(ctx: Context, nl: NeighborList, radius: float):
+    return ctx.nl_export_edges(nl, radius)
 
 
 def dimos_nl_export_pairs(ctx: Context, nl: NeighborList) -> torch.Tensor:

@@ -422,6 +422,21 @@ DIMOS_API int dimos_nl_export_pairs(dimos_ctx* c, const dimos_nl* l, int32_t* pa
     return nl_export_impl(ctx, nl, pairs, cap, n_pairs_host, nl->r_nl, (cudaStream_t)stream);
 }
 
+DIMOS_API int dimos_nl_export_edges(dimos_ctx* c, const dimos_nl* l, double radius, int32_t* pairs, void* dvec, int32_t* shift,
+                                    int64_t cap, int64_t* n_pairs_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!l || !n_pairs_host || (cap > 0 && !pairs)) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    const NL* nl = reinterpret_cast<const NL*>(l);
+    if (!list_belongs(ctx, nl) || nl->N <= 0) return set_error(ctx, DIMOS_EINVAL, "list not built with this context");
+    if (!(radius > 0) || radius > nl->r_nl) return set_error(ctx, DIMOS_EINVAL, "radius must be in (0, r_cut + skin]");
+    if (cap < 0) return set_error(ctx, DIMOS_EINVAL, "negative capacity");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return nl_export_impl(ctx, nl, pairs, cap, n_pairs_host, radius, (cudaStream_t)stream, cap > 0 ? dvec : nullptr,
+                          cap > 0 ? shift : nullptr);
+}
+
 DIMOS_API int dimos_nl_count_within(dimos_ctx* c, const dimos_nl* l, double radius, int64_t* n_pairs_host, void* stream)
 {
     if (!c) return DIMOS_EINVAL;

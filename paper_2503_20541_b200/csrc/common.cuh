@@ -135,7 +135,8 @@ void release(Ctx* ctx, DevBuf& b);
 // ---- entry points implemented per translation unit ---------------------------------------------
 int nl_build_impl(Ctx* ctx, NL* nl, const void* pos, const int32_t* excl_pairs, int64_t n_excl,
                   void* pos_at_build, cudaStream_t s);
-int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s);
+int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s,
+                   void* dvec = nullptr, int32_t* shift = nullptr);
 int needs_rebuild_impl(Ctx* ctx, const void* pos, const void* ref, int64_t N, double skin, int32_t* flag_dev,
                        cudaStream_t s);
 int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const int32_t* type,

@@ -738,7 +738,9 @@ static size_t build_smem_bytes(int m_res)
 // ------------------------------------------------------------------------------------------------
 template <typename real, int PBC>
 __global__ __launch_bounds__(128) void export_pairs_kernel(BuildParams<real> P, int2* __restrict__ pairs, int64_t cap,
-                                                           unsigned long long* __restrict__ counter)
+                                                           unsigned long long* __restrict__ counter,
+                                                           real* __restrict__ dvec, int* __restrict__ shift,
+                                                           const double* __restrict__ ref)
 {
     using real4 = typename vec4<real>::type;
     const int lane = threadIdx.x & 31;
@@ -801,6 +803,21 @@ __global__ __launch_bounds__(128) void export_pairs_kernel(BuildParams<real> P, 
                 if ((int64_t)w < cap) {
                     int a = pi[i], b = pj_orig;
                     pairs[w] = a < b ? make_int2(a, b) : make_int2(b, a);
+                    if (dvec || shift) {
+                        // edge (a, b), a < b:  d = r_a - r_b - n L (minimum image), n = shift.  With raw = cell-relative +
+                        // ref the image count follows from the origins: n L = (raw_i - raw_j) - d
+                        real d[3] = {xi[i] - px, yi[i] - py, zi[i] - pz};
+                        const real rel[3] = {xi[i] - pj.x, yi[i] - pj.y, zi[i] - pj.z};
+                        const real sgn = a < b ? (real)1 : (real)-1;
+#pragma unroll
+                        for (int ax = 0; ax < 3; ++ax) {
+                            if (PBC == 1) d[ax] -= P.L[ax] * rint_r(d[ax] / P.L[ax]);
+                            const double raw = (ref[3 * (U * UNIT + i) + ax] - ref[3 * (int64_t)j + ax]) + (double)rel[ax];
+                            const int n = (int)rint((raw - (double)d[ax]) / (double)P.g.L[ax]);
+                            if (dvec) dvec[3 * w + ax] = sgn * d[ax];
+                            if (shift) shift[3 * w + ax] = a < b ? n : -n;
+                        }
+                    }
                 }
                 ++w;
             }
@@ -996,7 +1013,8 @@ int nl_build_impl(Ctx* ctx, NL* nl, const void* pos, const int32_t* excl_pairs, 
 }
 
 template <typename real>
-static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s)
+static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, void* dvec,
+                           int32_t* shift, cudaStream_t s)
 {
     BuildParams<real> P = make_build_params<real>(nl);
     P.rnl2 = (real)radius * (real)radius;
@@ -1005,9 +1023,9 @@ static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, 
     DIMOS_LAUNCH_CHECK(ctx, "zero_counter");
     const unsigned nb = (unsigned)((nl->n_units + 3) / 4);
     if (nl->grid.pbc_mode == 0)
-        export_pairs_kernel<real, 0><<<nb, 128, 0, s>>>(P, (int2*)pairs, pairs ? cap : 0, counter);
+        export_pairs_kernel<real, 0><<<nb, 128, 0, s>>>(P, (int2*)pairs, pairs ? cap : 0, counter, (real*)dvec, shift, (const double*)nl->ref.p);
     else
-        export_pairs_kernel<real, 1><<<nb, 128, 0, s>>>(P, (int2*)pairs, pairs ? cap : 0, counter);
+        export_pairs_kernel<real, 1><<<nb, 128, 0, s>>>(P, (int2*)pairs, pairs ? cap : 0, counter, (real*)dvec, shift, (const double*)nl->ref.p);
     DIMOS_LAUNCH_CHECK(ctx, "export_pairs");
     unsigned long long* h = reinterpret_cast<unsigned long long*>(ctx->h_pinned + 16);
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h, counter, 8, cudaMemcpyDeviceToHost, s));
@@ -1017,10 +1035,11 @@ static int nl_export_typed(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, 
     return DIMOS_OK;
 }
 
-int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s)
+int nl_export_impl(Ctx* ctx, const NL* nl, int32_t* pairs, int64_t cap, int64_t* n_pairs_host, double radius, cudaStream_t s,
+                   void* dvec, int32_t* shift)
 {
-    if (ctx->precision == DIMOS_F64) return nl_export_typed<double>(ctx, nl, pairs, cap, n_pairs_host, radius, s);
-    return nl_export_typed<float>(ctx, nl, pairs, cap, n_pairs_host, radius, s);
+    if (ctx->precision == DIMOS_F64) return nl_export_typed<double>(ctx, nl, pairs, cap, n_pairs_host, radius, dvec, shift, s);
+    return nl_export_typed<float>(ctx, nl, pairs, cap, n_pairs_host, radius, dvec, shift, s);
 }
 
 }  // namespace dimos

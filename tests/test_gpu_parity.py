@@ -218,6 +218,42 @@ def test_exceptions_survive_rebuild_and_can_be_cleared_f32():
         ctx.close()
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,index", [("f32", 1), ("f64", 1), ("f32", 0), ("f64", 0)])
+def test_edge_list_with_vectors_and_shifts(precision, index):
+    """dimos_nl_export_edges: the edge set within r_cut equals the oracle's (outside the +-1e-5 nm
+    band), and every edge carries d = r_a - r_b - shift L and the shift the oracle computes.  configs[1] has 4 cells per
+    axis (image from the cell offsets), configs[0] a single cell (per-pair minimum image)."""
+    wb = wl.make_config(index)
+    r_cut = 1.0 if index == 1 else 0.9
+    db = DeviceBox(wb, precision)
+    ctx = dimos.Context(0, precision)
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, r_cut, 0.1, db.excl)
+        pairs, dvec, shift = dimos.dimos_nl_export_edges(ctx, nl, r_cut)
+        pairs = pairs.cpu().numpy().astype(np.int64)
+        dvec = dvec.double().cpu().numpy()
+        shift = shift.cpu().numpy().astype(np.int64)
+        pos64 = db.pos.double().cpu().numpy()
+        n = wb.n_atoms
+        key = pairs[:, 0] * n + pairs[:, 1]
+        assert np.all(pairs[:, 0] < pairs[:, 1]) and np.unique(key).size == key.size
+        must = oracle.neighbor_pairs(pos64, db.box, r_cut - BAND, wb.excl_pairs, "celllist").astype(np.int64)
+        may = oracle.neighbor_pairs(pos64, db.box, r_cut + BAND, wb.excl_pairs, "celllist").astype(np.int64)
+        assert np.setdiff1d(must[:, 0] * n + must[:, 1], key).size == 0
+        assert np.setdiff1d(key, may[:, 0] * n + may[:, 1]).size == 0
+        d_o, s_o = oracle.edge_vectors(pos64, db.box, pairs)
+        tol = 1e-12 if precision == "f64" else 2e-6
+        # a component within rounding of +-L/2 may legitimately take either image: compare d modulo L there
+        alt = np.abs(np.abs(d_o) - 0.5 * db.box) < 1e-5
+        assert np.all((shift == s_o) | alt)
+        assert np.abs(dvec - d_o)[~alt].max() <= tol
+        assert np.all(np.sqrt((dvec * dvec).sum(1)) < r_cut + BAND)
+        assert np.abs(pos64[pairs[:, 0]] - pos64[pairs[:, 1]] - shift * db.box - dvec).max() <= tol
+    finally:
+        ctx.close()
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)

@@ -499,3 +499,20 @@ def test_velocity_verlet_harmonic_oscillator_closed_form_and_reversibility():
     assert x[0, 0] == pytest.approx(0.7 * np.cos(n * phi), abs=1e-12)
     xb, vb = _vv_run(x, -v, lambda xx: -k * xx, np.array([1.0 / m]), dt, n)
     assert np.allclose(xb, x0, atol=1e-12) and np.allclose(vb, -v0, atol=1e-12)
+
+
+# --- edge list with distance vectors and shifts ------------------------------------------------
+def test_edge_vectors_identities():
+    """d = r_a - r_b - shift L with every component of d in [-L/2, L/2]; |d| < r_list for listed pairs; zero shifts when
+    the atoms sit far from the faces of a huge box; a pair across a face gets shift -1/+1 and the short vector."""
+    wb = small_box()
+    pairs = oracle.neighbor_pairs(wb.pos, wb.box, 0.9, wb.excl_pairs, "bruteforce")
+    d, s = oracle.edge_vectors(wb.pos, wb.box, pairs)
+    pos = wb.pos.astype(np.float64)
+    assert np.allclose(d, pos[pairs[:, 0]] - pos[pairs[:, 1]] - s * wb.box, atol=1e-15)
+    assert np.all(np.abs(d) <= 0.5 * wb.box + 1e-12) and np.all(np.sqrt((d * d).sum(1)) < 0.9)
+    two = np.array([[0.05, 1.0, 1.0], [2.95, 1.0, 1.0]])
+    d2, s2 = oracle.edge_vectors(two, [3.0, 3.0, 3.0], [[0, 1]])
+    assert np.allclose(d2, [[0.1, 0.0, 0.0]]) and s2.tolist() == [[-1, 0, 0]]
+    d3, s3 = oracle.edge_vectors([[10.0, 11.0, 12.0], [10.3, 11.0, 12.4]], BIGBOX, [[0, 1]])
+    assert s3.tolist() == [[0, 0, 0]] and np.allclose(d3, [[-0.3, 0.0, -0.4]])
