@@ -197,6 +197,26 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
             w[0] += (acc_t)(ddx * fx); w[1] += (acc_t)(ddx * fy); w[2] += (acc_t)(ddx * fz);         \
             w[3] += (acc_t)(ddy * fy); w[4] += (acc_t)(ddy * fz); w[5] += (acc_t)(ddz * fz);         \
         }                                                                                            \
+        if (E64 && in) { /* small fp32 box: the pair ENERGY in fp64 from the same fp32 inputs */     \
+            double ex_ = (double)xi[i] - (double)xj, ey_ = (double)yi[i] - (double)yj, ez_ = (double)zi[i] - (double)zj; \
+            ex_ -= P.d_L[0] * rint(ex_ / P.d_L[0]);                                                  \
+            ey_ -= P.d_L[1] * rint(ey_ / P.d_L[1]);                                                  \
+            ez_ -= P.d_L[2] * rint(ez_ / P.d_L[2]);                                                  \
+            const double r2d_ = ex_ * ex_ + ey_ * ey_ + ez_ * ez_, rd_ = sqrt(r2d_);                 \
+            const double qqd_ = (double)qraw[i] * (double)qj * P.d_ke;                               \
+            if (METHOD == DIMOS_RF) e_c64 += qqd_ * (1.0 / rd_ + P.d_krf * r2d_ - P.d_crf);          \
+            else e_c64 += qqd_ * erfc(P.d_alpha * rd_) / rd_;                                        \
+            if (LJ) {                                                                                \
+                const real4 cd_ = ljt[ti[i] + tj];                                                   \
+                const double ri6_ = 1.0 / (r2d_ * r2d_ * r2d_);                                      \
+                double el_ = ((double)cd_.y * ri6_ - (double)cd_.x) * ri6_;                          \
+                if (P.sw_on) {                                                                       \
+                    const double xs_ = (rd_ - P.d_rs) * P.d_inv_sw;                                  \
+                    if (xs_ > 0.0) el_ *= 1.0 + xs_ * xs_ * xs_ * (-10.0 + xs_ * (15.0 - 6.0 * xs_)); \
+                }                                                                                    \
+                e_lj64 += el_;                                                                       \
+            }                                                                                        \
+        }                                                                                            \
     } while (0)
 
 template <typename real, typename acc_t, int METHOD, int PBC>
@@ -219,6 +239,10 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
     const int wib = threadIdx.x >> 5;
     const int comp = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);  // reduce8_scatter's element of this lane
     double acc_d = 0.0;  // running fp64 total of component `comp` over all units of this warp
+    // Boxes with fewer than three cells per axis (per-pair minimum image) are small: their energy is a sum that cancels
+    // to ~1e-4 of the sum of magnitudes, below what fp32 pair terms resolve, so in fp32 mode the pair
+    // ENERGY of such boxes is evaluated in fp64 from the same fp32 inputs; forces and virial stay fp32.
+    constexpr bool E64 = PBC == 1 && sizeof(real) == 4 && sizeof(acc_t) == 4;
 
     // dynamic unit scheduling: every warp draws unit indices from one global counter, so no warp
     // waits for another (rows differ in length) and the tail is at most one unit long
@@ -230,7 +254,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
         if (lane == 0) U_next = (long long)atomicAdd(P.unit_counter, 1ull);  // in flight while this unit is processed
 
         // ---- the unit's 8 i-atoms in registers (uniform across the warp) ----
-        real xi[UNIT], yi[UNIT], zi[UNIT], qi[UNIT];
+        real xi[UNIT], yi[UNIT], zi[UNIT], qi[UNIT], qraw[UNIT];
         int ti[UNIT];
         real fix[UNIT], fiy[UNIT], fiz[UNIT];
 #pragma unroll
@@ -238,6 +262,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const real4 v = P.xyzq[U * UNIT + i];
             xi[i] = v.x; yi[i] = v.y; zi[i] = v.z;
             qi[i] = v.w * P.ke;  // k_e folded into the i-side charge
+            qraw[i] = v.w;
             const int t = P.stype[U * UNIT + i] & STYPE_MASK;
             ti[i] = P.row_active[t] ? t * P.nt : -1;
             fix[i] = fiy[i] = fiz[i] = 0;
@@ -246,6 +271,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
         const int total = ri.x & 0xFFFF;  // chunks in the row
         const int n_plain = ri.y;         // leading chunks that need no mask
         acc_t e_lj = 0, e_c = 0;
+        double e_lj64 = 0.0, e_c64 = 0.0;  // E64 only
         acc_t w[6] = {0, 0, 0, 0, 0, 0};
 
         // software pipeline: (jslot, meta) two chunks ahead, (xyzq, stype) one chunk ahead
@@ -307,7 +333,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             }
         }
         // ---- energy / virial of this unit: lane partials -> fp64 warp totals, kept per warp ----
-        double red[8] = {(double)e_lj, (double)e_c, (double)w[0], (double)w[1], (double)w[2], (double)w[3], (double)w[4], (double)w[5]};
+        double red[8] = {E64 ? e_lj64 : (double)e_lj, E64 ? e_c64 : (double)e_c, (double)w[0], (double)w[1], (double)w[2], (double)w[3], (double)w[4], (double)w[5]};
         acc_d += reduce8_scatter(red, lane);
 
         U = __shfl_sync(FULL, U_next, 0);
@@ -656,6 +682,13 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     P.sw_on = (prm->r_switch > 0.0 && prm->r_switch < rc_) ? 1 : 0;  // Eq. 6; otherwise plain truncation (reading C-8)
     P.rs = (real)prm->r_switch;
     P.inv_sw = P.sw_on ? (real)(1.0 / (rc_ - prm->r_switch)) : (real)0;
+    P.d_ke = prm->coulomb_const;
+    P.d_krf = (prm->eps_rf - 1.0) / ((2.0 * prm->eps_rf + 1.0) * rc_ * rc_ * rc_);
+    P.d_crf = 3.0 * prm->eps_rf / ((2.0 * prm->eps_rf + 1.0) * rc_);
+    P.d_alpha = prm->alpha;
+    P.d_rs = prm->r_switch;
+    P.d_inv_sw = P.sw_on ? 1.0 / (rc_ - prm->r_switch) : 0.0;
+    for (int a = 0; a < 3; ++a) P.d_L[a] = nl->grid.L[a];
     P.alpha = (real)prm->alpha;
     P.two_a_sqrtpi = (real)(2.0 * prm->alpha / sqrt(M_PI));
     for (int a = 0; a < 3; ++a) { P.L[a] = (real)nl->grid.L[a]; P.invL[a] = (real)(1.0 / nl->grid.L[a]); P.h[a] = (real)nl->grid.h[a]; }

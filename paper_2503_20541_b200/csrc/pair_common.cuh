@@ -47,6 +47,8 @@ struct ForceParams {
     real rc2, ke, krf, m2krf, crf, alpha, two_a_sqrtpi;
     real rs, inv_sw;  // LJ switch (Eq. 6): r_s and 1/(r_c - r_s)
     int sw_on;
+    // fp64 copies for the energy of small fp32 boxes (generic kernel, per-pair minimum image)
+    double d_ke, d_krf, d_crf, d_alpha, d_rs, d_inv_sw, d_L[3];
     real L[3], invL[3], h[3];
 };
 
