@@ -211,6 +211,20 @@ DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
                                     int64_t* n_pairs_host, void* stream);
 
+/* dimos_virtual_box -- non-periodic systems ("the system is ... embedded into a non-periodic box" for the
+ * neighbour-list computation).  Returns the edges of a virtual periodic box around the current positions that is large
+ * enough for the periodic routines to reproduce open boundaries exactly: box[a] = extent[a] + r_cut + 2 skin (at least
+ * 2 r_cut), so the periodic images of the system are farther apart than r_cut + skin and stay so while no atom has
+ * moved more than skin/2 since (the rebuild trigger).  Use the returned box in dimos_nl_build and dimos_nonbonded (positions
+ * need no shift: the routines wrap consistently), and call it again before every rebuild.  Meaningful with DIMOS_RF
+ * (or eps_rf = 1 for a plain shifted cutoff); the Ewald variant presumes a real periodic system.
+ *   pos        dev, N x 3, float or double per the context precision
+ *   box_host   host, 3 doubles, written (fp32-representable values)
+ *   lo_host    host, 3 doubles, written if not NULL: the lower corner of the bounding box
+ * Synchronises the stream.  DIMOS_EINVAL for a non-finite coordinate. */
+DIMOS_API int dimos_virtual_box(dimos_ctx* ctx, const void* pos, int64_t N, double r_cut, double skin, double* box_host,
+                                double* lo_host, void* stream);
+
 /* dimos_vv_kick_drift / dimos_vv_kick -- velocity Verlet, PAPER.md:281-292 (steps 1 + 2, and step 5; constraints and
  * thermostats, steps 3, 6, 7, are not built).  Units nm, ps, amu, kJ mol^-1 nm^-1: a = F / m needs no conversion factor.
  *   kick_drift:  v <- v + (dt/2) F / m;  x <- x + dt v      (in place)

@@ -29,7 +29,7 @@ EXPORTED_SYMBOLS = (
     "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats", "dimos_launch_count",
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
-    "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges",
+    "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
 )
 
 
@@ -95,6 +95,7 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_vv_kick_drift.argtypes = [vp, vp, vp, vp, vp, i64, dbl, vp, dbl, vp, ctypes.POINTER(i32), vp]
     lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
     lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
+    lib.dimos_virtual_box.argtypes = [vp, vp, i64, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -109,7 +110,7 @@ def load_library() -> ctypes.CDLL:
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
-                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges"):
+                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -304,6 +305,19 @@ class Context:
             nl.handle = h
         return nl, bool(rebuilt.value)
 
+    def virtual_box(self, pos, r_cut, skin):
+        """dimos_virtual_box: (box (3,) float64 numpy, lower corner (3,)) of the virtual periodic box of an open system."""
+        import numpy as np
+
+        pos = self._dev(pos, self.real, 3)
+        box = (ctypes.c_double * 3)()
+        lo = (ctypes.c_double * 3)()
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_virtual_box(self.handle, pos.data_ptr(), pos.shape[0], float(r_cut), float(skin), box, lo,
+                                            _stream_ptr())
+        self._check(rc)
+        return np.array(list(box), dtype=np.float64), np.array(list(lo), dtype=np.float64)
+
     def vv_kick_drift(self, pos, vel, F, inv_mass, dt, pos_at_build=None, skin=0.0, sync=True):
         """dimos_vv_kick_drift: velocity-Verlet steps 1 + 2 in place; with pos_at_build also the rebuild flag (bool when
         sync, else the device flag tensor)."""
@@ -426,6 +440,10 @@ def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = T
 
 def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
     return ctx.nonbonded(nl, pos, charge, type_, lj_table, **kw)
+
+
+def dimos_virtual_box(ctx: Context, pos, r_cut, skin):
+    return ctx.virtual_box(pos, r_cut, skin)
 
 
 def dimos_vv_kick_drift(ctx: Context, pos, vel, F, inv_mass, dt, **kw):

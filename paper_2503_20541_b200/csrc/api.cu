@@ -217,6 +217,51 @@ DIMOS_API int dimos_nl_needs_rebuild(dimos_ctx* c, const void* pos, const void* 
     return DIMOS_OK;
 }
 
+static float from_ordered_bits(unsigned u)
+{
+    const unsigned v = (u & 0x80000000u) ? (u & 0x7fffffffu) : ~u;
+    float f;
+    memcpy(&f, &v, 4);
+    return f;
+}
+
+DIMOS_API int dimos_virtual_box(dimos_ctx* c, const void* pos, int64_t N, double r_cut, double skin, double* box_host,
+                                double* lo_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!pos || !box_host) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || !(r_cut > 0) || !(skin >= 0)) return set_error(ctx, DIMOS_EINVAL, "bad N, r_cut or skin");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    // scratch for the ordered-int min / max words (this call runs once per rebuild and synchronises anyway)
+    unsigned* d = nullptr;
+    DIMOS_CUDA_TRY(ctx, cudaMalloc(&d, 8 * sizeof(unsigned)));
+    const unsigned init[8] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u, 0u, 0u};
+    cudaError_t e = cudaMemcpyAsync(d, init, sizeof(init), cudaMemcpyHostToDevice, s);
+    int rc = e == cudaSuccess ? bbox_impl(ctx, pos, N, d, s) : set_error(ctx, DIMOS_ECUDA, cudaGetErrorString(e));
+    unsigned h[8] = {0};
+    if (!rc) {
+        e = cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) rc = set_error(ctx, DIMOS_ECUDA, cudaGetErrorString(e));
+    }
+    cudaFree(d);
+    if (rc) return rc;
+    if (h[6]) return set_error(ctx, DIMOS_EINVAL, "non-finite coordinate");
+    for (int a = 0; a < 3; ++a) {
+        const double lo = from_ordered_bits(h[a]), hi = from_ordered_bits(h[3 + a]);
+        // images of the system are at least r_cut + 2 skin apart: no pair within r_cut + skin crosses the seam, and the
+        // system may still spread by skin (the trigger fires at skin/2 per atom) before the box must be recomputed
+        double L = (hi - lo) + r_cut + 2.0 * skin + 1e-3;
+        const double Lmin = 2.0 * r_cut + 1e-3;  // dimos_nl_build requires r_cut <= L / 2
+        if (L < Lmin) L = Lmin;
+        box_host[a] = (double)(float)L >= L ? (double)(float)L : (double)nextafterf((float)L, INFINITY);  // fp32-representable
+        if (lo_host) lo_host[a] = lo;
+    }
+    return DIMOS_OK;
+}
+
 DIMOS_API int dimos_vv_kick_drift(dimos_ctx* c, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
                                   const void* pos_at_build, double skin, int32_t* flag_dev, int32_t* flag_host, void* stream)
 {

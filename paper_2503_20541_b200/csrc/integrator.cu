@@ -4,6 +4,8 @@
 // the separate needs_rebuild pass.  Constraints (steps 3, 6) and thermostats (step 7) are not built.
 //
 // Units: nm, ps, amu, kJ mol^-1 nm^-1: a = F / m is in nm ps^-2 without a conversion factor.
+#include <math.h>
+
 #include "common.cuh"
 #include "trigger.cuh"
 
@@ -50,6 +52,55 @@ __global__ void vv_kick_kernel(real* __restrict__ vel, const real* __restrict__ 
 #pragma unroll
         for (int a = 0; a < 3; ++a) vel[3 * i + a] += F[3 * i + a] * s;
     }
+}
+
+// bounding box of all positions (virtual box of a non-periodic system): ordered-int atomics on 6 words
+__device__ __forceinline__ unsigned ordered_bits(float f)
+{
+    const unsigned u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+template <typename real>
+__global__ void bbox_kernel(const real* __restrict__ pos, int64_t N, unsigned* __restrict__ out /* min[3], max[3], bad */)
+{
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    bool bad = false;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const real x = pos[3 * i + a];
+            if (!isfinite(x)) bad = true;
+            // round outwards to fp32 so that the fp32 bounds enclose an fp64 coordinate
+            const float xl = __double2float_rd((double)x), xh = __double2float_ru((double)x);
+            lo[a] = fminf(lo[a], xl);
+            hi[a] = fmaxf(hi[a], xh);
+        }
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+    if ((threadIdx.x & 31) == 0)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            atomicMin(&out[a], ordered_bits(lo[a]));
+            atomicMax(&out[3 + a], ordered_bits(hi[a]));
+        }
+    if (bad) out[6] = 1u;
+}
+
+int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStream_t s)
+{
+    int blocks = (int)((N + 255) / 256);
+    const int maxb = ctx->sm_count * 8;
+    if (blocks > maxb) blocks = maxb;
+    if (blocks < 1) blocks = 1;
+    if (ctx->precision == DIMOS_F64) bbox_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos, N, out_dev);
+    else bbox_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos, N, out_dev);
+    DIMOS_LAUNCH_CHECK(ctx, "bbox");
+    return DIMOS_OK;
 }
 
 static int grid_for(const Ctx* ctx, int64_t N)

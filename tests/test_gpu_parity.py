@@ -254,6 +254,52 @@ def test_edge_list_with_vectors_and_shifts(precision, index):
         ctx.close()
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_open_boundaries_through_the_virtual_box(precision):
+    """Non-periodic system: a water droplet in vacuum, far from the origin and partly at negative
+    coordinates.  The GPU path runs in the virtual periodic box dimos_virtual_box returns; the oracle in a box twenty
+    times larger, where no periodic image exists at all: neighbour set, forces, energy and virial must agree."""
+    import dataclasses
+
+    full = wl.make_config(1)
+    centre = 0.5 * full.box
+    mol = np.arange(full.n_atoms) // 3
+    keep_mol = np.unique(mol[(np.linalg.norm(full.pos[::3].astype(np.float64) - centre, axis=1) < 1.6).repeat(3)])
+    sel = np.isin(mol, keep_mol)
+    new_index = -np.ones(full.n_atoms, dtype=np.int64)
+    new_index[sel] = np.arange(sel.sum())
+    excl = full.excl_pairs[sel[full.excl_pairs[:, 0]] & sel[full.excl_pairs[:, 1]]]
+    excl = new_index[excl].astype(np.int32)
+    np_real = np.float64 if precision == "f64" else np.float32
+    pos = (full.pos[sel].astype(np.float64) - centre + np.array([-0.7, 31.25, 5.5])).astype(np_real)
+    drop = dataclasses.replace(full, pos=pos, charge=full.charge[sel].copy(), type=full.type[sel].copy(), excl_pairs=excl,
+                               mass=full.mass[sel].copy())
+    dev = torch.device("cuda", 0)
+    ctx = dimos.Context(0, precision)
+    try:
+        box, lo = dimos.dimos_virtual_box(ctx, torch.from_numpy(pos).to(dev), 1.0, 0.1)
+        ext = pos.astype(np.float64).max(0) - pos.astype(np.float64).min(0)
+        assert np.all(box >= ext + 1.0 + 0.2) and np.all(box <= ext + 1.0 + 0.2 + 0.01) and np.allclose(lo, pos.min(0), atol=1e-6)
+    finally:
+        ctx.close()
+    db = DeviceBox(drop, precision, box=box)
+    ctx = dimos.Context(0, precision)
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, box, 1.0, 0.1, db.excl)
+        pos64 = db.pos.double().cpu().numpy()
+        big = 20.0 * box
+        gp = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy()
+        check_neighbor_set(gp, pos64, big, 1.1, drop.excl_pairs)
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, method="rf")
+        torch.cuda.synchronize()
+        orc = oracle.nonbonded(pos64, db.charge.double().cpu().numpy(), drop.type, db.lj_np, big, 1.0, method=METHOD["rf"],
+                               excl_pairs=drop.excl_pairs, band=BAND, algorithm="bruteforce")
+        check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision)
+    finally:
+        ctx.close()
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)

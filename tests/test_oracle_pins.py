@@ -516,3 +516,24 @@ def test_edge_vectors_identities():
     assert np.allclose(d2, [[0.1, 0.0, 0.0]]) and s2.tolist() == [[-1, 0, 0]]
     d3, s3 = oracle.edge_vectors([[10.0, 11.0, 12.0], [10.3, 11.0, 12.4]], BIGBOX, [[0, 1]])
     assert s3.tolist() == [[0, 0, 0]] and np.allclose(d3, [[-0.3, 0.0, -0.4]])
+
+
+# --- non-periodic systems by embedding into a virtual box ------------------------------------------
+def test_virtual_box_embedding_equals_open_boundaries():
+    """A periodic box of edge extent + r_c + 2 skin around an isolated cluster gives the same pair set, energy and
+    forces as a box so large that periodicity cannot matter: the images are farther away than r_c + skin."""
+    wb = small_box(m=30, edge=2.3, seed=21)
+    pos = wb.pos.astype(np.float64) + np.array([-0.4, 7.0, 3.3])  # anywhere, partly negative
+    ext = pos.max(0) - pos.min(0)
+    rc, skin = 0.9, 0.1
+    vbox = ext + rc + 2 * skin
+    huge = 20.0 * vbox
+    a = oracle.nonbonded(pos, wb.charge, wb.type, lj_table(), vbox, rc, excl_pairs=wb.excl_pairs, algorithm="bruteforce")
+    b = oracle.nonbonded(pos, wb.charge, wb.type, lj_table(), huge, rc, excl_pairs=wb.excl_pairs, algorithm="bruteforce")
+    assert a.n_pairs == b.n_pairs and np.abs(a.F - b.F).max() < 1e-9 and a.E[0] == pytest.approx(b.E[0], rel=1e-12)
+    pa = oracle.neighbor_pairs(pos, vbox, rc + skin, wb.excl_pairs, "celllist")
+    pb = oracle.neighbor_pairs(pos, huge, rc + skin, wb.excl_pairs, "bruteforce")
+    assert np.array_equal(pa, pb)
+    # one skin less and a pair across the seam can enter the list: the margin is needed
+    tight = ext + 0.5 * (rc + skin)
+    assert oracle.neighbor_pairs(pos, np.maximum(tight, 2 * rc + 1e-3), rc + skin, wb.excl_pairs, "bruteforce").shape[0] >= pb.shape[0]
