@@ -495,6 +495,12 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
     const int64_t U = (int64_t)blockIdx.x * BL_WARPS + wib;
+    __shared__ real4 code_off[27];  // image offset of every stencil code (saves the divisions by 9 and 3 per candidate)
+    if (threadIdx.x < 27) {
+        const int c = threadIdx.x;
+        code_off[c] = make4((real)(c / 9 - 1) * P.h[0], (real)((c / 3) % 3 - 1) * P.h[1], (real)(c % 3 - 1) * P.h[2], (real)0);
+    }
+    __syncthreads();
     if (U >= P.n_units) return;  // no block-wide barriers below
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -644,8 +650,8 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                 slot = v * UNIT + (t & 7);
                 if (P.perm[slot] >= 0) {
                     real4 pj = P.xyz[slot];
-                    const int dx = code / 9 - 1, dy = (code / 3) % 3 - 1, dz = code % 3 - 1;
-                    const real px = pj.x + (real)dx * P.h[0], py = pj.y + (real)dy * P.h[1], pz = pj.z + (real)dz * P.h[2];
+                    const real4 co = code_off[code];
+                    const real px = pj.x + co.x, py = pj.y + co.y, pz = pj.z + co.z;
                     unsigned bits = 0;
 #pragma unroll
                     for (int i = 0; i < UNIT; ++i) {
