@@ -653,16 +653,33 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                     const real4 co = code_off[code];
                     const real px = pj.x + co.x, py = pj.y + co.y, pz = pj.z + co.z;
                     unsigned bits = 0;
+                    if constexpr (sizeof(real) == 4 && PBC == 0) {
+                        // fp32, image from the cell offset: two i-atoms per packed instruction (FADD2/FMUL2/FFMA2)
+                        const float2 nx = make_float2(-(float)px, -(float)px), ny = make_float2(-(float)py, -(float)py),
+                                     nz = make_float2(-(float)pz, -(float)pz);
 #pragma unroll
-                    for (int i = 0; i < UNIT; ++i) {
-                        real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
-                        if (PBC == 1) {
-                            ddx -= P.L[0] * rint_r(ddx / P.L[0]);
-                            ddy -= P.L[1] * rint_r(ddy / P.L[1]);
-                            ddz -= P.L[2] * rint_r(ddz / P.L[2]);
+                        for (int q = 0; q < UNIT / 2; ++q) {
+                            const float2 ddx = __fadd2_rn(make_float2((float)xi[2 * q], (float)xi[2 * q + 1]), nx);
+                            const float2 ddy = __fadd2_rn(make_float2((float)yi[2 * q], (float)yi[2 * q + 1]), ny);
+                            const float2 ddz = __fadd2_rn(make_float2((float)zi[2 * q], (float)zi[2 * q + 1]), nz);
+                            float2 r2 = __fmul2_rn(ddx, ddx);
+                            r2 = __ffma2_rn(ddy, ddy, r2);
+                            r2 = __ffma2_rn(ddz, ddz, r2);
+                            bits |= (r2.x < (float)P.rnl2 ? 1u : 0u) << (2 * q);
+                            bits |= (r2.y < (float)P.rnl2 ? 1u : 0u) << (2 * q + 1);
                         }
-                        real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                        bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < UNIT; ++i) {
+                            real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
+                            if (PBC == 1) {
+                                ddx -= P.L[0] * rint_r(ddx / P.L[0]);
+                                ddy -= P.L[1] * rint_r(ddy / P.L[1]);
+                                ddz -= P.L[2] * rint_r(ddz / P.L[2]);
+                            }
+                            real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                            bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
+                        }
                     }
                     mask = valid_i & ~excl_bits(slot);
                     acc = (bits & mask) != 0;
