@@ -211,7 +211,9 @@ __device__ __forceinline__ void bitonic_sort_u64(unsigned long long* K, int npad
     }
 }
 
-constexpr int KD_SEGS = KD_MAX / UNIT;  // 512
+// segment arrays of the k-d bisection: a cell of npad (power of two) atoms ends in at most npad / UNIT segments; twice
+// that is allocated (the split step writes children 2s, 2s+1)
+__host__ __device__ inline int kd_segs(int npad_max) { return 2 * (npad_max / UNIT) < 8 ? 8 : 2 * (npad_max / UNIT); }
 
 template <typename real>
 __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const int* __restrict__ cell_start,
@@ -230,19 +232,20 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
     int npad = 32;
     while (npad < n) npad <<= 1;
 
+    const int KS = kd_segs(npad_max);
     unsigned long long* K = reinterpret_cast<unsigned long long*>(smem_raw);
     real* X = reinterpret_cast<real*>(K + npad_max);
     real* Y = X + npad_max;
     real* Z = Y + npad_max;
     int* ID = reinterpret_cast<int*>(Z + npad_max);
     int* segS = ID + npad_max;
-    int* segN = segS + KD_SEGS;
-    int* segS2 = segN + KD_SEGS;
-    int* segN2 = segS2 + KD_SEGS;
-    int* segAxis = segN2 + KD_SEGS;
-    int* bbmin = segAxis + KD_SEGS;  // [3][KD_SEGS]
-    int* bbmax = bbmin + 3 * KD_SEGS;
-    unsigned short* SEG = reinterpret_cast<unsigned short*>(bbmax + 3 * KD_SEGS);
+    int* segN = segS + KS;
+    int* segS2 = segN + KS;
+    int* segN2 = segS2 + KS;
+    int* segAxis = segN2 + KS;
+    int* bbmin = segAxis + KS;  // [3][KS]
+    int* bbmax = bbmin + 3 * KS;
+    unsigned short* SEG = reinterpret_cast<unsigned short*>(bbmax + 3 * KS);
     __shared__ int any_big;
 
     // canonical order: by original atom index (makes the result independent of the binning atomics)
@@ -284,8 +287,8 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
         __syncthreads();
         for (int s = threadIdx.x; s < nseg; s += blockDim.x) {
             if (cN[s] > UNIT) any_big = 1;
-            bbmin[s] = bbmin[KD_SEGS + s] = bbmin[2 * KD_SEGS + s] = 0x7fffffff;
-            bbmax[s] = bbmax[KD_SEGS + s] = bbmax[2 * KD_SEGS + s] = (int)0x80000000;
+            bbmin[s] = bbmin[KS + s] = bbmin[2 * KS + s] = 0x7fffffff;
+            bbmax[s] = bbmax[KS + s] = bbmax[2 * KS + s] = (int)0x80000000;
         }
         __syncthreads();
         if (!any_big) break;
@@ -298,8 +301,8 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
                 int oy = (int)(ordered_u32((float)Y[lid]) ^ 0x80000000u);
                 int oz = (int)(ordered_u32((float)Z[lid]) ^ 0x80000000u);
                 atomicMin(&bbmin[s], ox); atomicMax(&bbmax[s], ox);
-                atomicMin(&bbmin[KD_SEGS + s], oy); atomicMax(&bbmax[KD_SEGS + s], oy);
-                atomicMin(&bbmin[2 * KD_SEGS + s], oz); atomicMax(&bbmax[2 * KD_SEGS + s], oz);
+                atomicMin(&bbmin[KS + s], oy); atomicMax(&bbmax[KS + s], oy);
+                atomicMin(&bbmin[2 * KS + s], oz); atomicMax(&bbmax[2 * KS + s], oz);
             }
         }
         __syncthreads();
@@ -309,8 +312,8 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
                 float ext[3];
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
-                    unsigned lo = (unsigned)bbmin[a * KD_SEGS + s] ^ 0x80000000u;
-                    unsigned hi = (unsigned)bbmax[a * KD_SEGS + s] ^ 0x80000000u;
+                    unsigned lo = (unsigned)bbmin[a * KS + s] ^ 0x80000000u;
+                    unsigned hi = (unsigned)bbmax[a * KS + s] ^ 0x80000000u;
                     // undo ordered_u32
                     float flo = __uint_as_float((lo & 0x80000000u) ? (lo & 0x7fffffffu) : ~lo);
                     float fhi = __uint_as_float((hi & 0x80000000u) ? (hi & 0x7fffffffu) : ~hi);
@@ -402,7 +405,7 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
 
 static size_t kd_smem_bytes(int npad_max, size_t real_size)
 {
-    return (size_t)npad_max * (8 + 3 * real_size + 4 + 2) + (size_t)KD_SEGS * 4 * (5 + 6) + 64;
+    return (size_t)npad_max * (8 + 3 * real_size + 4 + 2) + (size_t)kd_segs(npad_max) * 4 * (5 + 6) + 64;
 }
 
 // ------------------------------------------------------------------------------------------------
