@@ -300,6 +300,20 @@ def test_open_boundaries_through_the_virtual_box(precision):
         ctx.close()
 
 
+@pytest.mark.gpu
+def test_uneven_density_grows_the_row_capacity_f32():
+    """configs[1] squeezed into half of its box along x (a slab at twice the mean density next to vacuum): the first
+    row-capacity estimate comes from the mean density, so the build must notice the overflow, grow and repeat
+    (n_rebuild_grow > 0), and the result must still match the oracle."""
+    import dataclasses
+
+    wb = wl.make_config(1)
+    pos = wb.pos.copy()
+    pos[:, 0] *= np.float32(0.5)
+    rep = run_case(dataclasses.replace(wb, pos=pos), "f32", 1.0, 0.1, "rf")
+    assert rep["stats"]["n_rebuild_grow"] >= 1, rep["stats"]
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)
