@@ -314,6 +314,27 @@ def test_uneven_density_grows_the_row_capacity_f32():
     assert rep["stats"]["n_rebuild_grow"] >= 1, rep["stats"]
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_exclusion_partner_limit(precision):
+    """Every atom of the mixture excluded from its 16 successors and 16 predecessors in index order: 32 partners, the
+    documented limit per atom (include/dimos.h), so every unit carries on the order of a hundred partially masked
+    entries; neighbour set, Ewald exclusion correction and forces must match.  One partner more is an error."""
+    import dataclasses
+
+    mix = _mixture_box(16, 4.6, 5)
+    n = mix.n_atoms
+    i = np.arange(n, dtype=np.int32)
+
+    def chain(kmax):
+        e = np.concatenate([np.stack([i[:-k], i[k:]], axis=1) for k in range(1, kmax + 1)]).astype(np.int32)
+        return e[np.lexsort((e[:, 1], e[:, 0]))]
+
+    run_case(dataclasses.replace(mix, excl_pairs=chain(16)), precision, 1.0, 0.1, "ewald")
+    with pytest.raises(dimos.DimosError):
+        run_case(dataclasses.replace(mix, excl_pairs=chain(17)), precision, 1.0, 0.1, "ewald")
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)
