@@ -29,3 +29,49 @@ def vv_kick(vel_half, force_new, inv_mass, dt):
     force_new = np.asarray(force_new, dtype=np.float64)
     inv_mass = np.asarray(inv_mass, dtype=np.float64).reshape(-1, 1)
     return vel_half + 0.5 * dt * (force_new * inv_mass)
+
+
+def dispersion_correction(type_, lj_table, box, r_cut, r_switch=0.0):
+    """Long-range dispersion (LJ tail) correction, PAPER.md:202 ("long-range dispersion corrections that approximate the
+    contributions beyond r_c"; no formula given: reading C-22).  Homogeneous fluid beyond the truncation, g(r) = 1:
+
+        E = (2 pi / V) sum_a sum_b N_a N_b  integral_0^inf [1 - S(r)] U_ab(r) r^2 dr
+
+    with U_ab the 12-6 potential of Eq. 4, S(r) = 1 for r < r_s, Eq. 6 for r_s <= r < r_c, 0 beyond r_c (r_switch <= 0 or
+    >= r_cut: S = 1 below r_c).  Evaluated by adaptive quadrature of exactly this integrand (scipy QUADPACK).
+    Returns (E, W) with W the 3x3 virial in the convention of reading C-7 (tr W = -dE/d lambda at fixed r_c): E scales as
+    1/V, so W = E * identity."""
+    from scipy import integrate
+
+    type_ = np.asarray(type_, dtype=np.int64)
+    lj_table = np.asarray(lj_table, dtype=np.float64)
+    nt = lj_table.shape[0]
+    counts = np.bincount(type_, minlength=nt).astype(np.float64)
+    vol = float(np.prod(np.asarray(box, dtype=np.float64)))
+    switched = 0.0 < r_switch < r_cut
+
+    def one_minus_s(r):
+        if r >= r_cut:
+            return 1.0
+        if not switched or r < r_switch:
+            return 0.0
+        x = (r - r_switch) / (r_cut - r_switch)
+        return 1.0 - (1.0 - 6.0 * x ** 5 + 15.0 * x ** 4 - 10.0 * x ** 3)
+
+    total = 0.0
+    for a in range(nt):
+        for b in range(nt):
+            sigma, eps = lj_table[a, b]
+            if eps == 0.0 or sigma == 0.0 or counts[a] == 0 or counts[b] == 0:
+                continue
+
+            def integrand(r, sigma=sigma, eps=eps):
+                sr6 = (sigma / r) ** 6
+                return one_minus_s(r) * 4.0 * eps * (sr6 * sr6 - sr6) * r * r
+
+            lo = r_switch if switched else r_cut
+            inner = integrate.quad(integrand, lo, r_cut, epsabs=0, epsrel=1e-13)[0] if switched else 0.0
+            outer = integrate.quad(integrand, r_cut, np.inf, epsabs=0, epsrel=1e-13)[0]
+            total += counts[a] * counts[b] * (inner + outer)
+    e = 2.0 * np.pi / vol * total
+    return e, e * np.eye(3)

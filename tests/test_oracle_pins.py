@@ -537,3 +537,27 @@ def test_virtual_box_embedding_equals_open_boundaries():
     # one skin less and a pair across the seam can enter the list: the margin is needed
     tight = ext + 0.5 * (rc + skin)
     assert oracle.neighbor_pairs(pos, np.maximum(tight, 2 * rc + 1e-3), rc + skin, wb.excl_pairs, "bruteforce").shape[0] >= pb.shape[0]
+
+
+# --- long-range dispersion correction (reading C-22) ------------------------------------------------
+def test_dispersion_correction_textbook_tail_and_switch_limits():
+    """Plain truncation: the textbook tail 8 pi N^2 eps / V [sigma^12 / (9 r_c^9) - sigma^6 / (3 r_c^3)] for one species.
+    With the switch the correction lies between the plain values at r_s and at r_c and tends to the plain value as
+    r_s -> r_c; it is extensive (doubling the box at constant density doubles it)."""
+    n_o, vol = 1000.0, 30.0
+    types = np.zeros(int(n_o), dtype=np.int32)
+    box = np.array([vol ** (1 / 3)] * 3)
+    tab = lj_table()
+    s, e, rc = wl.SIGMA_O, wl.EPS_O, 1.0
+    textbook = 8.0 * np.pi * n_o * n_o * e / vol * (s ** 12 / (9 * rc ** 9) - s ** 6 / (3 * rc ** 3))
+    got, w = oracle.dispersion_correction(types, tab, box, rc)
+    assert got == pytest.approx(textbook, rel=1e-12) and np.allclose(w, got * np.eye(3))
+    at_rs = oracle.dispersion_correction(types, tab, box, 0.8)[0]
+    sw = oracle.dispersion_correction(types, tab, box, rc, r_switch=0.8)[0]
+    assert at_rs < sw < got < 0.0  # attractive tail; more of it is missing the earlier the potential is cut
+    assert oracle.dispersion_correction(types, tab, box, rc, r_switch=rc - 1e-7)[0] == pytest.approx(got, rel=1e-6)
+    big = oracle.dispersion_correction(np.zeros(2000, dtype=np.int32), tab, box * 2 ** (1 / 3), rc)[0]
+    assert big == pytest.approx(2 * got, rel=1e-12)
+    # hydrogens (epsilon = 0) do not contribute
+    mixed = oracle.dispersion_correction(np.concatenate([types, np.ones(2000, dtype=np.int32)]), tab, box, rc)[0]
+    assert mixed == pytest.approx(got, rel=1e-14)
