@@ -211,6 +211,20 @@ DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
                                     int64_t* n_pairs_host, void* stream);
 
+/* dimos_dispersion_correction -- PAPER.md:202 ("long-range dispersion corrections that approximate the contributions
+ * beyond r_c"; the paper gives no formula: reading C-22).  The homogeneous-fluid tail of the 12-6 potential that the
+ * truncated (and, with r_switch, switched) pair sum leaves out:
+ *   E = (2 pi / V) sum_a sum_b N_a N_b  integral [1 - S(r)] U_ab(r) r^2 dr,   S = 1 below r_s, Eq. 6 up to r_c, 0 beyond
+ * A constant for a given composition, box, r_cut and r_switch; the type histogram is taken on the device, the
+ * integrals in closed form (tail) and by Gauss-Legendre quadrature (switching interval) on the host.
+ *   type      dev, N int32;   lj_table  dev, ntypes x ntypes x 2 doubles (sigma_ab, eps_ab) as for dimos_nonbonded
+ *   box       host, 3 doubles;   r_switch <= 0 or >= r_cut: plain truncation
+ *   E_host    host, 1 double, written;   virial_host  host, 9 doubles or NULL: E * identity (E ~ 1/V; reading C-7)
+ * Synchronises the stream. */
+DIMOS_API int dimos_dispersion_correction(dimos_ctx* ctx, const int32_t* type, int64_t N, const double* lj_table,
+                                          int32_t ntypes, const double* box, double r_cut, double r_switch, double* E_host,
+                                          double* virial_host, void* stream);
+
 /* dimos_virtual_box -- non-periodic systems ("the system is ... embedded into a non-periodic box" for the
  * neighbour-list computation).  Returns the edges of a virtual periodic box around the current positions that is large
  * enough for the periodic routines to reproduce open boundaries exactly: box[a] = extent[a] + r_cut + 2 skin (at least

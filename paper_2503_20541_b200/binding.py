@@ -30,6 +30,7 @@ EXPORTED_SYMBOLS = (
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
+    "dimos_dispersion_correction",
 )
 
 
@@ -96,6 +97,8 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
     lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
     lib.dimos_virtual_box.argtypes = [vp, vp, i64, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
+    lib.dimos_dispersion_correction.argtypes = [vp, vp, i64, vp, i32, ctypes.POINTER(dbl), dbl, dbl, ctypes.POINTER(dbl),
+                                                ctypes.POINTER(dbl), vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -110,7 +113,7 @@ def load_library() -> ctypes.CDLL:
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
-                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box"):
+                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -305,6 +308,21 @@ class Context:
             nl.handle = h
         return nl, bool(rebuilt.value)
 
+    def dispersion_correction(self, type_, lj_table, box, r_cut, r_switch=0.0):
+        """dimos_dispersion_correction: (E float, virial (3,3) float64 numpy) of the LJ tail correction."""
+        import numpy as np
+
+        type_ = self._dev(type_, torch.int32)
+        lj_table = self._dev(lj_table, torch.float64)
+        e = ctypes.c_double(0.0)
+        w = (ctypes.c_double * 9)()
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_dispersion_correction(self.handle, type_.data_ptr(), type_.numel(), lj_table.data_ptr(),
+                                                      lj_table.shape[0], _box3(box), float(r_cut), float(r_switch),
+                                                      ctypes.byref(e), w, _stream_ptr())
+        self._check(rc)
+        return float(e.value), np.array(list(w), dtype=np.float64).reshape(3, 3)
+
     def virtual_box(self, pos, r_cut, skin):
         """dimos_virtual_box: (box (3,) float64 numpy, lower corner (3,)) of the virtual periodic box of an open system."""
         import numpy as np
@@ -440,6 +458,10 @@ def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = T
 
 def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
     return ctx.nonbonded(nl, pos, charge, type_, lj_table, **kw)
+
+
+def dimos_dispersion_correction(ctx: Context, type_, lj_table, box, r_cut, r_switch=0.0):
+    return ctx.dispersion_correction(type_, lj_table, box, r_cut, r_switch)
 
 
 def dimos_virtual_box(ctx: Context, pos, r_cut, skin):

@@ -146,6 +146,8 @@ int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s);
 int vv_kick_drift_impl(Ctx* ctx, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
                        const void* pos_at_build, double skin, int32_t* flag_dev, cudaStream_t s);
 int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStream_t s);
+int type_histogram_impl(Ctx* ctx, const int32_t* type, int64_t N, int nt, unsigned long long* counts_dev, int* bad_dev,
+                        cudaStream_t s);
 int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, cudaStream_t s);
 
 // stencil code <-> offset

@@ -103,6 +103,35 @@ int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStrea
     return DIMOS_OK;
 }
 
+// histogram of the LJ types (dispersion correction): block-local counts in shared memory, then atomics
+__global__ void type_histogram_kernel(const int* __restrict__ type, int64_t N, int nt, unsigned long long* __restrict__ counts,
+                                      int* __restrict__ bad)
+{
+    __shared__ unsigned sh[MAX_TYPES];
+    for (int t = threadIdx.x; t < nt; t += blockDim.x) sh[t] = 0u;
+    __syncthreads();
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        const int t = type[i];
+        if (t < 0 || t >= nt) *bad = 1;
+        else atomicAdd(&sh[t], 1u);
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < nt; t += blockDim.x)
+        if (sh[t]) atomicAdd(&counts[t], (unsigned long long)sh[t]);
+}
+
+int type_histogram_impl(Ctx* ctx, const int32_t* type, int64_t N, int nt, unsigned long long* counts_dev, int* bad_dev,
+                        cudaStream_t s)
+{
+    int blocks = (int)((N + 255) / 256);
+    const int maxb = ctx->sm_count * 8;
+    if (blocks > maxb) blocks = maxb;
+    if (blocks < 1) blocks = 1;
+    type_histogram_kernel<<<blocks, 256, 0, s>>>(type, N, nt, counts_dev, bad_dev);
+    DIMOS_LAUNCH_CHECK(ctx, "type_histogram");
+    return DIMOS_OK;
+}
+
 static int grid_for(const Ctx* ctx, int64_t N)
 {
     int blocks = (int)((N + 255) / 256);

@@ -335,6 +335,25 @@ def test_exclusion_partner_limit(precision):
         run_case(dataclasses.replace(mix, excl_pairs=chain(17)), precision, 1.0, 0.1, "ewald")
 
 
+@pytest.mark.gpu
+def test_dispersion_correction_matches_oracle():
+    """LJ tail correction (reading C-22): device type histogram + host integrals against the oracle's
+    adaptive quadrature of the definition, for water (one LJ species) and the three-type mixture, with and without switch."""
+    ctx = dimos.Context(0, "f32")
+    try:
+        for wb in (wl.make_config(1), _mixture_box(16, 4.6, 3)):
+            db = DeviceBox(wb, "f32")
+            for rs in (0.0, 0.8, 0.95):
+                e, w = dimos.dimos_dispersion_correction(ctx, db.type, db.lj, db.box, 1.0, rs)
+                e_o, w_o = oracle.dispersion_correction(wb.type, db.lj_np, db.box, 1.0, rs)
+                assert e == pytest.approx(e_o, rel=1e-10) and np.allclose(w, w_o, rtol=1e-10, atol=0)
+                assert e < 0.0
+        with pytest.raises(dimos.DimosError):
+            dimos.dimos_dispersion_correction(ctx, db.type + 7, db.lj, db.box, 1.0, 0.0)  # type index out of range
+    finally:
+        ctx.close()
+
+
 def test_tiny_systems_f64():
     """One water (everything excluded => E = 0, F = 0 under RF) and two waters (9 pairs)."""
     two = wl.make_water_box(2, 5.0, 3)
