@@ -239,8 +239,8 @@ DIMOS_API int dimos_dispersion_correction(dimos_ctx* ctx, const int32_t* type, i
 DIMOS_API int dimos_virtual_box(dimos_ctx* ctx, const void* pos, int64_t N, double r_cut, double skin, double* box_host,
                                 double* lo_host, void* stream);
 
-/* dimos_vv_kick_drift / dimos_vv_kick -- velocity Verlet, PAPER.md:281-292 (steps 1 + 2, and step 5; constraints and
- * thermostats, steps 3, 6, 7, are not built).  Units nm, ps, amu, kJ mol^-1 nm^-1: a = F / m needs no conversion factor.
+/* dimos_vv_kick_drift / dimos_vv_kick -- velocity Verlet, PAPER.md:281-292 (steps 1 + 2, and step 5; steps 3 and 6 for rigid water are
+ * dimos_settle and dimos_settle_velocities; the thermostat of step 7 is not built).  Units nm, ps, amu, kJ mol^-1 nm^-1: a = F / m needs no conversion factor.
  *   kick_drift:  v <- v + (dt/2) F / m;  x <- x + dt v      (in place)
  *   kick:        v <- v + (dt/2) F / m                      (in place, with the forces at the new positions)
  *   pos, vel, F   dev, N x 3, float or double per the context precision
@@ -253,6 +253,32 @@ DIMOS_API int dimos_vv_kick_drift(dimos_ctx* ctx, void* pos, void* vel, const vo
                                   void* stream);
 DIMOS_API int dimos_vv_kick(dimos_ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
                             void* stream);
+
+/* dimos_settle -- step 3 of velocity Verlet for rigid three-site water: the SETTLE closed form that
+ * PAPER.md:327 names, i.e. the positions the three distance constraints |O-H1| = |O-H2| = d_OH, |H1-H2| = d_HH admit when
+ * the correction of every pair acts along its OLD bond vector, weighted by inverse mass (the converged SHAKE solution).
+ *   pos_old   dev, N x 3: positions before the drift; they must satisfy the constraints
+ *   pos       dev, N x 3: positions after the unconstrained drift, corrected in place
+ *   vel       dev, N x 3 or NULL: if given, v += (x_constrained - x_unconstrained) / dt, the half-step velocity that goes
+ *             with the constrained positions (step 6 is dimos_settle_velocities)
+ *   water     dev, n_w x 3 int32: atom indices (O, H1, H2) of each molecule; molecules must be whole (no atom of a molecule
+ *             wrapped into another periodic image), which dimos_vv_kick_drift preserves since it never wraps
+ *   m_O, m_H  masses; d_OH, d_HH the constraint lengths (0 < d_HH < 2 d_OH)
+ * float or double per the context precision (coordinates enter only as differences to the old oxygen).  Asynchronous on
+ * the stream; n_w = 0 is a no-op.  DIMOS_EINVAL for bad lengths, masses or dt. */
+DIMOS_API int dimos_settle(dimos_ctx* ctx, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w,
+                           double m_O, double m_H, double d_OH, double d_HH, double dt, void* stream);
+
+/* dimos_settle_velocities -- step 6 of velocity Verlet for rigid three-site water: after the second
+ * kick, remove the component of every relative velocity along its bond, (v_i - v_j) . (x_i - x_j) = 0 for the three bonds,
+ * by impulses along the bonds shared by inverse mass (the converged RATTLE velocity stage); the three multipliers of a
+ * molecule come from one direct 3 x 3 solve.  Linear and angular momentum of each molecule are unchanged.
+ *   pos     dev, N x 3: the (constrained) positions of the step
+ *   vel     dev, N x 3: corrected in place
+ *   water   dev, n_w x 3 int32 (O, H1, H2), molecules whole, as for dimos_settle
+ * Asynchronous on the stream; n_w = 0 is a no-op. */
+DIMOS_API int dimos_settle_velocities(dimos_ctx* ctx, const void* pos, void* vel, const int32_t* water, int64_t n_w,
+                                      double m_O, double m_H, void* stream);
 
 /* dimos_nl_set_exceptions -- PAPER.md:243 ("1-4 exceptions ... scale the strength of the non-bonded interactions by
  * some common factor", or an individual factor per pair; "handled explicitly by the non-bonded interaction method").

@@ -75,3 +75,54 @@ def dispersion_correction(type_, lj_table, box, r_cut, r_switch=0.0):
             total += counts[a] * counts[b] * (inner + outer)
     e = 2.0 * np.pi / vol * total
     return e, e * np.eye(3)
+
+
+def shake_water(pos_old, pos_new, mass, d_oh, d_hh, tol=1e-14, max_iter=500):
+    """Position constraints of rigid three-site water (step 3 of PAPER.md:281-292; PAPER.md:327 names SETTLE for it), as
+    the plain iterative SHAKE procedure run to convergence: for every molecule (atoms 3k, 3k+1, 3k+2 = O, H, H) the new
+    positions are corrected along the OLD bond vectors, x_i += g m_i^-1 r_ij_old, x_j -= g m_j^-1 r_ij_old with
+    g = (d_ij^2 - |r_ij_new|^2) / (2 (1/m_i + 1/m_j) r_ij_new . r_ij_old), until |r_ij| = d_ij for the three bonds.
+    SETTLE solves the same equations in closed form, so a converged SHAKE is its oracle.  Returns the constrained
+    positions (fp64); pos_old must satisfy the constraints."""
+    x0 = np.asarray(pos_old, dtype=np.float64).reshape(-1, 3, 3)
+    x = np.array(pos_new, dtype=np.float64).reshape(-1, 3, 3)
+    im = 1.0 / np.asarray(mass, dtype=np.float64).reshape(-1, 3)
+    bonds = ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh))
+    for _ in range(max_iter):
+        worst = 0.0
+        for i, j, d in bonds:
+            r_old = x0[:, i] - x0[:, j]
+            r_new = x[:, i] - x[:, j]
+            diff = d * d - (r_new * r_new).sum(1)
+            worst = max(worst, float(np.abs(diff).max()) / (d * d))
+            g = diff / (2.0 * (im[:, i] + im[:, j]) * (r_new * r_old).sum(1))
+            x[:, i] += (g * im[:, i])[:, None] * r_old
+            x[:, j] -= (g * im[:, j])[:, None] * r_old
+        if worst < tol:
+            break
+    return x.reshape(-1, 3)
+
+
+def rattle_water_velocities(pos, vel, mass, tol=1e-15, max_iter=2000):
+    """Velocity constraints of rigid three-site water (step 6 of PAPER.md:281-292), as the plain iterative RATTLE velocity
+    stage run to convergence: for every bond (i, j) of a molecule (atoms 3k, 3k+1, 3k+2) the component of the relative
+    velocity along the bond is removed by an impulse along r_ij shared by inverse mass,
+    k = (v_ij . r_ij) / (|r_ij|^2 (1/m_i + 1/m_j)),  v_i -= k r_ij / m_i,  v_j += k r_ij / m_j, until v_ij . r_ij = 0 for the
+    three bonds.  Returns the constrained velocities (fp64)."""
+    x = np.asarray(pos, dtype=np.float64).reshape(-1, 3, 3)
+    v = np.array(vel, dtype=np.float64).reshape(-1, 3, 3)
+    im = 1.0 / np.asarray(mass, dtype=np.float64).reshape(-1, 3)
+    scale = max(float(np.abs(v).max()), 1e-300)
+    for _ in range(max_iter):
+        worst = 0.0
+        for i, j in ((0, 1), (0, 2), (1, 2)):
+            r = x[:, i] - x[:, j]
+            rv = ((v[:, i] - v[:, j]) * r).sum(1)
+            r2 = (r * r).sum(1)
+            worst = max(worst, float((np.abs(rv) / np.sqrt(r2)).max()) / scale)
+            k = rv / (r2 * (im[:, i] + im[:, j]))
+            v[:, i] -= (k * im[:, i])[:, None] * r
+            v[:, j] += (k * im[:, j])[:, None] * r
+        if worst < tol:
+            break
+    return v.reshape(-1, 3)

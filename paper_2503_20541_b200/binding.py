@@ -30,7 +30,7 @@ EXPORTED_SYMBOLS = (
     "dimos_probe_fp32_peak", "dimos_status_string", "dimos_last_error", "dimos_version",
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
-    "dimos_dispersion_correction",
+    "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
 )
 
 
@@ -95,6 +95,8 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_nl_set_exceptions.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.dimos_vv_kick_drift.argtypes = [vp, vp, vp, vp, vp, i64, dbl, vp, dbl, vp, ctypes.POINTER(i32), vp]
     lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
+    lib.dimos_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp]
+    lib.dimos_settle_velocities.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, vp]
     lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
     lib.dimos_virtual_box.argtypes = [vp, vp, i64, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     lib.dimos_dispersion_correction.argtypes = [vp, vp, i64, vp, i32, ctypes.POINTER(dbl), dbl, dbl, ctypes.POINTER(dbl),
@@ -113,7 +115,8 @@ def load_library() -> ctypes.CDLL:
     for name in ("dimos_create", "dimos_destroy", "dimos_nl_build", "dimos_nl_destroy", "dimos_nl_needs_rebuild",
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
-                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction"):
+                 "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
+                 "dimos_settle", "dimos_settle_velocities"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -207,6 +210,13 @@ class Context:
             self.close()
         except Exception:
             pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+        return False
 
     # -- the C-ABI calls -------------------------------------------------------------------------
     def nl_build(self, pos, box, r_cut, skin, excl_pairs=None, pos_at_build=None, nl: NeighborList | None = None):
@@ -367,6 +377,29 @@ class Context:
                                         _stream_ptr())
         self._check(rc)
 
+    def settle(self, pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=None, dt=0.0):
+        """dimos_settle: rigid-water position constraints (velocity-Verlet step 3) in place on pos (and vel if given)."""
+        pos_old = self._dev(pos_old, self.real, 3)
+        pos = self._dev(pos, self.real, 3)
+        water = self._dev(water, torch.int32, 3)
+        if vel is not None:
+            vel = self._dev(vel, self.real, 3)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_settle(self.handle, pos_old.data_ptr(), pos.data_ptr(), vel.data_ptr() if vel is not None else None,
+                                       water.data_ptr(), water.shape[0], float(m_O), float(m_H), float(d_OH), float(d_HH),
+                                       float(dt), _stream_ptr())
+        self._check(rc)
+
+    def settle_velocities(self, pos, vel, water, m_O, m_H):
+        """dimos_settle_velocities: rigid-water velocity constraints (velocity-Verlet step 6) in place on vel."""
+        pos = self._dev(pos, self.real, 3)
+        vel = self._dev(vel, self.real, 3)
+        water = self._dev(water, torch.int32, 3)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_settle_velocities(self.handle, pos.data_ptr(), vel.data_ptr(), water.data_ptr(), water.shape[0],
+                                                  float(m_O), float(m_H), _stream_ptr())
+        self._check(rc)
+
     def nl_set_exceptions(self, nl: NeighborList, pairs, scale):
         """dimos_nl_set_exceptions: pairs (n,2) int32 i<j, scale (n,2) float64 = (Coulomb scale, LJ scale); None clears."""
         if pairs is None or len(pairs) == 0:
@@ -474,6 +507,14 @@ def dimos_vv_kick_drift(ctx: Context, pos, vel, F, inv_mass, dt, **kw):
 
 def dimos_vv_kick(ctx: Context, vel, F, inv_mass, dt):
     return ctx.vv_kick(vel, F, inv_mass, dt)
+
+
+def dimos_settle(ctx: Context, pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=None, dt=0.0):
+    return ctx.settle(pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=vel, dt=dt)
+
+
+def dimos_settle_velocities(ctx: Context, pos, vel, water, m_O, m_H):
+    return ctx.settle_velocities(pos, vel, water, m_O, m_H)
 
 
 def dimos_nl_set_exceptions(ctx: Context, nl: NeighborList, pairs, scale):

@@ -366,6 +366,34 @@ DIMOS_API int dimos_vv_kick(dimos_ctx* c, void* vel, const void* F, const void* 
     return vv_kick_impl(ctx, vel, F, inv_mass, N, dt, (cudaStream_t)stream);
 }
 
+DIMOS_API int dimos_settle(dimos_ctx* c, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w,
+                           double m_O, double m_H, double d_OH, double d_HH, double dt, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (n_w == 0) return DIMOS_OK;
+    if (!pos_old || !pos || !water) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (n_w < 0) return set_error(ctx, DIMOS_EINVAL, "n_w < 0");
+    if (!(m_O > 0) || !(m_H > 0)) return set_error(ctx, DIMOS_EINVAL, "masses must be > 0");
+    if (!(d_OH > 0) || !(d_HH > 0) || !(d_HH < 2.0 * d_OH)) return set_error(ctx, DIMOS_EINVAL, "need 0 < d_HH < 2 d_OH");
+    if (vel && !(dt > 0)) return set_error(ctx, DIMOS_EINVAL, "dt must be > 0 when vel is given");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return settle_impl(ctx, pos_old, pos, vel, water, n_w, m_O, m_H, d_OH, d_HH, dt, (cudaStream_t)stream);
+}
+
+DIMOS_API int dimos_settle_velocities(dimos_ctx* c, const void* pos, void* vel, const int32_t* water, int64_t n_w, double m_O,
+                                      double m_H, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (n_w == 0) return DIMOS_OK;
+    if (!pos || !vel || !water) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (n_w < 0) return set_error(ctx, DIMOS_EINVAL, "n_w < 0");
+    if (!(m_O > 0) || !(m_H > 0)) return set_error(ctx, DIMOS_EINVAL, "masses must be > 0");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return settle_vel_impl(ctx, pos, vel, water, n_w, m_O, m_H, (cudaStream_t)stream);
+}
+
 static int check_nb_args(Ctx* ctx, const NL* nl, int32_t ntypes, const double* box, const dimos_nb_params* p)
 {
     if (!list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");

@@ -149,6 +149,10 @@ int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStrea
 int type_histogram_impl(Ctx* ctx, const int32_t* type, int64_t N, int nt, unsigned long long* counts_dev, int* bad_dev,
                         cudaStream_t s);
 int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, cudaStream_t s);
+int settle_impl(Ctx* ctx, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w, double m_O,
+                double m_H, double d_OH, double d_HH, double dt, cudaStream_t s);
+int settle_vel_impl(Ctx* ctx, const void* pos, void* vel, const int32_t* water, int64_t n_w, double m_O, double m_H,
+                    cudaStream_t s);
 
 // stencil code <-> offset
 __host__ __device__ inline int stencil_code(int dx, int dy, int dz) { return (dx + 1) * 9 + (dy + 1) * 3 + (dz + 1); }

@@ -83,3 +83,162 @@ def test_md_loop_through_the_library_f32():
         assert bool(torch.isfinite(E).all())
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("n_w", [1, 33, 5000])
+def test_settle_matches_converged_shake(precision, n_w):
+    """dimos_settle (step 3; SETTLE) against the oracle's SHAKE iterated to 1e-14: same
+    constrained positions, bond lengths on the constraint, molecular centre of mass untouched, and the velocity picks up
+    (x_c - x_u) / dt.  Molecules are shuffled in memory so that the index table is exercised."""
+    rng = np.random.default_rng(900 + n_w)
+    np_real = np.float64 if precision == "f64" else np.float32
+    d_oh = wl.R_OH
+    d_hh = 2.0 * wl.R_OH * np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0)
+    m_O, m_H = 15.9994, 1.008
+    # rigid molecules with random orientations and positions (built from the canonical triangle by a random rotation)
+    half = np.radians(wl.ANGLE_HOH_DEG) / 2.0
+    tri = np.array([[0.0, 0.0, 0.0], [d_oh * np.sin(half), 0.0, d_oh * np.cos(half)], [-d_oh * np.sin(half), 0.0, d_oh * np.cos(half)]])
+    q = rng.normal(size=(n_w, 4))
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    w, x, y, z = q.T
+    R = np.stack([np.stack([1 - 2 * (y * y + z * z), 2 * (x * y - z * w), 2 * (x * z + y * w)], -1),
+                  np.stack([2 * (x * y + z * w), 1 - 2 * (x * x + z * z), 2 * (y * z - x * w)], -1),
+                  np.stack([2 * (x * z - y * w), 2 * (y * z + x * w), 1 - 2 * (x * x + y * y)], -1)], 1)
+    x0 = np.einsum("nij,kj->nki", R, tri) + rng.uniform(0.0, 6.0, size=(n_w, 1, 3))
+    x0 = x0.reshape(-1, 3).astype(np_real)  # what the device holds; rigid to the rounding of np_real
+    mass = np.tile([m_O, m_H, m_H], n_w)
+    dt = 0.002
+    v = rng.normal(0.0, 1.0, size=(3 * n_w, 3)) / np.sqrt(mass)[:, None] * 1.5   # thermal-sized velocities, nm/ps
+    x1 = (x0.astype(np.float64) + dt * v).astype(np_real)
+    # the oracle works on exactly the device's inputs, from an old configuration made rigid in fp64
+    x0_64 = oracle.shake_water(x0.astype(np.float64), x0.astype(np.float64), mass, d_oh, d_hh)
+    ref = oracle.shake_water(x0_64, x1.astype(np.float64), mass, d_oh, d_hh)
+    perm = rng.permutation(3 * n_w)          # atom k of the molecule order sits at memory index perm[k]
+    inv = np.empty_like(perm)
+    inv[perm] = np.arange(3 * n_w)
+    water = perm.reshape(n_w, 3).astype(np.int32)
+    dev = torch.device("cuda", 0)
+    with dimos.Context(0, precision) as ctx:
+        p_old = torch.from_numpy(np.ascontiguousarray(x0[inv])).to(dev)
+        p = torch.from_numpy(np.ascontiguousarray(x1[inv])).to(dev)
+        vel0 = v.astype(np_real)
+        vd = torch.from_numpy(np.ascontiguousarray(vel0[inv])).to(dev)
+        dimos.dimos_settle(ctx, p_old, p, torch.from_numpy(water).to(dev), m_O, m_H, d_oh, d_hh, vel=vd, dt=dt)
+        torch.cuda.synchronize()
+        got = p.cpu().numpy().astype(np.float64)[perm]
+        got_v = vd.cpu().numpy().astype(np.float64)[perm]
+        # without vel: positions identical, velocities untouched
+        p2 = torch.from_numpy(np.ascontiguousarray(x1[inv])).to(dev)
+        dimos.dimos_settle(ctx, p_old, p2, torch.from_numpy(water).to(dev), m_O, m_H, d_oh, d_hh)
+        torch.cuda.synchronize()
+        assert torch.equal(p2, p)
+        dimos.dimos_settle(ctx, p_old, p2, torch.from_numpy(water[:0].copy()).to(dev), m_O, m_H, d_oh, d_hh)  # n_w = 0
+        with pytest.raises(dimos.DimosError):
+            dimos.dimos_settle(ctx, p_old, p2, torch.from_numpy(water).to(dev), m_O, m_H, d_oh, 2.5 * d_oh)
+    # fp32: coordinates up to 6 nm carry 2.4e-7 nm of rounding each; fp64: the oracle's own convergence (1e-14 relative)
+    tol = 5e-12 if precision == "f64" else 3e-6
+    assert np.abs(got - ref).max() < tol
+    m = got.reshape(-1, 3, 3)
+    for i, j, d in ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh)):
+        assert np.abs(np.linalg.norm(m[:, i] - m[:, j], axis=1) - d).max() < tol
+    wgt = mass.reshape(-1, 3, 1)
+    com = lambda a: (a.reshape(-1, 3, 3) * wgt).sum(1) / wgt.sum(1)
+    assert np.abs(com(got) - com(x1.astype(np.float64))).max() < tol
+    ref_v = vel0.astype(np.float64) + (ref - x1.astype(np.float64)) / dt
+    assert np.abs(got_v - ref_v).max() < tol / dt * 2
+
+
+def _random_rigid_waters(rng, n_w, d_oh, d_hh, span=6.0):
+    half = np.arcsin(0.5 * d_hh / d_oh)
+    tri = np.array([[0.0, 0.0, 0.0], [d_oh * np.sin(half), 0.0, d_oh * np.cos(half)], [-d_oh * np.sin(half), 0.0, d_oh * np.cos(half)]])
+    q = rng.normal(size=(n_w, 4))
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    w, x, y, z = q.T
+    R = np.stack([np.stack([1 - 2 * (y * y + z * z), 2 * (x * y - z * w), 2 * (x * z + y * w)], -1),
+                  np.stack([2 * (x * y + z * w), 1 - 2 * (x * x + z * z), 2 * (y * z - x * w)], -1),
+                  np.stack([2 * (x * z - y * w), 2 * (y * z + x * w), 1 - 2 * (x * x + y * y)], -1)], 1)
+    return (np.einsum("nij,kj->nki", R, tri) + rng.uniform(0.0, span, size=(n_w, 1, 3))).reshape(-1, 3)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("n_w", [1, 33, 5000])
+def test_settle_velocities_match_converged_rattle(precision, n_w):
+    """dimos_settle_velocities (step 6) against the oracle's iterative RATTLE velocity stage, and the
+    properties that hold at any size: v_ij . r_ij = 0 on the three bonds, molecular linear and angular momentum kept."""
+    rng = np.random.default_rng(1200 + n_w)
+    np_real = np.float64 if precision == "f64" else np.float32
+    d_oh = wl.R_OH
+    d_hh = 2.0 * wl.R_OH * np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0)
+    m_O, m_H = 15.9994, 1.008
+    mass = np.tile([m_O, m_H, m_H], n_w)
+    x = _random_rigid_waters(rng, n_w, d_oh, d_hh).astype(np_real)
+    v = (rng.normal(0.0, 1.5, size=x.shape) / np.sqrt(mass)[:, None]).astype(np_real)
+    ref = oracle.rattle_water_velocities(x.astype(np.float64), v.astype(np.float64), mass)
+    water = np.arange(3 * n_w, dtype=np.int32).reshape(n_w, 3)
+    dev = torch.device("cuda", 0)
+    with dimos.Context(0, precision) as ctx:
+        vd = torch.from_numpy(v.copy()).to(dev)
+        dimos.dimos_settle_velocities(ctx, torch.from_numpy(x).to(dev), vd, torch.from_numpy(water).to(dev), m_O, m_H)
+        torch.cuda.synchronize()
+        got = vd.cpu().numpy().astype(np.float64)
+    vmax = np.abs(v).max()
+    tol = (1e-12 if precision == "f64" else 2e-5) * vmax
+    assert np.abs(got - ref).max() < tol
+    X, G, V0, M = x.astype(np.float64).reshape(-1, 3, 3), got.reshape(-1, 3, 3), v.astype(np.float64).reshape(-1, 3, 3), mass.reshape(-1, 3, 1)
+    for i, j in ((0, 1), (0, 2), (1, 2)):
+        r = X[:, i] - X[:, j]
+        assert np.abs(((G[:, i] - G[:, j]) * r).sum(1) / np.linalg.norm(r, axis=1)).max() < tol
+    assert np.abs((M * G).sum(1) - (M * V0).sum(1)).max() < tol * m_O
+    Xc = X - X[:, :1]
+    assert np.abs((M * np.cross(Xc, G)).sum(1) - (M * np.cross(Xc, V0)).sum(1)).max() < tol * m_O * d_oh * 4
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_constrained_velocity_verlet_steps_match_oracle(precision):
+    """Steps 1, 2, 3, 5, 6 of PAPER.md:281-292 chained on the device for rigid water with seeded forces, four time steps in
+    a row, against the same chain of oracle functions (kick+drift, SHAKE, kick, RATTLE velocities): positions, velocities,
+    and the rigid geometry at the end."""
+    n_w = 700
+    rng = np.random.default_rng(77)
+    np_real = np.float64 if precision == "f64" else np.float32
+    d_oh = wl.R_OH
+    d_hh = 2.0 * wl.R_OH * np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0)
+    m_O, m_H = 15.9994, 1.008
+    mass = np.tile([m_O, m_H, m_H], n_w)
+    inv_m = (1.0 / mass).astype(np_real)
+    dt = 0.002
+    x = _random_rigid_waters(rng, n_w, d_oh, d_hh).astype(np_real)
+    v0 = rng.normal(0.0, 1.5, size=x.shape) / np.sqrt(mass)[:, None]
+    v = oracle.rattle_water_velocities(x.astype(np.float64), v0, mass).astype(np_real)  # start on the constraint manifold
+    forces = [rng.normal(0.0, 600.0, size=x.shape).astype(np_real) for _ in range(5)]
+    water = np.arange(3 * n_w, dtype=np.int32).reshape(n_w, 3)
+    # oracle chain in fp64 from the same starting arrays
+    xo = oracle.shake_water(x.astype(np.float64), x.astype(np.float64), mass, d_oh, d_hh)
+    vo = v.astype(np.float64)
+    for s in range(4):
+        xu, vh = oracle.vv_kick_drift(xo, vo, forces[s].astype(np.float64), inv_m.astype(np.float64), dt)
+        xc = oracle.shake_water(xo, xu, mass, d_oh, d_hh)
+        vh = vh + (xc - xu) / dt
+        vn = oracle.vv_kick(vh, forces[s + 1].astype(np.float64), inv_m.astype(np.float64), dt)
+        xo, vo = xc, oracle.rattle_water_velocities(xc, vn, mass)
+    dev = torch.device("cuda", 0)
+    with dimos.Context(0, precision) as ctx:
+        xd, vd = torch.from_numpy(x.copy()).to(dev), torch.from_numpy(v.copy()).to(dev)
+        wd, imd = torch.from_numpy(water).to(dev), torch.from_numpy(inv_m).to(dev)
+        fd = [torch.from_numpy(f).to(dev) for f in forces]
+        for s in range(4):
+            x_old = xd.clone()
+            dimos.dimos_vv_kick_drift(ctx, xd, vd, fd[s], imd, dt)
+            dimos.dimos_settle(ctx, x_old, xd, wd, m_O, m_H, d_oh, d_hh, vel=vd, dt=dt)
+            dimos.dimos_vv_kick(ctx, vd, fd[s + 1], imd, dt)
+            dimos.dimos_settle_velocities(ctx, xd, vd, wd, m_O, m_H)
+        torch.cuda.synchronize()
+        gx, gv = xd.cpu().numpy().astype(np.float64), vd.cpu().numpy().astype(np.float64)
+    tol_x = 1e-11 if precision == "f64" else 1e-5      # fp32: 4 steps x (rounding of 6 nm coordinates ~ 5e-7)
+    tol_v = 1e-9 if precision == "f64" else 4e-3       # (x_c - x_u) / dt amplifies position rounding by 1/dt = 500
+    assert np.abs(gx - xo).max() < tol_x
+    assert np.abs(gv - vo).max() < tol_v
+    m = gx.reshape(-1, 3, 3)
+    for i, j, d in ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh)):
+        assert np.abs(np.linalg.norm(m[:, i] - m[:, j], axis=1) - d).max() < (1e-12 if precision == "f64" else 3e-6)

@@ -561,3 +561,51 @@ def test_dispersion_correction_textbook_tail_and_switch_limits():
     # hydrogens (epsilon = 0) do not contribute
     mixed = oracle.dispersion_correction(np.concatenate([types, np.ones(2000, dtype=np.int32)]), tab, box, rc)[0]
     assert mixed == pytest.approx(got, rel=1e-14)
+
+
+# --- rigid-water position constraints (step 3 of PAPER.md:281-292; SETTLE) ---------------------------
+def test_shake_water_satisfies_constraints_and_conserves_momentum():
+    """The constrained positions have the rigid geometry to 1e-12; the correction is a sum of pair displacements weighted
+    by inverse mass, so it leaves every molecule's centre of mass where the unconstrained step put it; an already rigid
+    configuration is left untouched; a rigid translation + small rotation of the old molecule is reproduced."""
+    wb = small_box(m=40, edge=2.4, seed=4)
+    d_hh = 2.0 * wl.R_OH * np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0)
+    x0 = wb.pos.astype(np.float64)
+    x0 = oracle.shake_water(x0, x0, wb.mass, wl.R_OH, d_hh)  # the workload stores fp32: make it rigid in fp64 first
+    rng = np.random.default_rng(1)
+    x1 = x0 + rng.normal(0.0, 0.004, size=x0.shape)  # an unconstrained step of a few pm
+    xc = oracle.shake_water(x0, x1, wb.mass, wl.R_OH, d_hh)
+    m = xc.reshape(-1, 3, 3)
+    for i, j, d in ((0, 1, wl.R_OH), (0, 2, wl.R_OH), (1, 2, d_hh)):
+        assert np.abs(np.linalg.norm(m[:, i] - m[:, j], axis=1) - d).max() < 1e-12
+    w = wb.mass.reshape(-1, 3, 1)
+    com = lambda p: (p.reshape(-1, 3, 3) * w).sum(1) / w.sum(1)
+    assert np.abs(com(xc) - com(x1)).max() < 1e-13
+    assert np.abs(oracle.shake_water(x0, x0, wb.mass, wl.R_OH, d_hh) - x0).max() < 1e-13
+    shift = x0 + np.array([0.01, -0.02, 0.005])
+    assert np.abs(oracle.shake_water(x0, shift, wb.mass, wl.R_OH, d_hh) - shift).max() < 1e-12
+
+
+def test_rattle_water_velocities_pins():
+    """Step 6 (PAPER.md:281-292): after the velocity constraint no bond length changes to first order (v_ij . r_ij = 0);
+    the impulses are internal and central, so each molecule keeps its linear and angular momentum; a rigid-body velocity
+    field v = V + omega x r already satisfies the constraints and is returned unchanged; and the result is the projection
+    that removes exactly the three internal degrees of freedom: kinetic energy never increases."""
+    wb = small_box(m=40, edge=2.4, seed=5)
+    x = wb.pos.astype(np.float64)
+    mass = wb.mass.astype(np.float64)
+    rng = np.random.default_rng(2)
+    v = rng.normal(0.0, 1.0, size=x.shape) / np.sqrt(mass)[:, None]
+    vc = oracle.rattle_water_velocities(x, v, mass)
+    X, V, VC, M = x.reshape(-1, 3, 3), v.reshape(-1, 3, 3), vc.reshape(-1, 3, 3), mass.reshape(-1, 3, 1)
+    for i, j in ((0, 1), (0, 2), (1, 2)):
+        assert np.abs(((VC[:, i] - VC[:, j]) * (X[:, i] - X[:, j])).sum(1)).max() < 1e-15
+    assert np.abs((M * VC).sum(1) - (M * V).sum(1)).max() < 1e-13
+    assert np.abs((M * np.cross(X, VC)).sum(1) - (M * np.cross(X, V)).sum(1)).max() < 1e-13
+    assert (M * VC * VC).sum() < (M * V * V).sum()
+    com = (M * X).sum(1, keepdims=True) / M.sum(1, keepdims=True)
+    omega = rng.normal(0.0, 3.0, size=(X.shape[0], 1, 3))
+    rigid = rng.normal(0.0, 0.5, size=(X.shape[0], 1, 3)) + np.cross(omega, X - com)
+    assert np.abs(oracle.rattle_water_velocities(x, rigid.reshape(-1, 3), mass) - rigid.reshape(-1, 3)).max() < 1e-14
+    # 9 velocity components - 3 constraints: the removed part is 3-dimensional per molecule and mass-orthogonal to the rest
+    assert np.abs((M * (V - VC) * VC).sum((1, 2))).max() < 1e-13
