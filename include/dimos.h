@@ -240,7 +240,7 @@ DIMOS_API int dimos_virtual_box(dimos_ctx* ctx, const void* pos, int64_t N, doub
                                 double* lo_host, void* stream);
 
 /* dimos_vv_kick_drift / dimos_vv_kick -- velocity Verlet, PAPER.md:281-292 (steps 1 + 2, and step 5; steps 3 and 6 for rigid water are
- * dimos_settle and dimos_settle_velocities; the thermostat of step 7 is not built).  Units nm, ps, amu, kJ mol^-1 nm^-1: a = F / m needs no conversion factor.
+ * dimos_settle and dimos_settle_velocities; step 7 is dimos_berendsen).  Units nm, ps, amu, kJ mol^-1 nm^-1: a = F / m needs no conversion factor.
  *   kick_drift:  v <- v + (dt/2) F / m;  x <- x + dt v      (in place)
  *   kick:        v <- v + (dt/2) F / m                      (in place, with the forces at the new positions)
  *   pos, vel, F   dev, N x 3, float or double per the context precision
@@ -279,6 +279,23 @@ DIMOS_API int dimos_settle(dimos_ctx* ctx, const void* pos_old, void* pos, void*
  * Asynchronous on the stream; n_w = 0 is a no-op. */
 DIMOS_API int dimos_settle_velocities(dimos_ctx* ctx, const void* pos, void* vel, const int32_t* water, int64_t n_w,
                                       double m_O, double m_H, void* stream);
+
+/* dimos_kinetic_energy / dimos_berendsen -- step 7 of velocity Verlet with the Berendsen thermostat,
+ * the velocity-rescaling thermostat of PAPER.md:306.  Units nm, ps, amu, kJ/mol, K; k_B = 8.314462618e-3 kJ mol^-1 K^-1.
+ *   kinetic_energy:  K = 1/2 sum_i m_i |v_i|^2  -> *ke_dev (and *ke_host if not NULL, which synchronises the stream)
+ *   berendsen:       T = 2 K / (n_dof k_B);  v <- v sqrt(1 + (dt/tau) (T0/T - 1))  in place, lambda taken from the
+ *                    device-resident K (no host round trip); *ke_dev holds K BEFORE the scaling, *T_host (if not NULL,
+ *                    synchronises) the temperature before the scaling
+ *   vel        dev, N x 3, float or double per the context precision;  inv_mass  dev, N, same type: 1 / m_i
+ *   n_dof      degrees of freedom, e.g. 3 N - 3 or, with rigid water, 6 n_w - 3
+ *   ke_dev     dev, one double, written (the caller owns it)
+ * The sum is accumulated in fp64 with one atomic per thread block: its last bits depend on the block order.
+ * DIMOS_EINVAL unless T0 >= 0 and 0 < dt <= tau.  A system at rest (K = 0) has no temperature to rescale: velocities
+ * become NaN, as the formula says. */
+DIMOS_API int dimos_kinetic_energy(dimos_ctx* ctx, const void* vel, const void* inv_mass, int64_t N, double* ke_dev,
+                                   double* ke_host, void* stream);
+DIMOS_API int dimos_berendsen(dimos_ctx* ctx, void* vel, const void* inv_mass, int64_t N, int64_t n_dof, double T0, double tau,
+                              double dt, double* ke_dev, double* T_host, void* stream);
 
 /* dimos_nl_set_exceptions -- PAPER.md:243 ("1-4 exceptions ... scale the strength of the non-bonded interactions by
  * some common factor", or an individual factor per pair; "handled explicitly by the non-bonded interaction method").

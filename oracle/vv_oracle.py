@@ -126,3 +126,21 @@ def rattle_water_velocities(pos, vel, mass, tol=1e-15, max_iter=2000):
         if worst < tol:
             break
     return v.reshape(-1, 3)
+
+
+K_B = 8.314462618e-3  # kJ mol^-1 K^-1 (molar gas constant, CODATA 2018): the units of PAPER.md's MD (nm, ps, amu)
+
+
+def kinetic_energy(vel, mass):
+    """K = 1/2 sum_i m_i |v_i|^2 in kJ/mol (amu nm^2 ps^-2 = kJ/mol), fp64."""
+    v = np.asarray(vel, dtype=np.float64)
+    return 0.5 * float((np.asarray(mass, dtype=np.float64)[:, None] * v * v).sum())
+
+
+def berendsen(vel, mass, n_dof, T0, tau, dt):
+    """Step 7 of PAPER.md:281-292 with the Berendsen thermostat (a thermostat that rescales the velocities):
+    T = 2 K / (n_dof k_B); every velocity is multiplied by lambda = sqrt(1 + (dt / tau) (T0 / T - 1)).
+    Returns (scaled velocities fp64, T before scaling)."""
+    T = 2.0 * kinetic_energy(vel, mass) / (n_dof * K_B)
+    lam = np.sqrt(1.0 + (dt / tau) * (T0 / T - 1.0))
+    return np.asarray(vel, dtype=np.float64) * lam, T

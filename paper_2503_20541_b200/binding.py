@@ -31,6 +31,7 @@ EXPORTED_SYMBOLS = (
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
+    "dimos_kinetic_energy", "dimos_berendsen",
 )
 
 
@@ -97,6 +98,8 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
     lib.dimos_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp]
     lib.dimos_settle_velocities.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, vp]
+    lib.dimos_kinetic_energy.argtypes = [vp, vp, vp, i64, vp, ctypes.POINTER(dbl), vp]
+    lib.dimos_berendsen.argtypes = [vp, vp, vp, i64, i64, dbl, dbl, dbl, vp, ctypes.POINTER(dbl), vp]
     lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
     lib.dimos_virtual_box.argtypes = [vp, vp, i64, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     lib.dimos_dispersion_correction.argtypes = [vp, vp, i64, vp, i32, ctypes.POINTER(dbl), dbl, dbl, ctypes.POINTER(dbl),
@@ -116,7 +119,7 @@ def load_library() -> ctypes.CDLL:
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
                  "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
-                 "dimos_settle", "dimos_settle_velocities"):
+                 "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -400,6 +403,34 @@ class Context:
                                                   float(m_O), float(m_H), _stream_ptr())
         self._check(rc)
 
+    def _ke_scratch(self):
+        if getattr(self, "_ke", None) is None:
+            self._ke = torch.zeros(1, dtype=torch.float64, device=self.device)
+        return self._ke
+
+    def kinetic_energy(self, vel, inv_mass) -> float:
+        """dimos_kinetic_energy: K = 1/2 sum m v^2 in kJ/mol (synchronises)."""
+        vel = self._dev(vel, self.real, 3)
+        inv_mass = self._dev(inv_mass, self.real)
+        out = ctypes.c_double(0.0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_kinetic_energy(self.handle, vel.data_ptr(), inv_mass.data_ptr(), vel.shape[0],
+                                               self._ke_scratch().data_ptr(), ctypes.byref(out), _stream_ptr())
+        self._check(rc)
+        return out.value
+
+    def berendsen(self, vel, inv_mass, n_dof, T0, tau, dt, sync=True):
+        """dimos_berendsen: rescale vel in place; returns the temperature before the scaling (None with sync=False)."""
+        vel = self._dev(vel, self.real, 3)
+        inv_mass = self._dev(inv_mass, self.real)
+        out = ctypes.c_double(0.0)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_berendsen(self.handle, vel.data_ptr(), inv_mass.data_ptr(), vel.shape[0], int(n_dof), float(T0),
+                                          float(tau), float(dt), self._ke_scratch().data_ptr(),
+                                          ctypes.byref(out) if sync else None, _stream_ptr())
+        self._check(rc)
+        return out.value if sync else None
+
     def nl_set_exceptions(self, nl: NeighborList, pairs, scale):
         """dimos_nl_set_exceptions: pairs (n,2) int32 i<j, scale (n,2) float64 = (Coulomb scale, LJ scale); None clears."""
         if pairs is None or len(pairs) == 0:
@@ -515,6 +546,14 @@ def dimos_settle(ctx: Context, pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=No
 
 def dimos_settle_velocities(ctx: Context, pos, vel, water, m_O, m_H):
     return ctx.settle_velocities(pos, vel, water, m_O, m_H)
+
+
+def dimos_kinetic_energy(ctx: Context, vel, inv_mass):
+    return ctx.kinetic_energy(vel, inv_mass)
+
+
+def dimos_berendsen(ctx: Context, vel, inv_mass, n_dof, T0, tau, dt, sync=True):
+    return ctx.berendsen(vel, inv_mass, n_dof, T0, tau, dt, sync=sync)
 
 
 def dimos_nl_set_exceptions(ctx: Context, nl: NeighborList, pairs, scale):

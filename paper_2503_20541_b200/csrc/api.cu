@@ -394,6 +394,49 @@ DIMOS_API int dimos_settle_velocities(dimos_ctx* c, const void* pos, void* vel, 
     return settle_vel_impl(ctx, pos, vel, water, n_w, m_O, m_H, (cudaStream_t)stream);
 }
 
+DIMOS_API int dimos_kinetic_energy(dimos_ctx* c, const void* vel, const void* inv_mass, int64_t N, double* ke_dev,
+                                   double* ke_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!vel || !inv_mass || !ke_dev) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0) return set_error(ctx, DIMOS_EINVAL, "N must be > 0");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = kinetic_energy_impl(ctx, vel, inv_mass, N, ke_dev, s);
+    if (rc != DIMOS_OK) return rc;
+    if (ke_host) {
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ke_host, ke_dev, sizeof(double), cudaMemcpyDeviceToHost, s));
+        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    }
+    return DIMOS_OK;
+}
+
+DIMOS_API int dimos_berendsen(dimos_ctx* c, void* vel, const void* inv_mass, int64_t N, int64_t n_dof, double T0, double tau,
+                              double dt, double* ke_dev, double* T_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!vel || !inv_mass || !ke_dev) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || n_dof <= 0) return set_error(ctx, DIMOS_EINVAL, "N and n_dof must be > 0");
+    if (!(T0 >= 0) || !(tau > 0) || !(dt > 0) || !(dt <= tau)) return set_error(ctx, DIMOS_EINVAL, "need T0 >= 0 and 0 < dt <= tau");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    const double kB = 8.314462618e-3;  // kJ mol^-1 K^-1
+    const double two_over_dof_kb = 2.0 / ((double)n_dof * kB);
+    int rc = kinetic_energy_impl(ctx, vel, inv_mass, N, ke_dev, s);
+    if (rc != DIMOS_OK) return rc;
+    rc = berendsen_scale_impl(ctx, vel, N, ke_dev, two_over_dof_kb, T0, dt / tau, s);
+    if (rc != DIMOS_OK) return rc;
+    if (T_host) {
+        double ke = 0.0;
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(&ke, ke_dev, sizeof(double), cudaMemcpyDeviceToHost, s));
+        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+        *T_host = ke * two_over_dof_kb;
+    }
+    return DIMOS_OK;
+}
+
 static int check_nb_args(Ctx* ctx, const NL* nl, int32_t ntypes, const double* box, const dimos_nb_params* p)
 {
     if (!list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");

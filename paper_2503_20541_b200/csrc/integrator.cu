@@ -181,6 +181,39 @@ __global__ void settle_vel_kernel(const real* __restrict__ pos, real* __restrict
     }
 }
 
+// Step 7 (Berendsen rescaling).  kinetic_energy: K = 1/2 sum m v^2, products in `real`,
+// accumulated in fp64 per thread, warp shuffle, one fp64 atomic per block.  berendsen_scale: every thread derives lambda
+// from the device-resident K (no host round trip) and scales its velocities.
+template <typename real>
+__global__ void kinetic_energy_kernel(const real* __restrict__ vel, const real* __restrict__ inv_mass, int64_t N,
+                                      double* __restrict__ ke)
+{
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        const real vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        acc += (double)(vx * vx + vy * vy + vz * vz) / (double)inv_mass[i];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    __shared__ double sh[8];
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += sh[w];
+        atomicAdd(ke, 0.5 * t);
+    }
+}
+
+template <typename real>
+__global__ void berendsen_scale_kernel(real* __restrict__ vel, int64_t n3, const double* __restrict__ ke, double two_over_dof_kb,
+                                       double T0, double dt_over_tau)
+{
+    const double T = *ke * two_over_dof_kb;
+    const real lam = (real)sqrt(1.0 + dt_over_tau * (T0 / T - 1.0));
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (int64_t)gridDim.x * blockDim.x) vel[i] *= lam;
+}
+
 // bounding box of all positions (virtual box of a non-periodic system): ordered-int atomics on 6 words
 __device__ __forceinline__ unsigned ordered_bits(float f)
 {
@@ -329,6 +362,30 @@ int settle_vel_impl(Ctx* ctx, const void* pos, void* vel, const int32_t* water, 
         settle_vel_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos, (float*)vel, water, n_w, (float)(1.0 / m_O),
                                                         (float)(1.0 / m_H));
     DIMOS_LAUNCH_CHECK(ctx, "settle_velocities");
+    return DIMOS_OK;
+}
+
+int kinetic_energy_impl(Ctx* ctx, const void* vel, const void* inv_mass, int64_t N, double* ke_dev, cudaStream_t s)
+{
+    DIMOS_CUDA_TRY(ctx, cudaMemsetAsync(ke_dev, 0, sizeof(double), s));
+    const int blocks = grid_for(ctx, N);
+    if (ctx->precision == DIMOS_F64)
+        kinetic_energy_kernel<double><<<blocks, 256, 0, s>>>((const double*)vel, (const double*)inv_mass, N, ke_dev);
+    else
+        kinetic_energy_kernel<float><<<blocks, 256, 0, s>>>((const float*)vel, (const float*)inv_mass, N, ke_dev);
+    DIMOS_LAUNCH_CHECK(ctx, "kinetic_energy");
+    return DIMOS_OK;
+}
+
+int berendsen_scale_impl(Ctx* ctx, void* vel, int64_t N, const double* ke_dev, double two_over_dof_kb, double T0,
+                         double dt_over_tau, cudaStream_t s)
+{
+    const int blocks = grid_for(ctx, 3 * N);
+    if (ctx->precision == DIMOS_F64)
+        berendsen_scale_kernel<double><<<blocks, 256, 0, s>>>((double*)vel, 3 * N, ke_dev, two_over_dof_kb, T0, dt_over_tau);
+    else
+        berendsen_scale_kernel<float><<<blocks, 256, 0, s>>>((float*)vel, 3 * N, ke_dev, two_over_dof_kb, T0, dt_over_tau);
+    DIMOS_LAUNCH_CHECK(ctx, "berendsen_scale");
     return DIMOS_OK;
 }
 

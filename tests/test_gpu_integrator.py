@@ -242,3 +242,40 @@ def test_constrained_velocity_verlet_steps_match_oracle(precision):
     m = gx.reshape(-1, 3, 3)
     for i, j, d in ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh)):
         assert np.abs(np.linalg.norm(m[:, i] - m[:, j], axis=1) - d).max() < (1e-12 if precision == "f64" else 3e-6)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("n", [1, 999, 300000])
+def test_kinetic_energy_and_berendsen_match_oracle(precision, n):
+    """dimos_kinetic_energy and dimos_berendsen (step 7; Berendsen rescaling) against the
+    numpy fp64 oracle: K, the temperature before scaling, the scaled velocities element by element, and the relaxation
+    T' = T + (dt/tau)(T0 - T) measured on the device's own output."""
+    rng = np.random.default_rng(5000 + n)
+    np_real = np.float64 if precision == "f64" else np.float32
+    mass = rng.choice(np.array([15.9994, 1.008]), size=n)
+    inv_m = (1.0 / mass).astype(np_real)
+    m_dev = 1.0 / inv_m.astype(np.float64)  # the masses the device sees
+    v = (1.25 * rng.normal(size=(n, 3)) * np.sqrt(oracle.K_B * 300.0 / mass)[:, None]).astype(np_real)
+    n_dof = max(3 * n - 3, 1)
+    T0, tau, dt = 300.0, 0.1, 0.002
+    K_o = oracle.kinetic_energy(v, m_dev)
+    v_o, T_o = oracle.berendsen(v, m_dev, n_dof, T0, tau, dt)
+    dev = torch.device("cuda", 0)
+    with dimos.Context(0, precision) as ctx:
+        vd, imd = torch.from_numpy(v.copy()).to(dev), torch.from_numpy(inv_m).to(dev)
+        K = dimos.dimos_kinetic_energy(ctx, vd, imd)
+        T = dimos.dimos_berendsen(ctx, vd, imd, n_dof, T0, tau, dt)
+        got = vd.cpu().numpy().astype(np.float64)
+        K2 = dimos.dimos_kinetic_energy(ctx, vd, imd)
+        v_async = torch.from_numpy(v.copy()).to(dev)
+        assert dimos.dimos_berendsen(ctx, v_async, imd, n_dof, T0, tau, dt, sync=False) is None
+        torch.cuda.synchronize()
+        assert torch.allclose(v_async, vd, rtol=1e-6, atol=0)
+        with pytest.raises(dimos.DimosError):
+            dimos.dimos_berendsen(ctx, vd, imd, n_dof, T0, 0.001, 0.002)  # dt > tau
+    rel = 1e-13 if precision == "f64" else 2e-7   # fp32 squares, fp64 accumulation: independent roundings average out
+    assert K == pytest.approx(K_o, rel=rel)
+    assert T == pytest.approx(T_o, rel=rel)
+    assert np.abs(got - v_o).max() <= (1e-14 if precision == "f64" else 2e-7) * np.abs(v_o).max()
+    T_after = 2.0 * K2 / (n_dof * oracle.K_B)
+    assert T_after == pytest.approx(T_o + dt / tau * (T0 - T_o), rel=1e-12 if precision == "f64" else 1e-6)

@@ -609,3 +609,32 @@ def test_rattle_water_velocities_pins():
     assert np.abs(oracle.rattle_water_velocities(x, rigid.reshape(-1, 3), mass) - rigid.reshape(-1, 3)).max() < 1e-14
     # 9 velocity components - 3 constraints: the removed part is 3-dimensional per molecule and mass-orthogonal to the rest
     assert np.abs((M * (V - VC) * VC).sum((1, 2))).max() < 1e-13
+
+
+def test_berendsen_thermostat_pins():
+    """Step 7 (Berendsen rescaling).  The rescaled temperature obeys the linear relaxation
+    T' = T + (dt/tau)(T0 - T) exactly, so n applications give T0 + (T - T0)(1 - dt/tau)^n; dt = tau lands on T0 in one
+    step; T = T0 is a fixed point; one atom of mass m and speed v has K = m v^2 / 2; velocities drawn from the
+    Maxwell-Boltzmann distribution at T0 (sigma^2 = k_B T0 / m per component) measure T0 within 4 standard errors; and k_B
+    is R = N_A k (both exact SI constants)."""
+    assert oracle.K_B == pytest.approx(6.02214076e23 * 1.380649e-23 * 1e-3, rel=1e-12)
+    assert oracle.kinetic_energy([[3.0, 4.0, 12.0]], [2.0]) == pytest.approx(169.0, rel=1e-15)
+    rng = np.random.default_rng(3)
+    n = 20000
+    mass = rng.choice(np.array([15.9994, 1.008]), size=n)
+    T0 = 300.0
+    v = rng.normal(size=(n, 3)) * np.sqrt(oracle.K_B * T0 / mass)[:, None]
+    n_dof = 3 * n
+    T = 2.0 * oracle.kinetic_energy(v, mass) / (n_dof * oracle.K_B)
+    assert abs(T - T0) < 4.0 * T0 * np.sqrt(2.0 / n_dof)
+    hot = v * 1.3
+    Th = 2.0 * oracle.kinetic_energy(hot, mass) / (n_dof * oracle.K_B)
+    cur, dt, tau = hot, 0.002, 0.1
+    for k in range(1, 6):
+        cur, T_before = oracle.berendsen(cur, mass, n_dof, T0, tau, dt)
+        T_after = 2.0 * oracle.kinetic_energy(cur, mass) / (n_dof * oracle.K_B)
+        assert T_after == pytest.approx(T0 + (Th - T0) * (1.0 - dt / tau) ** k, rel=1e-12)
+    one, _ = oracle.berendsen(hot, mass, n_dof, T0, 0.05, 0.05)
+    assert 2.0 * oracle.kinetic_energy(one, mass) / (n_dof * oracle.K_B) == pytest.approx(T0, rel=1e-13)
+    same, T_same = oracle.berendsen(v, mass, n_dof, T, tau, dt)
+    assert np.array_equal(same, v) and T_same == T
