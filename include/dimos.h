@@ -297,6 +297,23 @@ DIMOS_API int dimos_kinetic_energy(dimos_ctx* ctx, const void* vel, const void* 
 DIMOS_API int dimos_berendsen(dimos_ctx* ctx, void* vel, const void* inv_mass, int64_t N, int64_t n_dof, double T0, double tau,
                               double dt, double* ke_dev, double* T_host, void* stream);
 
+/* dimos_water_kick_drift_settle / dimos_water_kick_settle_velocities -- the velocity-Verlet loop of PAPER.md:281-292 for a
+ * system of rigid three-site waters in two passes instead of five: each thread holds one molecule in registers.
+ *   kick_drift_settle:       steps 1 + 2 + 3 = dimos_vv_kick_drift, then dimos_settle with vel and the pre-drift positions
+ *                            (no copy of the old positions is needed), then the rebuild trigger of dimos_nl_needs_rebuild
+ *                            on the CONSTRAINED positions (pos_at_build, skin, flag_dev, flag_host as in dimos_vv_kick_drift)
+ *   kick_settle_velocities:  steps 5 + 6 = dimos_vv_kick, then dimos_settle_velocities; if ke_dev is not NULL it receives
+ *                            the kinetic energy of the constrained velocities (step 8; one double, fp64 accumulation)
+ * Same arithmetic as the separate calls, in the same order.  Only atoms listed in `water` (dev, n_w x 3 int32: O, H1, H2)
+ * are moved; masses come from m_O, m_H.  pos must satisfy the constraints on entry to kick_drift_settle.  Asynchronous on
+ * the stream unless flag_host is given. */
+DIMOS_API int dimos_water_kick_drift_settle(dimos_ctx* ctx, void* pos, void* vel, const void* F, const int32_t* water,
+                                            int64_t n_w, double m_O, double m_H, double d_OH, double d_HH, double dt,
+                                            const void* pos_at_build, double skin, int32_t* flag_dev, int32_t* flag_host,
+                                            void* stream);
+DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* ctx, const void* pos, void* vel, const void* F, const int32_t* water,
+                                                 int64_t n_w, double m_O, double m_H, double dt, double* ke_dev, void* stream);
+
 /* dimos_nl_set_exceptions -- PAPER.md:243 ("1-4 exceptions ... scale the strength of the non-bonded interactions by
  * some common factor", or an individual factor per pair; "handled explicitly by the non-bonded interaction method").
  * Reading C-21 (the paper gives no formula): every exception pair must ALSO be one of the excluded pairs the list was

@@ -31,7 +31,7 @@ EXPORTED_SYMBOLS = (
     "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read", "dimos_step_host", "dimos_nl_set_exceptions",
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
-    "dimos_kinetic_energy", "dimos_berendsen",
+    "dimos_kinetic_energy", "dimos_berendsen", "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities",
 )
 
 
@@ -98,6 +98,9 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
     lib.dimos_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp]
     lib.dimos_settle_velocities.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, vp]
+    lib.dimos_water_kick_drift_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp, dbl, vp,
+                                                  ctypes.POINTER(i32), vp]
+    lib.dimos_water_kick_settle_velocities.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, vp, vp]
     lib.dimos_kinetic_energy.argtypes = [vp, vp, vp, i64, vp, ctypes.POINTER(dbl), vp]
     lib.dimos_berendsen.argtypes = [vp, vp, vp, i64, i64, dbl, dbl, dbl, vp, ctypes.POINTER(dbl), vp]
     lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
@@ -119,7 +122,8 @@ def load_library() -> ctypes.CDLL:
                  "dimos_nonbonded", "dimos_nonbonded_host", "dimos_nl_export_pairs", "dimos_nl_stats",
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
                  "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
-                 "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen"):
+                 "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen",
+                 "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -403,6 +407,42 @@ class Context:
                                                   float(m_O), float(m_H), _stream_ptr())
         self._check(rc)
 
+    def water_kick_drift_settle(self, pos, vel, F, water, m_O, m_H, d_OH, d_HH, dt, pos_at_build=None, skin=0.0, sync=True):
+        """dimos_water_kick_drift_settle: steps 1 + 2 + 3 for rigid waters in one pass; returns the rebuild flag like
+        vv_kick_drift (None without pos_at_build)."""
+        pos = self._dev(pos, self.real, 3)
+        vel = self._dev(vel, self.real, 3)
+        F = self._dev(F, self.real, 3)
+        water = self._dev(water, torch.int32, 3)
+        host = ctypes.c_int32(0)
+        trig = pos_at_build is not None
+        if trig:
+            pos_at_build = self._dev(pos_at_build, self.real, 3)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_water_kick_drift_settle(
+                self.handle, pos.data_ptr(), vel.data_ptr(), F.data_ptr(), water.data_ptr(), water.shape[0], float(m_O),
+                float(m_H), float(d_OH), float(d_HH), float(dt), pos_at_build.data_ptr() if trig else None, float(skin),
+                self._flag.data_ptr() if trig else None, ctypes.byref(host) if (trig and sync) else None, _stream_ptr())
+        self._check(rc)
+        if not trig:
+            return None
+        return bool(host.value) if sync else self._flag
+
+    def water_kick_settle_velocities(self, pos, vel, F, water, m_O, m_H, dt, want_ke=False):
+        """dimos_water_kick_settle_velocities: steps 5 + 6 for rigid waters in one pass; with want_ke returns the device
+        tensor (1 double) that receives the kinetic energy of the constrained velocities."""
+        pos = self._dev(pos, self.real, 3)
+        vel = self._dev(vel, self.real, 3)
+        F = self._dev(F, self.real, 3)
+        water = self._dev(water, torch.int32, 3)
+        ke = self._ke_scratch() if want_ke else None
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_water_kick_settle_velocities(self.handle, pos.data_ptr(), vel.data_ptr(), F.data_ptr(),
+                                                             water.data_ptr(), water.shape[0], float(m_O), float(m_H), float(dt),
+                                                             ke.data_ptr() if want_ke else None, _stream_ptr())
+        self._check(rc)
+        return ke
+
     def _ke_scratch(self):
         if getattr(self, "_ke", None) is None:
             self._ke = torch.zeros(1, dtype=torch.float64, device=self.device)
@@ -546,6 +586,14 @@ def dimos_settle(ctx: Context, pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=No
 
 def dimos_settle_velocities(ctx: Context, pos, vel, water, m_O, m_H):
     return ctx.settle_velocities(pos, vel, water, m_O, m_H)
+
+
+def dimos_water_kick_drift_settle(ctx: Context, pos, vel, F, water, m_O, m_H, d_OH, d_HH, dt, **kw):
+    return ctx.water_kick_drift_settle(pos, vel, F, water, m_O, m_H, d_OH, d_HH, dt, **kw)
+
+
+def dimos_water_kick_settle_velocities(ctx: Context, pos, vel, F, water, m_O, m_H, dt, want_ke=False):
+    return ctx.water_kick_settle_velocities(pos, vel, F, water, m_O, m_H, dt, want_ke=want_ke)
 
 
 def dimos_kinetic_energy(ctx: Context, vel, inv_mass):

@@ -394,6 +394,43 @@ DIMOS_API int dimos_settle_velocities(dimos_ctx* c, const void* pos, void* vel, 
     return settle_vel_impl(ctx, pos, vel, water, n_w, m_O, m_H, (cudaStream_t)stream);
 }
 
+DIMOS_API int dimos_water_kick_drift_settle(dimos_ctx* c, void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w,
+                                            double m_O, double m_H, double d_OH, double d_HH, double dt, const void* pos_at_build,
+                                            double skin, int32_t* flag_dev, int32_t* flag_host, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!pos || !vel || !F || !water) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (n_w <= 0) return set_error(ctx, DIMOS_EINVAL, "n_w must be > 0");
+    if (!(m_O > 0) || !(m_H > 0)) return set_error(ctx, DIMOS_EINVAL, "masses must be > 0");
+    if (!(d_OH > 0) || !(d_HH > 0) || !(d_HH < 2.0 * d_OH)) return set_error(ctx, DIMOS_EINVAL, "need 0 < d_HH < 2 d_OH");
+    if (!(dt > 0) || !(skin >= 0)) return set_error(ctx, DIMOS_EINVAL, "need dt > 0 and skin >= 0");
+    if ((pos_at_build != nullptr) != (flag_dev != nullptr)) return set_error(ctx, DIMOS_EINVAL, "pos_at_build and flag_dev go together");
+    if (flag_host && !flag_dev) return set_error(ctx, DIMOS_EINVAL, "flag_host needs flag_dev");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = water_step_a_impl(ctx, pos, vel, F, water, n_w, m_O, m_H, d_OH, d_HH, dt, pos_at_build, skin, flag_dev, s);
+    if (rc) return rc;
+    if (flag_host) {
+        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 32, flag_dev, sizeof(int), cudaMemcpyDeviceToHost, s));
+        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+        *flag_host = ctx->h_pinned[32];
+    }
+    return DIMOS_OK;
+}
+
+DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* c, const void* pos, void* vel, const void* F, const int32_t* water,
+                                                 int64_t n_w, double m_O, double m_H, double dt, double* ke_dev, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!pos || !vel || !F || !water) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (n_w <= 0) return set_error(ctx, DIMOS_EINVAL, "n_w must be > 0");
+    if (!(m_O > 0) || !(m_H > 0) || !(dt == dt)) return set_error(ctx, DIMOS_EINVAL, "bad masses or dt");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return water_step_b_impl(ctx, pos, vel, F, water, n_w, m_O, m_H, dt, ke_dev, (cudaStream_t)stream);
+}
+
 DIMOS_API int dimos_kinetic_energy(dimos_ctx* c, const void* vel, const void* inv_mass, int64_t N, double* ke_dev,
                                    double* ke_host, void* stream)
 {

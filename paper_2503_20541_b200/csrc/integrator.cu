@@ -1,7 +1,8 @@
 // integrator.cu -- velocity-Verlet update (steps 1, 2 and 5), with the
 // skin-displacement rebuild trigger (row A3) fused into the position update: the drift kernel already
 // holds every new position in registers, so max |x - x_at_build|^2 costs one more 12-byte read per atom and saves
-// the separate needs_rebuild pass.  Constraints (steps 3, 6) and thermostats (step 7) are not built.
+// the separate needs_rebuild pass.  Below: SETTLE for rigid water (steps 3, 6), the Berendsen thermostat (step 7) and
+// the two fused per-molecule passes that run steps 1-3 and 5-6 for a water system.
 //
 // Units: nm, ps, amu, kJ mol^-1 nm^-1: a = F / m is in nm ps^-2 without a conversion factor.
 #include <math.h>
@@ -61,122 +62,230 @@ __global__ void vv_kick_kernel(real* __restrict__ vel, const real* __restrict__ 
 // coordinates only ever enter as differences.  The constraint forces lie in the old molecular plane, hence the component
 // along its normal Z is unchanged and the rest is three rotations (phi, psi, theta) of the canonical triangle.
 template <typename real>
+struct SettleGeom {
+    real wO, wH;      // m_O / M, m_H / M
+    real ra, rb, rc;  // O and the HH midpoint from the centre of mass, half the HH distance
+    real d_hh2;
+};
+
+// b0, c0: old hydrogens relative to the old oxygen; A, B, C: unconstrained new atoms relative to the old oxygen;
+// overwritten with the constrained new atoms in the same frame
+template <typename real>
+__device__ __forceinline__ void settle_molecule(const real* b0, const real* c0, real* A, real* B, real* C, const SettleGeom<real>& g)
+{
+    const real ra = g.ra, rb = g.rb, rc = g.rc, d_hh2 = g.d_hh2;
+    real com[3], a1[3], b1[3], c1[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        com[k] = g.wO * A[k] + g.wH * (B[k] + C[k]);
+        a1[k] = A[k] - com[k];
+        b1[k] = B[k] - com[k];
+        c1[k] = C[k] - com[k];
+    }
+    // orthonormal frame: Z normal to the old plane, X = a1 x Z, Y = Z x X
+    real Z[3] = {b0[1] * c0[2] - b0[2] * c0[1], b0[2] * c0[0] - b0[0] * c0[2], b0[0] * c0[1] - b0[1] * c0[0]};
+    real X[3] = {a1[1] * Z[2] - a1[2] * Z[1], a1[2] * Z[0] - a1[0] * Z[2], a1[0] * Z[1] - a1[1] * Z[0]};
+    real Y[3] = {Z[1] * X[2] - Z[2] * X[1], Z[2] * X[0] - Z[0] * X[2], Z[0] * X[1] - Z[1] * X[0]};
+    const real nz = rsqrt(Z[0] * Z[0] + Z[1] * Z[1] + Z[2] * Z[2]);
+    const real nx = rsqrt(X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);
+    const real ny = rsqrt(Y[0] * Y[0] + Y[1] * Y[1] + Y[2] * Y[2]);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { X[k] *= nx; Y[k] *= ny; Z[k] *= nz; }
+    auto dot = [](const real* u, const real* v) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; };
+    const real xb0 = dot(b0, X), yb0 = dot(b0, Y), xc0 = dot(c0, X), yc0 = dot(c0, Y);
+    const real za1 = dot(a1, Z);
+    const real xb1 = dot(b1, X), yb1 = dot(b1, Y), zb1 = dot(b1, Z);
+    const real xc1 = dot(c1, X), yc1 = dot(c1, Y), zc1 = dot(c1, Z);
+    // tilt angles from the unchanged normal components
+    const real sinphi = za1 / ra;
+    const real cosphi = sqrt((real)1 - sinphi * sinphi);
+    const real sinpsi = (zb1 - zc1) / ((real)2 * rc * cosphi);
+    const real cospsi = sqrt((real)1 - sinpsi * sinpsi);
+    const real ya2 = ra * cosphi;
+    real xb2 = -rc * cospsi;
+    const real yb2 = -rb * cosphi - rc * sinpsi * sinphi;
+    const real yc2 = -rb * cosphi + rc * sinpsi * sinphi;
+    // re-impose |bc| = d_HH on xb2 (zero in exact arithmetic; removes the rounding of the two square roots)
+    const real dy = yb2 - yc2, dz = zb1 - zc1;
+    xb2 = (real)-0.5 * sqrt(fmax(d_hh2 - dy * dy - dz * dz, (real)0));
+    // in-plane rotation theta from the zero-torque condition about Z
+    const real alpha = xb2 * (xb0 - xc0) + yb0 * yb2 + yc0 * yc2;
+    const real beta = xb2 * (yc0 - yb0) + xb0 * yb2 + xc0 * yc2;
+    const real gamma = xb0 * yb1 - xb1 * yb0 + xc0 * yc1 - xc1 * yc0;
+    const real al2be2 = alpha * alpha + beta * beta;
+    const real sintheta = (alpha * gamma - beta * sqrt(fmax(al2be2 - gamma * gamma, (real)0))) / al2be2;
+    const real costheta = sqrt((real)1 - sintheta * sintheta);
+    const real a3[3] = {-ya2 * sintheta, ya2 * costheta, za1};
+    const real b3[3] = {xb2 * costheta - yb2 * sintheta, xb2 * sintheta + yb2 * costheta, zb1};
+    const real c3[3] = {-xb2 * costheta - yc2 * sintheta, -xb2 * sintheta + yc2 * costheta, zc1};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        A[k] = com[k] + X[k] * a3[0] + Y[k] * a3[1] + Z[k] * a3[2];
+        B[k] = com[k] + X[k] * b3[0] + Y[k] * b3[1] + Z[k] * b3[2];
+        C[k] = com[k] + X[k] * c3[0] + Y[k] * c3[1] + Z[k] * c3[2];
+    }
+}
+
+template <typename real>
 __global__ void settle_kernel(const real* __restrict__ pos_old, real* __restrict__ pos, real* __restrict__ vel,
-                              const int32_t* __restrict__ water, int64_t n_w, real wO, real wH, real ra, real rb, real rc,
-                              real d_hh2, real inv_dt)
+                              const int32_t* __restrict__ water, int64_t n_w, SettleGeom<real> g, real inv_dt)
 {
     for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_w; w += (int64_t)gridDim.x * blockDim.x) {
         const int64_t ia = water[3 * w], ib = water[3 * w + 1], ic = water[3 * w + 2];
-        real a0[3], b0[3], c0[3], A[3], B[3], C[3], com[3], a1[3], b1[3], c1[3];
+        real a0[3], b0[3], c0[3], A[3], B[3], C[3], Au[3], Bu[3], Cu[3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             a0[k] = pos_old[3 * ia + k];
             b0[k] = pos_old[3 * ib + k] - a0[k];
             c0[k] = pos_old[3 * ic + k] - a0[k];
-            A[k] = pos[3 * ia + k] - a0[k];
-            B[k] = pos[3 * ib + k] - a0[k];
-            C[k] = pos[3 * ic + k] - a0[k];
-            com[k] = wO * A[k] + wH * (B[k] + C[k]);  // wO = m_O / M, wH = m_H / M
-            a1[k] = A[k] - com[k];
-            b1[k] = B[k] - com[k];
-            c1[k] = C[k] - com[k];
+            Au[k] = A[k] = pos[3 * ia + k] - a0[k];
+            Bu[k] = B[k] = pos[3 * ib + k] - a0[k];
+            Cu[k] = C[k] = pos[3 * ic + k] - a0[k];
         }
-        // orthonormal frame: Z normal to the old plane, X = a1 x Z, Y = Z x X
-        real Z[3] = {b0[1] * c0[2] - b0[2] * c0[1], b0[2] * c0[0] - b0[0] * c0[2], b0[0] * c0[1] - b0[1] * c0[0]};
-        real X[3] = {a1[1] * Z[2] - a1[2] * Z[1], a1[2] * Z[0] - a1[0] * Z[2], a1[0] * Z[1] - a1[1] * Z[0]};
-        real Y[3] = {Z[1] * X[2] - Z[2] * X[1], Z[2] * X[0] - Z[0] * X[2], Z[0] * X[1] - Z[1] * X[0]};
-        const real nz = rsqrt(Z[0] * Z[0] + Z[1] * Z[1] + Z[2] * Z[2]);
-        const real nx = rsqrt(X[0] * X[0] + X[1] * X[1] + X[2] * X[2]);
-        const real ny = rsqrt(Y[0] * Y[0] + Y[1] * Y[1] + Y[2] * Y[2]);
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { X[k] *= nx; Y[k] *= ny; Z[k] *= nz; }
-        auto dot = [](const real* u, const real* v) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; };
-        const real xb0 = dot(b0, X), yb0 = dot(b0, Y), xc0 = dot(c0, X), yc0 = dot(c0, Y);
-        const real za1 = dot(a1, Z);
-        const real xb1 = dot(b1, X), yb1 = dot(b1, Y), zb1 = dot(b1, Z);
-        const real xc1 = dot(c1, X), yc1 = dot(c1, Y), zc1 = dot(c1, Z);
-        // tilt angles from the unchanged normal components
-        const real sinphi = za1 / ra;
-        const real cosphi = sqrt((real)1 - sinphi * sinphi);
-        const real sinpsi = (zb1 - zc1) / ((real)2 * rc * cosphi);
-        const real cospsi = sqrt((real)1 - sinpsi * sinpsi);
-        const real ya2 = ra * cosphi;
-        real xb2 = -rc * cospsi;
-        const real yb2 = -rb * cosphi - rc * sinpsi * sinphi;
-        const real yc2 = -rb * cosphi + rc * sinpsi * sinphi;
-        // re-impose |bc| = d_HH on xb2 (zero in exact arithmetic; removes the rounding of the two square roots)
-        const real dy = yb2 - yc2, dz = zb1 - zc1;
-        xb2 = (real)-0.5 * sqrt(fmax(d_hh2 - dy * dy - dz * dz, (real)0));
-        // in-plane rotation theta from the zero-torque condition about Z
-        const real alpha = xb2 * (xb0 - xc0) + yb0 * yb2 + yc0 * yc2;
-        const real beta = xb2 * (yc0 - yb0) + xb0 * yb2 + xc0 * yc2;
-        const real gamma = xb0 * yb1 - xb1 * yb0 + xc0 * yc1 - xc1 * yc0;
-        const real al2be2 = alpha * alpha + beta * beta;
-        const real sintheta = (alpha * gamma - beta * sqrt(fmax(al2be2 - gamma * gamma, (real)0))) / al2be2;
-        const real costheta = sqrt((real)1 - sintheta * sintheta);
-        const real a3[3] = {-ya2 * sintheta, ya2 * costheta, za1};
-        const real b3[3] = {xb2 * costheta - yb2 * sintheta, xb2 * sintheta + yb2 * costheta, zb1};
-        const real c3[3] = {-xb2 * costheta - yc2 * sintheta, -xb2 * sintheta + yc2 * costheta, zc1};
+        settle_molecule<real>(b0, c0, A, B, C, g);
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const real na = com[k] + X[k] * a3[0] + Y[k] * a3[1] + Z[k] * a3[2];
-            const real nb = com[k] + X[k] * b3[0] + Y[k] * b3[1] + Z[k] * b3[2];
-            const real nc = com[k] + X[k] * c3[0] + Y[k] * c3[1] + Z[k] * c3[2];
             if (vel) {  // the constraint displacement is a velocity change over dt
-                vel[3 * ia + k] += (na - A[k]) * inv_dt;
-                vel[3 * ib + k] += (nb - B[k]) * inv_dt;
-                vel[3 * ic + k] += (nc - C[k]) * inv_dt;
+                vel[3 * ia + k] += (A[k] - Au[k]) * inv_dt;
+                vel[3 * ib + k] += (B[k] - Bu[k]) * inv_dt;
+                vel[3 * ic + k] += (C[k] - Cu[k]) * inv_dt;
             }
-            pos[3 * ia + k] = a0[k] + na;
-            pos[3 * ib + k] = a0[k] + nb;
-            pos[3 * ic + k] = a0[k] + nc;
+            pos[3 * ia + k] = a0[k] + A[k];
+            pos[3 * ib + k] = a0[k] + B[k];
+            pos[3 * ic + k] = a0[k] + C[k];
         }
     }
+}
+
+// Steps 1 + 2 + 3 for a system of rigid waters in one pass: kick, drift, SETTLE, the constraint's velocity change, and the
+// rebuild trigger on the constrained positions.  The old positions live in registers, so no copy of them is needed.
+template <typename real, bool TRIGGER>
+__global__ void water_kick_drift_settle_kernel(real* __restrict__ pos, real* __restrict__ vel, const real* __restrict__ F,
+                                               const int32_t* __restrict__ water, int64_t n_w, SettleGeom<real> g, real imO,
+                                               real imH, real dt, const real* __restrict__ ref, real thr2,
+                                               unsigned long long* __restrict__ state, int* __restrict__ flag)
+{
+    real m = 0;
+    const real hdt = (real)0.5 * dt, inv_dt = (real)1 / dt;
+    for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_w; w += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t id[3] = {water[3 * w], water[3 * w + 1], water[3 * w + 2]};
+        real a0[3], b0[3], c0[3], P[3][3], U[3][3], V[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            a0[k] = pos[3 * id[0] + k];
+            b0[k] = pos[3 * id[1] + k] - a0[k];
+            c0[k] = pos[3 * id[2] + k] - a0[k];
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const real im = a == 0 ? imO : imH;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                V[a][k] = vel[3 * id[a] + k] + hdt * (F[3 * id[a] + k] * im);
+                const real rel0 = a == 0 ? (real)0 : (a == 1 ? b0[k] : c0[k]);
+                U[a][k] = P[a][k] = rel0 + dt * V[a][k];
+            }
+        }
+        settle_molecule<real>(b0, c0, P[0], P[1], P[2], g);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            real d2 = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const real x = a0[k] + P[a][k];
+                vel[3 * id[a] + k] = V[a][k] + (P[a][k] - U[a][k]) * inv_dt;
+                pos[3 * id[a] + k] = x;
+                if (TRIGGER) {
+                    const real d = x - ref[3 * id[a] + k];
+                    d2 += d * d;
+                }
+            }
+            if (TRIGGER) {
+                m = d2 > m ? d2 : m;
+                if (!(d2 == d2)) m = (real)INFINITY;
+            }
+        }
+    }
+    if (TRIGGER) trigger_reduce_and_flag<real>(m, thr2, state, flag);
 }
 
 // Step 6 for rigid three-site water (PAPER.md:281-292 step 6): remove the relative velocity along the three bonds with
 // impulses mu_k r_k shared by inverse mass.  Bonds k = (O,H1), (O,H2), (H1,H2) with r_k = x_i - x_j; the multipliers solve
 // the 3 x 3 system  sum_k c_lk (r_l . r_k) mu_k = -(v_i - v_j)_l . r_l,  c_lk = sum_a s_l(a) s_k(a) / m_a  (s = +1, -1 on the
 // two ends of a bond), directly (Cramer), one thread per molecule.
+// x: positions of O, H1, H2 (any common origin); v: their velocities, corrected in place
 template <typename real>
-__global__ void settle_vel_kernel(const real* __restrict__ pos, real* __restrict__ vel, const int32_t* __restrict__ water,
-                                  int64_t n_w, real imO, real imH)
+__device__ __forceinline__ void settle_vel_molecule(const real (*x)[3], real (*v)[3], real imO, real imH)
 {
+    real r0[3], r1[3], r2[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        r0[k] = x[0][k] - x[1][k];
+        r1[k] = x[0][k] - x[2][k];
+        r2[k] = x[1][k] - x[2][k];
+    }
+    auto dot = [](const real* u, const real* w) { return u[0] * w[0] + u[1] * w[1] + u[2] * w[2]; };
+    const real a00 = (imO + imH) * dot(r0, r0), a11 = (imO + imH) * dot(r1, r1), a22 = (imH + imH) * dot(r2, r2);
+    const real a01 = imO * dot(r0, r1), a02 = -imH * dot(r0, r2), a12 = imH * dot(r1, r2);
+    real b0 = 0, b1 = 0, b2 = 0;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        b0 -= (v[0][k] - v[1][k]) * r0[k];
+        b1 -= (v[0][k] - v[2][k]) * r1[k];
+        b2 -= (v[1][k] - v[2][k]) * r2[k];
+    }
+    // symmetric 3 x 3 solve by cofactors
+    const real c00 = a11 * a22 - a12 * a12, c01 = a02 * a12 - a01 * a22, c02 = a01 * a12 - a02 * a11;
+    const real c11 = a00 * a22 - a02 * a02, c12 = a01 * a02 - a00 * a12, c22 = a00 * a11 - a01 * a01;
+    const real idet = (real)1 / (a00 * c00 + a01 * c01 + a02 * c02);
+    const real mu0 = (c00 * b0 + c01 * b1 + c02 * b2) * idet;
+    const real mu1 = (c01 * b0 + c11 * b1 + c12 * b2) * idet;
+    const real mu2 = (c02 * b0 + c12 * b1 + c22 * b2) * idet;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        v[0][k] += imO * (mu0 * r0[k] + mu1 * r1[k]);
+        v[1][k] += imH * (mu2 * r2[k] - mu0 * r0[k]);
+        v[2][k] -= imH * (mu1 * r1[k] + mu2 * r2[k]);
+    }
+}
+
+// KICK: first v += (dt/2) F / m (step 5), then the velocity constraint (step 6); ke (if not NULL) accumulates the kinetic
+// energy of the constrained velocities (step 8), fp64, one atomic per block
+template <typename real, bool KICK>
+__global__ void settle_vel_kernel(const real* __restrict__ pos, real* __restrict__ vel, const real* __restrict__ F,
+                                  const int32_t* __restrict__ water, int64_t n_w, real imO, real imH, real hdt,
+                                  double* __restrict__ ke)
+{
+    double acc = 0.0;
     for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_w; w += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t ia = water[3 * w], ib = water[3 * w + 1], ic = water[3 * w + 2];
-        real r0[3], r1[3], r2[3], va[3], vb[3], vc[3];
+        const int64_t id[3] = {water[3 * w], water[3 * w + 1], water[3 * w + 2]};
+        real x[3][3], v[3][3];
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const real xa = pos[3 * ia + k], xb = pos[3 * ib + k], xc = pos[3 * ic + k];
-            r0[k] = xa - xb;
-            r1[k] = xa - xc;
-            r2[k] = xb - xc;
-            va[k] = vel[3 * ia + k];
-            vb[k] = vel[3 * ib + k];
-            vc[k] = vel[3 * ic + k];
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                x[a][k] = pos[3 * id[a] + k];
+                v[a][k] = vel[3 * id[a] + k];
+                if (KICK) v[a][k] += hdt * (F[3 * id[a] + k] * (a == 0 ? imO : imH));
+            }
+        settle_vel_molecule<real>(x, v, imO, imH);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) vel[3 * id[a] + k] = v[a][k];
+            if (KICK) acc += (double)(v[a][0] * v[a][0] + v[a][1] * v[a][1] + v[a][2] * v[a][2]) / (double)(a == 0 ? imO : imH);
         }
-        auto dot = [](const real* u, const real* v) { return u[0] * v[0] + u[1] * v[1] + u[2] * v[2]; };
-        const real a00 = (imO + imH) * dot(r0, r0), a11 = (imO + imH) * dot(r1, r1), a22 = (imH + imH) * dot(r2, r2);
-        const real a01 = imO * dot(r0, r1), a02 = -imH * dot(r0, r2), a12 = imH * dot(r1, r2);
-        real b0 = 0, b1 = 0, b2 = 0;
+    }
+    if (KICK && ke) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            b0 -= (va[k] - vb[k]) * r0[k];
-            b1 -= (va[k] - vc[k]) * r1[k];
-            b2 -= (vb[k] - vc[k]) * r2[k];
-        }
-        // symmetric 3 x 3 solve by cofactors
-        const real c00 = a11 * a22 - a12 * a12, c01 = a02 * a12 - a01 * a22, c02 = a01 * a12 - a02 * a11;
-        const real c11 = a00 * a22 - a02 * a02, c12 = a01 * a02 - a00 * a12, c22 = a00 * a11 - a01 * a01;
-        const real idet = (real)1 / (a00 * c00 + a01 * c01 + a02 * c02);
-        const real mu0 = (c00 * b0 + c01 * b1 + c02 * b2) * idet;
-        const real mu1 = (c01 * b0 + c11 * b1 + c12 * b2) * idet;
-        const real mu2 = (c02 * b0 + c12 * b1 + c22 * b2) * idet;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            vel[3 * ia + k] = va[k] + imO * (mu0 * r0[k] + mu1 * r1[k]);
-            vel[3 * ib + k] = vb[k] + imH * (mu2 * r2[k] - mu0 * r0[k]);
-            vel[3 * ic + k] = vc[k] - imH * (mu1 * r1[k] + mu2 * r2[k]);
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        __shared__ double sh[8];
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int q = 0; q < (int)(blockDim.x >> 5); ++q) t += sh[q];
+            atomicAdd(ke, 0.5 * t);
         }
     }
 }
@@ -334,20 +443,25 @@ int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64
     return DIMOS_OK;
 }
 
+template <typename real>
+static SettleGeom<real> settle_geom(double m_O, double m_H, double d_OH, double d_HH)
+{
+    const double M = m_O + 2.0 * m_H, rc = 0.5 * d_HH, h = sqrt(d_OH * d_OH - rc * rc);
+    const double ra = h * 2.0 * m_H / M;
+    return SettleGeom<real>{(real)(m_O / M), (real)(m_H / M), (real)ra, (real)(h - ra), (real)rc, (real)(d_HH * d_HH)};
+}
+
 int settle_impl(Ctx* ctx, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w, double m_O,
                 double m_H, double d_OH, double d_HH, double dt, cudaStream_t s)
 {
-    const double M = m_O + 2.0 * m_H, rc = 0.5 * d_HH, h = sqrt(d_OH * d_OH - rc * rc);
-    const double ra = h * 2.0 * m_H / M, rb = h - ra;  // O and the HH midpoint from the centre of mass
     const double inv_dt = dt > 0 ? 1.0 / dt : 0.0;
     const int blocks = grid_for(ctx, n_w);
     if (ctx->precision == DIMOS_F64)
-        settle_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos_old, (double*)pos, (double*)vel, water, n_w, m_O / M,
-                                                     m_H / M, ra, rb, rc, d_HH * d_HH, inv_dt);
+        settle_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos_old, (double*)pos, (double*)vel, water, n_w,
+                                                     settle_geom<double>(m_O, m_H, d_OH, d_HH), inv_dt);
     else
         settle_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos_old, (float*)pos, (float*)vel, water, n_w,
-                                                    (float)(m_O / M), (float)(m_H / M), (float)ra, (float)rb, (float)rc,
-                                                    (float)(d_HH * d_HH), (float)inv_dt);
+                                                    settle_geom<float>(m_O, m_H, d_OH, d_HH), (float)inv_dt);
     DIMOS_LAUNCH_CHECK(ctx, "settle");
     return DIMOS_OK;
 }
@@ -357,11 +471,54 @@ int settle_vel_impl(Ctx* ctx, const void* pos, void* vel, const int32_t* water, 
 {
     const int blocks = grid_for(ctx, n_w);
     if (ctx->precision == DIMOS_F64)
-        settle_vel_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos, (double*)vel, water, n_w, 1.0 / m_O, 1.0 / m_H);
+        settle_vel_kernel<double, false><<<blocks, 256, 0, s>>>((const double*)pos, (double*)vel, nullptr, water, n_w, 1.0 / m_O,
+                                                                1.0 / m_H, 0.0, nullptr);
     else
-        settle_vel_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos, (float*)vel, water, n_w, (float)(1.0 / m_O),
-                                                        (float)(1.0 / m_H));
+        settle_vel_kernel<float, false><<<blocks, 256, 0, s>>>((const float*)pos, (float*)vel, nullptr, water, n_w,
+                                                               (float)(1.0 / m_O), (float)(1.0 / m_H), 0.f, nullptr);
     DIMOS_LAUNCH_CHECK(ctx, "settle_velocities");
+    return DIMOS_OK;
+}
+
+template <typename real>
+static void launch_water_a(Ctx* ctx, void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O,
+                           double m_H, double d_OH, double d_HH, double dt, const void* ref, double skin, int32_t* flag_dev,
+                           cudaStream_t s)
+{
+    const int blocks = grid_for(ctx, n_w);
+    const real h = (real)0.5 * (real)skin;
+    const SettleGeom<real> g = settle_geom<real>(m_O, m_H, d_OH, d_HH);
+    if (ref && flag_dev)
+        water_kick_drift_settle_kernel<real, true><<<blocks, 256, 0, s>>>((real*)pos, (real*)vel, (const real*)F, water, n_w, g,
+                                                                          (real)(1.0 / m_O), (real)(1.0 / m_H), (real)dt,
+                                                                          (const real*)ref, h * h, ctx->d_rebuild_state, flag_dev);
+    else
+        water_kick_drift_settle_kernel<real, false><<<blocks, 256, 0, s>>>((real*)pos, (real*)vel, (const real*)F, water, n_w, g,
+                                                                           (real)(1.0 / m_O), (real)(1.0 / m_H), (real)dt, nullptr,
+                                                                           (real)0, nullptr, nullptr);
+}
+
+int water_step_a_impl(Ctx* ctx, void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O, double m_H,
+                      double d_OH, double d_HH, double dt, const void* ref, double skin, int32_t* flag_dev, cudaStream_t s)
+{
+    if (ctx->precision == DIMOS_F64) launch_water_a<double>(ctx, pos, vel, F, water, n_w, m_O, m_H, d_OH, d_HH, dt, ref, skin, flag_dev, s);
+    else launch_water_a<float>(ctx, pos, vel, F, water, n_w, m_O, m_H, d_OH, d_HH, dt, ref, skin, flag_dev, s);
+    DIMOS_LAUNCH_CHECK(ctx, "water_kick_drift_settle");
+    return DIMOS_OK;
+}
+
+int water_step_b_impl(Ctx* ctx, const void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O,
+                      double m_H, double dt, double* ke_dev, cudaStream_t s)
+{
+    if (ke_dev) DIMOS_CUDA_TRY(ctx, cudaMemsetAsync(ke_dev, 0, sizeof(double), s));
+    const int blocks = grid_for(ctx, n_w);
+    if (ctx->precision == DIMOS_F64)
+        settle_vel_kernel<double, true><<<blocks, 256, 0, s>>>((const double*)pos, (double*)vel, (const double*)F, water, n_w,
+                                                               1.0 / m_O, 1.0 / m_H, 0.5 * dt, ke_dev);
+    else
+        settle_vel_kernel<float, true><<<blocks, 256, 0, s>>>((const float*)pos, (float*)vel, (const float*)F, water, n_w,
+                                                              (float)(1.0 / m_O), (float)(1.0 / m_H), (float)(0.5 * dt), ke_dev);
+    DIMOS_LAUNCH_CHECK(ctx, "water_kick_settle_velocities");
     return DIMOS_OK;
 }
 

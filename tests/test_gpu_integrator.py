@@ -194,11 +194,14 @@ def test_settle_velocities_match_converged_rattle(precision, n_w):
     assert np.abs((M * np.cross(Xc, G)).sum(1) - (M * np.cross(Xc, V0)).sum(1)).max() < tol * m_O * d_oh * 4
 
 
+@pytest.mark.parametrize("fused", [False, True])
 @pytest.mark.parametrize("precision", ["f32", "f64"])
-def test_constrained_velocity_verlet_steps_match_oracle(precision):
+def test_constrained_velocity_verlet_steps_match_oracle(precision, fused):
     """Steps 1, 2, 3, 5, 6 of PAPER.md:281-292 chained on the device for rigid water with seeded forces, four time steps in
     a row, against the same chain of oracle functions (kick+drift, SHAKE, kick, RATTLE velocities): positions, velocities,
-    and the rigid geometry at the end."""
+    and the rigid geometry at the end.  fused: the same chain through dimos_water_kick_drift_settle and
+    dimos_water_kick_settle_velocities (two passes per step), with the rebuild flag and the kinetic energy they report
+    checked against the oracle's on the last step."""
     n_w = 700
     rng = np.random.default_rng(77)
     np_real = np.float64 if precision == "f64" else np.float32
@@ -227,13 +230,24 @@ def test_constrained_velocity_verlet_steps_match_oracle(precision):
         xd, vd = torch.from_numpy(x.copy()).to(dev), torch.from_numpy(v.copy()).to(dev)
         wd, imd = torch.from_numpy(water).to(dev), torch.from_numpy(inv_m).to(dev)
         fd = [torch.from_numpy(f).to(dev) for f in forces]
+        ref_d = xd.clone()
+        skin = 2.0 * float(np.sqrt(((xo - x.astype(np.float64)) ** 2).sum(1).max())) * 0.9   # fires on the last step only?
         for s in range(4):
-            x_old = xd.clone()
-            dimos.dimos_vv_kick_drift(ctx, xd, vd, fd[s], imd, dt)
-            dimos.dimos_settle(ctx, x_old, xd, wd, m_O, m_H, d_oh, d_hh, vel=vd, dt=dt)
-            dimos.dimos_vv_kick(ctx, vd, fd[s + 1], imd, dt)
-            dimos.dimos_settle_velocities(ctx, xd, vd, wd, m_O, m_H)
+            if fused:
+                fired = dimos.dimos_water_kick_drift_settle(ctx, xd, vd, fd[s], wd, m_O, m_H, d_oh, d_hh, dt, pos_at_build=ref_d, skin=skin)
+                ke = dimos.dimos_water_kick_settle_velocities(ctx, xd, vd, fd[s + 1], wd, m_O, m_H, dt, want_ke=True)
+            else:
+                x_old = xd.clone()
+                dimos.dimos_vv_kick_drift(ctx, xd, vd, fd[s], imd, dt)
+                dimos.dimos_settle(ctx, x_old, xd, wd, m_O, m_H, d_oh, d_hh, vel=vd, dt=dt)
+                dimos.dimos_vv_kick(ctx, vd, fd[s + 1], imd, dt)
+                dimos.dimos_settle_velocities(ctx, xd, vd, wd, m_O, m_H)
         torch.cuda.synchronize()
+        if fused:
+            want, m_disp = oracle.needs_rebuild(xd.cpu().numpy(), x, skin)
+            assert fired == want and fired  # skin was chosen 10 % below twice the oracle's largest displacement
+            assert float(ke[0]) == pytest.approx(oracle.kinetic_energy(vo, mass), rel=1e-9 if precision == "f64" else 1e-4)
+            assert dimos.dimos_water_kick_drift_settle(ctx, xd.clone(), vd.clone(), fd[0], wd, m_O, m_H, d_oh, d_hh, dt) is None
         gx, gv = xd.cpu().numpy().astype(np.float64), vd.cpu().numpy().astype(np.float64)
     tol_x = 1e-11 if precision == "f64" else 1e-5      # fp32: 4 steps x (rounding of 6 nm coordinates ~ 5e-7)
     tol_v = 1e-9 if precision == "f64" else 4e-3       # (x_c - x_u) / dt amplifies position rounding by 1/dt = 500
@@ -281,8 +295,9 @@ def test_kinetic_energy_and_berendsen_match_oracle(precision, n):
     assert T_after == pytest.approx(T_o + dt / tau * (T0 - T_o), rel=1e-12 if precision == "f64" else 1e-6)
 
 
+@pytest.mark.parametrize("fused", [False, True])
 @pytest.mark.parametrize("precision", ["f32", "f64"])
-def test_rigid_water_nve_conserves_total_energy(precision):
+def test_rigid_water_nve_conserves_total_energy(precision, fused):
     """The whole loop of PAPER.md:281-292 on the device (steps 1-6: kick+drift with the fused trigger, SETTLE, list rebuild
     when the trigger fires, pair forces, kick, velocity constraints) for the 3000-molecule box, started from the
     un-equilibrated synthetic configuration: some 6e4 kJ/mol flow from potential into kinetic energy within a few dozen
@@ -319,17 +334,26 @@ def test_rigid_water_nve_conserves_total_energy(precision):
         K0 = dimos.dimos_kinetic_energy(ctx, vel, inv_m)
         tot, pot, rebuilds = [U0 + K0], [U0], 0
         for _ in range(100):
-            old = pos.clone()
-            fired = dimos.dimos_vv_kick_drift(ctx, pos, vel, F, inv_m, dt, pos_at_build=nl.pos_at_build, skin=0.1)
-            dimos.dimos_settle(ctx, old, pos, water, m_O, m_H, d_oh, d_hh, vel=vel, dt=dt)
-            if fired or dimos.dimos_nl_needs_rebuild(ctx, pos, nl.pos_at_build, 0.1):  # SETTLE moved atoms after the drift
+            if fused:  # two passes per step; the trigger sees the constrained positions
+                fired = dimos.dimos_water_kick_drift_settle(ctx, pos, vel, F, water, m_O, m_H, d_oh, d_hh, dt,
+                                                            pos_at_build=nl.pos_at_build, skin=0.1)
+            else:
+                old = pos.clone()
+                fired = dimos.dimos_vv_kick_drift(ctx, pos, vel, F, inv_m, dt, pos_at_build=nl.pos_at_build, skin=0.1)
+                dimos.dimos_settle(ctx, old, pos, water, m_O, m_H, d_oh, d_hh, vel=vel, dt=dt)
+                fired = fired or dimos.dimos_nl_needs_rebuild(ctx, pos, nl.pos_at_build, 0.1)  # SETTLE moved atoms after the drift
+            if fired:
                 nl = dimos.dimos_nl_build(ctx, pos, L, 1.0, 0.1, excl, nl=nl)
                 rebuilds += 1
             F, E, W = dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F)
-            dimos.dimos_vv_kick(ctx, vel, F, inv_m, dt)
-            dimos.dimos_settle_velocities(ctx, pos, vel, water, m_O, m_H)
+            if fused:
+                K = float(dimos.dimos_water_kick_settle_velocities(ctx, pos, vel, F, water, m_O, m_H, dt, want_ke=True)[0])
+            else:
+                dimos.dimos_vv_kick(ctx, vel, F, inv_m, dt)
+                dimos.dimos_settle_velocities(ctx, pos, vel, water, m_O, m_H)
+                K = dimos.dimos_kinetic_energy(ctx, vel, inv_m)
             pot.append(float(E[0]))
-            tot.append(pot[-1] + dimos.dimos_kinetic_energy(ctx, vel, inv_m))
+            tot.append(pot[-1] + K)
         m = pos.cpu().numpy().astype(np.float64).reshape(-1, 3, 3)
     flow = U0 - min(pot)
     assert rebuilds >= 1 and flow > 2.0 * K0
