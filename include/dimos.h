@@ -296,6 +296,10 @@ DIMOS_API int dimos_kinetic_energy(dimos_ctx* ctx, const void* vel, const void* 
                                    double* ke_host, void* stream);
 DIMOS_API int dimos_berendsen(dimos_ctx* ctx, void* vel, const void* inv_mass, int64_t N, int64_t n_dof, double T0, double tau,
                               double dt, double* ke_dev, double* T_host, void* stream);
+/* dimos_berendsen_scale -- the rescaling half of dimos_berendsen with the kinetic energy taken from *ke_dev as some earlier
+ * call on the same stream left it (dimos_kinetic_energy, dimos_water_kick_settle_velocities): one pass over vel, no sum. */
+DIMOS_API int dimos_berendsen_scale(dimos_ctx* ctx, void* vel, int64_t N, int64_t n_dof, double T0, double tau, double dt,
+                                    const double* ke_dev, void* stream);
 
 /* dimos_water_kick_drift_settle / dimos_water_kick_settle_velocities -- the velocity-Verlet loop of PAPER.md:281-292 for a
  * system of rigid three-site waters in two passes instead of five: each thread holds one molecule in registers.

@@ -32,6 +32,7 @@ EXPORTED_SYMBOLS = (
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
     "dimos_kinetic_energy", "dimos_berendsen", "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities",
+    "dimos_berendsen_scale",
 )
 
 
@@ -101,6 +102,7 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_water_kick_drift_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp, dbl, vp,
                                                   ctypes.POINTER(i32), vp]
     lib.dimos_water_kick_settle_velocities.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, vp, vp]
+    lib.dimos_berendsen_scale.argtypes = [vp, vp, i64, i64, dbl, dbl, dbl, vp, vp]
     lib.dimos_kinetic_energy.argtypes = [vp, vp, vp, i64, vp, ctypes.POINTER(dbl), vp]
     lib.dimos_berendsen.argtypes = [vp, vp, vp, i64, i64, dbl, dbl, dbl, vp, ctypes.POINTER(dbl), vp]
     lib.dimos_nl_export_edges.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ctypes.POINTER(i64), vp]
@@ -123,7 +125,7 @@ def load_library() -> ctypes.CDLL:
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
                  "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
                  "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen",
-                 "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities"):
+                 "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities", "dimos_berendsen_scale"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -471,6 +473,15 @@ class Context:
         self._check(rc)
         return out.value if sync else None
 
+    def berendsen_scale(self, vel, n_dof, T0, tau, dt, ke):
+        """dimos_berendsen_scale: rescale vel with the kinetic energy already in the device tensor `ke` (1 double)."""
+        vel = self._dev(vel, self.real, 3)
+        ke = self._dev(ke, torch.float64)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_berendsen_scale(self.handle, vel.data_ptr(), vel.shape[0], int(n_dof), float(T0), float(tau),
+                                                float(dt), ke.data_ptr(), _stream_ptr())
+        self._check(rc)
+
     def nl_set_exceptions(self, nl: NeighborList, pairs, scale):
         """dimos_nl_set_exceptions: pairs (n,2) int32 i<j, scale (n,2) float64 = (Coulomb scale, LJ scale); None clears."""
         if pairs is None or len(pairs) == 0:
@@ -594,6 +605,10 @@ def dimos_water_kick_drift_settle(ctx: Context, pos, vel, F, water, m_O, m_H, d_
 
 def dimos_water_kick_settle_velocities(ctx: Context, pos, vel, F, water, m_O, m_H, dt, want_ke=False):
     return ctx.water_kick_settle_velocities(pos, vel, F, water, m_O, m_H, dt, want_ke=want_ke)
+
+
+def dimos_berendsen_scale(ctx: Context, vel, n_dof, T0, tau, dt, ke):
+    return ctx.berendsen_scale(vel, n_dof, T0, tau, dt, ke)
 
 
 def dimos_kinetic_energy(ctx: Context, vel, inv_mass):

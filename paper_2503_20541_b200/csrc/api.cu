@@ -474,6 +474,18 @@ DIMOS_API int dimos_berendsen(dimos_ctx* c, void* vel, const void* inv_mass, int
     return DIMOS_OK;
 }
 
+DIMOS_API int dimos_berendsen_scale(dimos_ctx* c, void* vel, int64_t N, int64_t n_dof, double T0, double tau, double dt,
+                                    const double* ke_dev, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!vel || !ke_dev) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || n_dof <= 0) return set_error(ctx, DIMOS_EINVAL, "N and n_dof must be > 0");
+    if (!(T0 >= 0) || !(tau > 0) || !(dt > 0) || !(dt <= tau)) return set_error(ctx, DIMOS_EINVAL, "need T0 >= 0 and 0 < dt <= tau");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return berendsen_scale_impl(ctx, vel, N, ke_dev, 2.0 / ((double)n_dof * 8.314462618e-3), T0, dt / tau, (cudaStream_t)stream);
+}
+
 static int check_nb_args(Ctx* ctx, const NL* nl, int32_t ntypes, const double* box, const dimos_nb_params* p)
 {
     if (!list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");

@@ -281,6 +281,11 @@ def test_kinetic_energy_and_berendsen_match_oracle(precision, n):
         T = dimos.dimos_berendsen(ctx, vd, imd, n_dof, T0, tau, dt)
         got = vd.cpu().numpy().astype(np.float64)
         K2 = dimos.dimos_kinetic_energy(ctx, vd, imd)
+        v_split = torch.from_numpy(v.copy()).to(dev)   # the two halves called separately give the same velocities
+        dimos.dimos_kinetic_energy(ctx, v_split, imd)
+        dimos.dimos_berendsen_scale(ctx, v_split, n_dof, T0, tau, dt, ctx._ke_scratch())
+        torch.cuda.synchronize()
+        assert torch.allclose(v_split, vd, rtol=1e-6, atol=0)
         v_async = torch.from_numpy(v.copy()).to(dev)
         assert dimos.dimos_berendsen(ctx, v_async, imd, n_dof, T0, tau, dt, sync=False) is None
         torch.cuda.synchronize()
