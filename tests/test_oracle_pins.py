@@ -106,6 +106,75 @@ def test_rf_energy_vanishes_at_cutoff_and_force_limit(eps_rf, rc):
     assert res.E[0] == 0.0 and f == 0.0 and res.n_pairs == 0
 
 
+# --- the cutoff-band force allowance of reading C-10 (the `allow` output) ------------------------------------
+# SURVEY.md §8(c) C-10 prints the values: at r_c = 1.0, eps_rf = 78.5 the RF force jump at the cutoff is
+# f(r_c) = 3 k_e q_i q_j / ((2 eps_rf + 1) r_c^2) = 1.835 (O-O), 0.917 (O-H), 0.459 (H-H) kJ mol^-1 nm^-1.
+C10_JUMP = {("O", "O"): 1.835, ("O", "H"): 0.917, ("H", "H"): 0.459}
+
+
+@pytest.mark.parametrize("kinds", sorted(C10_JUMP))
+@pytest.mark.parametrize("offset,inside_band", [(-5e-6, True), (5e-6, True), (-2e-5, False), (2e-5, False)])
+def test_allow_is_the_rf_force_jump_inside_the_band_and_zero_outside(kinds, offset, inside_band):
+    """allow_i = sum over pairs with |r - r_c| < band of |f_ij| (reading C-10): for one pair at r_c + offset both atoms get
+    the RF force jump f(r_c) when |offset| < band = 1e-5 and exactly 0 otherwise, on either side of the cutoff."""
+    a, b = kinds
+    rc = 1.0
+    res, f = two_particles(a, b, rc + offset, rc, band=1e-5)
+    closed = 3.0 * KE * abs(Q[a] * Q[b]) / ((2 * 78.5 + 1) * rc * rc)
+    assert closed == pytest.approx(C10_JUMP[kinds], abs=5e-4)  # the survey's printed value (3 decimals)
+    if inside_band:
+        # f_RF(r) = k_e qq (1/r^2 - 2 k_rf r) is small at r_c because the two terms nearly cancel (1 - 2 k_rf = 0.019), so
+        # d ln f / dr = -(2 + 2 k_rf) / (1 - 2 k_rf) = -157 per nm: |offset| = 5e-6 moves it by 7.8e-4 relative; LJ adds
+        # its own 0.015 for O-O (SURVEY C-10)
+        lj = 0.016 if kinds == ("O", "O") else 0.0
+        assert res.allow[0] == pytest.approx(closed, abs=lj + 160 * abs(offset) * closed)
+        assert res.allow[1] == res.allow[0]
+    else:
+        assert res.allow[0] == 0.0 and res.allow[1] == 0.0
+    # the allowance never changes what is computed: forces only from the in-cutoff side
+    assert (f != 0.0) == (offset < 0)
+
+
+def test_allow_is_none_without_band_and_sparse_with_it():
+    """band = 0 disables the allowance; with band = 1e-5 only atoms owning a pair within the band get a non-zero value
+    (SURVEY C-10 expects ~2.8 % of atoms; a band 100x too wide, or an allowance summed over all pairs, fails here), and
+    each value equals the sum of |f_ij| over exactly those pairs (recounted here by brute force in numpy)."""
+    wb = wl.make_config(1)  # 9,000 atoms
+    tab = lj_table()
+    rc, band = 1.0, 1e-5
+    res0 = oracle.nonbonded(wb.pos, wb.charge, wb.type, tab, wb.box, rc, excl_pairs=wb.excl_pairs, band=0.0)
+    assert res0.allow is None
+    res = oracle.nonbonded(wb.pos, wb.charge, wb.type, tab, wb.box, rc, excl_pairs=wb.excl_pairs, band=band)
+    assert np.array_equal(res.F, res0.F) and np.array_equal(res.E, res0.E)
+    n = wb.n_atoms
+    frac = (res.allow > 0).mean()
+    assert 0.0 < frac < 0.05, frac
+    # independent recount: pairs within the band from scipy's periodic k-d tree, |f| from the closed RF form
+    from scipy.spatial import cKDTree
+
+    pos = wb.pos.astype(np.float64)
+    tree = cKDTree(pos, boxsize=wb.box)
+    outer = tree.query_pairs(rc + band, output_type="ndarray")
+    d = pos[outer[:, 0]] - pos[outer[:, 1]]
+    d -= wb.box * np.rint(d / wb.box)
+    r = np.sqrt((d * d).sum(1))
+    sel = np.abs(r - rc) < band
+    i, j, r = outer[sel, 0], outer[sel, 1], r[sel]
+    keep = (i // 3) != (j // 3)  # workloads.py: atoms 3m..3m+2 form one molecule and exclude one another
+    i, j, r = i[keep], j[keep], r[keep]
+    assert len(i) > 20 and len(np.unique(np.concatenate([i, j]))) == (res.allow > 0).sum()
+    k_rf = (78.5 - 1) / ((2 * 78.5 + 1) * rc**3)
+    qq = KE * wb.charge[i].astype(np.float64) * wb.charge[j].astype(np.float64)
+    f_c = qq * (1.0 / r**3 - 2 * k_rf) * r
+    both_o = (wb.type[i] == 0) & (wb.type[j] == 0)
+    s6 = (wl.SIGMA_O / r) ** 6
+    f_lj = np.where(both_o, 24 * wl.EPS_O * (2 * s6 * s6 - s6) / r, 0.0)
+    want = np.zeros(n)
+    np.add.at(want, i, np.abs(f_c + f_lj))
+    np.add.at(want, j, np.abs(f_c + f_lj))
+    assert np.allclose(res.allow, want, rtol=1e-9, atol=1e-12)
+
+
 def test_rf_with_unit_dielectric_is_shifted_coulomb():
     # eps_rf = 1 => k_rf = 0, c_rf = 1/r_c: the textbook shifted Coulomb potential k_e qq (1/r - 1/r_c)
     res, f = two_particles("H", "H", 0.5, 2.0, eps_rf=1.0)
