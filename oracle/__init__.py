@@ -7,6 +7,7 @@ from .dimos_oracle import (  # noqa: F401
     METHOD_EWALD_REAL,
     METHOD_RF,
     NonbondedResult,
+    count_pairs,
     edge_vectors,
     lorentz_berthelot,
     needs_rebuild,

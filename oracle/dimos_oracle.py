@@ -151,6 +151,18 @@ def neighbor_pairs(pos, box, r_list, excl_pairs=None, algorithm="celllist") -> n
     return pairs
 
 
+def count_pairs(pos, box, r_list, excl_pairs=None, algorithm="celllist") -> int:
+    """Number of pairs neighbor_pairs would return (the C routine's count-only call)."""
+    lib = _load()
+    pos, box = _d(pos), _d(box)
+    excl = _i(excl_pairs if excl_pairs is not None else np.zeros((0, 2), np.int32)).reshape(-1, 2)
+    fn = {"bruteforce": lib.orc_neighbor_pairs_bruteforce, "celllist": lib.orc_neighbor_pairs_celllist}[algorithm]
+    total = fn(pos.shape[0], _dp(pos), _dp(box), float(r_list), _ip(excl), excl.shape[0], None, 0)
+    if total < 0:
+        raise MemoryError(f"oracle count_pairs failed rc={total}")
+    return int(total)
+
+
 def needs_rebuild(pos, pos_at_build, skin):
     """(flag, max displacement): PAPER.md:175, strict max |dr| > skin/2 on raw coordinates."""
     pos, ref = _d(pos), _d(pos_at_build)

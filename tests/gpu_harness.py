@@ -66,6 +66,32 @@ def check_neighbor_set(gpu_pairs, pos, box, r_nl, excl_pairs):
     return len(gk), len(must), len(may)
 
 
+def check_neighbor_set_device(gpu_pairs, pos, box, r_nl, excl_pairs):
+    """check_neighbor_set for lists of 1e7 ... 3e8 pairs: the same comparison (sorted int64 keys i * n + j; every oracle
+    pair with r < r_nl - BAND is in the GPU set, every GPU pair has r < r_nl + BAND in the oracle) with the sorting and
+    the membership tests done by torch on the device.  gpu_pairs: (m, 2) int32 CUDA tensor."""
+    n = pos.shape[0]
+    assert bool((gpu_pairs[:, 0] < gpu_pairs[:, 1]).all()), "exported pairs must have i < j"
+    gk = torch.sort(gpu_pairs[:, 0].long() * n + gpu_pairs[:, 1].long()).values
+    assert bool((gk[1:] > gk[:-1]).all()), "duplicate pair in the exported neighbour set"
+    counts = {}
+    for name, radius in (("must", r_nl - BAND), ("may", r_nl + BAND)):
+        op = torch.from_numpy(oracle.neighbor_pairs(pos, box, radius, excl_pairs, "celllist")).to(gk.device)
+        ok = torch.sort(op[:, 0].long() * n + op[:, 1].long()).values
+        del op
+        counts[name] = int(ok.numel())
+        if name == "must":  # every oracle pair is in the GPU set
+            idx = torch.searchsorted(gk, ok).clamp_(max=gk.numel() - 1)
+            bad = ok[gk[idx] != ok]
+            assert bad.numel() == 0, f"{bad.numel()} oracle pairs missing from the GPU list, first (i,j)={divmod(int(bad[0]), n)}"
+        else:  # every GPU pair is in the oracle's wider set
+            idx = torch.searchsorted(ok, gk).clamp_(max=ok.numel() - 1)
+            bad = gk[ok[idx] != gk]
+            assert bad.numel() == 0, f"{bad.numel()} GPU pairs not in the oracle set, first (i,j)={divmod(int(bad[0]), n)}"
+        del ok, idx, bad
+    return int(gk.numel()), counts["must"], counts["may"]
+
+
 def check_nonbonded(F, E, W, orc, precision, use_allow=True):
     """Element-by-element force comparison + energy components + virial against an oracle result."""
     e_tol, f_tol = TOL[precision]
@@ -75,6 +101,8 @@ def check_nonbonded(F, E, W, orc, precision, use_allow=True):
     rms = float(np.sqrt((orc.F ** 2).sum(axis=1).mean()))
     dF = np.sqrt(((F - orc.F) ** 2).sum(axis=1))
     allow = orc.allow if (use_allow and orc.allow is not None and precision != "f64") else np.zeros_like(dF)
+    # reading C-10: the allowance is rare (SURVEY expects ~2.8 % of atoms own a pair within 1e-5 nm of r_c)
+    assert (allow > 0).mean() <= 0.05, f"{(allow > 0).mean():.3f} of the atoms carry a cutoff-band allowance"
     excess = dF - allow
     worst = int(np.argmax(excess))
     assert excess[worst] <= f_tol * rms, (
@@ -92,8 +120,11 @@ def check_nonbonded(F, E, W, orc, precision, use_allow=True):
 
 
 def run_case(wb, precision, r_cut, skin, method, box=None, pos=None, eps_rf=78.5, alpha=3.12, oracle_alg="celllist",
-             check_set=True, r_switch=0.0, exceptions=None):
-    """Build + export + nonbonded on the GPU, compare all of it with the oracle.  Returns a small report."""
+             check_set=True, r_switch=0.0, exceptions=None, on_device=False):
+    """Build + export + nonbonded on the GPU, compare all of it with the oracle.  Returns a small report.
+    on_device: sort / compare the pair keys with torch on the GPU (the 1e8-pair sets of the full-size configs), and
+    compare the in-cutoff pair count dimos_nl_count_within(r_cut) -- the numerator of bench.py's metric -- with the
+    oracle's, up to the pairs within BAND of r_cut."""
     db = DeviceBox(wb, precision, box=box, pos=pos)
     ctx = dimos.Context(0, precision)
     try:
@@ -101,7 +132,12 @@ def run_case(wb, precision, r_cut, skin, method, box=None, pos=None, eps_rf=78.5
         rep = {"stats": nl.stats()}
         assert torch.equal(nl.pos_at_build, db.pos)
         pos64 = db.pos.double().cpu().numpy()
-        if check_set:
+        if check_set and on_device:
+            gp = dimos.dimos_nl_export_pairs(ctx, nl)
+            rep["set"] = check_neighbor_set_device(gp, pos64, db.box, r_cut + skin, wb.excl_pairs)
+            del gp
+            torch.cuda.empty_cache()
+        elif check_set:
             gp = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy()
             rep["set"] = check_neighbor_set(gp, pos64, db.box, r_cut + skin, wb.excl_pairs)
         if exceptions is not None:
@@ -115,6 +151,13 @@ def run_case(wb, precision, r_cut, skin, method, box=None, pos=None, eps_rf=78.5
                                r_switch=r_switch, exceptions=exceptions)
         rep.update(check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision))
         rep["n_pairs_cut"] = orc.n_pairs
+        if on_device:
+            lo = oracle.count_pairs(pos64, db.box, r_cut - BAND, wb.excl_pairs)
+            hi = oracle.count_pairs(pos64, db.box, r_cut + BAND, wb.excl_pairs)
+            got = ctx.nl_count_within(nl, r_cut)
+            assert lo <= orc.n_pairs <= hi
+            assert lo <= got <= hi, f"dimos_nl_count_within(r_cut) = {got}, oracle {orc.n_pairs} (band [{lo}, {hi}])"
+            rep["count_within"] = (got, lo, hi)
         return rep
     finally:
         ctx.close()
