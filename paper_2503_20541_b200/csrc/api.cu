@@ -54,7 +54,7 @@ static void free_list(Ctx* ctx, NL* nl)
 {
     DevBuf* bufs[] = {&nl->cell_count, &nl->cell_start, &nl->unit_start, &nl->scan_tmp, &nl->atom_cell, &nl->atom_rank,
                       &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
-                      &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->jslot, &nl->meta, &nl->row_info,
+                      &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->entry, &nl->emask, &nl->row_info,
                       &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials, &nl->accum,
                       &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW, &nl->st_ref, &nl->st_flag,
                       &nl->export_count};
@@ -66,7 +66,7 @@ static size_t list_workspace_bytes(const NL* nl)
 {
     const DevBuf* bufs[] = {&nl->cell_count, &nl->cell_start, &nl->unit_start, &nl->scan_tmp, &nl->atom_cell, &nl->atom_rank,
                             &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
-                            &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->jslot, &nl->meta,
+                            &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->entry, &nl->emask,
                             &nl->row_info, &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials,
                             &nl->accum, &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW,
                             &nl->st_ref, &nl->st_flag, &nl->export_count};
@@ -749,7 +749,7 @@ DIMOS_API int dimos_nl_stats(const dimos_nl* l, dimos_nl_stats_t* out)
     out->n_entries = nl->n_entries;
     out->n_entries_padded = nl->n_entries_padded;
     out->n_pair_slots = nl->n_entries_padded * UNIT;
-    out->list_bytes = nl->n_entries_padded * 6 + nl->n_units * 8;
+    out->list_bytes = nl->n_entries_padded * 4 + nl->n_units * 8;
     out->workspace_bytes = (int64_t)list_workspace_bytes(nl);
     for (int a = 0; a < 3; ++a) out->n_cells[a] = nl->grid.n[a];
     out->pbc_mode = nl->grid.pbc_mode;

@@ -18,6 +18,11 @@ constexpr int MAX_EXCL_PER_ATOM = 32;
 constexpr int MAX_TYPES = 64;
 constexpr int LIST_SLACK = 1024;  // entries readable past the last row (the force kernels prefetch two chunks ahead unguarded)
 constexpr int SELF_CODE = 13;  // stencil code of offset (0,0,0): (dx+1)*9+(dy+1)*3+(dz+1)
+// one list entry = one 32-bit word: slot of the j-atom (low 27 bits) | stencil code of its periodic image (high 5 bits);
+// the 8-bit i-mask of an entry lives in a parallel byte array and is read for the masked chunks only
+constexpr unsigned ENTRY_SLOT_BITS = 27;
+constexpr unsigned ENTRY_SLOT_MASK = (1u << ENTRY_SLOT_BITS) - 1u;
+__host__ __device__ inline unsigned entry_pack(int slot, int code) { return (unsigned)slot | ((unsigned)code << ENTRY_SLOT_BITS); }
 
 // device error flag bits (NL::d_flags[0])
 enum : int {
@@ -75,7 +80,7 @@ struct NL {
     int row_cap = 0;  // entries per unit row (multiple of 32), includes m_res
     int m_res = 128;  // max masked entries per row staged by the builder (multiple of 32); rows start m_res entries into their slab
     int n_grow = 0;
-    bool rows_sorted = false;  // plain entries partitioned LJ-active-j first (done lazily by the first force call after a build)
+    bool rows_sorted = false;  // rows partitioned [LJ-active plain | masked | LJ-free plain] (done lazily by the first force call after a build)
     int64_t n_entries = 0, n_entries_padded = 0;
     int64_t n_excl = 0;
     int max_cell_count = 0;
@@ -93,9 +98,11 @@ struct NL {
     DevBuf excl_pairs;            // int2[n_excl] copy (Ewald exclusion correction)
     DevBuf exc_pairs, exc_scale;  // 1-4 exceptions: int2[n_exc], double2[n_exc] = (Coulomb scale, LJ scale); survive rebuilds
     int64_t n_exc = 0;
-    DevBuf jslot;      // int[n_units*row_cap]
-    DevBuf meta;       // uint16[n_units*row_cap]: mask | code<<8
-    DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, leading mask-free chunks}
+    DevBuf entry;      // uint32[n_units*row_cap]: slot | code << 27
+    DevBuf emask;      // uint8[n_units*row_cap]: i-mask of the entry (all-ones in the mask-free chunks)
+    DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, nA | nM << 16}: the row is nA mask-free
+                       // chunks, then nM chunks that need their masks, then the remaining mask-free chunks (after
+                       // reorder_rows: nA = chunks of j-atoms with LJ partners, the trailing ones have none)
     DevBuf flags;      // int[8]: [0] error flags, [1] max cell count, [2..3] entry counters (u64), [4..5] padded
     // per-step device arrays
     DevBuf xyzq;       // real4[n_slots]

@@ -462,8 +462,8 @@ struct BuildParams {
     const real4* bb_hi;
     const int* excl_start;
     const int* excl_adj;
-    int* jslot;
-    unsigned short* meta;
+    unsigned* entry;
+    unsigned char* emask;
     int2* row_info;
     int* flags;
 };
@@ -573,13 +573,13 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         unsigned bp = __ballot_sync(FULL, is_plain);
         if (is_masked) {
             int pos = nm + __popc(bm & lt_mask);
-            if (pos < P.m_res) { st_j[pos] = j; st_meta[pos] = (unsigned short)(mask | (code << 8)); }
+            if (pos < P.m_res) { st_j[pos] = (int)entry_pack(j, code); st_meta[pos] = (unsigned short)mask; }
         }
         if (is_plain) {
             int pos = nu + __popc(bp & lt_mask);
             if (pos < nu_cap) {
-                P.jslot[row + P.m_res + pos] = j;
-                P.meta[row + P.m_res + pos] = (unsigned short)(0xFFu | (code << 8));
+                P.entry[row + P.m_res + pos] = entry_pack(j, code);
+                P.emask[row + P.m_res + pos] = 0xFFu;
             }
         }
         nm += __popc(bm);
@@ -593,8 +593,8 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         if (accept) {
             int pos = nu + __popc(bp & lt_mask);
             if (pos < nu_cap) {
-                P.jslot[row + P.m_res + pos] = j;
-                P.meta[row + P.m_res + pos] = (unsigned short)(mask | (code << 8));
+                P.entry[row + P.m_res + pos] = entry_pack(j, code);
+                P.emask[row + P.m_res + pos] = (unsigned char)mask;
             }
         }
         nu += __popc(bp);
@@ -739,14 +739,14 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         n_pad = 0;
     }
     const int self = (int)(U * UNIT);
-    const unsigned short pad_meta = (unsigned short)(SELF_CODE << 8);  // mask 0
     for (int k = lane; k < n_pad - nu; k += 32) {
         const int64_t e = row + P.m_res + nu + k;
-        P.jslot[e] = k < nm ? st_j[k] : self;
-        P.meta[e] = k < nm ? st_meta[k] : pad_meta;
+        P.entry[e] = k < nm ? (unsigned)st_j[k] : entry_pack(self, SELF_CODE);  // padding: the unit itself, mask 0
+        P.emask[e] = k < nm ? (unsigned char)st_meta[k] : (unsigned char)0;
     }
     if (lane == 0) {
-        P.row_info[U] = make_int2((n_pad >> 5) | (unit_full ? 0 : 0x10000), unit_full ? (nu >> 5) : 0);
+        const int n_a = unit_full ? (nu >> 5) : 0;  // leading mask-free chunks; everything after them reads its masks
+        P.row_info[U] = make_int2((n_pad >> 5) | (unit_full ? 0 : 0x10000), n_a | (((n_pad >> 5) - n_a) << 16));
         atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[2]), (unsigned long long)(nm + nu));
         atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[4]), (unsigned long long)n_pad);
     }
@@ -790,10 +790,10 @@ __global__ __launch_bounds__(128) void export_pairs_kernel(BuildParams<real> P, 
     const int64_t row = U * (int64_t)P.row_cap + P.m_res;
     for (int c = 0; c < nch; ++c) {
         const int64_t e = row + (int64_t)c * 32 + lane;
-        const int j = P.jslot[e];
-        const unsigned m = P.meta[e];
-        const unsigned mask = m & 0xFFu;
-        const int code = (int)(m >> 8);
+        const unsigned wd = P.entry[e];
+        const int j = (int)(wd & ENTRY_SLOT_MASK);
+        const unsigned mask = P.emask[e];
+        const int code = (int)(wd >> ENTRY_SLOT_BITS);
         real4 pj = P.xyz[j];
         const int pj_orig = P.perm[j];
         const int dx = code / 9 - 1, dy = (code / 3) % 3 - 1, dz = code % 3 - 1;
@@ -874,8 +874,8 @@ static BuildParams<real> make_build_params(const NL* nl)
     P.bb_hi = (const real4*)nl->bb_hi.p;
     P.excl_start = (const int*)nl->excl_start.p;
     P.excl_adj = (const int*)nl->excl_adj.p;
-    P.jslot = (int*)nl->jslot.p;
-    P.meta = (unsigned short*)nl->meta.p;
+    P.entry = (unsigned*)nl->entry.p;
+    P.emask = (unsigned char*)nl->emask.p;
     P.row_info = (int2*)nl->row_info.p;
     P.flags = (int*)nl->flags.p;
     return P;
@@ -957,6 +957,7 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
     if (h[1] > KD_MAX) return set_error(ctx, DIMOS_EOVERFLOW, "more than 4096 atoms in one cell (r_cut+skin too large for this density)");
     nl->n_units = h[2];
     nl->n_slots = nl->n_units * UNIT;
+    if (nl->n_slots > (int64_t)ENTRY_SLOT_MASK) return set_error(ctx, DIMOS_EOVERFLOW, "more than 2^27 atom slots: list entries hold 27-bit slot indices");
     const int64_t nun = nl->n_units, nsl = nl->n_slots;
 
     if ((rc = ensure(ctx, nl->perm, nsl * sizeof(int), s))) return rc;
@@ -988,8 +989,8 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
         nl->row_cap = nl->m_res + (((int)est + 31) & ~31);
     }
     for (int attempt = 0; attempt < 6; ++attempt) {
-        if ((rc = ensure(ctx, nl->jslot, ((size_t)nun * nl->row_cap + LIST_SLACK) * sizeof(int), s))) return rc;
-        if ((rc = ensure(ctx, nl->meta, ((size_t)nun * nl->row_cap + LIST_SLACK) * sizeof(unsigned short), s))) return rc;
+        if ((rc = ensure(ctx, nl->entry, ((size_t)nun * nl->row_cap + LIST_SLACK) * sizeof(unsigned), s))) return rc;
+        if ((rc = ensure(ctx, nl->emask, ((size_t)nun * nl->row_cap + LIST_SLACK) * sizeof(unsigned char), s))) return rc;
         zero_int_kernel<<<1, 32, 0, s>>>(flags + 2, 8);
         DIMOS_LAUNCH_CHECK(ctx, "zero_counters");
         BuildParams<real> P = make_build_params<real>(nl);

@@ -94,7 +94,8 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
                               const int* __restrict__ perm, const double* __restrict__ ref, int64_t n_slots,
                               typename vec4<real>::type* __restrict__ xyzq, int* __restrict__ stype,
                               typename vec4<real>::type* __restrict__ Facc, const double* __restrict__ lj_table, int nt,
-                              real* __restrict__ lj_out, int* __restrict__ row_active, double* __restrict__ accum)
+                              real* __restrict__ lj_out, int* __restrict__ row_active, double* __restrict__ accum,
+                              int* __restrict__ order_stale, int check_order)
 {
     // per type: does it have any non-zero LJ partner?  (every block recomputes the tiny table: no inter-block order)
     __shared__ int act_sh[MAX_TYPES];
@@ -115,7 +116,11 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
         const double z = (double)pos[3 * (int64_t)o + 2] - ref[3 * s + 2];
         xyzq[s] = mk4((real)x, (real)y, (real)z, pad ? (real)0 : charge[o]);
         const int t = type[o];
-        stype[s] = t | (act_sh[t] ? STYPE_ACTIVE : 0);  // bit 30: the atom has LJ partners
+        const int st = t | (act_sh[t] ? STYPE_ACTIVE : 0);  // bit 30: the atom has LJ partners
+        // the rows were ordered by this bit (reorder_rows): if it changes for any atom, the pair kernel is told to
+        // evaluate LJ in every chunk until the next build
+        if (check_order && !pad && ((stype[s] ^ st) & STYPE_ACTIVE)) atomicOr(order_stale, 1);
+        stype[s] = st;
         Facc[s] = mk4((real)0, (real)0, (real)0, (real)0);
     }
     if (blockIdx.x == 0) {
@@ -269,36 +274,39 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
         }
         const int2 ri = P.row_info[U];
         const int total = ri.x & 0xFFFF;  // chunks in the row
-        const int n_plain = ri.y;         // leading chunks that need no mask
+        const int n_a = ri.y & 0xFFFF;    // leading mask-free chunks ...
+        const unsigned n_m = (unsigned)ri.y >> 16;  // ... then this many chunks that read their masks, then mask-free again
         acc_t e_lj = 0, e_c = 0;
         double e_lj64 = 0.0, e_c64 = 0.0;  // E64 only
         acc_t w[6] = {0, 0, 0, 0, 0, 0};
 
         // software pipeline: (jslot, meta) two chunks ahead, (xyzq, stype) one chunk ahead
         int64_t e = U * (int64_t)P.row_cap + P.m_res + lane;
-        int jn = 0, jn2 = 0, tjn = 0;
-        unsigned mn = 0, mn2 = 0;
+        unsigned jn = 0, jn2 = 0;  // packed entries
+        int tjn = 0;
+        unsigned mn = 0, mn2 = 0;  // i-masks
         real4 pjn = mk4((real)0, (real)0, (real)0, (real)0);
-        if (total > 0) { jn = P.jslot[e]; mn = P.meta[e]; }
-        if (total > 1) { jn2 = P.jslot[e + 32]; mn2 = P.meta[e + 32]; }
-        if (total > 0) { pjn = P.xyzq[jn]; tjn = P.stype[jn] & STYPE_MASK; }
+        if (total > 0) { jn = P.entry[e]; mn = P.emask[e]; }
+        if (total > 1) { jn2 = P.entry[e + 32]; mn2 = P.emask[e + 32]; }
+        if (total > 0) { pjn = P.xyzq[jn & ENTRY_SLOT_MASK]; tjn = P.stype[jn & ENTRY_SLOT_MASK] & STYPE_MASK; }
 
         for (int c = 0; c < total; ++c) {
-            const int j = jn;
+            const int j = (int)(jn & ENTRY_SLOT_MASK);
+            const unsigned code = jn >> ENTRY_SLOT_BITS;
             const unsigned m = mn;
             const real4 pj = pjn;
             const int tj = tjn;
             jn = jn2; mn = mn2;
-            if (c + 1 < total) { pjn = P.xyzq[jn]; tjn = P.stype[jn] & STYPE_MASK; }
-            if (c + 2 < total) { jn2 = P.jslot[e + 64]; mn2 = P.meta[e + 64]; }
+            if (c + 1 < total) { pjn = P.xyzq[jn & ENTRY_SLOT_MASK]; tjn = P.stype[jn & ENTRY_SLOT_MASK] & STYPE_MASK; }
+            if (c + 2 < total) { jn2 = P.entry[e + 64]; mn2 = P.emask[e + 64]; }
             e += 32;
 
-            const real4 off = off_s[m >> 8];
+            const real4 off = off_s[code];
             const real xj = pj.x + off.x, yj = pj.y + off.y, zj = pj.z + off.z;
             const real qj = pj.w;
-            const unsigned mask = m & 0xFFu;
+            const bool plain = !((unsigned)(c - n_a) < n_m);  // warp-uniform: no mask needed
+            const unsigned mask = plain ? 0xFFu : m;
             real fjx = 0, fjy = 0, fjz = 0;
-            const bool plain = c < n_plain;  // warp-uniform: no mask needed
 
             if (plain) {
 #pragma unroll
@@ -657,10 +665,11 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     const int T = 256;
     gather_kernel<real><<<(unsigned)((nsl + T - 1) / T), T, 0, s>>>(pos, charge, type, (const int*)nl->perm.p, (const double*)nl->ref.p,
                                                                     nsl, (real4*)nl->xyzq.p, (int*)nl->stype.p, (real4*)nl->Facc.p,
-                                                                    lj_table, nt, lj_dev, row_active, (double*)nl->accum.p);
+                                                                    lj_table, nt, lj_dev, row_active, (double*)nl->accum.p,
+                                                                    (int*)nl->flags.p + 8, nl->rows_sorted ? 1 : 0);
     DIMOS_LAUNCH_CHECK(ctx, "gather");
     if (!nl->rows_sorted) {  // once per build: partition every row's mask-free entries, LJ-active j-atoms first
-        launch_reorder_rows((int*)nl->jslot.p, (unsigned short*)nl->meta.p, (const int2*)nl->row_info.p, (const int*)nl->stype.p,
+        launch_reorder_rows((unsigned*)nl->entry.p, (unsigned char*)nl->emask.p, (int2*)nl->row_info.p, (const int*)nl->stype.p,
                             nun, nl->row_cap, nl->m_res, s);
         DIMOS_LAUNCH_CHECK(ctx, "reorder_rows");
         nl->rows_sorted = true;
@@ -669,8 +678,8 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     ForceParams<real> P;
     P.n_units = nun; P.n_slots = nsl; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;
     P.xyzq = (const real4*)nl->xyzq.p; P.stype = (const int*)nl->stype.p;
-    P.jslot = (const int*)nl->jslot.p; P.meta = (const unsigned short*)nl->meta.p; P.row_info = (const int2*)nl->row_info.p;
-    P.lj4 = (const real4*)lj_dev; P.row_active = row_active;
+    P.entry = (const unsigned*)nl->entry.p; P.emask = (const unsigned char*)nl->emask.p; P.row_info = (const int2*)nl->row_info.p;
+    P.lj4 = (const real4*)lj_dev; P.row_active = row_active; P.order_stale = (const int*)nl->flags.p + 8;
     P.unit_counter = reinterpret_cast<unsigned long long*>((double*)nl->accum.p + 14);
     P.Facc = (real4*)nl->Facc.p; P.Fown = (real4*)nl->Fown.p; P.partials = (double*)nl->partials.p;
     const double rc_ = prm->r_cut;

@@ -33,14 +33,16 @@ struct ForceParams {
     using real4 = typename vec4<real>::type;
     int64_t n_units, n_slots;
     int row_cap, m_res, nt;
+    int row_words;  // packed kernel: words per shared-memory row buffer (row capacity + slack, multiple of 32)
     const real4* xyzq;
     const int* stype;
-    const int* jslot;
-    const unsigned short* meta;
-    const int2* row_info;
+    const unsigned* entry;        // slot | code << 27
+    const unsigned char* emask;   // i-mask per entry (read for the masked chunks)
+    const int2* row_info;         // {chunks | partial << 16, nA | nM << 16}
     const typename vec4<real>::type* lj4;  // (c6, c12, 6 c6, 12 c12) per type pair
     unsigned long long* unit_counter;      // dynamic unit scheduling (zeroed by gather_kernel)
     const int* row_active;   // per type: any non-zero LJ partner
+    const int* order_stale;  // != 0: an atom's LJ activity changed since reorder_rows ran (evaluate LJ everywhere)
     real4* Facc;
     real4* Fown;
     double* partials;        // [gridDim.x][N_PART]
@@ -82,7 +84,7 @@ __device__ __forceinline__ T reduce8_scatter(T (&v)[8], int lane)
 }
 
 // packed-FP32 pair kernel (pair_f32x2.cu); returns false when the case is not covered (caller uses the generic kernel)
-void launch_reorder_rows(int* jslot, unsigned short* meta, const int2* row_info, const int* stype, int64_t n_units,
+void launch_reorder_rows(unsigned* entry, unsigned char* emask, int2* row_info, const int* stype, int64_t n_units,
                          int row_cap, int m_res, cudaStream_t s);
 bool launch_pair_force_f32x2(const ForceParams<float>& P, int method, unsigned nb, size_t dyn, cudaStream_t s);
 

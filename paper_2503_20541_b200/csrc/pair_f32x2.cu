@@ -34,6 +34,13 @@ __device__ __forceinline__ float rsqrt_f(float x)
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float2 bc(float a) { return make_float2(a, a); }
 
+__device__ __forceinline__ float4 lds_f4(unsigned addr)
+{
+    float4 v;
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 struct UnitRegs {
     float2 x[NPAIR], y[NPAIR], z[NPAIR], q[NPAIR];     // i-atoms (q pre-multiplied by k_e)
     float2 fx[NPAIR], fy[NPAIR], fz[NPAIR];            // F_i accumulators over the row
@@ -79,8 +86,8 @@ __device__ __forceinline__ void erfc_exp2(float2 x, float2& erfc_x, float2& exp_
 //   MASKED: honour the entry's i-mask (exclusions, intra-unit half, padding); LJ: evaluate Eq. 4 for the
 //   i-pairs flagged in lj_pairs.  Returns F_j = -sum_i fs_i * d_i.
 template <int METHOD, bool SW, bool MASKED, bool LJ>
-__device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const float4* __restrict__ ljt, const int* __restrict__ ti, float nxj,
-                                           float nyj, float nzj, float qj, int tj, unsigned mask, unsigned lj_pairs,
+__device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, unsigned ljrow, const unsigned (&ti16)[UNIT], float nxj,
+                                           float nyj, float nzj, float qj, unsigned mask, unsigned lj_pairs,
                                            float& sx, float& sy, float& sz)
 {
     const float2 nx2 = bc(nxj), ny2 = bc(nyj), nz2 = bc(nzj), qj2 = bc(qj);
@@ -129,7 +136,9 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
         }
         if (LJ) {
             if (lj_pairs & (1u << p)) {  // warp-uniform
-                const float4 ca = ljt[ti[2 * p] + (tj & STYPE_MASK)], cb = ljt[ti[2 * p + 1] + (tj & STYPE_MASK)];  // c6, c12, 6 c6, 12 c12
+                // (c6, c12, 6 c6, 12 c12) of the two i-atoms with the lane's j-atom: ljrow = shared address of the table
+                // column of the j-type, ti16 = byte offset of the i-type's row (warp-uniform)
+                const float4 ca = lds_f4(ljrow + ti16[2 * p]), cb = lds_f4(ljrow + ti16[2 * p + 1]);
                 float2 rinv6 = __fmul2_rn(__fmul2_rn(rinvsq, rinvsq), rinvsq);
                 rinv6.x = in_a ? rinv6.x : 0.f;
                 rinv6.y = in_b ? rinv6.y : 0.f;
@@ -173,34 +182,82 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
 }
 
 
-// One chunk of the software pipeline.  (j0, m0) are the list entries of chunk c and (PJ, TJ) its gathered j-atoms;
-// (j1, m1) / (j2, m2) are the entries of chunks c+1 / c+2, loaded two and three steps before their coordinates are
-// gathered.  The step loads the entries of chunk c+3, gathers chunk c+1 into the other coordinate buffer,
-// evaluates chunk c and rotates the entry registers.  Reads past the row's last chunk stay inside the list
-// allocation (LIST_SLACK) and their indices are clamped, so the pipeline needs no guards.
-#define DIMOS_CHUNK_STEP(PJ, TJ, PJn, TJn, EOFF, C)                                                              \
+// ---- shared-memory / TMA helpers (explicit shared-space addresses) ----
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// list rows are read once per force call: evict-first in L2 so that the gathered j-atom coordinates (14.7 MB, re-read
+// ~60 times) stay resident; the bulk copy bypasses L1 altogether
+__device__ __forceinline__ unsigned long long policy_evict_first()
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void bulk_row_to_smem(unsigned dst, const void* src, unsigned bytes, unsigned bar, unsigned long long pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ unsigned lds_u32(unsigned addr)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+// image offset of an entry from the CTA's shared table
+__device__ __forceinline__ float4 lds_offset(unsigned base, unsigned w)
+{
+    float4 v;
+    const unsigned addr = base + ((w >> (ENTRY_SLOT_BITS - 4)) & 0x1F0u);
+    asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
+// One chunk of the software pipeline.  The unit's row of packed entries (slot | code << 27) sits in the warp's
+// shared-memory buffer (one TMA bulk copy per row, issued one unit ahead).  EC is the entry of chunk c and (PJ, TJ) its
+// gathered j-atom; EN is the entry of chunk c+1.  The step gathers chunk c+1 into the other coordinate buffer,
+// replaces EC by the entry of chunk c+2 (two entry registers, two coordinate buffers: nothing is copied at the loop
+// back-edge), and evaluates chunk c.  Reads past the row's last chunk stay inside the buffer's slack and their slot
+// is clamped, so the pipeline needs no guards.
+//   A row (reorder_rows) is three phases, each with its own loop: KIND 0 = mask-free chunks whose j-atoms have LJ
+//   partners, KIND 1 = chunks that read their i-masks (always with LJ), KIND 2 = mask-free chunks without LJ.  Only
+//   phases 0 and 1 gather the j-atom types (for the chunk after them, too: harmless at the phase boundary).
+#define DIMOS_CHUNK_STEP(KIND, PJ, TJ, PJn, TJn, EC, EN, SOFF)                                                   \
     do {                                                                                                         \
-        const int jc = j0;          /* rotate FIRST (old values), then load straight into the freed registers */ \
-        const unsigned mk = m0;                                                                                  \
-        j0 = j1; m0 = m1; j1 = j2; m1 = m2;                                                                      \
-        j2 = jp[(EOFF) + 96];                                                                                    \
-        m2 = mp[(EOFF) + 96];                                                                                    \
+        const float4 off = lds_offset(off_base, EC);                                                             \
+        const unsigned jc = EC & ENTRY_SLOT_MASK;                                                                \
         {                                                                                                        \
-            const unsigned jj = min((unsigned)j0, slot_max);                                                     \
+            const unsigned jj = min(EN & ENTRY_SLOT_MASK, slot_max);                                             \
             PJn = P.xyzq[jj];                                                                                    \
-            TJn = P.stype[jj];                                                                                   \
+            if ((KIND) != 2) TJn = P.stype[jj];                                                                  \
         }                                                                                                        \
-        const float4 off = off_s[mk >> 8];                                                                       \
+        EC = lds_u32(sa + (SOFF) + 256u);                                                                        \
+        unsigned mk = 0xFFu;                                                                                     \
+        if ((KIND) == 1) { mk = mk_n; mk_n = mp[32]; }                                                           \
         const float nxj = off.x - PJ.x, nyj = off.y - PJ.y, nzj = off.z - PJ.z; /* -(x_j + image shift) */       \
         float sx, sy, sz;                                                                                        \
-        if ((unsigned)((C) - c_plain) < n_plain) { /* warp-uniform: full chunk of a full unit, all masks 0xFF */ \
-            if (lj_pairs != 0u && __any_sync(FULL, (TJ & STYPE_ACTIVE) != 0))                                    \
-                chunk_body<METHOD, SW, false, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, lj_pairs, sx, sy, sz);  \
-            else                                                                                                 \
-                chunk_body<METHOD, SW, false, false>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, 0xFFu, 0u, sx, sy, sz);       \
-        } else {                                                                                                 \
-            chunk_body<METHOD, SW, true, true>(u, k, ljt, ti_w, nxj, nyj, nzj, PJ.w, TJ, mk & 0xFFu, lj_pairs, sx, sy, sz);  \
-        }                                                                                                        \
+        const unsigned ljrow = (KIND) != 2 ? ljt_base + ((unsigned)(TJ & STYPE_MASK) << 4) : 0u;                  \
+        chunk_body<METHOD, SW, (KIND) == 1, (KIND) != 2>(u, k, ljrow, ti16, nxj, nyj, nzj, PJ.w, mk, lj_pairs, sx, sy, sz);      \
         /* virial: x_j' (x) F_j in unit-local coordinates, x_j' = -nxj */                                        \
         w[0] = fmaf(-nxj, sx, w[0]); w[1] = fmaf(-nxj, sy, w[1]); w[2] = fmaf(-nxj, sz, w[2]);                   \
         w[3] = fmaf(-nyj, sy, w[3]); w[4] = fmaf(-nyj, sz, w[4]); w[5] = fmaf(-nzj, sz, w[5]);                   \
@@ -210,67 +267,99 @@ __device__ __forceinline__ void chunk_body(UnitRegs& u, const Consts& k, const f
 template <int METHOD, bool SW>
 __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x2_kernel(ForceParams<float> P)
 {
-    __shared__ float4 off_s[27];
-    __shared__ int ti_s[FX_WARPS][UNIT];  // type * nt of the warp's current i-atoms
-    extern __shared__ __align__(16) unsigned char dyn_smem[];
-    float4* ljt = reinterpret_cast<float4*>(dyn_smem);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
-
-    for (int t = threadIdx.x; t < P.nt * P.nt; t += blockDim.x) ljt[t] = P.lj4[t];
-    if (threadIdx.x < 27) {  // NEGATED image offsets: the kernel works with -x_j
-        const int c = threadIdx.x;
-        off_s[c] = make_float4(-(float)(c / 9 - 1) * P.h[0], -(float)((c / 3) % 3 - 1) * P.h[1], -(float)(c % 3 - 1) * P.h[2], 0.f);
-    }
-    __syncthreads();  // the only CTA-wide barrier: warps are independent from here on
+    __shared__ float4 off_s[32];
+    __shared__ __align__(8) unsigned long long bars[FX_WARPS][2];
+    extern __shared__ __align__(128) unsigned char dyn_smem[];
+    // dynamic shared memory: FX_WARPS x 2 row buffers of P.row_words words (128-byte aligned), then the LJ table
+    float4* ljt = reinterpret_cast<float4*>(dyn_smem + (size_t)FX_WARPS * 2 * P.row_words * 4);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
 
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;
-    int* ti_w = ti_s[wib];
+    for (int t = threadIdx.x; t < P.nt * P.nt; t += blockDim.x) ljt[t] = P.lj4[t];
+    if (threadIdx.x < 32) {  // NEGATED image offsets: the kernel works with -x_j
+        const int c = threadIdx.x < 27 ? threadIdx.x : SELF_CODE;
+        off_s[threadIdx.x] = make_float4(-(float)(c / 9 - 1) * P.h[0], -(float)((c / 3) % 3 - 1) * P.h[1], -(float)(c % 3 - 1) * P.h[2], 0.f);
+    }
+    const unsigned bar0 = smem_u32(&bars[wib][0]);
+    if (lane == 0) {
+        mbar_init(bar0, 1);
+        mbar_init(bar0 + 8, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();  // the only CTA-wide barrier: warps are independent from here on
+
+    const unsigned ljt_base = smem_u32(ljt);
     const int comp = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);  // reduce8_scatter's element of this lane
     const unsigned slot_max = (unsigned)(P.n_slots - 1);
+    const unsigned long long pol_stream = policy_evict_first();
+    const unsigned off_base = smem_u32(off_s);
+    const unsigned row_bytes = (unsigned)P.row_words * 4u;
+    const unsigned buf0 = smem_u32(dyn_smem) + (unsigned)wib * 2u * row_bytes;  // this warp's two row buffers
+    const bool lj_all = *P.order_stale != 0;  // the LJ activity of some atom changed since the rows were ordered
     double acc_d = 0.0;  // running fp64 total of component `comp` over all units of this warp
     Consts k;
     k.rc2 = P.rc2; k.krf = P.krf; k.m2krf = P.m2krf; k.mcrf = -P.crf;
     k.alpha = P.alpha; k.two_a_sqrtpi = P.two_a_sqrtpi;
     k.rs = P.rs; k.inv_sw = P.inv_sw;
 
-    long long U = 0, U_next = 0;
+    // dynamic unit scheduling: every warp draws unit indices from one global counter (rows differ in length); the next
+    // unit is claimed at the start of the current one, its row_info read after the first phase and its row copied
+    // after the second, so that none of the three waits on the one before
+    long long U = 0;
     if (lane == 0) U = (long long)atomicAdd(P.unit_counter, 1ull);
     U = __shfl_sync(FULL, U, 0);
+    if (U >= P.n_units) {
+        const int64_t prow0 = ((int64_t)blockIdx.x * FX_WARPS + wib) * N_PART;
+        if (lane < N_PART) P.partials[prow0 + lane] = 0.0;
+        return;
+    }
+    int2 ri = P.row_info[U];
+    unsigned kbuf = 0;  // units processed by this warp: buffer = kbuf & 1, mbarrier phase = (kbuf >> 1) & 1
+    if (lane == 0 && (ri.x & 0xFFFF) != 0) {
+        const unsigned bytes = (unsigned)(ri.x & 0xFFFF) * 128u;
+        mbar_expect_tx(bar0, bytes);
+        bulk_row_to_smem(buf0, P.entry + U * (int64_t)P.row_cap + P.m_res, bytes, bar0, pol_stream);
+    }
+    // pipeline state handed from one unit to the next: first two entries, first j-atom, the unit's own atoms
+    unsigned ea = 0, eb = 0;
+    float4 pA = make_float4(0.f, 0.f, 0.f, 0.f), pB;
+    int tA = 0, tB = 0;
+    float4 mine = make_float4(0.f, 0.f, 0.f, 0.f);
+    int my_t = 0;
+    if ((ri.x & 0xFFFF) != 0) {
+        mbar_wait(bar0, 0);
+        ea = lds_u32(buf0 + lane * 4u);
+        eb = lds_u32(buf0 + lane * 4u + 128u);
+        const unsigned jj = min(ea & ENTRY_SLOT_MASK, slot_max);
+        pA = P.xyzq[jj];
+        tA = P.stype[jj];
+    }
+    if (lane < UNIT) { mine = P.xyzq[U * UNIT + lane]; my_t = P.stype[U * UNIT + lane]; }
 
-    while (U < P.n_units) {
-        if (lane == 0) U_next = (long long)atomicAdd(P.unit_counter, 1ull);  // in flight while this unit is processed
+    while (true) {
+        long long Un = 0;
+        if (lane == 0) Un = (long long)atomicAdd(P.unit_counter, 1ull);  // in flight during the first phase
+        const int total = ri.x & 0xFFFF;                  // chunks in the row
+        // lj_all: every chunk takes the masked-with-LJ path (mask-free chunks carry all-ones masks)
+        const int n_a = lj_all ? 0 : (ri.y & 0xFFFF);                  // mask-free chunks whose j-atoms have LJ partners
+        const int n_m = lj_all ? total : (int)((unsigned)ri.y >> 16);  // masked chunks after them
+        const int n_b = total - n_a - n_m;                             // mask-free chunks without LJ
+        const unsigned b = kbuf & 1u;
 
-        const int2 ri = P.row_info[U];
-        const int total = ri.x & 0xFFFF;        // chunks in the row
-        const int c_plain = 0;                  // the mask-free chunks come first ...
-        const unsigned n_plain = (unsigned)ri.y;  // ... this many of them
+        const unsigned char* mp = P.emask + U * (int64_t)P.row_cap + P.m_res + lane + n_a * 32;
+        unsigned mk_n = mp[0];  // i-mask of the first masked chunk
+        unsigned sa = buf0 + b * row_bytes + lane * 4u;  // shared address of this lane's entry of the current chunk
 
-        // pipeline prologue: indices of chunks 0 and 1, coordinates of chunk 0
-        const int64_t e0 = U * (int64_t)P.row_cap + P.m_res + lane;
-        const int* jp = P.jslot + e0;
-        const unsigned short* mp = P.meta + e0;
-        int j0 = jp[0], j1 = jp[32], j2 = jp[64];
-        unsigned m0 = mp[0], m1 = mp[32], m2 = mp[64];
-        float4 pA, pB;
-        int tA, tB;
-        {
-            const unsigned jj = min((unsigned)j0, slot_max);
-            pA = P.xyzq[jj];
-            tA = P.stype[jj];
-        }
-
-        // ---- the unit's 8 i-atoms: lanes 0..7 load one each; shuffles broadcast them straight into register pairs ----
+        // ---- the unit's 8 i-atoms: lanes 0..7 hold one each; shuffles broadcast them straight into register pairs ----
         UnitRegs u;
-        float4 mine = make_float4(0.f, 0.f, 0.f, 0.f);
-        int my_t = 0;
-        if (lane < UNIT) { mine = P.xyzq[U * UNIT + lane]; my_t = P.stype[U * UNIT + lane]; }
-        __syncwarp();
-        if (lane < UNIT) ti_w[lane] = (my_t & STYPE_MASK) * P.nt;
-        __syncwarp();
+        unsigned ti16[UNIT];  // byte offset of every i-atom's row in the shared LJ table (warp-uniform)
+#pragma unroll
+        for (int i = 0; i < UNIT; ++i) ti16[i] = __shfl_sync(FULL, (unsigned)((my_t & STYPE_MASK) * P.nt) << 4, i);
         const unsigned act_bits = __ballot_sync(FULL, (my_t & STYPE_ACTIVE) != 0) & 0xFFu;
         const unsigned act_or = act_bits | (act_bits >> 1);  // bit 2p: pair p has an LJ-active atom
         const unsigned lj_pairs = (act_or & 1u) | ((act_or >> 1) & 2u) | ((act_or >> 2) & 4u) | ((act_or >> 3) & 8u);
+        const float4 own = mine;  // kept for the virial term x_i (x) F_i
         mine.w *= P.ke;  // k_e folded into the i-side charge
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
@@ -284,12 +373,53 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         u.e_lj = f2(0.f, 0.f);
         float w[6] = {0, 0, 0, 0, 0, 0};
 
-        // ---- the row, two chunks per iteration (ping-pong buffers A/B: no register rotation) ----
-        for (int c = 0; c < total; c += 2) {
-            DIMOS_CHUNK_STEP(pA, tA, pB, tB, 0, c);
-            if (c + 1 < total) DIMOS_CHUNK_STEP(pB, tB, pA, tA, 32, c + 1);
-            jp += 64;
-            mp += 64;
+        // ---- the row: three phases, two chunks per iteration (ping-pong entry registers and coordinate buffers; a
+        //      phase with an odd number of chunks ends with one swap) ----
+        for (int c = 0; c < n_a; c += 2) {
+            DIMOS_CHUNK_STEP(0, pA, tA, pB, tB, ea, eb, 0u);
+            if (c + 1 < n_a) { DIMOS_CHUNK_STEP(0, pB, tB, pA, tA, eb, ea, 128u); sa += 256u; }
+            else { pA = pB; tA = tB; const unsigned t_ = ea; ea = eb; eb = t_; sa += 128u; }
+        }
+        Un = __shfl_sync(FULL, Un, 0);
+        const bool more = Un < P.n_units;
+        int2 ri_n = make_int2(0, 0);
+        if (more) ri_n = P.row_info[Un];
+        for (int c = 0; c < n_m; ++c) {
+            DIMOS_CHUNK_STEP(1, pA, tA, pB, tB, ea, eb, 0u);
+            pA = pB; tA = tB;
+            { const unsigned t_ = ea; ea = eb; eb = t_; }
+            sa += 128u;
+            mp += 32;
+        }
+        // the next unit's row: bulk copy into the other buffer (last read by the previous unit, which is finished)
+        const int total_n = ri_n.x & 0xFFFF;
+        __syncwarp();
+        if (lane == 0 && total_n != 0) {
+            const unsigned bytes = (unsigned)total_n * 128u;
+            mbar_expect_tx(bar0 + 8u * (b ^ 1u), bytes);
+            bulk_row_to_smem(buf0 + (b ^ 1u) * row_bytes, P.entry + Un * (int64_t)P.row_cap + P.m_res, bytes, bar0 + 8u * (b ^ 1u), pol_stream);
+        }
+        for (int c = 0; c < n_b; c += 2) {
+            DIMOS_CHUNK_STEP(2, pA, tA, pB, tB, ea, eb, 0u);
+            if (c + 1 < n_b) { DIMOS_CHUNK_STEP(2, pB, tB, pA, tA, eb, ea, 128u); }
+            sa += 256u;
+        }
+
+        // ---- hand-off: the next unit's first two entries, its first j-atom and its own atoms are requested BEFORE this
+        //      unit's reductions, so their latency is covered by the shuffles below ----
+        float4 mine_n = make_float4(0.f, 0.f, 0.f, 0.f);
+        int my_t_n = 0;
+        if (more) {
+            if (total_n != 0) {
+                mbar_wait(bar0 + 8u * (b ^ 1u), ((kbuf + 1u) >> 1) & 1u);
+                const unsigned sn = buf0 + (b ^ 1u) * row_bytes + lane * 4u;
+                ea = lds_u32(sn);
+                eb = lds_u32(sn + 128u);
+                const unsigned jj = min(ea & ENTRY_SLOT_MASK, slot_max);
+                pA = P.xyzq[jj];
+                tA = P.stype[jj];
+            }
+            if (lane < UNIT) { mine_n = P.xyzq[Un * UNIT + lane]; my_t_n = P.stype[Un * UNIT + lane]; }
         }
 
         // ---- F_i: reduce over the warp once per unit; lanes 0,4,..,28 end up holding one i-atom each ----
@@ -303,17 +433,22 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         const float rx = reduce8_scatter(fix, lane);
         const float ry = reduce8_scatter(fiy, lane);
         const float rz = reduce8_scatter(fiz, lane);
+        const float vx = __shfl_sync(FULL, own.x, comp), vy = __shfl_sync(FULL, own.y, comp), vz = __shfl_sync(FULL, own.z, comp);
         if ((lane & 3) == 0) {
             P.Fown[U * UNIT + comp] = make_float4(rx, ry, rz, 0.f);
-            const float4 v = P.xyzq[U * UNIT + comp];  // x_i (x) F_i^unit
-            w[0] += v.x * rx; w[1] += v.x * ry; w[2] += v.x * rz;
-            w[3] += v.y * ry; w[4] += v.y * rz; w[5] += v.z * rz;
+            w[0] += vx * rx; w[1] += vx * ry; w[2] += vx * rz;  // x_i (x) F_i^unit
+            w[3] += vy * ry; w[4] += vy * rz; w[5] += vz * rz;
         }
-        double red[8] = {(double)u.e_lj.x + (double)u.e_lj.y, (double)u.e_c.x + (double)u.e_c.y,
-                         (double)w[0], (double)w[1], (double)w[2], (double)w[3], (double)w[4], (double)w[5]};
-        acc_d += reduce8_scatter(red, lane);
+        // energy / virial of this unit: per-lane fp32 partials -> fp32 warp sums -> fp64 running totals (reading C-11)
+        float red[8] = {u.e_lj.x + u.e_lj.y, u.e_c.x + u.e_c.y, w[0], w[1], w[2], w[3], w[4], w[5]};
+        acc_d += (double)reduce8_scatter(red, lane);
 
-        U = __shfl_sync(FULL, U_next, 0);
+        if (!more) break;
+        U = Un;
+        ri = ri_n;
+        mine = mine_n;
+        my_t = my_t_n;
+        ++kbuf;
     }
 
     const int64_t prow = ((int64_t)blockIdx.x * FX_WARPS + wib) * N_PART;
@@ -322,12 +457,15 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
 }
 #undef DIMOS_CHUNK_STEP
 
-// Stable partition of every full unit's mask-free entries: j-atoms with LJ partners first.  After it, only the
-// leading ~1/3 of a water row's chunks take the LJ path of the pair kernel (which still decides per chunk by a
-// warp vote, so a stale order costs time, never correctness).
+// Once per build (first force call): every full unit's row is rewritten as
+//   [ mask-free chunks of j-atoms WITH LJ partners | chunks that read their i-masks | mask-free chunks WITHOUT LJ ]
+// The middle region takes the entries whose mask is not all-ones (exclusions, the unit's own half, padding) and the
+// leftovers of the two mask-free classes that do not fill a chunk.  The pair kernel then needs the j-atom types only
+// for the first two regions and no per-chunk vote.  Should an atom's LJ activity change afterwards (gather_kernel
+// notices), the kernel evaluates LJ in every chunk: the order is an optimisation, never a correctness condition.
 constexpr int RO_WARPS = 4;
-__global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(int* __restrict__ jslot, unsigned short* __restrict__ meta,
-                                                                     const int2* __restrict__ row_info,
+__global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(unsigned* __restrict__ entry, unsigned char* __restrict__ emask,
+                                                                     int2* __restrict__ row_info,
                                                                      const int* __restrict__ stype, int64_t n_units,
                                                                      int row_cap, int m_res)
 {
@@ -336,80 +474,100 @@ __global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(int* __rest
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int64_t U = (int64_t)blockIdx.x * RO_WARPS + wib;
     if (U >= n_units) return;
-    int* sj = reinterpret_cast<int*>(ro_smem) + (size_t)wib * cap;
-    unsigned short* sm = reinterpret_cast<unsigned short*>(reinterpret_cast<int*>(ro_smem) + (size_t)RO_WARPS * cap) + (size_t)wib * cap;
+    unsigned* se = reinterpret_cast<unsigned*>(ro_smem) + (size_t)wib * cap;
+    unsigned short* sm = reinterpret_cast<unsigned short*>(reinterpret_cast<unsigned*>(ro_smem) + (size_t)RO_WARPS * cap) + (size_t)wib * cap;
     const int2 ri = row_info[U];
-    const int nu = ri.y * 32 < cap ? ri.y * 32 : cap;  // entries of the mask-free chunks (0 for a partial unit)
-    if (nu == 0) return;
+    if (ri.x & 0x10000) return;  // partial unit: every chunk stays masked
+    const int n = (ri.x & 0xFFFF) * 32 < cap ? (ri.x & 0xFFFF) * 32 : cap;
+    if (n == 0) return;
     const int64_t base = U * (int64_t)row_cap + m_res;
     const unsigned FULL = 0xffffffffu, lt = (1u << lane) - 1u;
-    int n_act = 0;
-    for (int k0 = 0; k0 < nu; k0 += 32) {
+    // class of an entry: 0 = mask-free with LJ, 1 = masked (real), 2 = mask-free without LJ, 3 = padding (mask 0, goes last in the masked region)
+    int cnt[4] = {0, 0, 0, 0};
+    for (int k0 = 0; k0 < n; k0 += 32) {
         const int k = k0 + lane;
-        bool act = false;
-        if (k < nu) {
-            const int j = jslot[base + k];
-            sj[k] = j;
-            act = (stype[j] & STYPE_ACTIVE) != 0;
-            sm[k] = (unsigned short)(meta[base + k] | (act ? 0x8000u : 0u));  // bit 15 is free: remember the flag
-        }
-        n_act += __popc(__ballot_sync(FULL, act));
+        const unsigned wd = entry[base + k];
+        const unsigned m = emask[base + k];
+        int cls;
+        if (m == 0u) cls = 3;
+        else if (m != 0xFFu) cls = 1;
+        else cls = (stype[wd & ENTRY_SLOT_MASK] & STYPE_ACTIVE) ? 0 : 2;
+        se[k] = wd;
+        sm[k] = (unsigned short)(m | (cls << 8));
+#pragma unroll
+        for (int q = 0; q < 4; ++q) cnt[q] += __popc(__ballot_sync(FULL, cls == q));
     }
     __syncwarp();
-    int pa = 0, pi = n_act;
-    for (int k0 = 0; k0 < nu; k0 += 32) {
+    const int fullA = cnt[0] & ~31, fullB = cnt[2] & ~31;         // entries in whole mask-free chunks
+    const int remA = cnt[0] - fullA, remB = cnt[2] - fullB;
+    const int nM = cnt[1] + cnt[3] + remA + remB;                 // multiple of 32 because n, fullA, fullB are
+    // destination offsets: A_full | remA, masked, remB, padding | B_full
+    int posM = fullA + remA, posB = fullA + nM, posP = fullA + remA + cnt[1] + remB;
+    int seenA = 0, seenB = 0;
+    for (int k0 = 0; k0 < n; k0 += 32) {
         const int k = k0 + lane;
-        bool act = false, ina = false;
-        int j = 0;
-        unsigned short m = 0;
-        if (k < nu) {
-            j = sj[k];
-            m = sm[k];
-            act = (m & 0x8000u) != 0;
-            ina = !act;
+        const unsigned wd = se[k];
+        const unsigned short mm = sm[k];
+        const int cls = mm >> 8;
+        const unsigned b0 = __ballot_sync(FULL, cls == 0), b1 = __ballot_sync(FULL, cls == 1), b2 = __ballot_sync(FULL, cls == 2),
+                       b3 = __ballot_sync(FULL, cls == 3);
+        int dst;
+        if (cls == 0) {
+            const int r = seenA + __popc(b0 & lt);  // rank among the LJ class: the first fullA go to the front, the rest into the masked region
+            dst = r < fullA ? r : fullA + (r - fullA);
+        } else if (cls == 1) {
+            dst = posM + __popc(b1 & lt);
+        } else if (cls == 2) {
+            const int r = seenB + __popc(b2 & lt);
+            dst = r < fullB ? posB + r : fullA + remA + cnt[1] + (r - fullB);
+        } else {
+            dst = posP + __popc(b3 & lt);
         }
-        const unsigned ba = __ballot_sync(FULL, act), bi = __ballot_sync(FULL, ina);
-        if (k < nu) {
-            const int pos = act ? pa + __popc(ba & lt) : pi + __popc(bi & lt);
-            jslot[base + pos] = j;
-            meta[base + pos] = (unsigned short)(m & 0x7FFFu);
-        }
-        pa += __popc(ba);
-        pi += __popc(bi);
+        entry[base + dst] = wd;
+        emask[base + dst] = (unsigned char)(mm & 0xFFu);
+        seenA += __popc(b0);
+        posM += __popc(b1);
+        seenB += __popc(b2);
+        posP += __popc(b3);
     }
+    if (lane == 0) row_info[U] = make_int2(ri.x, (fullA >> 5) | ((nM >> 5) << 16));
 }
 
 }  // namespace
 
-void launch_reorder_rows(int* jslot, unsigned short* meta, const int2* row_info, const int* stype, int64_t n_units,
+void launch_reorder_rows(unsigned* entry, unsigned char* emask, int2* row_info, const int* stype, int64_t n_units,
                          int row_cap, int m_res, cudaStream_t s)
 {
     const size_t smem = (size_t)RO_WARPS * (row_cap - m_res) * 6;
     if (smem > 48 * 1024) cudaFuncSetAttribute(reorder_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const unsigned nb = (unsigned)((n_units + RO_WARPS - 1) / RO_WARPS);
-    reorder_rows_kernel<<<nb, RO_WARPS * 32, smem, s>>>(jslot, meta, row_info, stype, n_units, row_cap, m_res);
+    reorder_rows_kernel<<<nb, RO_WARPS * 32, smem, s>>>(entry, emask, row_info, stype, n_units, row_cap, m_res);
 }
 
 template <int METHOD, bool SW>
-static void launch_one(const ForceParams<float>& P, unsigned nb, size_t dyn, cudaStream_t s)
+static bool launch_one(const ForceParams<float>& P, unsigned nb, size_t dyn, cudaStream_t s)
 {
-    if (dyn > 48 * 1024)
-        cudaFuncSetAttribute(pair_force_f32x2_kernel<METHOD, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-    pair_force_f32x2_kernel<METHOD, SW><<<nb, FX_WARPS * 32, dyn, s>>>(P);
-}
-
-bool launch_pair_force_f32x2(const ForceParams<float>& P, int method, unsigned nb, size_t dyn, cudaStream_t s)
-{
-    if (method == DIMOS_RF) {
-        if (P.sw_on) launch_one<DIMOS_RF, true>(P, nb, dyn, s);
-        else launch_one<DIMOS_RF, false>(P, nb, dyn, s);
-    } else if (method == DIMOS_EWALD_REAL) {
-        if (P.sw_on) launch_one<DIMOS_EWALD_REAL, true>(P, nb, dyn, s);
-        else launch_one<DIMOS_EWALD_REAL, false>(P, nb, dyn, s);
-    } else {
+    if (dyn > 48 * 1024 &&
+        cudaFuncSetAttribute(pair_force_f32x2_kernel<METHOD, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn) != cudaSuccess) {
+        cudaGetLastError();
         return false;
     }
+    pair_force_f32x2_kernel<METHOD, SW><<<nb, FX_WARPS * 32, dyn, s>>>(P);
     return true;
+}
+
+// Returns false when the case is not covered (the caller then runs the generic kernel): an unknown method, or rows too
+// long for the two shared-memory row buffers per warp.
+bool launch_pair_force_f32x2(const ForceParams<float>& P_in, int method, unsigned nb, size_t lj_bytes, cudaStream_t s)
+{
+    ForceParams<float> P = P_in;
+    P.row_words = ((P.row_cap - P.m_res) + 64 + 31) & ~31;  // two chunks of slack: the pipeline reads two chunks ahead
+    const size_t dyn = (size_t)FX_WARPS * 2 * P.row_words * 4 + lj_bytes;
+    if (dyn > 110 * 1024) return false;  // two CTAs per SM must fit
+    if (method == DIMOS_RF) return P.sw_on ? launch_one<DIMOS_RF, true>(P, nb, dyn, s) : launch_one<DIMOS_RF, false>(P, nb, dyn, s);
+    if (method == DIMOS_EWALD_REAL)
+        return P.sw_on ? launch_one<DIMOS_EWALD_REAL, true>(P, nb, dyn, s) : launch_one<DIMOS_EWALD_REAL, false>(P, nb, dyn, s);
+    return false;
 }
 
 }  // namespace dimos
