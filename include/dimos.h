@@ -211,6 +211,33 @@ DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_
 DIMOS_API int dimos_nl_export_pairs(dimos_ctx* ctx, const dimos_nl* nl, int32_t* pairs, int64_t cap,
                                     int64_t* n_pairs_host, void* stream);
 
+/* dimos_pme_recip -- reciprocal-space electrostatics by smooth particle-mesh Ewald ("we implement smooth
+ * PME ... B-splines based on the recursive definition") and the self energy, i.e. the two terms of Eq. 9
+ * that dimos_nonbonded with DIMOS_EWALD_REAL does not return:
+ *   U_recip = k_e / (2 pi V) sum_{k != 0} exp(-(pi k / alpha)^2) / k^2 |sum_j q_j exp(2 pi i k . r_j)|^2
+ *             (Eq. 11, with the charges and the imaginary unit the printed formula lost: reading C-25),
+ *             approximated on a K1 x K2 x K3 mesh with cardinal B-splines of the given order (Essmann et al. 1995);
+ *   U_self  = -k_e alpha / sqrt(pi) sum_i q_i^2   (Eq. 12).
+ * Steps: charge spreading (hand-written kernel), 3-D real-to-complex FFT (cuFFT), influence function B(m) C(m) with energy
+ * and virial (hand-written), inverse FFT (cuFFT), force interpolation (hand-written).
+ *   pos, charge  dev, N x 3 and N (element type of the context; positions need not be wrapped)
+ *   box          host, 3 doubles;   alpha  Ewald splitting parameter (nm^-1), the one given to dimos_nonbonded
+ *   mesh         host, 3 int32: mesh points per axis, each in [2 * order, 4096] with prime factors 2, 3, 5, 7
+ *                (dimos_pme_mesh_size gives the paper's heuristic);   order  spline order n, 3..6 (OpenMM's 5)
+ *   F            dev, N x 3 or NULL (energy only): reciprocal forces, ADDED to F when accumulate != 0, else overwriting
+ *   E            dev, 2 doubles, overwritten: {U_recip, U_self};   virial  dev, 9 doubles or NULL: the reciprocal-space
+ *                virial W_ab = -dU_recip/d(strain_ab) (reading C-7; the self term has none)
+ * F32/MIXED contexts spread, transform and interpolate in fp32 and reduce energy/virial in fp64; F64 contexts are fp64
+ * throughout.  The mesh, the cuFFT plans and their work area are kept in the context and re-made when mesh or order
+ * change (that first call synchronises the stream); otherwise the call does not synchronise. */
+DIMOS_API int dimos_pme_recip(dimos_ctx* ctx, const void* pos, const void* charge, int64_t N, const double* box, double alpha,
+                              const int32_t* mesh, int32_t order, double coulomb_const, void* F, int32_t accumulate, double* E,
+                              double* virial, void* stream);
+
+/* dimos_pme_mesh_size -- the paper's mesh heuristic n_mesh = 2 alpha d / (3 delta^(1/5)) per box edge d,
+ * rounded up to the next size with prime factors 2, 3, 5, 7.  Host only; mesh_out receives 3 int32. */
+DIMOS_API int dimos_pme_mesh_size(double alpha, const double* box, double delta, int32_t* mesh_out);
+
 /* dimos_dispersion_correction -- PAPER.md:202 ("long-range dispersion corrections that approximate the contributions
  * beyond r_c"; the paper gives no formula: reading C-22).  The homogeneous-fluid tail of the 12-6 potential that the
  * truncated (and, with r_switch, switched) pair sum leaves out:

@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = (
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
     "dimos_kinetic_energy", "dimos_berendsen", "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities",
-    "dimos_berendsen_scale",
+    "dimos_berendsen_scale", "dimos_pme_recip", "dimos_pme_mesh_size",
 )
 
 
@@ -109,6 +109,8 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_virtual_box.argtypes = [vp, vp, i64, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     lib.dimos_dispersion_correction.argtypes = [vp, vp, i64, vp, i32, ctypes.POINTER(dbl), dbl, dbl, ctypes.POINTER(dbl),
                                                 ctypes.POINTER(dbl), vp]
+    lib.dimos_pme_recip.argtypes = [vp, vp, vp, i64, ctypes.POINTER(dbl), dbl, ctypes.POINTER(i32), i32, dbl, vp, i32, vp, vp, vp]
+    lib.dimos_pme_mesh_size.argtypes = [dbl, ctypes.POINTER(dbl), dbl, ctypes.POINTER(i32)]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -125,7 +127,8 @@ def load_library() -> ctypes.CDLL:
                  "dimos_probe_fp32_peak", "dimos_nl_count_within", "dimos_profile_enable", "dimos_profile_read",
                  "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
                  "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen",
-                 "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities", "dimos_berendsen_scale"):
+                 "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities", "dimos_berendsen_scale",
+                 "dimos_pme_recip", "dimos_pme_mesh_size"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -326,6 +329,27 @@ class Context:
         else:
             nl.handle = h
         return nl, bool(rebuilt.value)
+
+    def pme_recip(self, pos, charge, box, alpha, mesh, order=5, coulomb_const=138.935456, F=None, accumulate=False,
+                  want_forces=True, E=None, virial=None):
+        """dimos_pme_recip: (F (N,3) or None, E (2,) = {U_recip, U_self}, virial (3,3)) device tensors; no sync."""
+        real = torch.float64 if self.precision == "f64" else torch.float32
+        pos = self._dev(pos, real, 3)
+        charge = self._dev(charge, real)
+        n = pos.shape[0]
+        if F is None and want_forces:
+            F = torch.zeros((n, 3), dtype=real, device=pos.device) if accumulate else torch.empty((n, 3), dtype=real, device=pos.device)
+        if E is None:
+            E = torch.empty(2, dtype=torch.float64, device=pos.device)
+        if virial is None:
+            virial = torch.empty((3, 3), dtype=torch.float64, device=pos.device)
+        m = (ctypes.c_int32 * 3)(*[int(k) for k in mesh])
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_pme_recip(self.handle, pos.data_ptr(), charge.data_ptr(), n, _box3(box), float(alpha), m, int(order),
+                                          float(coulomb_const), F.data_ptr() if F is not None else None, 1 if accumulate else 0,
+                                          E.data_ptr(), virial.data_ptr(), _stream_ptr())
+        self._check(rc)
+        return F, E, virial
 
     def dispersion_correction(self, type_, lj_table, box, r_cut, r_switch=0.0):
         """dimos_dispersion_correction: (E float, virial (3,3) float64 numpy) of the LJ tail correction."""
@@ -573,6 +597,19 @@ def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = T
 
 def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
     return ctx.nonbonded(nl, pos, charge, type_, lj_table, **kw)
+
+
+def dimos_pme_recip(ctx: Context, pos, charge, box, alpha, mesh, **kw):
+    return ctx.pme_recip(pos, charge, box, alpha, mesh, **kw)
+
+
+def dimos_pme_mesh_size(alpha, box, delta):
+    """The paper's mesh heuristic, rounded up to 7-smooth sizes: tuple of 3 ints.  Host only."""
+    m = (ctypes.c_int32 * 3)()
+    rc = load_library().dimos_pme_mesh_size(float(alpha), _box3(box), float(delta), m)
+    if rc != 0:
+        raise DimosError(rc, "dimos_pme_mesh_size: bad argument")
+    return tuple(int(k) for k in m)
 
 
 def dimos_dispersion_correction(ctx: Context, type_, lj_table, box, r_cut, r_switch=0.0):

@@ -121,6 +121,7 @@ DIMOS_API int dimos_destroy(dimos_ctx* c)
     cudaSetDevice(ctx->device);
     for (NL* nl : ctx->lists) free_list(ctx, nl);
     ctx->lists.clear();
+    pme_release(ctx);
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     if (ctx->d_rebuild_state) cudaFree(ctx->d_rebuild_state);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
@@ -286,6 +287,42 @@ static double switch_region_integral(double sigma, double eps, double rs, double
             sum += wg[k] * (1.0 - S) * 4.0 * eps * (sr6 * sr6 - sr6) * r * r;
         }
     return half * sum;
+}
+
+DIMOS_API int dimos_pme_mesh_size(double alpha, const double* box, double delta, int32_t* mesh_out)
+{
+    if (!box || !mesh_out || !(alpha > 0) || !(delta > 0) || !(delta < 1)) return DIMOS_EINVAL;
+    for (int a = 0; a < 3; ++a) {
+        if (!(box[a] > 0) || !std::isfinite(box[a])) return DIMOS_EINVAL;
+        const double want = ceil(2.0 * alpha * box[a] / (3.0 * pow(delta, 0.2)));
+        if (!(want < 4096.0)) return DIMOS_EINVAL;
+        int k = want < 8.0 ? 8 : (int)want;
+        for (;; ++k) {  // next size whose prime factors are 2, 3, 5, 7 (the radices cuFFT has kernels for)
+            int r = k;
+            for (int f : {2, 3, 5, 7})
+                while (r % f == 0) r /= f;
+            if (r == 1) break;
+        }
+        mesh_out[a] = k;
+    }
+    return DIMOS_OK;
+}
+
+DIMOS_API int dimos_pme_recip(dimos_ctx* c, const void* pos, const void* charge, int64_t N, const double* box, double alpha,
+                              const int32_t* mesh, int32_t order, double coulomb_const, void* F, int32_t accumulate, double* E,
+                              double* virial, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!pos || !charge || !box || !mesh || !E) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || !(alpha > 0) || !std::isfinite(alpha) || !std::isfinite(coulomb_const)) return set_error(ctx, DIMOS_EINVAL, "bad N, alpha or coulomb_const");
+    if (order < 3 || order > 6) return set_error(ctx, DIMOS_EINVAL, "PME spline order must be 3..6");
+    for (int a = 0; a < 3; ++a) {
+        if (!(box[a] > 0) || !std::isfinite(box[a])) return set_error(ctx, DIMOS_EINVAL, "bad box");
+        if (mesh[a] < 2 * order || mesh[a] > 4096) return set_error(ctx, DIMOS_EINVAL, "mesh size must lie in [2 * order, 4096] per axis");
+    }
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return pme_recip_impl(ctx, pos, charge, N, box, alpha, mesh, order, coulomb_const, F, E, virial, accumulate ? 1 : 0, (cudaStream_t)stream);
 }
 
 DIMOS_API int dimos_dispersion_correction(dimos_ctx* c, const int32_t* type, int64_t N, const double* lj_table, int32_t ntypes,

@@ -54,6 +54,7 @@ struct Ctx {
     int* h_pinned = nullptr;        // 64 ints pinned scratch for read-backs
     unsigned long long* d_rebuild_state = nullptr;  // {max bits, ticket}
     std::vector<struct NL*> lists;
+    struct PmePlan* pme = nullptr;  // cuFFT plans, mesh and accumulators of dimos_pme_recip (pme.cu), rebuilt when the mesh changes
     // optional per-kernel timing of the pair-force kernel (dimos_profile_enable / dimos_profile_read)
     bool profiling = false;
     std::vector<cudaEvent_t> prof_events;  // pairs (start, stop), recycled after each read
@@ -150,6 +151,9 @@ int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const 
                    const double* lj_table, int32_t ntypes, const dimos_nb_params* prm, void* F, double* E,
                    double* virial, cudaStream_t s);
 int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s);
+int pme_recip_impl(Ctx* ctx, const void* pos, const void* charge, int64_t n, const double* box, double alpha, const int32_t* mesh,
+                   int32_t order, double ke, void* F, double* E, double* W, int accumulate, cudaStream_t s);
+void pme_release(Ctx* ctx);
 int vv_kick_drift_impl(Ctx* ctx, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
                        const void* pos_at_build, double skin, int32_t* flag_dev, cudaStream_t s);
 int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStream_t s);
