@@ -139,12 +139,13 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
-def load_traffic(kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), or None."""
+def load_traffic(kernel: str, config_index: int):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture of the same workload
+    (profiles/traffic.json, keyed "<kernel>@configs[<i>]"), or None."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(path):
         try:
-            return json.load(open(path)).get(kernel)
+            return json.load(open(path)).get(f"{kernel}@configs[{config_index}]")
         except Exception:
             return None
     return None
@@ -153,10 +154,12 @@ def load_traffic(kernel: str):
 # ------------------------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle as it stands, on the host cores, on a bounded sample
 # ------------------------------------------------------------------------------------------------------
-def oracle_sample_box(method: str, big: bool):
-    """A constant-density box of the same recipe as the headline workload, small enough for the CPU."""
-    n_mol = 30000 if big else 3000
-    return wl.make_scaled(n_mol, seed=wl.SEED_BASE + 50, method=method)
+def oracle_box(spec, size: str):
+    """The workload's own box ("config"), or a constant-density box of the same recipe 10x / 100x smaller."""
+    if size == "config":
+        return wl.make_water_box(spec.n_molecules, wl.box_edge_for(spec), wl.SEED_BASE + spec.index, spec)
+    n_mol = {"tenth": max(spec.n_molecules // 10, 216), "hundredth": max(spec.n_molecules // 100, 216)}[size]
+    return wl.make_scaled(n_mol, seed=wl.SEED_BASE + 50, r_cut=spec.r_cut, skin=spec.skin, method=spec.method)
 
 
 def time_oracle_step(box, method: str):
@@ -170,19 +173,32 @@ def time_oracle_step(box, method: str):
     return time.perf_counter() - t0, res.n_pairs
 
 
-def cpu_baseline(method: str, budget_s: float = 20.0) -> dict:
+def pick_oracle_box(spec, n_evals: int, budget_s: float):
+    """Largest box of the workload's recipe whose n_evals oracle evaluations fit the time budget: the config itself when
+    it does (the oracle's cost is linear in N: a probe on the 100x smaller box is scaled up)."""
+    probe = oracle_box(spec, "hundredth")
+    t_probe, _ = time_oracle_step(probe, spec.method)
+    per_atom = t_probe / probe.n_atoms
+    for size in ("config", "tenth"):
+        n_atoms = 3 * spec.n_molecules if size == "config" else 3 * max(spec.n_molecules // 10, 216)
+        if 1.5 * per_atom * n_atoms * n_evals <= budget_s:
+            return oracle_box(spec, size), size
+    return probe, "hundredth"
+
+
+def sample_text(box, spec, size):
+    what = "the workload's own box" if size == "config" else f"a box of the same recipe, {size} of the atoms (the full box would exceed the time budget)"
+    return (f"one oracle cell-list force evaluation (fp64, C, OpenMP over all host cores) of {what}: {box.n_atoms} atoms, "
+            f"r_cut={spec.r_cut}, method={spec.method}")
+
+
+def cpu_baseline(spec, budget_s: float = 30.0) -> dict:
     import oracle
 
-    small = oracle_sample_box(method, big=False)
-    t_small, n_small = time_oracle_step(small, method)
-    cores = oracle.num_threads()
-    if t_small * 10.0 <= budget_s:  # a 10x larger box fits the budget: use it (less cache-friendly, more honest)
-        big = oracle_sample_box(method, big=True)
-        t, n = time_oracle_step(big, method)
-        sample = f"one oracle cell-list force evaluation (fp64, OpenMP) of a {big.n_atoms}-atom box of the same recipe"
-    else:
-        t, n, sample = t_small, n_small, f"one oracle cell-list force evaluation (fp64, OpenMP) of a {small.n_atoms}-atom box of the same recipe"
-    return {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": t}
+    box, size = pick_oracle_box(spec, 1, budget_s)
+    t, n = time_oracle_step(box, spec.method)
+    return {"value": n / t, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample_text(box, spec, size),
+            "seconds": t, "same_config": size == "config", "n_atoms": int(box.n_atoms), "pairs_in_cutoff": int(n)}
 
 
 def run_reference(args, spec, precision):
@@ -191,28 +207,22 @@ def run_reference(args, spec, precision):
         return
     import oracle
 
-    method = spec.method
-    small = oracle_sample_box(method, big=False)
-    t_probe, _ = time_oracle_step(small, method)
-    total_steps = args.steps + args.warmup
-    big = t_probe * 10.0 * total_steps <= 150.0
-    box = oracle_sample_box(method, big=big)
+    box, size = pick_oracle_box(spec, args.steps + args.warmup, 240.0)
     for _ in range(args.warmup):
-        time_oracle_step(box, method)
+        time_oracle_step(box, spec.method)
     t0 = time.perf_counter()
     pairs = 0
     for _ in range(args.steps):
-        _, n = time_oracle_step(box, method)
+        _, n = time_oracle_step(box, spec.method)
         pairs += n
     dt = time.perf_counter() - t0
     value = pairs / dt
-    sample = (f"each step = one oracle cell-list force evaluation (fp64, OpenMP) of a {box.n_atoms}-atom box of the same recipe "
-              f"(density, r_cut={box.spec.r_cut}, method={method})")
+    sample = "each step = " + sample_text(box, spec, size)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(spec, precision), "sample": sample},
+        "config": {"workload": workload_name(spec, precision), "sample": sample, "same_config": size == "config"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -252,6 +262,50 @@ def tau_vs_n(ctx, dimos, dev, spec, precision, timed, tau_force_main, tau_build_
     rows.append({"n_atoms": int(n_main), "tau_force_s": tau_force_main, "tau_build_s": tau_build_main,
                  "pairs_in_cutoff": int(n_cut_main), "pairs_per_s_force_only": n_cut_main / tau_force_main})
     return rows
+
+
+def md_step_tau(ctx, dimos, torch, box, spec, pos0, vel_np, charge, typ, excl, lj, kw, steps=60, warmup=10, dt=0.0005):
+    """tau of one rigid-water MD step made of library calls only (the quantity the paper's Fig. 1 plots):
+    dimos_water_kick_drift_settle (velocity-Verlet steps 1-3 of PAPER.md:281-292 + the rebuild trigger) -> dimos_nl_build when
+    it fired -> dimos_nonbonded (step 4) -> dimos_water_kick_settle_velocities (steps 5-6).  NVE from Maxwell-Boltzmann 300 K
+    velocities on the seeded (unrelaxed) box, dt = 0.5 fs (the time step of the paper's water-box benchmark)."""
+    dev = pos0.device
+    n = pos0.shape[0]
+    water = torch.arange(n, dtype=torch.int32, device=dev).reshape(-1, 3)
+    m_O, m_H = float(box.mass[0]), float(box.mass[1])
+    d_oh = wl.R_OH
+    d_hh = 2.0 * wl.R_OH * float(np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0))
+    pos = pos0.clone()
+    vel = torch.from_numpy(vel_np.astype(np.float64 if pos0.dtype == torch.float64 else np.float32)).to(dev)
+    dimos.dimos_settle_velocities(ctx, pos, vel, water, m_O, m_H)
+    nl = dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl)
+    F = torch.empty_like(pos)
+    E = torch.empty(4, dtype=torch.float64, device=dev)
+    W = torch.empty(3, 3, dtype=torch.float64, device=dev)
+    dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw)
+    rebuilds = 0
+
+    def one():
+        nonlocal rebuilds
+        if dimos.dimos_water_kick_drift_settle(ctx, pos, vel, F, water, m_O, m_H, d_oh, d_hh, dt, pos_at_build=nl.pos_at_build, skin=spec.skin):
+            dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl, nl=nl)
+            rebuilds += 1
+        dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw)
+        dimos.dimos_water_kick_settle_velocities(ctx, pos, vel, F, water, m_O, m_H, dt)
+
+    for _ in range(warmup):
+        one()
+    rebuilds = 0
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(steps):
+        one()
+    b.record()
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(E).all()) and bool(torch.isfinite(pos).all()), "non-finite state in the MD-step timing"
+    return {"tau_s": a.elapsed_time(b) * 1e-3 / steps, "steps": steps, "rebuilds": rebuilds, "dt_fs": 1e3 * dt,
+            "what": "rigid-water velocity-Verlet step: water_kick_drift_settle -> (nl_build) -> nonbonded -> water_kick_settle_velocities"}
 
 
 def workload_name(spec, precision):
@@ -374,9 +428,12 @@ def run_ours(args, spec, precision):
         h_W = torch.empty((3, 3), dtype=torch.float64).pin_memory()
         hnl = None
         k = 0
+        # charge / type / lj_table travel once (first call); afterwards only the positions do
+        hnl, _ = ctx.step_host(None, host_pos[0], h_charge, h_type, h_lj, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E, h_W, **kw)
+        k = 1
         for _ in range(max(args.warmup, 3)):
-            hnl, _ = ctx.step_host(hnl, host_pos[k % ring], h_charge, h_type, h_lj, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E,
-                                   h_W, **kw)
+            hnl, _ = ctx.step_host(hnl, host_pos[k % ring], None, None, None, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E,
+                                   h_W, ntypes=h_lj.shape[0], **kw)
             k += 1
         torch.cuda.synchronize()
         if dist:
@@ -386,10 +443,11 @@ def run_ours(args, spec, precision):
         a.record()
         e2e_rebuilds = 0
         for _ in range(args.steps):
-            hnl, rb = ctx.step_host(hnl, host_pos[k % ring], h_charge, h_type, h_lj, box.box, spec.r_cut, spec.skin, h_excl, h_F,
-                                    h_E, h_W, **kw)
+            hnl, rb = ctx.step_host(hnl, host_pos[k % ring], None, None, None, box.box, spec.r_cut, spec.skin, h_excl, h_F,
+                                    h_E, h_W, ntypes=h_lj.shape[0], **kw)
             e2e_rebuilds += int(rb)
             k += 1
+        assert bool(torch.isfinite(h_E).all()) and bool(torch.isfinite(h_F).all()), "non-finite result in the e2e region"
         b.record()
         torch.cuda.synchronize()
         e2e_seconds = max(a.elapsed_time(b) * 1e-3, 0.0)
@@ -398,9 +456,9 @@ def run_ours(args, spec, precision):
             dist.barrier()
         rs = 8 if precision == "f64" else 4
         e2e_t, e2e_units = aggregate_over_ranks(e2e_seconds, float(n_cut) * args.steps, world, dist, dev)
-        e2e = {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": n * (3 * rs + rs + 4) + int(h_lj.numel()) * 8,
+        e2e = {"value": e2e_units / e2e_t, "unit": UNIT, "h2d_bytes_per_step": n * 3 * rs,
                "d2h_bytes_per_step": n * 3 * rs + 13 * 8 + 4, "ms_per_step": 1e3 * e2e_t / args.steps, "rebuilds": e2e_rebuilds,
-               "wall_ms_per_step": 1e3 * wall / args.steps, "api": "dimos_step_host (pinned host buffers)"}
+               "wall_ms_per_step": 1e3 * wall / args.steps, "api": "dimos_step_host (pinned host buffers; positions up and F/E/W down every step, charge/type/lj_table once)"}
 
     total_t, total_units = aggregate_over_ranks(seconds, float(n_cut) * args.steps, world, dist, dev)
     if rank != 0:
@@ -413,14 +471,18 @@ def run_ours(args, spec, precision):
     flops_per_launch = FLOPS_PER_LISTED_PAIR * n_listed + FLOPS_PER_CUTOFF_PAIR[spec.method] * n_cut
     pair_s = pair_ms * 1e-3 / max(pair_n, 1)
     achieved_tflops = flops_per_launch / pair_s * 1e-12 if pair_n else None
-    fp32_peak = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 * 1e-12  # TFLOP/s
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    fp32_peak = n_sm * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 * 1e-12  # TFLOP/s
     if precision == "f64":
         fp32_peak = 40.0  # NVIDIA's nominal B200 FP64 vector rate (no measured figure on this pool); context only
+    # the packed kernel runs fp32 boxes with at least three cells per axis, either method (csrc/nonbonded.cu use_f32x2)
+    kernel_name = "pair_force_f32x2_kernel" if (precision == "f32" and stats["pbc_mode"] == 0) else "pair_force_kernel"
     list_bytes = stats["list_bytes"] + stats["n_slots"] * (16 + 4 + 16 + 16)
     roofline = {
-        "bound": "alu", "kernel": "pair_force_f32x2_kernel" if (precision == "f32" and spec.method == "rf") else "pair_force_kernel", "achieved": achieved_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
-        "frac": (achieved_tflops / fp32_peak) if achieved_tflops else None, "traffic": load_traffic("pair_force_kernel"),
-        "peak_source": f"derived: 148 SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md); FFMA probe measured "
+        "bound": "alu", "kernel": kernel_name, "achieved": achieved_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
+        "frac": (achieved_tflops / fp32_peak) if achieved_tflops else None, "traffic": load_traffic(kernel_name, spec.index),
+        "traffic_source": "committed ncu --set full capture of this kernel on this workload (profiles/traffic.json), not this run",
+        "peak_source": f"derived: {n_sm} SMs x 128 FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md); FFMA probe measured "
                        f"{fp32_probe:.1f} TFLOP/s in this run",
         "fp32_probe_tflops": fp32_probe,
         "flops_per_launch": flops_per_launch, "flop_model": f"{FLOPS_PER_LISTED_PAIR}*N_nl + {FLOPS_PER_CUTOFF_PAIR[spec.method]}*N_c",
@@ -445,8 +507,10 @@ def run_ours(args, spec, precision):
     }
     if not args.no_scan and world == 1 and precision != "f64":
         line["tau_vs_n"] = tau_vs_n(ctx, dimos, dev, spec, precision, timed, tau_force, tau_build, n, n_cut)
+    if not args.no_scan and world == 1 and box.n_atoms % 3 == 0:
+        line["md_step"] = md_step_tau(ctx, dimos, torch, box, spec, pos0, vel, charge, typ, excl, lj, kw)
     if not args.no_cpu_baseline and world >= 1:
-        line["cpu_baseline"] = cpu_baseline(spec.method)
+        line["cpu_baseline"] = cpu_baseline(spec)
     ctx.close()
     if dist:
         dist.destroy_process_group()

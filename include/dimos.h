@@ -25,7 +25,9 @@
  *   the legacy default stream).  A call does not synchronise with the host unless stated.
  *   Every call returns a dimos_status (0 = DIMOS_OK, negative = error); on error no output array
  *   is guaranteed to be written.  dimos_last_error(ctx) gives a human-readable message.
- *   Calls on one context must not overlap in time (no internal locking).
+ *   Host calls on one context must not overlap in time (no internal locking).  Their device work may: calls may use
+ *   different streams and several lists, and up to 64 rebuild-trigger evaluations (dimos_nl_needs_rebuild and the
+ *   integrator steps that fuse it) may be in flight at once, each with its own reduction state.
  *   There is no CPU fallback: without a usable CUDA device every compute call fails with
  *   DIMOS_ECUDA.
  */
@@ -59,7 +61,11 @@ typedef enum {
 } dimos_status;
 
 /* Element type of pos/charge/F and arithmetic of the pair kernel (reading C-11):
- *   DIMOS_F32   float in/out, float pair math, per-thread float partial sums, fp64 final reduction
+ *   DIMOS_F32   float in/out, float pair math, per-thread float partial sums, fp64 final reduction.
+ *               Exception: boxes with fewer than three cells per axis (N of a few thousand at most; the per-pair
+ *               minimum-image kernel) evaluate the pair ENERGY in fp64 from the same fp32 inputs, because their
+ *               total is a ~1e-4 remainder of cancelling terms that fp32 pair energies cannot resolve to 1e-5
+ *               (DESIGN.md section 3); forces and virial stay fp32.  Larger boxes are fp32 throughout.
  *   DIMOS_F64   double everywhere
  *   DIMOS_MIXED float in/out, float pair math, energy and virial accumulated in fp64 from the
  *               first add */
@@ -191,6 +197,8 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* ctx, dimos_nl* nl, const void* pos
  *                 built from pos_host and returned; otherwise reused / rebuilt in place
  *   excl_pairs_host  host, n_excl x 2 int32 (read only when the list is first built; the list keeps
  *                 its device copy for later rebuilds)
+ *   charge_host, type_host, lj_table_host   each may be NULL once a call on this list has passed it: the device copy
+ *                 kept in the list is used again, so that only what changed travels (positions travel every step)
  *   rebuilt_host  host, may be NULL: receives 1 if this call (re)built the list, else 0
  * Other arguments as in dimos_nonbonded_host.  Synchronises the stream (twice: once to read the
  * trigger, once at the end). */
@@ -237,6 +245,11 @@ DIMOS_API int dimos_pme_recip(dimos_ctx* ctx, const void* pos, const void* charg
 /* dimos_pme_mesh_size -- the paper's mesh heuristic n_mesh = 2 alpha d / (3 delta^(1/5)) per box edge d,
  * rounded up to the next size with prime factors 2, 3, 5, 7.  Host only; mesh_out receives 3 int32. */
 DIMOS_API int dimos_pme_mesh_size(double alpha, const double* box, double delta, int32_t* mesh_out);
+
+/* dimos_lj_table_fill -- Lorentz-Berthelot combining rules, Eq. 5: sigma_ab = (sigma_a + sigma_b) / 2,
+ * eps_ab = sqrt(eps_a eps_b), written as the ntypes x ntypes x 2 table (sigma_ab, eps_ab) that dimos_nonbonded takes
+ * (reading C-16).  Host only: sigma, eps host arrays of ntypes doubles, table_out host array of 2 ntypes^2 doubles. */
+DIMOS_API int dimos_lj_table_fill(const double* sigma, const double* eps, int32_t ntypes, double* table_out);
 
 /* dimos_dispersion_correction -- PAPER.md:202 ("long-range dispersion corrections that approximate the contributions
  * beyond r_c"; the paper gives no formula: reading C-22).  The homogeneous-fluid tail of the 12-6 potential that the

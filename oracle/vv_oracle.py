@@ -1,10 +1,12 @@
-"""Velocity-Verlet steps 1, 2 and 5 of PAPER.md:281-292 (section III C 1), written out in numpy fp64.
+"""The velocity-Verlet loop of PAPER.md:281-292 (section III C 1) written out in numpy fp64: steps 1, 2, 5 (kicks and
+drift), steps 3 and 6 for rigid three-site water (SHAKE / RATTLE iterated to convergence, reading C-23), step 7 as the
+Berendsen thermostat (reading C-24) and the Langevin update of PAPER.md:309 (reading C-26), plus the long-range dispersion
+correction of PAPER.md:202 (reading C-22).
 
 TEST INFRASTRUCTURE ONLY (see oracle/__init__.py): the product package never imports this.
 
 Units: positions nm, velocities nm/ps, forces kJ mol^-1 nm^-1, masses amu, time ps.  With these units the
 acceleration a = F / m is in nm/ps^2 without any conversion factor (1 kJ/mol = 1 amu nm^2 ps^-2).
-Constraints (steps 3, 6) and the thermostat (step 7) are not part of this oracle: the library does not build them.
 """
 from __future__ import annotations
 

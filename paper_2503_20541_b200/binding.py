@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = (
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
     "dimos_kinetic_energy", "dimos_berendsen", "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities",
-    "dimos_berendsen_scale", "dimos_pme_recip", "dimos_pme_mesh_size",
+    "dimos_berendsen_scale", "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill",
 )
 
 
@@ -111,6 +111,7 @@ def load_library() -> ctypes.CDLL:
                                                 ctypes.POINTER(dbl), vp]
     lib.dimos_pme_recip.argtypes = [vp, vp, vp, i64, ctypes.POINTER(dbl), dbl, ctypes.POINTER(i32), i32, dbl, vp, i32, vp, vp, vp]
     lib.dimos_pme_mesh_size.argtypes = [dbl, ctypes.POINTER(dbl), dbl, ctypes.POINTER(i32)]
+    lib.dimos_lj_table_fill.argtypes = [vp, vp, i32, vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -128,7 +129,7 @@ def load_library() -> ctypes.CDLL:
                  "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
                  "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen",
                  "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities", "dimos_berendsen_scale",
-                 "dimos_pme_recip", "dimos_pme_mesh_size"):
+                 "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -308,20 +309,23 @@ class Context:
         return F, E, virial
 
     def step_host(self, nl: "NeighborList | None", pos, charge, type_, lj_table, box, r_cut, skin, excl_pairs, F, E, virial, *,
-                  method="rf", eps_rf=78.5, alpha=3.12, coulomb_const=138.935456, r_switch=0.0):
-        """dimos_step_host: HOST tensors in and out; returns (NeighborList, rebuilt: bool)."""
-        for t in (pos, charge, type_, lj_table, F, E, virial) + ((excl_pairs,) if excl_pairs is not None else ()):
-            if t.is_cuda or not t.is_contiguous():
+                  method="rf", eps_rf=78.5, alpha=3.12, coulomb_const=138.935456, r_switch=0.0, ntypes=None):
+        """dimos_step_host: HOST tensors in and out; returns (NeighborList, rebuilt: bool).  charge / type_ / lj_table may be
+        None after a call on this list has passed them (the list keeps its device copies); give ntypes then."""
+        for t in (pos, charge, type_, lj_table, F, E, virial, excl_pairs):
+            if t is not None and (t.is_cuda or not t.is_contiguous()):
                 raise ValueError("step_host takes contiguous host tensors")
         prm = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method], float(r_switch))
         h = ctypes.c_void_p(nl.handle.value if nl is not None else None)
         rebuilt = ctypes.c_int32(0)
         n_excl = 0 if excl_pairs is None else excl_pairs.shape[0]
+        nt = lj_table.shape[0] if lj_table is not None else int(ntypes)
+        ptr = lambda t: t.data_ptr() if t is not None else None
         with torch.cuda.device(self.device):
-            rc = self.lib.dimos_step_host(self.handle, ctypes.byref(h), pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
-                                          lj_table.data_ptr(), lj_table.shape[0], pos.shape[0], _box3(box), float(skin),
-                                          excl_pairs.data_ptr() if n_excl else None, n_excl, ctypes.byref(prm), F.data_ptr(),
-                                          E.data_ptr(), virial.data_ptr(), ctypes.byref(rebuilt), _stream_ptr())
+            rc = self.lib.dimos_step_host(self.handle, ctypes.byref(h), pos.data_ptr(), ptr(charge), ptr(type_), ptr(lj_table), nt,
+                                          pos.shape[0], _box3(box), float(skin), excl_pairs.data_ptr() if n_excl else None, n_excl,
+                                          ctypes.byref(prm), F.data_ptr(), E.data_ptr(), virial.data_ptr(), ctypes.byref(rebuilt),
+                                          _stream_ptr())
         self._check(rc)
         boxt = tuple(float(b) for b in (box.tolist() if hasattr(box, "tolist") else box))
         if nl is None:
@@ -670,9 +674,13 @@ def dimos_nl_export_pairs(ctx: Context, nl: NeighborList) -> torch.Tensor:
 
 def lj_table_from_types(sigma, epsilon) -> torch.Tensor:
     """Host-side fill of the (sigma_ab, eps_ab) table by Lorentz-Berthelot, Eq. (5) PAPER.md:195."""
-    s = torch.as_tensor(sigma, dtype=torch.float64)
-    e = torch.as_tensor(epsilon, dtype=torch.float64)
+    s = torch.as_tensor(sigma, dtype=torch.float64).contiguous()
+    e = torch.as_tensor(epsilon, dtype=torch.float64).contiguous()
     table = torch.empty(s.numel(), s.numel(), 2, dtype=torch.float64)
-    table[:, :, 0] = 0.5 * (s[:, None] + s[None, :])
-    table[:, :, 1] = torch.sqrt(e[:, None] * e[None, :])
+    rc = load_library().dimos_lj_table_fill(s.data_ptr(), e.data_ptr(), s.numel(), table.data_ptr())  # dimos_lj_table_fill
+    if rc != 0:
+        raise DimosError(rc, "dimos_lj_table_fill: bad argument")
     return table
+
+
+dimos_lj_table_fill = lj_table_from_types

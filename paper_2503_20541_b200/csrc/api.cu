@@ -106,10 +106,10 @@ DIMOS_API int dimos_create(dimos_ctx** out, int device, int precision, const dim
     ctx->sm_count = prop.multiProcessorCount;
     if (prop.major < 10) { delete ctx; return DIMOS_ECUDA; }  // built for sm_100a only
     if (cudaMallocHost((void**)&ctx->h_pinned, 64 * sizeof(int)) != cudaSuccess) { delete ctx; return DIMOS_ENOMEM; }
-    if (cudaMalloc((void**)&ctx->d_rebuild_state, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+    if (cudaMalloc((void**)&ctx->d_rebuild_state, 2 * TRIGGER_RING * sizeof(unsigned long long)) != cudaSuccess) {
         cudaFreeHost(ctx->h_pinned); delete ctx; return DIMOS_ENOMEM;
     }
-    cudaMemset(ctx->d_rebuild_state, 0, 2 * sizeof(unsigned long long));
+    cudaMemset(ctx->d_rebuild_state, 0, 2 * TRIGGER_RING * sizeof(unsigned long long));
     *out = reinterpret_cast<dimos_ctx*>(ctx);
     return DIMOS_OK;
 }
@@ -122,6 +122,7 @@ DIMOS_API int dimos_destroy(dimos_ctx* c)
     for (NL* nl : ctx->lists) free_list(ctx, nl);
     ctx->lists.clear();
     pme_release(ctx);
+    release(ctx, ctx->scratch);
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     if (ctx->d_rebuild_state) cudaFree(ctx->d_rebuild_state);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
@@ -289,6 +290,19 @@ static double switch_region_integral(double sigma, double eps, double rs, double
     return half * sum;
 }
 
+DIMOS_API int dimos_lj_table_fill(const double* sigma, const double* eps, int32_t ntypes, double* table_out)
+{
+    if (!sigma || !eps || !table_out || ntypes < 1 || ntypes > MAX_TYPES) return DIMOS_EINVAL;
+    for (int a = 0; a < ntypes; ++a)
+        if (!(sigma[a] >= 0) || !(eps[a] >= 0) || !std::isfinite(sigma[a]) || !std::isfinite(eps[a])) return DIMOS_EINVAL;
+    for (int a = 0; a < ntypes; ++a)
+        for (int b = 0; b < ntypes; ++b) {  // Eq. 5
+            table_out[2 * ((size_t)a * ntypes + b)] = 0.5 * (sigma[a] + sigma[b]);
+            table_out[2 * ((size_t)a * ntypes + b) + 1] = sqrt(eps[a] * eps[b]);
+        }
+    return DIMOS_OK;
+}
+
 DIMOS_API int dimos_pme_mesh_size(double alpha, const double* box, double delta, int32_t* mesh_out)
 {
     if (!box || !mesh_out || !(alpha > 0) || !(delta > 0) || !(delta < 1)) return DIMOS_EINVAL;
@@ -337,8 +351,9 @@ DIMOS_API int dimos_dispersion_correction(dimos_ctx* c, const int32_t* type, int
     if (!(box[0] > 0 && box[1] > 0 && box[2] > 0)) return set_error(ctx, DIMOS_EINVAL, "bad box");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
     cudaStream_t s = (cudaStream_t)stream;
-    unsigned long long* d = nullptr;
-    DIMOS_CUDA_TRY(ctx, cudaMalloc(&d, (MAX_TYPES + 1) * sizeof(unsigned long long)));
+    int rc0;
+    if ((rc0 = ensure(ctx, ctx->scratch, (MAX_TYPES + 1) * sizeof(unsigned long long), s))) return rc0;
+    unsigned long long* d = (unsigned long long*)ctx->scratch.p;
     std::vector<double> tab((size_t)ntypes * ntypes * 2);
     unsigned long long h[MAX_TYPES + 1] = {0};
     cudaError_t e = cudaMemsetAsync(d, 0, (MAX_TYPES + 1) * sizeof(unsigned long long), s);
@@ -350,7 +365,6 @@ DIMOS_API int dimos_dispersion_correction(dimos_ctx* c, const int32_t* type, int
         if (e == cudaSuccess) e = cudaStreamSynchronize(s);
         if (e != cudaSuccess) rc = set_error(ctx, DIMOS_ECUDA, cudaGetErrorString(e));
     }
-    cudaFree(d);
     if (rc) return rc;
     if (h[MAX_TYPES]) return set_error(ctx, DIMOS_EINVAL, "type index out of range");
     const bool sw = r_switch > 0.0 && r_switch < r_cut;
@@ -596,8 +610,7 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
 {
     if (!c) return DIMOS_EINVAL;
     Ctx* ctx = reinterpret_cast<Ctx*>(c);
-    if (!inout || !pos_host || !charge_host || !type_host || !lj_table_host || !box || !params || !F_host || !E_host)
-        return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (!inout || !pos_host || !box || !params || !F_host || !E_host) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
     if (N <= 0 || n_excl < 0 || (n_excl > 0 && !excl_pairs_host)) return set_error(ctx, DIMOS_EINVAL, "bad N or exclusion list");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
     cudaStream_t s = (cudaStream_t)stream;
@@ -606,6 +619,11 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
     int rc;
     int rebuilt = 0;
     bool static_uploaded = false;
+    // charge / type / lj_table may be NULL: the device copies of the last call that passed them are used again
+    const bool have_static = nl && list_belongs(ctx, nl) && nl->N == N && nl->st_static_ntypes == ntypes && nl->st_charge.p &&
+                             nl->st_type.p && nl->st_lj.p;
+    if ((!charge_host || !type_host || !lj_table_host) && !have_static)
+        return set_error(ctx, DIMOS_EINVAL, "charge_host / type_host / lj_table_host are NULL but this list holds no copy of them yet");
     bool fresh = nl == nullptr || !list_belongs(ctx, nl) || nl->N != N || nl->r_cut != params->r_cut || nl->skin != skin ||
                  nl->box[0] != box[0] || nl->box[1] != box[1] || nl->box[2] != box[2] || nl->n_excl != n_excl ||
                  nl->st_ref.p == nullptr;
@@ -617,12 +635,12 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
         rc = needs_rebuild_impl(ctx, nl->st_pos.p, nl->st_ref.p, N, skin, (int32_t*)nl->st_flag.p, s);
         if (rc) return rc;
         DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 33, nl->st_flag.p, sizeof(int), cudaMemcpyDeviceToHost, s));
-        // the other per-step inputs go up while the host waits for the flag
+        // the other inputs the caller passed go up while the host waits for the flag
         if (nl->st_charge.p && nl->st_type.p && nl->st_lj.p && nl->st_charge.bytes >= (size_t)N * rs &&
             nl->st_type.bytes >= (size_t)N * sizeof(int) && nl->st_lj.bytes >= (size_t)ntypes * ntypes * 2 * sizeof(double)) {
-            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
-            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
-            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
+            if (charge_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
+            if (type_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
+            if (lj_table_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
             static_uploaded = true;
         }
         DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
@@ -671,10 +689,11 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
     if ((rc = ensure(ctx, nl->st_F, 3 * (size_t)N * rs, s))) return rc;
     if ((rc = ensure(ctx, nl->st_EW, 16 * sizeof(double), s))) return rc;
     if (!static_uploaded) {
-        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
-        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
-        DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
+        if (charge_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_charge.p, charge_host, (size_t)N * rs, cudaMemcpyHostToDevice, s));
+        if (type_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_type.p, type_host, (size_t)N * sizeof(int), cudaMemcpyHostToDevice, s));
+        if (lj_table_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
     }
+    nl->st_static_ntypes = ntypes;
     double* EW = (double*)nl->st_EW.p;
     rc = nonbonded_impl(ctx, nl, nl->st_pos.p, nl->st_charge.p, (const int32_t*)nl->st_type.p, (const double*)nl->st_lj.p, ntypes,
                         params, nl->st_F.p, EW, EW + 4, s);

@@ -52,7 +52,9 @@ struct Ctx {
     int64_t launches = 0;
     int sm_count = 148;
     int* h_pinned = nullptr;        // 64 ints pinned scratch for read-backs
-    unsigned long long* d_rebuild_state = nullptr;  // {max bits, ticket}
+    unsigned long long* d_rebuild_state = nullptr;  // TRIGGER_RING x {max bits, ticket}: one pair per trigger call in flight
+    unsigned trigger_seq = 0;
+    DevBuf scratch;  // small per-context device scratch (type histogram of dimos_dispersion_correction)
     std::vector<struct NL*> lists;
     struct PmePlan* pme = nullptr;  // cuFFT plans, mesh and accumulators of dimos_pme_recip (pme.cu), rebuilt when the mesh changes
     // optional per-kernel timing of the pair-force kernel (dimos_profile_enable / dimos_profile_read)
@@ -61,6 +63,10 @@ struct Ctx {
     size_t prof_used = 0;                  // events handed out since the last read
 };
 constexpr size_t PROF_MAX_EVENTS = 8192;
+constexpr unsigned TRIGGER_RING = 64;
+// reduction state of the next rebuild-trigger kernel: consecutive calls (possibly on different streams, several lists per
+// context) never share a {max, ticket} pair unless more than TRIGGER_RING of them are in flight at once
+inline unsigned long long* next_trigger_state(Ctx* ctx) { return ctx->d_rebuild_state + 2 * (ctx->trigger_seq++ % TRIGGER_RING); }
 
 // geometry of the cell grid / list, passed by value to kernels
 struct Grid {
@@ -115,6 +121,7 @@ struct NL {
     DevBuf accum;      // double[16] + unsigned ticket
     // host-call staging (dimos_nonbonded_host)
     DevBuf st_pos, st_charge, st_type, st_lj, st_F, st_EW, st_ref, st_flag;
+    int st_static_ntypes = 0;  // ntypes of the charge / type / lj_table copies held in st_* (dimos_step_host), 0 = none
     DevBuf export_count;  // unsigned long long[1]
 };
 

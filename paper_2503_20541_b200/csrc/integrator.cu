@@ -319,7 +319,10 @@ __global__ void berendsen_scale_kernel(real* __restrict__ vel, int64_t n3, const
                                        double T0, double dt_over_tau)
 {
     const double T = *ke * two_over_dof_kb;
-    const real lam = (real)sqrt(1.0 + dt_over_tau * (T0 / T - 1.0));
+    // a system at rest (T = 0) has nothing to rescale: lambda = 1 instead of a division by zero; the radicand is
+    // kept non-negative (dt > tau with T far above T0 would otherwise give NaN velocities)
+    const double rad = T > 0.0 ? 1.0 + dt_over_tau * (T0 / T - 1.0) : 1.0;
+    const real lam = (real)sqrt(rad > 0.0 ? rad : 0.0);
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (int64_t)gridDim.x * blockDim.x) vel[i] *= lam;
 }
 
@@ -417,7 +420,7 @@ static void launch_kick_drift(Ctx* ctx, void* pos, void* vel, const void* F, con
     const real h = (real)0.5 * (real)skin;
     if (ref && flag_dev)
         vv_kick_drift_kernel<real, true><<<blocks, 256, 0, s>>>((real*)pos, (real*)vel, (const real*)F, (const real*)inv_mass, N,
-                                                                 (real)dt, (const real*)ref, h * h, ctx->d_rebuild_state, flag_dev);
+                                                                 (real)dt, (const real*)ref, h * h, next_trigger_state(ctx), flag_dev);
     else
         vv_kick_drift_kernel<real, false><<<blocks, 256, 0, s>>>((real*)pos, (real*)vel, (const real*)F, (const real*)inv_mass,
                                                                   N, (real)dt, nullptr, (real)0, nullptr, nullptr);
@@ -491,7 +494,7 @@ static void launch_water_a(Ctx* ctx, void* pos, void* vel, const void* F, const 
     if (ref && flag_dev)
         water_kick_drift_settle_kernel<real, true><<<blocks, 256, 0, s>>>((real*)pos, (real*)vel, (const real*)F, water, n_w, g,
                                                                           (real)(1.0 / m_O), (real)(1.0 / m_H), (real)dt,
-                                                                          (const real*)ref, h * h, ctx->d_rebuild_state, flag_dev);
+                                                                          (const real*)ref, h * h, next_trigger_state(ctx), flag_dev);
     else
         water_kick_drift_settle_kernel<real, false><<<blocks, 256, 0, s>>>((real*)pos, (real*)vel, (const real*)F, water, n_w, g,
                                                                            (real)(1.0 / m_O), (real)(1.0 / m_H), (real)dt, nullptr,

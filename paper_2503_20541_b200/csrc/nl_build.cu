@@ -378,7 +378,7 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
         int64_t slot = (int64_t)u0 * UNIT + p;
         perm[slot] = p < n ? id : ~id;
         if (p < n) inv_perm[id] = (int)slot;
-        xyz_build[slot] = make4(X[lid], Y[lid], Z[lid], (real)0);
+        xyz_build[slot] = make4(X[lid], Y[lid], Z[lid], p < n ? (real)1 : (real)0);  // w: 1 = real atom, 0 = padding slot
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             double x = (double)pos[3 * (int64_t)id + a];
@@ -651,8 +651,8 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                 const int v = cand_unit[t >> 3];
                 code = cand_code[t >> 3];
                 slot = v * UNIT + (t & 7);
-                if (P.perm[slot] >= 0) {
-                    real4 pj = P.xyz[slot];
+                const real4 pj = P.xyz[slot];
+                if (pj.w != (real)0) {  // not a padding slot
                     const real4 co = code_off[code];
                     const real px = pj.x + co.x, py = pj.y + co.y, pz = pj.z + co.z;
                     unsigned bits = 0;
@@ -693,34 +693,71 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         ncand = 0;
     };
 
-    for (int ix = 0; ix < sn[0]; ++ix)
-        for (int iy = 0; iy < sn[1]; ++iy)
-            for (int iz = 0; iz < sn[2]; ++iz) {
-                const int c2 = (sc[0][ix] * P.g.n[1] + sc[1][iy]) * P.g.n[2] + sc[2][iz];
-                const int code = stencil_code(sd[0][ix], sd[1][iy], sd[2][iz]);
-                const real ox = (real)sd[0][ix] * P.h[0], oy = (real)sd[1][iy] * P.h[1], oz = (real)sd[2][iz] * P.h[2];
-                const int us = P.unit_start[c2], ue = P.unit_start[c2 + 1];
-                for (int v0 = us; v0 < ue; v0 += 32) {
-                    if (ncand + 32 > CAND_MAX) flush();
-                    const int v = v0 + lane;
-                    bool acc = false;
-                    if (v < ue && v != U && owns(U, v, P.n_units)) {
-                        real4 lo = P.bb_lo[v], hi = P.bb_hi[v];
-                        real gx = axis_gap<real, PBC>(ulo.x, uhi.x, lo.x + ox, hi.x + ox, P.L[0]);
-                        real gy = axis_gap<real, PBC>(ulo.y, uhi.y, lo.y + oy, hi.y + oy, P.L[1]);
-                        real gz = axis_gap<real, PBC>(ulo.z, uhi.z, lo.z + oz, hi.z + oz, P.L[2]);
-                        acc = gx * gx + gy * gy + gz * gz < P.rnl2;
-                    }
-                    unsigned b = __ballot_sync(FULL, acc);
-                    if (acc) {
-                        int pos = ncand + __popc(b & lt_mask);
-                        cand_unit[pos] = v;
-                        cand_code[pos] = (unsigned char)code;
-                    }
-                    ncand += __popc(b);
-                    __syncwarp();
-                }
+    // Stencil table, one lane per (de-duplicated) stencil cell: its unit range, image code, and whether any of its units
+    // can be owned by U.  Ownership is an arc of n_units/2 consecutive unit indices, far longer than a cell's range, so
+    // a cell neither of whose end units is owned (and that does not hold U itself) has no owned unit at all.
+    int my_us = 0, my_cnt = 0, my_code = SELF_CODE;
+    {
+        const int ns = sn[0] * sn[1] * sn[2];
+        if (lane < ns) {
+            const int iz = lane % sn[2], iy = (lane / sn[2]) % sn[1], ix = lane / (sn[2] * sn[1]);
+            int scx = 0, scy = 0, scz = 0, sdx = 0, sdy = 0, sdz = 0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                if (k == ix) { scx = sc[0][k]; sdx = sd[0][k]; }
+                if (k == iy) { scy = sc[1][k]; sdy = sd[1][k]; }
+                if (k == iz) { scz = sc[2][k]; sdz = sd[2][k]; }
             }
+            const int c2 = (scx * P.g.n[1] + scy) * P.g.n[2] + scz;
+            my_code = stencil_code(sdx, sdy, sdz);
+            const int us = P.unit_start[c2], ue = P.unit_start[c2 + 1];
+            my_us = us;
+            my_cnt = ue - us;
+            if (my_cnt > 0 && P.n_units >= 256 && !(U >= us && U < ue) && !owns(U, us, P.n_units) && !owns(U, ue - 1, P.n_units))
+                my_cnt = 0;
+        }
+    }
+    int my_pre = my_cnt;  // exclusive prefix sum of the unit counts over the stencil lanes
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(FULL, my_pre, o);
+        if (lane >= o) my_pre += y;
+    }
+    const int n_scan = __shfl_sync(FULL, my_pre, 31);
+    my_pre -= my_cnt;
+
+    // flat scan over the candidate units of all stencil cells, 32 per batch
+    for (int f0 = 0; f0 < n_scan; f0 += 32) {
+        if (ncand + 32 > CAND_MAX) flush();
+        const int f = f0 + lane;
+        // stencil lane of flat index f: the largest c with prefix[c] <= f (binary search over the lanes' prefixes)
+        int c = 0;
+#pragma unroll
+        for (int step = 16; step > 0; step >>= 1) {
+            const int t = c + step;
+            const int pt = __shfl_sync(FULL, my_pre, t & 31);
+            if (t < 32 && pt <= f) c = t;
+        }
+        const int c_us = __shfl_sync(FULL, my_us, c), c_pre = __shfl_sync(FULL, my_pre, c), code = __shfl_sync(FULL, my_code, c);
+        const int v = c_us + (f - c_pre);
+        bool acc = false;
+        if (f < n_scan && v != U && owns(U, v, P.n_units)) {
+            const real4 co = code_off[code];
+            real4 lo = P.bb_lo[v], hi = P.bb_hi[v];
+            real gx = axis_gap<real, PBC>(ulo.x, uhi.x, lo.x + co.x, hi.x + co.x, P.L[0]);
+            real gy = axis_gap<real, PBC>(ulo.y, uhi.y, lo.y + co.y, hi.y + co.y, P.L[1]);
+            real gz = axis_gap<real, PBC>(ulo.z, uhi.z, lo.z + co.z, hi.z + co.z, P.L[2]);
+            acc = gx * gx + gy * gy + gz * gz < P.rnl2;
+        }
+        unsigned b = __ballot_sync(FULL, acc);
+        if (acc) {
+            int pos = ncand + __popc(b & lt_mask);
+            cand_unit[pos] = v;
+            cand_code[pos] = (unsigned char)code;
+        }
+        ncand += __popc(b);
+        __syncwarp();
+    }
     flush();
     __syncwarp();
 

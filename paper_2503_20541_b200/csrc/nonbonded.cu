@@ -77,10 +77,10 @@ int needs_rebuild_impl(Ctx* ctx, const void* pos, const void* ref, int64_t N, do
     if (blocks < 1) blocks = 1;
     if (ctx->precision == DIMOS_F64) {
         double h = 0.5 * skin;
-        needs_rebuild_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos, (const double*)ref, N, h * h, ctx->d_rebuild_state, flag_dev);
+        needs_rebuild_kernel<double><<<blocks, 256, 0, s>>>((const double*)pos, (const double*)ref, N, h * h, next_trigger_state(ctx), flag_dev);
     } else {
         float h = 0.5f * (float)skin;
-        needs_rebuild_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos, (const float*)ref, N, h * h, ctx->d_rebuild_state, flag_dev);
+        needs_rebuild_kernel<float><<<blocks, 256, 0, s>>>((const float*)pos, (const float*)ref, N, h * h, next_trigger_state(ctx), flag_dev);
     }
     DIMOS_LAUNCH_CHECK(ctx, "needs_rebuild");
     return DIMOS_OK;

@@ -65,3 +65,20 @@ def test_product_never_imports_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), f
                 assert "liboracle" not in text and "dimos_oracle" not in text, f
+
+
+def test_lj_table_fill_is_eq5_and_matches_the_oracle():
+    """dimos_lj_table_fill (host-only entry point, Eq. 5) against the oracle's Lorentz-Berthelot table
+    and against the rule written out: sigma_ab arithmetic mean, eps_ab geometric mean, symmetric."""
+    import numpy as np
+
+    import oracle
+
+    sigma, eps = [0.315061, 0.0, 0.25, 0.4], [0.6364, 0.0, 0.3, 1.2]
+    t = binding.dimos_lj_table_fill(sigma, eps).numpy()
+    assert np.allclose(t, oracle.lorentz_berthelot(sigma, eps), rtol=1e-15, atol=0)
+    assert t[0, 2, 0] == 0.5 * (0.315061 + 0.25) and t[0, 2, 1] == pytest.approx((0.6364 * 0.3) ** 0.5, rel=1e-15)
+    assert np.array_equal(t, t.transpose(1, 0, 2))
+    assert t[1, 1, 1] == 0.0 and t[0, 1, 1] == 0.0  # a type with eps = 0 has no LJ partner
+    with pytest.raises(binding.DimosError):
+        binding.dimos_lj_table_fill([0.3, -1.0], [0.1, 0.1])

@@ -42,7 +42,10 @@ def test_step_host_trajectory_matches_oracle_every_step(precision, method):
             h_F.fill_(float("nan"))
             h_E.fill_(float("nan"))
             h_W.fill_(float("nan"))
-            nl, rebuilt = ctx.step_host(nl, h_pos, h_charge, h_type, h_lj, wb.box, rc, skin, h_excl, h_F, h_E, h_W, method=method)
+            if step % 3 == 1:  # static inputs omitted: the list's device copies are used again
+                nl, rebuilt = ctx.step_host(nl, h_pos, None, None, None, wb.box, rc, skin, h_excl, h_F, h_E, h_W, method=method, ntypes=2)
+            else:
+                nl, rebuilt = ctx.step_host(nl, h_pos, h_charge, h_type, h_lj, wb.box, rc, skin, h_excl, h_F, h_E, h_W, method=method)
             if step == 0:
                 assert rebuilt, "the first call builds the list"
             else:
@@ -63,5 +66,8 @@ def test_step_host_trajectory_matches_oracle_every_step(precision, method):
         orc = oracle.nonbonded(p, 0.5 * wb.charge.astype(np.float64), wb.type, lj_np, wb.box, rc, method=ometh,
                                excl_pairs=wb.excl_pairs, band=BAND)
         check_nonbonded(h_F.numpy(), h_E.numpy(), h_W.numpy(), orc, precision)
+        # without a list there is nothing to reuse
+        with pytest.raises(dimos.DimosError):
+            ctx.step_host(None, h_pos, None, None, None, wb.box, rc, skin, h_excl, h_F, h_E, h_W, method=method, ntypes=2)
     finally:
         ctx.close()
