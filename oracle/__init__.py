@@ -15,4 +15,4 @@ from .dimos_oracle import (  # noqa: F401
     nonbonded,
     num_threads,
 )
-from .vv_oracle import K_B, berendsen, dispersion_correction, kinetic_energy, rattle_water_velocities, shake_water, vv_kick, vv_kick_drift  # noqa: F401,E402
+from .vv_oracle import K_B, berendsen, langevin_ou, dispersion_correction, kinetic_energy, rattle_water_velocities, shake_water, vv_kick, vv_kick_drift  # noqa: F401,E402

@@ -146,3 +146,17 @@ def berendsen(vel, mass, n_dof, T0, tau, dt):
     T = 2.0 * kinetic_energy(vel, mass) / (n_dof * K_B)
     lam = np.sqrt(1.0 + (dt / tau) * (T0 / T - 1.0))
     return np.asarray(vel, dtype=np.float64) * lam, T
+
+
+def langevin_ou(vel, mass, xi, gamma, dt, T):
+    """Langevin dynamics (PAPER.md:309 names it and gives no formula: reading C-26): the friction + noise part of the
+    Langevin equation dv = -gamma v dt + sqrt(2 gamma k_B T / m) dW integrated EXACTLY over one time step (the
+    Ornstein-Uhlenbeck update, applied where velocity Verlet has its step 7):
+        v <- a v + sqrt((1 - a^2) k_B T / m) xi,   a = exp(-gamma dt),
+    xi = one standard normal number per velocity component, passed in (both sides of the parity test read the same
+    array).  gamma in ps^-1, T in K, masses in amu, velocities in nm/ps.  Returns fp64 velocities."""
+    v = np.asarray(vel, dtype=np.float64)
+    m = np.asarray(mass, dtype=np.float64)[:, None]
+    x = np.asarray(xi, dtype=np.float64)
+    a = np.exp(-gamma * dt)
+    return a * v + np.sqrt((1.0 - a * a) * K_B * T / m) * x

@@ -707,3 +707,40 @@ def test_berendsen_thermostat_pins():
     assert 2.0 * oracle.kinetic_energy(one, mass) / (n_dof * oracle.K_B) == pytest.approx(T0, rel=1e-13)
     same, T_same = oracle.berendsen(v, mass, n_dof, T, tau, dt)
     assert np.array_equal(same, v) and T_same == T
+
+
+def test_langevin_ou_pins():
+    """Reading C-26: the exact Ornstein-Uhlenbeck velocity update.  Pins that do not re-type it: without
+    noise the velocity decays by exactly e^(-gamma t) over any number of steps (the velocity autocorrelation of free
+    Langevin dynamics); gamma = 0 leaves v unchanged and gamma -> infinity replaces it by a Maxwell-Boltzmann sample; the
+    Maxwell-Boltzmann distribution is stationary (variance k_B T / m kept exactly in expectation, checked by sampling);
+    from rest <v^2> relaxes as (k_B T / m)(1 - e^(-2 gamma t)); and <v(0) v(t)> over a sampled ensemble is e^(-gamma t)."""
+    rng = np.random.default_rng(12)
+    n = 200000
+    mass = np.where(np.arange(n) % 3 == 0, 15.9994, 1.008)
+    T, gamma, dt = 300.0, 5.0, 0.002
+    kT_m = oracle.K_B * T / mass[:, None]
+    v0 = rng.normal(size=(n, 3)) * np.sqrt(kT_m)
+    zero = np.zeros((n, 3))
+    v = v0.copy()
+    for _ in range(25):
+        v = oracle.langevin_ou(v, mass, zero, gamma, dt, T)
+    assert np.allclose(v, v0 * math.exp(-gamma * 25 * dt), rtol=1e-13, atol=0)
+    assert np.array_equal(oracle.langevin_ou(v0, mass, rng.normal(size=(n, 3)), 0.0, dt, T), v0)
+    xi = rng.normal(size=(n, 3))
+    assert np.allclose(oracle.langevin_ou(v0, mass, xi, 1e6, dt, T), np.sqrt(kT_m) * xi, rtol=1e-12, atol=1e-300)
+    # stationarity and relaxation from rest, in units of k_B T / m (standard error of the variance estimate ~ sqrt(2/3n))
+    v1 = oracle.langevin_ou(v0, mass, rng.normal(size=(n, 3)), gamma, dt, T)
+    assert ((v1**2) / kT_m).mean() == pytest.approx(1.0, abs=6 * math.sqrt(2.0 / (3 * n)))
+    v = zero.copy()
+    for k in range(1, 41):
+        v = oracle.langevin_ou(v, mass, rng.normal(size=(n, 3)), gamma, dt, T)
+        if k in (5, 20, 40):
+            assert ((v**2) / kT_m).mean() == pytest.approx(1.0 - math.exp(-2 * gamma * k * dt), abs=8 * math.sqrt(2.0 / (3 * n)))
+    # velocity autocorrelation over the ensemble
+    v = v0.copy()
+    for k in range(1, 31):
+        v = oracle.langevin_ou(v, mass, rng.normal(size=(n, 3)), gamma, dt, T)
+        if k in (10, 30):
+            c = ((v * v0) / kT_m).mean()
+            assert c == pytest.approx(math.exp(-gamma * k * dt), abs=8 / math.sqrt(3 * n))
