@@ -166,7 +166,8 @@ DIMOS_API int dimos_nl_needs_rebuild(dimos_ctx* ctx, const void* pos, const void
  * more than skin/2 since dimos_nl_build), which the caller checks with dimos_nl_needs_rebuild.
  *   pos      dev, N x 3
  *   charge   dev, N (e)
- *   type     dev, N int32 in [0, ntypes)
+ *   type     dev, N int32 in [0, ntypes); an index outside that range is evaluated as type 0 and reported as DIMOS_EINVAL by
+ *            the next call on this list that synchronises (dimos_nonbonded_host, dimos_step_host)
  *   lj_table dev, ntypes x ntypes x 2 doubles = (sigma_ab, eps_ab), symmetric (Eq. 5 filled by the
  *            caller, reading C-16); ntypes <= 64
  *   box      host, 3 doubles, must equal the build box (else DIMOS_ESTALE)
@@ -330,12 +331,21 @@ DIMOS_API int dimos_settle_velocities(dimos_ctx* ctx, const void* pos, void* vel
  *   n_dof      degrees of freedom, e.g. 3 N - 3 or, with rigid water, 6 n_w - 3
  *   ke_dev     dev, one double, written (the caller owns it)
  * The sum is accumulated in fp64 with one atomic per thread block: its last bits depend on the block order.
- * DIMOS_EINVAL unless T0 >= 0 and 0 < dt <= tau.  A system at rest (K = 0) has no temperature to rescale: velocities
- * become NaN, as the formula says. */
+ * DIMOS_EINVAL unless T0 >= 0 and 0 < dt <= tau.  A system at rest (K = 0) has no temperature to rescale: its
+ * velocities are left as they are (lambda = 1).  Atoms with inv_mass = 0 (frozen) carry no kinetic energy. */
 DIMOS_API int dimos_kinetic_energy(dimos_ctx* ctx, const void* vel, const void* inv_mass, int64_t N, double* ke_dev,
                                    double* ke_host, void* stream);
 DIMOS_API int dimos_berendsen(dimos_ctx* ctx, void* vel, const void* inv_mass, int64_t N, int64_t n_dof, double T0, double tau,
                               double dt, double* ke_dev, double* T_host, void* stream);
+/* dimos_langevin_ou -- Langevin dynamics (PAPER.md:309 names it and gives no formula: reading C-26): the friction + noise
+ * part of dv = -gamma v dt + sqrt(2 gamma k_B T / m) dW integrated exactly over one time step, applied where velocity Verlet
+ * has its step 7:   v <- a v + sqrt((1 - a^2) k_B T / m) xi,   a = exp(-gamma dt).
+ *   vel       dev, N x 3, in place;   inv_mass  dev, N (1 / m_i; 0 = frozen atom: its velocity only decays)
+ *   xi        dev, N x 3 standard normal numbers supplied by the caller (e.g. torch.randn on the device), same type
+ *   gamma     friction in ps^-1 (0: no-op up to rounding);   T in K;   k_B = 8.314462618e-3 kJ mol^-1 K^-1
+ * With rigid water the velocity constraints (dimos_settle_velocities) must be applied again afterwards. */
+DIMOS_API int dimos_langevin_ou(dimos_ctx* ctx, void* vel, const void* inv_mass, const void* xi, int64_t N, double gamma, double dt,
+                                double T, void* stream);
 /* dimos_berendsen_scale -- the rescaling half of dimos_berendsen with the kinetic energy taken from *ke_dev as some earlier
  * call on the same stream left it (dimos_kinetic_energy, dimos_water_kick_settle_velocities): one pass over vel, no sum. */
 DIMOS_API int dimos_berendsen_scale(dimos_ctx* ctx, void* vel, int64_t N, int64_t n_dof, double T0, double tau, double dt,
@@ -368,6 +378,8 @@ DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* ctx, const void* pos
  *   pairs   dev, n_exc x 2 int32, (i, j) with i < j, original atom indices; read (copied into the list)
  *   scale   dev, n_exc x 2 double, (s_c, s_lj) per pair; read (copied)
  *   n_exc   >= 0; 0 removes the exceptions.  The copy belongs to the list and survives rebuilds in place.
+ * The list is checked once here (indices in range, i < j, every pair among the list's excluded pairs: DIMOS_EINVAL
+ * otherwise); the call synchronises the stream.
  * Not checked: that the pairs are excluded pairs (the caller's precondition). */
 DIMOS_API int dimos_nl_set_exceptions(dimos_ctx* ctx, dimos_nl* nl, const int32_t* pairs, const double* scale,
                                       int64_t n_exc, void* stream);

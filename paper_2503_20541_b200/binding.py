@@ -32,7 +32,7 @@ EXPORTED_SYMBOLS = (
     "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box",
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
     "dimos_kinetic_energy", "dimos_berendsen", "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities",
-    "dimos_berendsen_scale", "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill",
+    "dimos_berendsen_scale", "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill", "dimos_langevin_ou",
 )
 
 
@@ -112,6 +112,7 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_pme_recip.argtypes = [vp, vp, vp, i64, ctypes.POINTER(dbl), dbl, ctypes.POINTER(i32), i32, dbl, vp, i32, vp, vp, vp]
     lib.dimos_pme_mesh_size.argtypes = [dbl, ctypes.POINTER(dbl), dbl, ctypes.POINTER(i32)]
     lib.dimos_lj_table_fill.argtypes = [vp, vp, i32, vp]
+    lib.dimos_langevin_ou.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, vp]
     lib.dimos_profile_enable.argtypes = [vp, ctypes.c_int]
     lib.dimos_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(i64)]
     lib.dimos_nl_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
@@ -129,7 +130,7 @@ def load_library() -> ctypes.CDLL:
                  "dimos_nl_set_exceptions", "dimos_vv_kick_drift", "dimos_vv_kick", "dimos_nl_export_edges", "dimos_virtual_box", "dimos_dispersion_correction",
                  "dimos_settle", "dimos_settle_velocities", "dimos_kinetic_energy", "dimos_berendsen",
                  "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities", "dimos_berendsen_scale",
-                 "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill"):
+                 "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill", "dimos_langevin_ou"):
         getattr(lib, name).restype = ctypes.c_int
     _lib_handle = lib
     return lib
@@ -256,16 +257,17 @@ class Context:
             return nl
         return NeighborList(h, self, pos_at_build, boxt, float(r_cut), float(skin))
 
-    def nl_needs_rebuild(self, pos, pos_at_build, skin, sync: bool = True):
+    def nl_needs_rebuild(self, pos, pos_at_build, skin, sync: bool = True, flag=None):
         """dimos_nl_needs_rebuild: bool when sync=True, else the device flag tensor (no host sync)."""
         pos = self._dev(pos, self.real, 3)
         ref = self._dev(pos_at_build, self.real, 3)
         host = ctypes.c_int32(0)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_nl_needs_rebuild(self.handle, pos.data_ptr(), ref.data_ptr(), pos.shape[0], float(skin),
-                                                 self._flag.data_ptr(), ctypes.byref(host) if sync else None, _stream_ptr())
+                                                 (flag if flag is not None else self._flag).data_ptr(),
+                                                 ctypes.byref(host) if sync else None, _stream_ptr())
         self._check(rc)
-        return bool(host.value) if sync else self._flag
+        return bool(host.value) if sync else (flag if flag is not None else self._flag)
 
     def _params(self, nl, method, eps_rf, alpha, coulomb_const, r_switch=0.0):
         return _Params(float(nl.r_cut), float(eps_rf), float(alpha), float(coulomb_const),
@@ -412,6 +414,16 @@ class Context:
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_vv_kick(self.handle, vel.data_ptr(), F.data_ptr(), inv_mass.data_ptr(), vel.shape[0], float(dt),
                                         _stream_ptr())
+        self._check(rc)
+
+    def langevin_ou(self, vel, inv_mass, xi, gamma, dt, T):
+        """dimos_langevin_ou: exact Ornstein-Uhlenbeck velocity update in place on vel with the caller's normal numbers xi."""
+        vel = self._dev(vel, self.real, 3)
+        inv_mass = self._dev(inv_mass, self.real)
+        xi = self._dev(xi, self.real, 3)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_langevin_ou(self.handle, vel.data_ptr(), inv_mass.data_ptr(), xi.data_ptr(), vel.shape[0], float(gamma),
+                                            float(dt), float(T), _stream_ptr())
         self._check(rc)
 
     def settle(self, pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=None, dt=0.0):
@@ -595,8 +607,9 @@ def dimos_nl_build(ctx: Context, pos, box, r_cut, skin, excl_pairs=None, pos_at_
     return ctx.nl_build(pos, box, r_cut, skin, excl_pairs, pos_at_build, nl)
 
 
-def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = True):
-    return ctx.nl_needs_rebuild(pos, pos_at_build, skin, sync)
+def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = True, flag=None):
+    """flag: int32 device tensor of one element to receive the result (default: one shared by the context's calls)."""
+    return ctx.nl_needs_rebuild(pos, pos_at_build, skin, sync, flag)
 
 
 def dimos_nonbonded(ctx: Context, nl: NeighborList, pos, charge, type_, lj_table, **kw):
@@ -630,6 +643,10 @@ def dimos_vv_kick_drift(ctx: Context, pos, vel, F, inv_mass, dt, **kw):
 
 def dimos_vv_kick(ctx: Context, vel, F, inv_mass, dt):
     return ctx.vv_kick(vel, F, inv_mass, dt)
+
+
+def dimos_langevin_ou(ctx: Context, vel, inv_mass, xi, gamma, dt, T):
+    return ctx.langevin_ou(vel, inv_mass, xi, gamma, dt, T)
 
 
 def dimos_settle(ctx: Context, pos_old, pos, water, m_O, m_H, d_OH, d_HH, vel=None, dt=0.0):

@@ -537,6 +537,18 @@ DIMOS_API int dimos_berendsen_scale(dimos_ctx* c, void* vel, int64_t N, int64_t 
     return berendsen_scale_impl(ctx, vel, N, ke_dev, 2.0 / ((double)n_dof * 8.314462618e-3), T0, dt / tau, (cudaStream_t)stream);
 }
 
+DIMOS_API int dimos_langevin_ou(dimos_ctx* c, void* vel, const void* inv_mass, const void* xi, int64_t N, double gamma, double dt,
+                                double T, void* stream)
+{
+    if (!c) return DIMOS_EINVAL;
+    Ctx* ctx = reinterpret_cast<Ctx*>(c);
+    if (!vel || !inv_mass || !xi) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (N <= 0 || !(gamma >= 0) || !(dt > 0) || !(T >= 0) || !std::isfinite(gamma) || !std::isfinite(dt) || !std::isfinite(T))
+        return set_error(ctx, DIMOS_EINVAL, "need N > 0, gamma >= 0, dt > 0, T >= 0");
+    if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
+    return langevin_ou_impl(ctx, vel, inv_mass, xi, N, gamma, dt, T, (cudaStream_t)stream);
+}
+
 static int check_nb_args(Ctx* ctx, const NL* nl, int32_t ntypes, const double* box, const dimos_nb_params* p)
 {
     if (!list_belongs(ctx, nl)) return set_error(ctx, DIMOS_EINVAL, "list does not belong to this context");
@@ -598,7 +610,9 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* c, dimos_nl* l, const void* pos_ho
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(F_host, nl->st_F.p, 3 * N * rs, cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(E_host, EW, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
     if (virial_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(virial_host, EW + 4, 9 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 35, (int*)nl->flags.p + 9, sizeof(int), cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    if (ctx->h_pinned[35]) return set_error(ctx, DIMOS_EINVAL, "type index out of range [0, ntypes)");
     return DIMOS_OK;
 }
 
@@ -701,7 +715,9 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(F_host, nl->st_F.p, 3 * (size_t)N * rs, cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(E_host, EW, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
     if (virial_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(virial_host, EW + 4, 9 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 35, (int*)nl->flags.p + 9, sizeof(int), cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    if (ctx->h_pinned[35]) return set_error(ctx, DIMOS_EINVAL, "type index out of range [0, ntypes)");
     return DIMOS_OK;
 }
 
@@ -759,8 +775,17 @@ DIMOS_API int dimos_nl_set_exceptions(dimos_ctx* c, dimos_nl* l, const int32_t* 
     int rc;
     if ((rc = ensure(ctx, nl->exc_pairs, (size_t)n_exc * 2 * sizeof(int32_t), s))) return rc;
     if ((rc = ensure(ctx, nl->exc_scale, (size_t)n_exc * 2 * sizeof(double), s))) return rc;
+    if (nl->N <= 0 || !nl->flags.p) return set_error(ctx, DIMOS_ESTALE, "build the list before setting its exceptions");
+    // every pair must be in range, i < j, and also an excluded pair (reading C-21): checked here, once
+    int* bad = (int*)nl->flags.p + 10;
+    DIMOS_CUDA_TRY(ctx, cudaMemsetAsync(bad, 0, sizeof(int), s));
+    if ((rc = check_exceptions_impl(ctx, nl, pairs, n_exc, bad, s))) return rc;
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 34, bad, sizeof(int), cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->exc_pairs.p, pairs, (size_t)n_exc * 2 * sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->exc_scale.p, scale, (size_t)n_exc * 2 * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    if (ctx->h_pinned[34] & 1) return set_error(ctx, DIMOS_EINVAL, "exception pair out of range or not i < j");
+    if (ctx->h_pinned[34] & 2) return set_error(ctx, DIMOS_EINVAL, "every exception pair must also be an excluded pair of this list");
     nl->n_exc = n_exc;
     return DIMOS_OK;
 }

@@ -110,7 +110,8 @@ struct NL {
     DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, nA | nM << 16}: the row is nA mask-free
                        // chunks, then nM chunks that need their masks, then the remaining mask-free chunks (after
                        // reorder_rows: nA = chunks of j-atoms with LJ partners, the trailing ones have none)
-    DevBuf flags;      // int[8]: [0] error flags, [1] max cell count, [2..3] entry counters (u64), [4..5] padded
+    DevBuf flags;      // int[16]: [0] error flags, [1] max cell count, [2..3] entry counters (u64), [4..5] padded, [6..7] needed
+                       // capacities, [8] row order stale (an atom became LJ-active), [9] type index out of range, [10] exception check
     // per-step device arrays
     DevBuf xyzq;       // real4[n_slots]
     DevBuf stype;      // int[n_slots]
@@ -158,6 +159,7 @@ int nonbonded_impl(Ctx* ctx, NL* nl, const void* pos, const void* charge, const 
                    const double* lj_table, int32_t ntypes, const dimos_nb_params* prm, void* F, double* E,
                    double* virial, cudaStream_t s);
 int probe_fp32_impl(Ctx* ctx, double ms_target, double* tflops, cudaStream_t s);
+int check_exceptions_impl(Ctx* ctx, const NL* nl, const int32_t* pairs, int64_t n_exc, int* bad_dev, cudaStream_t s);
 int pme_recip_impl(Ctx* ctx, const void* pos, const void* charge, int64_t n, const double* box, double alpha, const int32_t* mesh,
                    int32_t order, double ke, void* F, double* E, double* W, int accumulate, cudaStream_t s);
 void pme_release(Ctx* ctx);
@@ -167,6 +169,7 @@ int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStrea
 int type_histogram_impl(Ctx* ctx, const int32_t* type, int64_t N, int nt, unsigned long long* counts_dev, int* bad_dev,
                         cudaStream_t s);
 int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, cudaStream_t s);
+int langevin_ou_impl(Ctx* ctx, void* vel, const void* inv_mass, const void* xi, int64_t N, double gamma, double dt, double T, cudaStream_t s);
 int settle_impl(Ctx* ctx, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w, double m_O,
                 double m_H, double d_OH, double d_HH, double dt, cudaStream_t s);
 int water_step_a_impl(Ctx* ctx, void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O, double m_H,

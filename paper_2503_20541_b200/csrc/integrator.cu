@@ -98,9 +98,9 @@ __device__ __forceinline__ void settle_molecule(const real* b0, const real* c0, 
     const real xc1 = dot(c1, X), yc1 = dot(c1, Y), zc1 = dot(c1, Z);
     // tilt angles from the unchanged normal components
     const real sinphi = za1 / ra;
-    const real cosphi = sqrt((real)1 - sinphi * sinphi);
+    const real cosphi = sqrt(fmax((real)1 - sinphi * sinphi, (real)0));  // a molecule distorted beyond recovery gives 0, not NaN
     const real sinpsi = (zb1 - zc1) / ((real)2 * rc * cosphi);
-    const real cospsi = sqrt((real)1 - sinpsi * sinpsi);
+    const real cospsi = sqrt(fmax((real)1 - sinpsi * sinpsi, (real)0));
     const real ya2 = ra * cosphi;
     real xb2 = -rc * cospsi;
     const real yb2 = -rb * cosphi - rc * sinpsi * sinphi;
@@ -114,7 +114,7 @@ __device__ __forceinline__ void settle_molecule(const real* b0, const real* c0, 
     const real gamma = xb0 * yb1 - xb1 * yb0 + xc0 * yc1 - xc1 * yc0;
     const real al2be2 = alpha * alpha + beta * beta;
     const real sintheta = (alpha * gamma - beta * sqrt(fmax(al2be2 - gamma * gamma, (real)0))) / al2be2;
-    const real costheta = sqrt((real)1 - sintheta * sintheta);
+    const real costheta = sqrt(fmax((real)1 - sintheta * sintheta, (real)0));
     const real a3[3] = {-ya2 * sintheta, ya2 * costheta, za1};
     const real b3[3] = {xb2 * costheta - yb2 * sintheta, xb2 * sintheta + yb2 * costheta, zb1};
     const real c3[3] = {-xb2 * costheta - yc2 * sintheta, -xb2 * sintheta + yc2 * costheta, zc1};
@@ -300,7 +300,8 @@ __global__ void kinetic_energy_kernel(const real* __restrict__ vel, const real* 
     double acc = 0.0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
         const real vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
-        acc += (double)(vx * vx + vy * vy + vz * vz) / (double)inv_mass[i];
+        const real im = inv_mass[i];
+        if (im > (real)0) acc += (double)(vx * vx + vy * vy + vz * vz) / (double)im;  // inv_mass = 0: a frozen atom, no kinetic energy
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -432,6 +433,30 @@ int vv_kick_drift_impl(Ctx* ctx, void* pos, void* vel, const void* F, const void
     if (ctx->precision == DIMOS_F64) launch_kick_drift<double>(ctx, pos, vel, F, inv_mass, N, dt, pos_at_build, skin, flag_dev, s);
     else launch_kick_drift<float>(ctx, pos, vel, F, inv_mass, N, dt, pos_at_build, skin, flag_dev, s);
     DIMOS_LAUNCH_CHECK(ctx, "vv_kick_drift");
+    return DIMOS_OK;
+}
+
+// Langevin dynamics, reading C-26: exact Ornstein-Uhlenbeck velocity update v <- a v + sqrt((1 - a^2) k_B T / m) xi
+template <typename real>
+__global__ void langevin_ou_kernel(real* __restrict__ vel, const real* __restrict__ inv_mass, const real* __restrict__ xi, int64_t N,
+                                   real a, real b2 /* (1 - a^2) k_B T */)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
+        const real sg = sqrt(b2 * inv_mass[i]);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) vel[3 * i + c] = a * vel[3 * i + c] + sg * xi[3 * i + c];
+    }
+}
+
+int langevin_ou_impl(Ctx* ctx, void* vel, const void* inv_mass, const void* xi, int64_t N, double gamma, double dt, double T, cudaStream_t s)
+{
+    const int blocks = grid_for(ctx, N);
+    const double a = exp(-gamma * dt), b2 = (1.0 - a * a) * 8.314462618e-3 * T;
+    if (ctx->precision == DIMOS_F64)
+        langevin_ou_kernel<double><<<blocks, 256, 0, s>>>((double*)vel, (const double*)inv_mass, (const double*)xi, N, a, b2);
+    else
+        langevin_ou_kernel<float><<<blocks, 256, 0, s>>>((float*)vel, (const float*)inv_mass, (const float*)xi, N, (float)a, (float)b2);
+    DIMOS_LAUNCH_CHECK(ctx, "langevin_ou");
     return DIMOS_OK;
 }
 

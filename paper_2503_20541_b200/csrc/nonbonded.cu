@@ -115,7 +115,11 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
         const double y = (double)pos[3 * (int64_t)o + 1] - ref[3 * s + 1];
         const double z = (double)pos[3 * (int64_t)o + 2] - ref[3 * s + 2];
         xyzq[s] = mk4((real)x, (real)y, (real)z, pad ? (real)0 : charge[o]);
-        const int t = type[o];
+        int t = type[o];
+        if (t < 0 || t >= nt) {  // reported by the next synchronising call on this list; evaluated as type 0 meanwhile
+            atomicOr(order_stale + 1, 1);
+            t = 0;
+        }
         const int st = t | (act_sh[t] ? STYPE_ACTIVE : 0);  // bit 30: the atom has LJ partners
         // the rows were ordered by this bit (reorder_rows): if it changes for any atom, the pair kernel is told to
         // evaluate LJ in every chunk until the next build
@@ -475,6 +479,27 @@ __global__ void exceptions_kernel(const int2* __restrict__ pairs, const double2*
             for (int ww = 0; ww < (int)(blockDim.x >> 5); ++ww) sum += sh[ww][threadIdx.x];
         partials[(int64_t)blockIdx.x * N_PART + threadIdx.x] = sum;
     }
+}
+
+// setup-time check of a 1-4 exception list: indices in range, i < j, and every pair also in the exclusion list (C-21)
+__global__ void check_exceptions_kernel(const int2* __restrict__ pairs, int64_t n_exc, int64_t N, const int* __restrict__ excl_start,
+                                        const int* __restrict__ excl_adj, int* __restrict__ bad)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_exc) return;
+    const int2 p = pairs[k];
+    if (p.x < 0 || p.y < 0 || p.x >= N || p.y >= N || p.x >= p.y) { atomicOr(bad, 1); return; }
+    bool found = false;
+    for (int e = excl_start[p.x]; e < excl_start[p.x + 1]; ++e) found = found || excl_adj[e] == p.y;
+    if (!found) atomicOr(bad, 2);
+}
+
+int check_exceptions_impl(Ctx* ctx, const NL* nl, const int32_t* pairs, int64_t n_exc, int* bad_dev, cudaStream_t s)
+{
+    check_exceptions_kernel<<<(unsigned)((n_exc + 255) / 256), 256, 0, s>>>((const int2*)pairs, n_exc, nl->N, (const int*)nl->excl_start.p,
+                                                                            (const int*)nl->excl_adj.p, bad_dev);
+    DIMOS_LAUNCH_CHECK(ctx, "check_exceptions");
+    return DIMOS_OK;
 }
 
 // ------------------------------------------------------------------------------------------------

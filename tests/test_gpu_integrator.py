@@ -419,3 +419,34 @@ def test_thermostatted_rigid_water_loop():
         r = x[:, i] - x[:, j]
         assert np.abs(np.linalg.norm(r, axis=1) - d).max() < 3e-6
         assert np.abs(((v[:, i] - v[:, j]) * r).sum(1) / d).max() < 2e-5 * np.abs(v).max()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("n", [1, 1000, 300001])
+def test_langevin_ou_matches_oracle(precision, n):
+    """dimos_langevin_ou (reading C-26) against the numpy oracle on the same velocities, masses and normal
+    numbers, element by element; gamma = 0 returns the input; a frozen atom (inv_mass = 0) only decays."""
+    rng = np.random.default_rng(900 + n)
+    np_real = np.float64 if precision == "f64" else np.float32
+    mass = rng.choice(np.array([15.9994, 1.008]), size=n)
+    inv_m = (1.0 / mass).astype(np_real)
+    v = (rng.normal(size=(n, 3)) * np.sqrt(oracle.K_B * 300.0 / mass)[:, None]).astype(np_real)
+    xi = rng.normal(size=(n, 3)).astype(np_real)
+    gamma, dt, T = 5.0, 0.002, 310.0
+    want = oracle.langevin_ou(v, 1.0 / inv_m.astype(np.float64), xi, gamma, dt, T)
+    dev = torch.device("cuda", 0)
+    with dimos.Context(0, precision) as ctx:
+        vd = torch.from_numpy(v.copy()).to(dev)
+        dimos.dimos_langevin_ou(ctx, vd, torch.from_numpy(inv_m).to(dev), torch.from_numpy(xi).to(dev), gamma, dt, T)
+        got = vd.cpu().numpy().astype(np.float64)
+        scale = np.abs(want).max()
+        assert np.abs(got - want).max() <= (1e-14 if precision == "f64" else 4e-7) * scale
+        v0 = torch.from_numpy(v.copy()).to(dev)
+        dimos.dimos_langevin_ou(ctx, v0, torch.from_numpy(inv_m).to(dev), torch.from_numpy(xi).to(dev), 0.0, dt, T)
+        assert np.array_equal(v0.cpu().numpy(), v)
+        frozen = torch.zeros(n, dtype=vd.dtype, device=dev)
+        vf = torch.from_numpy(v.copy()).to(dev)
+        dimos.dimos_langevin_ou(ctx, vf, frozen, torch.from_numpy(xi).to(dev), gamma, dt, T)
+        assert np.allclose(vf.cpu().numpy(), v * np.exp(-gamma * dt), rtol=1e-6, atol=0)
+        with pytest.raises(dimos.DimosError):
+            dimos.dimos_langevin_ou(ctx, vd, torch.from_numpy(inv_m).to(dev), torch.from_numpy(xi).to(dev), -1.0, dt, T)

@@ -560,3 +560,63 @@ def test_config4_water100k_ewald_whole_system(precision):
     wb = wl.make_config(4)
     rep = run_case(wb, precision, 1.0, 0.1, "ewald", alpha=3.12, on_device=True)
     assert rep["stats"]["n_cells"] == (13, 13, 13) and rep["stats"]["pbc_mode"] == 0
+
+
+def test_invalid_types_and_exception_lists_are_reported():
+    """a type index outside [0, ntypes) and an exception pair that is not an excluded pair return DIMOS_EINVAL
+    instead of garbage (types: at the next synchronising call on the list; exceptions: when they are set)."""
+    wb = wl.make_config(0)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 0.9, 0.1, db.excl)
+        good = db.excl[:5].clone()
+        scale = torch.full((5, 2), 0.5, dtype=torch.float64, device="cuda")
+        dimos.dimos_nl_set_exceptions(ctx, nl, good, scale)
+        bad = good.clone()
+        bad[2, 1] = bad[2, 0] + 5  # (O of one molecule, an atom of the next): in range, i < j, not excluded
+        with pytest.raises(dimos.DimosError) as ei:
+            dimos.dimos_nl_set_exceptions(ctx, nl, bad, scale)
+        assert ei.value.status == -1
+        bad[2, 1] = wb.n_atoms
+        with pytest.raises(dimos.DimosError):
+            dimos.dimos_nl_set_exceptions(ctx, nl, bad, scale)
+        dimos.dimos_nl_set_exceptions(ctx, nl, good[:0], scale[:0])
+        # out-of-range type through the host entry point
+        n = wb.n_atoms
+        h = dict(pos=torch.from_numpy(wb.pos).pin_memory(), charge=torch.from_numpy(wb.charge).pin_memory(),
+                 lj=torch.from_numpy(db.lj_np).pin_memory(), F=torch.empty((n, 3)).pin_memory(),
+                 E=torch.empty(4, dtype=torch.float64).pin_memory(), W=torch.empty((3, 3), dtype=torch.float64).pin_memory())
+        t_bad = torch.from_numpy(wb.type.copy())
+        t_bad[17] = 2
+        with pytest.raises(dimos.DimosError) as ei:
+            ctx.nonbonded_host(nl, h["pos"], h["charge"], t_bad.pin_memory(), h["lj"], h["F"], h["E"], h["W"])
+        assert ei.value.status == -1
+    finally:
+        ctx.close()
+
+
+def test_needs_rebuild_on_two_streams_at_once():
+    """Two trigger evaluations in flight on different streams: each has its own reduction state, so
+    neither sees the other's partial maximum or ticket count."""
+    n = 2_000_000
+    g = torch.Generator(device="cuda").manual_seed(3)
+    ref = torch.rand((n, 3), device="cuda", generator=g) * 20
+    moved = ref.clone()
+    moved[n - 7, 1] += 0.2       # beyond skin/2 = 0.05
+    still = ref + 1e-3
+    ctx = dimos.Context(0, "f32")
+    try:
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        f1 = torch.zeros(1, dtype=torch.int32, device="cuda")
+        f2 = torch.zeros(1, dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        for _ in range(20):
+            with torch.cuda.stream(s1):
+                dimos.dimos_nl_needs_rebuild(ctx, moved, ref, 0.1, sync=False, flag=f1)
+            with torch.cuda.stream(s2):
+                dimos.dimos_nl_needs_rebuild(ctx, still, ref, 0.1, sync=False, flag=f2)
+            torch.cuda.synchronize()
+            assert int(f1.item()) == 1 and int(f2.item()) == 0
+    finally:
+        ctx.close()
