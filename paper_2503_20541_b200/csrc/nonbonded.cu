@@ -47,6 +47,39 @@ __device__ __forceinline__ double erf_r(double x) { return erf(x); }
 __device__ __forceinline__ float exp_r(float x) { return expf(x); }
 __device__ __forceinline__ double exp_r(double x) { return exp(x); }
 
+__constant__ double ERFC_CHEB[28] = {
+#include "erfc_cheb.inc"
+};
+constexpr double ERFC_CHEB_XMAX = 3.6;
+// erfc(x) and exp(-x^2), x >= 0.  fp64 with `fast`: erfc(x) = g(x) exp(-x^2), g = erfc(x) exp(x^2) from its degree-27
+// Chebyshev series on [0, 3.6] (Clenshaw recurrence, 6e-16 relative; the host sets `fast` only when alpha r_cut <= 3.6, and
+// larger arguments belong to slots beyond the cutoff, whose result is discarded: they are clamped).  One exp instead of
+// libm's erfc + exp: the fp64 Ewald pair kernel spent most of its time there.
+__device__ __forceinline__ void erfc_exp_r(float x, bool, float& erfc_x, float& ex)
+{
+    erfc_x = erfcf(x);
+    ex = expf(-x * x);
+}
+__device__ __forceinline__ void erfc_exp_r(double x, bool fast, double& erfc_x, double& ex)
+{
+    if (!fast) {
+        erfc_x = erfc(x);
+        ex = exp(-x * x);
+        return;
+    }
+    const double xc = fmin(x, ERFC_CHEB_XMAX);
+    ex = exp(-xc * xc);
+    const double t2 = 2.0 * (2.0 * xc - ERFC_CHEB_XMAX) / ERFC_CHEB_XMAX;  // 2 t, t in [-1, 1]
+    double b1 = 0.0, b2 = 0.0;
+#pragma unroll
+    for (int j = 27; j >= 1; --j) {
+        const double b0 = fma(t2, b1, ERFC_CHEB[j] - b2);
+        b2 = b1;
+        b1 = b0;
+    }
+    erfc_x = (fma(0.5 * t2, b1, ERFC_CHEB[0] - b2)) * ex;
+}
+
 // ------------------------------------------------------------------------------------------------
 // A3: rebuild trigger
 // ------------------------------------------------------------------------------------------------
@@ -173,8 +206,8 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
         } else {                                                                                     \
             const real r = r2 * rinv;                                                                \
             const real ar = P.alpha * r;                                                             \
-            const real erfc_ar = erfc_r(ar);                                                         \
-            const real ex = exp_r(-ar * ar);                                                         \
+            real erfc_ar, ex;                                                                        \
+            erfc_exp_r(ar, P.erfc_fast != 0, erfc_ar, ex);                                           \
             const real qr = qq * rinv;                                                               \
             e_c = fma_acc(qr, erfc_ar, e_c);                    /* Eq. 10, n = 0 */                  \
             fr2 = fma_r(qq * P.two_a_sqrtpi, ex, qr * erfc_ar);                                      \
@@ -252,6 +285,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
     // to ~1e-4 of the sum of magnitudes, below what fp32 pair terms resolve, so in fp32 mode the pair
     // ENERGY of such boxes is evaluated in fp64 from the same fp32 inputs; forces and virial stay fp32.
     constexpr bool E64 = PBC == 1 && sizeof(real) == 4 && sizeof(acc_t) == 4;
+    const bool lj_all = *P.order_stale != 0;  // an atom became LJ-active after the rows were ordered: LJ in every chunk
 
     // dynamic unit scheduling: every warp draws unit indices from one global counter, so no warp
     // waits for another (rows differ in length) and the tail is at most one unit long
@@ -312,10 +346,12 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const unsigned mask = plain ? 0xFFu : m;
             real fjx = 0, fjy = 0, fjz = 0;
 
+            // after reorder_rows only the chunks in front of and inside the masked region hold j-atoms with LJ partners
+            const bool lj_chunk = lj_all || c < n_a + (int)n_m;
             if (plain) {
 #pragma unroll
                 for (int i = 0; i < UNIT; ++i) {
-                    if (ti[i] >= 0) DIMOS_SLOT(i, true, false);
+                    if (ti[i] >= 0 && lj_chunk) DIMOS_SLOT(i, true, false);
                     else DIMOS_SLOT(i, false, false);
                 }
             } else {
@@ -650,6 +686,10 @@ static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P,
     if constexpr (std::is_same<real, float>::value && std::is_same<acc_t, float>::value) {
         if (use_f32x2(ctx, nl, method)) done = launch_pair_force_f32x2(P, method, nb, dyn, s);
     }
+    if constexpr (std::is_same<real, double>::value) {
+        static const bool generic64 = [] { const char* e = getenv("DIMOS_PAIR_KERNEL"); return e && std::string(e) == "generic"; }();
+        if (!generic64) done = launch_pair_force_f64(P, method, pbc, nb, s);
+    }
     if (done) {}
     else if (method == DIMOS_RF) { if (pbc == 0) DIMOS_PF(DIMOS_RF, 0); else DIMOS_PF(DIMOS_RF, 1); }
     else { if (pbc == 0) DIMOS_PF(DIMOS_EWALD_REAL, 0); else DIMOS_PF(DIMOS_EWALD_REAL, 1); }
@@ -671,7 +711,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     const bool fx = sizeof(real) == 4 && use_f32x2(ctx, nl, prm->method);
     const int wpb = fx ? FX_WARPS : PF_WARPS;  // warps per CTA
     const unsigned nb_full = (unsigned)((nun + wpb - 1) / wpb);
-    const unsigned nb_res = (unsigned)ctx->sm_count * (fx ? (unsigned)FX_CTAS_PER_SM : (sizeof(real) == 4 ? 2u : 1u));
+    const unsigned nb_res = (unsigned)ctx->sm_count * (fx ? (unsigned)FX_CTAS_PER_SM : 2u);
     const unsigned nb_force = nb_full < nb_res ? nb_full : nb_res;
     const size_t n_force_rows = (size_t)nb_force * wpb;  // one fp64 partial row per warp
     const bool ewald = prm->method == DIMOS_EWALD_REAL;
@@ -724,6 +764,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     P.d_inv_sw = P.sw_on ? 1.0 / (rc_ - prm->r_switch) : 0.0;
     for (int a = 0; a < 3; ++a) P.d_L[a] = nl->grid.L[a];
     P.alpha = (real)prm->alpha;
+    P.erfc_fast = (prm->alpha * rc_ <= ERFC_CHEB_XMAX) ? 1 : 0;
     P.two_a_sqrtpi = (real)(2.0 * prm->alpha / sqrt(M_PI));
     for (int a = 0; a < 3; ++a) { P.L[a] = (real)nl->grid.L[a]; P.invL[a] = (real)(1.0 / nl->grid.L[a]); P.h[a] = (real)nl->grid.h[a]; }
     const size_t dyn = (size_t)nt * nt * sizeof(real4);

@@ -49,6 +49,7 @@ struct ForceParams {
     real rc2, ke, krf, m2krf, crf, alpha, two_a_sqrtpi;
     real rs, inv_sw;  // LJ switch (Eq. 6): r_s and 1/(r_c - r_s)
     int sw_on;
+    int erfc_fast;  // fp64 Ewald: alpha r_cut <= 3.6, erfc from the Chebyshev series (nonbonded.cu)
     // fp64 copies for the energy of small fp32 boxes (generic kernel, per-pair minimum image)
     double d_ke, d_krf, d_crf, d_alpha, d_rs, d_inv_sw, d_L[3];
     real L[3], invL[3], h[3];
@@ -86,6 +87,8 @@ __device__ __forceinline__ T reduce8_scatter(T (&v)[8], int lane)
 // packed-FP32 pair kernel (pair_f32x2.cu); returns false when the case is not covered (caller uses the generic kernel)
 void launch_reorder_rows(unsigned* entry, unsigned char* emask, int2* row_info, const int* stype, int64_t n_units,
                          int row_cap, int m_res, cudaStream_t s);
+// rolled fp64 kernel (pair_f64.cu); false = not covered
+bool launch_pair_force_f64(const ForceParams<double>& P, int method, int pbc, unsigned nb, cudaStream_t s);
 bool launch_pair_force_f32x2(const ForceParams<float>& P, int method, unsigned nb, size_t dyn, cudaStream_t s);
 
 }  // namespace dimos
