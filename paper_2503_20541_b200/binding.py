@@ -163,7 +163,10 @@ class NeighborList:
 class Context:
     """One library context: device + precision + torch-backed allocator."""
 
-    def __init__(self, device: int = 0, precision: str = "f32", torch_allocator: bool = True):
+    def __init__(self, device: int = 0, precision: str = "f32", torch_allocator: bool = True, guard_bytes: int = 0):
+        """guard_bytes > 0 (a multiple of 256): every workspace block the library asks for is allocated with that many
+        bytes of 0xA5 in front of and behind it; check_guards() reports blocks whose guards were overwritten (the
+        out-of-bounds-write check of tests/test_gpu_guards.py; compute-sanitizer is not available on every pool)."""
         if not torch.cuda.is_available():
             raise RuntimeError("dimos_b200 needs a CUDA device: there is no CPU fallback")
         self.lib = load_library()
@@ -172,19 +175,29 @@ class Context:
         self.real = torch.float64 if precision == "f64" else torch.float32
         self._blocks: dict[int, torch.Tensor] = {}
         self._alloc_struct = None
+        self._guard = int(guard_bytes)
+        self._guard_violations: list[tuple[int, int]] = []
+        if self._guard % 256 != 0:
+            raise ValueError("guard_bytes must be a multiple of 256")
         if torch_allocator:
             dev = torch.device("cuda", self.device)
 
             def _alloc(nbytes, _stream, _user):
+                g = self._guard
                 try:
-                    t = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+                    t = torch.empty(int(nbytes) + 2 * g, dtype=torch.uint8, device=dev)
+                    if g:
+                        t[:g] = 0xA5
+                        t[g + int(nbytes):] = 0xA5
                 except Exception:
                     return None
-                self._blocks[t.data_ptr()] = t
-                return t.data_ptr()
+                self._blocks[t.data_ptr() + g] = t
+                return t.data_ptr() + g
 
             def _free(ptr, _user):
-                self._blocks.pop(int(ptr), None)
+                t = self._blocks.pop(int(ptr), None)
+                if t is not None and self._guard:
+                    self._check_block(int(ptr), t)
 
             self._alloc_cb = _ALLOC_FN(_alloc)
             self._free_cb = _FREE_FN(_free)
@@ -211,6 +224,25 @@ class Context:
         if shape_last is not None and (t.dim() != 2 or t.shape[1] != shape_last):
             raise ValueError(f"expected shape (N, {shape_last})")
         return t
+
+    def _check_block(self, ptr: int, t: torch.Tensor):
+        g = self._guard
+        torch.cuda.synchronize(self.device)
+        bad = int((t[:g] != 0xA5).sum()) + int((t[t.numel() - g:] != 0xA5).sum())
+        if bad:
+            self._guard_violations.append((t.numel() - 2 * g, bad))
+
+    def check_guards(self) -> list:
+        """(block size, overwritten guard bytes) of every workspace block, live or freed, whose guards were touched."""
+        if not self._guard:
+            raise RuntimeError("context was created without guard_bytes")
+        live = list(self._guard_violations)
+        for ptr, t in self._blocks.items():
+            before = len(self._guard_violations)
+            self._check_block(ptr, t)
+            live += self._guard_violations[before:]
+            del self._guard_violations[before:]
+        return live
 
     def close(self):
         if getattr(self, "handle", None):
