@@ -112,3 +112,13 @@ def test_pme_total_ewald_energy_is_independent_of_alpha_f64():
         assert abs(totals[1] - totals[0]) <= 2e-7 * scale, (totals, scale)
     finally:
         ctx.close()
+
+
+def test_pme_recip_config4_full_size_f32():
+    """configs[4] (300,000 atoms) with the mesh bench.py times (the paper's heuristic): the whole force array,
+    energy and virial against the numpy oracle."""
+    wb = wl.make_config(4)
+    delta = float(np.exp(-(3.12 * 1.0) ** 2) / 2.0)
+    mesh = dimos.dimos_pme_mesh_size(3.12, wb.box, delta)
+    F, E, W, p64, q64 = run(wb.pos, wb.charge, wb.box, 3.12, mesh, 5, "f32")
+    compare(F, E, W, pme.pme_recip(p64, q64, wb.box, 3.12, mesh, 5), "f32", q64, 3.12)
