@@ -54,7 +54,7 @@ static void free_list(Ctx* ctx, NL* nl)
 {
     DevBuf* bufs[] = {&nl->cell_count, &nl->cell_start, &nl->unit_start, &nl->scan_tmp, &nl->atom_cell, &nl->atom_rank,
                       &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
-                      &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->entry, &nl->emask, &nl->row_info,
+                      &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->entry, &nl->emask, &nl->row_info, &nl->slot_hint, &nl->atom_active,
                       &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials, &nl->accum,
                       &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW, &nl->st_ref, &nl->st_flag,
                       &nl->export_count};
@@ -66,7 +66,7 @@ static size_t list_workspace_bytes(const NL* nl)
 {
     const DevBuf* bufs[] = {&nl->cell_count, &nl->cell_start, &nl->unit_start, &nl->scan_tmp, &nl->atom_cell, &nl->atom_rank,
                             &nl->cell_atoms, &nl->perm, &nl->inv_perm, &nl->ref, &nl->xyz_build, &nl->bb_lo, &nl->bb_hi,
-                            &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->entry, &nl->emask,
+                            &nl->unit_cell, &nl->excl_start, &nl->excl_adj, &nl->excl_pairs, &nl->exc_pairs, &nl->exc_scale, &nl->entry, &nl->emask, &nl->slot_hint, &nl->atom_active,
                             &nl->row_info, &nl->flags, &nl->xyzq, &nl->stype, &nl->Facc, &nl->Fown, &nl->lj, &nl->partials,
                             &nl->accum, &nl->st_pos, &nl->st_charge, &nl->st_type, &nl->st_lj, &nl->st_F, &nl->st_EW,
                             &nl->st_ref, &nl->st_flag, &nl->export_count};

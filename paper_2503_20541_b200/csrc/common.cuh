@@ -22,6 +22,10 @@ constexpr int SELF_CODE = 13;  // stencil code of offset (0,0,0): (dx+1)*9+(dy+1
 // the 8-bit i-mask of an entry lives in a parallel byte array and is read for the masked chunks only
 constexpr unsigned ENTRY_SLOT_BITS = 27;
 constexpr unsigned ENTRY_SLOT_MASK = (1u << ENTRY_SLOT_BITS) - 1u;
+// Offset (in entries, from the row's first entry) of chunk c of a row of `total` chunks: the first n_am = nA + nM chunks
+// sit at the row's start, the remaining (mask-free, LJ-free) ones END at the row's capacity nu_cap = row_cap - m_res
+// (the list builder fills the row from both ends).
+__host__ __device__ inline int row_chunk_offset(int c, int total, int n_am, int nu_cap) { return c < n_am ? c * 32 : nu_cap - (total - c) * 32; }
 __host__ __device__ inline unsigned entry_pack(int slot, int code) { return (unsigned)slot | ((unsigned)code << ENTRY_SLOT_BITS); }
 
 // device error flag bits (NL::d_flags[0])
@@ -87,7 +91,6 @@ struct NL {
     int row_cap = 0;  // entries per unit row (multiple of 32), includes m_res
     int m_res = 128;  // max masked entries per row staged by the builder (multiple of 32); rows start m_res entries into their slab
     int n_grow = 0;
-    bool rows_sorted = false;  // rows partitioned [LJ-active plain | masked | LJ-free plain] (done lazily by the first force call after a build)
     int64_t n_entries = 0, n_entries_padded = 0;
     int64_t n_excl = 0;
     int max_cell_count = 0;
@@ -107,9 +110,12 @@ struct NL {
     int64_t n_exc = 0;
     DevBuf entry;      // uint32[n_units*row_cap]: slot | code << 27
     DevBuf emask;      // uint8[n_units*row_cap]: i-mask of the entry (all-ones in the mask-free chunks)
-    DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, nA | nM << 16}: the row is nA mask-free
-                       // chunks, then nM chunks that need their masks, then the remaining mask-free chunks (after
-                       // reorder_rows: nA = chunks of j-atoms with LJ partners, the trailing ones have none)
+    DevBuf row_info;   // int2[n_units]: {chunks in the row | partial-unit flag << 16, nA | nM << 16}: nA mask-free chunks of
+                       // j-atoms assumed LJ-active, then nM chunks that read their masks, then (at the end of the row's
+                       // capacity, see row_chunk_offset) the mask-free chunks of j-atoms assumed LJ-free
+    DevBuf slot_hint;  // uint8[n_slots]: the LJ-activity flag the builder assumed for the slot's atom (1 without a hint)
+    DevBuf atom_active;  // uint8[N]: LJ-activity of every atom at the last force call = the next build's hint
+    bool hint_valid = false;
     DevBuf flags;      // int[16]: [0] error flags, [1] max cell count, [2..3] entry counters (u64), [4..5] padded, [6..7] needed
                        // capacities, [8] row order stale (an atom became LJ-active), [9] type index out of range, [10] exception check
     // per-step device arrays

@@ -211,6 +211,26 @@ __device__ __forceinline__ void bitonic_sort_u64(unsigned long long* K, int npad
     }
 }
 
+// Rank sort inside segments: position p (< n) carries local id Kin[p] and the 32-bit key KEY[p]; if its segment
+// [st, st + cnt) is to be sorted (`sort_it`), p moves to st + #{q in the segment: KEY[q] < KEY[p], or equal and q < p}.
+// One pass, no barrier inside, ~3 instructions per comparison: a cell of ~150 atoms needs ~450 comparisons per thread
+// over all levels of the bisection, where full bitonic sorts of the padded cell cost six times 36 barrier-separated stages.
+__device__ __forceinline__ void rank_scatter(const unsigned short* __restrict__ Lin, unsigned short* __restrict__ Lout,
+                                             const unsigned* __restrict__ KEY, int p, int st, int cnt, bool sort_it)
+{
+    int dst = p;
+    if (sort_it) {
+        const unsigned kp = KEY[p];
+        int r = 0;
+        for (int q = st; q < st + cnt; ++q) {
+            const unsigned kq = KEY[q];
+            r += (kq < kp || (kq == kp && q < p)) ? 1 : 0;
+        }
+        dst = st + r;
+    }
+    Lout[dst] = Lin[p];
+}
+
 // segment arrays of the k-d bisection: a cell of npad (power of two) atoms ends in at most npad / UNIT segments; twice
 // that is allocated (the split step writes children 2s, 2s+1)
 __host__ __device__ inline int kd_segs(int npad_max) { return 2 * (npad_max / UNIT) < 8 ? 8 : 2 * (npad_max / UNIT); }
@@ -222,7 +242,8 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
                                   typename vec4<real>::type* __restrict__ xyz_build,
                                   typename vec4<real>::type* __restrict__ bb_lo,
                                   typename vec4<real>::type* __restrict__ bb_hi, int* __restrict__ unit_cell,
-                                  int npad_max)
+                                  int npad_max, const unsigned char* __restrict__ atom_active,
+                                  unsigned char* __restrict__ slot_hint)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int cell = blockIdx.x;
@@ -233,8 +254,10 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
     while (npad < n) npad <<= 1;
 
     const int KS = kd_segs(npad_max);
-    unsigned long long* K = reinterpret_cast<unsigned long long*>(smem_raw);
-    real* X = reinterpret_cast<real*>(K + npad_max);
+    unsigned* KEY = reinterpret_cast<unsigned*>(smem_raw);                       // sort key of the atom at a position
+    unsigned short* LA = reinterpret_cast<unsigned short*>(KEY + npad_max);      // position -> local id, two buffers
+    unsigned short* LB = LA + npad_max;
+    real* X = reinterpret_cast<real*>(smem_raw + (size_t)npad_max * 8);
     real* Y = X + npad_max;
     real* Z = Y + npad_max;
     int* ID = reinterpret_cast<int*>(Z + npad_max);
@@ -248,19 +271,19 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
     unsigned short* SEG = reinterpret_cast<unsigned short*>(bbmax + 3 * KS);
     __shared__ int any_big;
 
-    // canonical order: by original atom index (makes the result independent of the binning atomics)
-    for (int p = threadIdx.x; p < npad; p += blockDim.x)
-        K[p] = p < n ? (((unsigned long long)(unsigned)cell_atoms[a0 + p]) << 12) : ~0ull;
+    // canonical order: by original atom index (makes the units independent of the order the binning atomics produced)
+    for (int p = threadIdx.x; p < n; p += blockDim.x) { KEY[p] = (unsigned)cell_atoms[a0 + p]; LA[p] = (unsigned short)p; }
     __syncthreads();
-    bitonic_sort_u64(K, npad);
+    for (int p = threadIdx.x; p < n; p += blockDim.x) rank_scatter(LA, LB, KEY, p, 0, n, true);
+    __syncthreads();
 
     const int cz = cell % g.n[2];
     const int cy = (cell / g.n[2]) % g.n[1];
     const int cx = cell / (g.n[2] * g.n[1]);
     const double org[3] = {cx * g.h[0], cy * g.h[1], cz * g.h[2]};
 
-    for (int p = threadIdx.x; p < n; p += blockDim.x) {
-        int id = (int)(K[p] >> 12);
+    for (int p = threadIdx.x; p < n; p += blockDim.x) {  // local id = canonical rank
+        const int id = cell_atoms[a0 + LB[p]];
         ID[p] = id;
         double r[3];
 #pragma unroll
@@ -276,12 +299,13 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
         SEG[p] = 0;
     }
     __syncthreads();
-    for (int p = threadIdx.x; p < npad; p += blockDim.x) K[p] = p < n ? (unsigned long long)p : ~0ull;
+    for (int p = threadIdx.x; p < n; p += blockDim.x) LA[p] = (unsigned short)p;  // position -> local id
     if (threadIdx.x == 0) { segS[0] = 0; segN[0] = n; }
     __syncthreads();
 
     int nseg = 1;
     int *cS = segS, *cN = segN, *nS = segS2, *nN = segN2;
+    unsigned short *Lc = LA, *Ln = LB;
     for (int level = 0; level < 10; ++level) {
         if (threadIdx.x == 0) any_big = 0;
         __syncthreads();
@@ -296,7 +320,7 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
         for (int p = threadIdx.x; p < n; p += blockDim.x) {
             int s = SEG[p];
             if (cN[s] > UNIT) {
-                int lid = (int)(K[p] & 0xFFF);
+                int lid = Lc[p];
                 int ox = (int)(ordered_u32((float)X[lid]) ^ 0x80000000u);
                 int oy = (int)(ordered_u32((float)Y[lid]) ^ 0x80000000u);
                 int oz = (int)(ordered_u32((float)Z[lid]) ^ 0x80000000u);
@@ -325,21 +349,20 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
             segAxis[s] = ax;
         }
         __syncthreads();
+        // key of every atom of a segment to be split: its coordinate along the segment's longest axis
         for (int p = threadIdx.x; p < n; p += blockDim.x) {
-            int s = SEG[p];
-            int lid = (int)(K[p] & 0xFFF);
-            unsigned c;
+            const int s = SEG[p];
             if (cN[s] > UNIT) {
-                int ax = segAxis[s];
-                float v = ax == 0 ? (float)X[lid] : (ax == 1 ? (float)Y[lid] : (float)Z[lid]);
-                c = ordered_u32(v);
-            } else {
-                c = (unsigned)(p - cS[s]);
+                const int lid = Lc[p], ax = segAxis[s];
+                const float v = ax == 0 ? (float)X[lid] : (ax == 1 ? (float)Y[lid] : (float)Z[lid]);
+                KEY[p] = ordered_u32(v);
             }
-            K[p] = ((unsigned long long)s << 44) | ((unsigned long long)c << 12) | (unsigned long long)lid;
         }
         __syncthreads();
-        bitonic_sort_u64(K, npad);
+        for (int p = threadIdx.x; p < n; p += blockDim.x) {
+            const int s = SEG[p];
+            rank_scatter(Lc, Ln, KEY, p, cS[s], cN[s], cN[s] > UNIT);
+        }
         // split every big segment: the left child takes a multiple of UNIT atoms
         for (int s = threadIdx.x; s < nseg; s += blockDim.x) {
             int cnt = cN[s], st = cS[s];
@@ -354,7 +377,7 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
             }
         }
         __syncthreads();
-        for (int p = threadIdx.x; p < n; p += blockDim.x) {
+        for (int p = threadIdx.x; p < n; p += blockDim.x) {  // segments are position ranges: the scatter stayed inside them
             int s = SEG[p];
             int child = 2 * s;
             if (cN[s] > UNIT && p >= nS[2 * s + 1]) child = 2 * s + 1;
@@ -364,6 +387,7 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
         int* t;
         t = cS; cS = nS; nS = t;
         t = cN; cN = nN; nN = t;
+        unsigned short* tl = Lc; Lc = Ln; Ln = tl;
         nseg *= 2;
     }
 
@@ -371,14 +395,35 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
     const int u0 = unit_start[cell];
     const int nu = (n + UNIT - 1) / UNIT;
     using real4 = typename vec4<real>::type;
+    // LJ-activity hint of every position (remembered from the last force call; all active without one).  Inside a unit the
+    // atoms with LJ partners come first, so that they share as few of the pair kernel's i-atom pairs as possible; the
+    // list builder files j-atoms by the same flag.  Both are optimisations: the pair kernel checks the real types.
+    for (int p = threadIdx.x; p < n; p += blockDim.x) SEG[p] = atom_active ? (unsigned short)(atom_active[ID[Lc[p]]] != 0) : (unsigned short)1;
+    __syncthreads();
+    for (int p = threadIdx.x; p < n; p += blockDim.x) {  // stable partition of every unit's atoms: active first
+        const int b = p & ~(UNIT - 1), e = min(b + UNIT, n);
+        const int mine = SEG[p];
+        int n_act = 0, before_same = 0;
+        for (int k = b; k < e; ++k) {
+            n_act += SEG[k];
+            before_same += (k < p && SEG[k] == mine) ? 1 : 0;
+        }
+        const int dst = b + (mine ? before_same : n_act + before_same);
+        Ln[dst] = Lc[p];
+        KEY[dst] = (unsigned)mine;
+    }
+    __syncthreads();
     for (int p = threadIdx.x; p < nu * UNIT; p += blockDim.x) {
-        int q = p < n ? p : n - 1;  // padding slots mirror the cell's last atom
-        int lid = (int)(K[q] & 0xFFF);
+        const int q = p < n ? p : n - 1;  // padding slots mirror the cell's last atom
+        int lid = Ln[q];
         int id = ID[lid];
         int64_t slot = (int64_t)u0 * UNIT + p;
         perm[slot] = p < n ? id : ~id;
         if (p < n) inv_perm[id] = (int)slot;
-        xyz_build[slot] = make4(X[lid], Y[lid], Z[lid], p < n ? (real)1 : (real)0);  // w: 1 = real atom, 0 = padding slot
+        const int act = p < n ? (int)KEY[q] : 0;
+        slot_hint[slot] = (unsigned char)act;
+        // w: 0 = padding slot, 1 = real atom assumed without LJ partners, 2 = real atom assumed with
+        xyz_build[slot] = make4(X[lid], Y[lid], Z[lid], p < n ? (real)(1 + act) : (real)0);
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             double x = (double)pos[3 * (int64_t)id + a];
@@ -392,7 +437,7 @@ __global__ void kd_cluster_kernel(const real* __restrict__ pos, Grid g, const in
         for (int k = 0; k < UNIT; ++k) {
             int p = u * UNIT + k;
             if (p >= n) break;
-            int lid = (int)(K[p] & 0xFFF);
+            int lid = Lc[p];
             real v[3] = {X[lid], Y[lid], Z[lid]};
 #pragma unroll
             for (int a = 0; a < 3; ++a) { lo[a] = v[a] < lo[a] ? v[a] : lo[a]; hi[a] = v[a] > hi[a] ? v[a] : hi[a]; }
@@ -561,43 +606,44 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
     __syncwarp();
 
     const int64_t row = U * (int64_t)P.row_cap;
-    int nm = 0;  // masked entries staged
-    int nu = 0;  // unmasked entries written (or needed, once overflowing)
+    int nm = 0;   // masked entries staged
+    int nua = 0;  // mask-free entries of j-atoms assumed LJ-active: written upwards from the start of the row
+    int nub = 0;  // mask-free entries of the others: written downwards from the end of the row's capacity
+    bool lost = false;  // warp-uniform: the cursors met
     const int nu_cap = P.row_cap - P.m_res;
 
-    // append one warp-wide batch of entries
-    auto append = [&](bool accept, unsigned mask, int j, int code) {
-        const bool is_masked = accept && (mask != (unit_full ? 0xFFu : valid_i) || !unit_full);
-        const bool is_plain = accept && !is_masked;
-        unsigned bm = __ballot_sync(FULL, is_masked);
-        unsigned bp = __ballot_sync(FULL, is_plain);
+    // append one warp-wide batch of entries; cls_b: the j-atom is assumed to have no LJ partners
+    auto append = [&](bool accept, unsigned mask, int j, int code, bool cls_b) {
+        const bool is_masked = accept && mask != 0xFFu;
+        const bool is_a = accept && !is_masked && !cls_b;
+        const bool is_b = accept && !is_masked && cls_b;
+        const unsigned bm = __ballot_sync(FULL, is_masked), ba = __ballot_sync(FULL, is_a), bb = __ballot_sync(FULL, is_b);
         if (is_masked) {
             int pos = nm + __popc(bm & lt_mask);
             if (pos < P.m_res) { st_j[pos] = (int)entry_pack(j, code); st_meta[pos] = (unsigned short)mask; }
         }
-        if (is_plain) {
-            int pos = nu + __popc(bp & lt_mask);
-            if (pos < nu_cap) {
-                P.entry[row + P.m_res + pos] = entry_pack(j, code);
-                P.emask[row + P.m_res + pos] = 0xFFu;
-            }
-        }
+        // the two cursors never write into each other's current batch; once they would, nothing more is written and
+        // the row is reported as overflowed (the host grows row_cap and rebuilds)
+        if (nua + nub + 64 > nu_cap) lost = true;
+        if (is_a && !lost) P.entry[row + P.m_res + nua + __popc(ba & lt_mask)] = entry_pack(j, code);
+        if (is_b && !lost) P.entry[row + P.m_res + nu_cap - 1 - (nub + __popc(bb & lt_mask))] = entry_pack(j, code);
         nm += __popc(bm);
-        nu += __popc(bp);
+        nua += __popc(ba);
+        nub += __popc(bb);
     };
-    // Partial units (fewer than UNIT real atoms, one per cell) keep every entry in the row's plain
-    // region with mask = valid_i: the force kernel runs them through its masked path.
-    auto append_any = [&](bool accept, unsigned mask, int j, int code) {
-        if (unit_full) { append(accept, mask, j, code); return; }
+    // Partial units (fewer than UNIT real atoms, one per cell) keep every entry, with its mask, in the upward region:
+    // the force kernels run them through their masked path.
+    auto append_any = [&](bool accept, unsigned mask, int j, int code, bool cls_b) {
+        if (unit_full) { append(accept, mask, j, code, cls_b); return; }
         unsigned bp = __ballot_sync(FULL, accept);
         if (accept) {
-            int pos = nu + __popc(bp & lt_mask);
+            int pos = nua + __popc(bp & lt_mask);
             if (pos < nu_cap) {
                 P.entry[row + P.m_res + pos] = entry_pack(j, code);
                 P.emask[row + P.m_res + pos] = (unsigned char)mask;
             }
         }
-        nu += __popc(bp);
+        nua += __popc(bp);
     };
 
     auto excl_bits = [&](int slot) -> unsigned {
@@ -617,7 +663,7 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
             mask = ((1u << lane) - 1u) & valid_i & ~excl_bits(slot);
             acc = mask != 0;
         }
-        append_any(acc, mask, slot, SELF_CODE);
+        append_any(acc, mask, slot, SELF_CODE, false);
     }
 
     // ---- stencil: unique neighbour cells per axis (reading C-18) ----
@@ -644,7 +690,7 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         const int T = ncand * UNIT;
         for (int t0 = 0; t0 < T; t0 += 32) {
             const int t = t0 + lane;
-            bool acc = false;
+            bool acc = false, cls_b = false;
             unsigned mask = 0;
             int slot = 0, code = SELF_CODE;
             if (t < T) {
@@ -686,9 +732,10 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                     }
                     mask = valid_i & ~excl_bits(slot);
                     acc = (bits & mask) != 0;
+                    cls_b = pj.w == (real)1;
                 }
             }
-            append_any(acc, mask, slot, code);
+            append_any(acc, mask, slot, code, cls_b);
         }
         ncand = 0;
     };
@@ -766,26 +813,52 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         if (lane == 0) { atomicOr(&P.flags[0], FLAG_MASKED_OVERFLOW); atomicMax(&P.flags[7], nm); }
         nm = P.m_res;
     }
-    // Row layout: the mask-free entries first (the leading nu/32 full chunks are the force kernels' mask-free
-    // chunks), then the masked entries, then padding up to a multiple of 32: one chunk sequence, no hole.
-    int n_pad = (nu + nm + 31) & ~31;
-    if (n_pad > nu_cap) {
-        if (lane == 0) { atomicOr(&P.flags[0], FLAG_ROW_OVERFLOW); atomicMax(&P.flags[6], n_pad); }
-        nu = 0;  // the row is unusable; the host grows row_cap and rebuilds
+    // Row layout (what the force kernels' three phases walk):
+    //   [ A: whole chunks of mask-free entries, LJ-active j ][ M: the chunks that read their i-masks ] ... gap ... [ B: whole
+    //   chunks of mask-free entries, LJ-free j, ending at the row's capacity ]
+    // M holds A's leftover entries (already in place behind A's last whole chunk), the staged masked entries, B's
+    // leftover entries (the last ones written, at the low end of the downward region) and padding up to a chunk.
+    int full_a = unit_full ? (nua & ~31) : 0, full_b = nub & ~31;
+    const int rem_a = nua - full_a, rem_b = nub - full_b;
+    int n_mpad = (rem_a + nm + rem_b + 31) & ~31;
+    if (lost || full_a + n_mpad + full_b > nu_cap) {
+        if (lane == 0) { atomicOr(&P.flags[0], FLAG_ROW_OVERFLOW); atomicMax(&P.flags[6], nua + nub + nm + 160); }
+        full_a = full_b = n_mpad = 0;  // the row is unusable; the host grows row_cap and rebuilds
         nm = 0;
-        n_pad = 0;
-    }
-    const int self = (int)(U * UNIT);
-    for (int k = lane; k < n_pad - nu; k += 32) {
-        const int64_t e = row + P.m_res + nu + k;
-        P.entry[e] = k < nm ? (unsigned)st_j[k] : entry_pack(self, SELF_CODE);  // padding: the unit itself, mask 0
-        P.emask[e] = k < nm ? (unsigned char)st_meta[k] : (unsigned char)0;
+    } else if (unit_full) {
+        unsigned wb = 0;
+        if (lane < rem_b) wb = P.entry[row + P.m_res + (nu_cap - nub) + lane];  // read B's leftovers before M may overwrite them
+        __syncwarp();
+        const int self = (int)(U * UNIT);
+        for (int k = lane; k < n_mpad; k += 32) {
+            const int64_t e = row + P.m_res + full_a + k;
+            if (k < rem_a) {
+                P.emask[e] = 0xFFu;
+            } else if (k < rem_a + nm) {
+                P.entry[e] = (unsigned)st_j[k - rem_a];
+                P.emask[e] = (unsigned char)st_meta[k - rem_a];
+            } else if (k < rem_a + nm + rem_b) {
+                P.emask[e] = 0xFFu;  // the entry itself (one of B's leftovers) is written below
+            } else {
+                P.entry[e] = entry_pack(self, SELF_CODE);  // padding: the unit itself, mask 0
+                P.emask[e] = 0;
+            }
+        }
+        __syncwarp();
+        if (lane < rem_b) P.entry[row + P.m_res + full_a + rem_a + nm + lane] = wb;
+    } else {
+        // partial unit: pad the upward region to a whole chunk; every chunk is a masked chunk
+        const int self = (int)(U * UNIT);
+        for (int k = nua + lane; k < n_mpad; k += 32) {
+            P.entry[row + P.m_res + k] = entry_pack(self, SELF_CODE);
+            P.emask[row + P.m_res + k] = 0;
+        }
     }
     if (lane == 0) {
-        const int n_a = unit_full ? (nu >> 5) : 0;  // leading mask-free chunks; everything after them reads its masks
-        P.row_info[U] = make_int2((n_pad >> 5) | (unit_full ? 0 : 0x10000), n_a | (((n_pad >> 5) - n_a) << 16));
-        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[2]), (unsigned long long)(nm + nu));
-        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[4]), (unsigned long long)n_pad);
+        const int total = (full_a + n_mpad + full_b) >> 5;
+        P.row_info[U] = make_int2(total | (unit_full ? 0 : 0x10000), (full_a >> 5) | ((n_mpad >> 5) << 16));
+        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[2]), (unsigned long long)(nm + nua + nub));
+        atomicAdd(reinterpret_cast<unsigned long long*>(&P.flags[4]), (unsigned long long)(total * 32));
     }
 }
 
@@ -823,13 +896,14 @@ __global__ __launch_bounds__(128) void export_pairs_kernel(BuildParams<real> P, 
         pi[i] = __shfl_sync(FULL, my_perm, i);
     }
     const int2 ri = P.row_info[U];
-    const int nch = ri.x & 0xFFFF;  // chunks in the row (mask-free chunks first, then masked entries and padding)
+    const int nch = ri.x & 0xFFFF;  // chunks in the row
+    const int n_a = ri.y & 0xFFFF, n_am = n_a + (int)((unsigned)ri.y >> 16);
     const int64_t row = U * (int64_t)P.row_cap + P.m_res;
     for (int c = 0; c < nch; ++c) {
-        const int64_t e = row + (int64_t)c * 32 + lane;
+        const int64_t e = row + row_chunk_offset(c, nch, n_am, P.row_cap - P.m_res) + lane;
         const unsigned wd = P.entry[e];
         const int j = (int)(wd & ENTRY_SLOT_MASK);
-        const unsigned mask = P.emask[e];
+        const unsigned mask = (c >= n_a && c < n_am) ? (unsigned)P.emask[e] : 0xFFu;  // only the masked chunks store masks
         const int code = (int)(wd >> ENTRY_SLOT_BITS);
         real4 pj = P.xyz[j];
         const int pj_orig = P.perm[j];
@@ -1004,6 +1078,7 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
     if ((rc = ensure(ctx, nl->bb_hi, nun * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->unit_cell, nun * sizeof(int), s))) return rc;
     if ((rc = ensure(ctx, nl->row_info, nun * sizeof(int2), s))) return rc;
+    if ((rc = ensure(ctx, nl->slot_hint, nsl, s))) return rc;
 
     int npad_max = 32;
     while (npad_max < nl->max_cell_count) npad_max <<= 1;
@@ -1012,7 +1087,8 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
     kd_cluster_kernel<real><<<(unsigned)ncells, 256, kd_smem, s>>>(
         pos, g, (const int*)nl->cell_start.p, (const int*)nl->unit_start.p, (const int*)nl->cell_atoms.p, (int*)nl->perm.p,
         (int*)nl->inv_perm.p, (double*)nl->ref.p, (real4*)nl->xyz_build.p, (real4*)nl->bb_lo.p, (real4*)nl->bb_hi.p,
-        (int*)nl->unit_cell.p, npad_max);
+        (int*)nl->unit_cell.p, npad_max, nl->hint_valid ? (const unsigned char*)nl->atom_active.p : nullptr,
+        (unsigned char*)nl->slot_hint.p);
     DIMOS_LAUNCH_CHECK(ctx, "kd_cluster");
 
     // ---- row capacity estimate (grown on overflow) ----
@@ -1049,7 +1125,6 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
             memcpy(&np, h + 4, 8);
             nl->n_entries = (int64_t)ne;
             nl->n_entries_padded = (int64_t)np;
-            nl->rows_sorted = false;  // the next force call re-partitions the rows by LJ activity
             return DIMOS_OK;
         }
         nl->n_grow++;

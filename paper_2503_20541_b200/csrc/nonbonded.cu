@@ -128,7 +128,8 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
                               typename vec4<real>::type* __restrict__ xyzq, int* __restrict__ stype,
                               typename vec4<real>::type* __restrict__ Facc, const double* __restrict__ lj_table, int nt,
                               real* __restrict__ lj_out, int* __restrict__ row_active, double* __restrict__ accum,
-                              int* __restrict__ order_stale, int check_order)
+                              int* __restrict__ order_stale, const unsigned char* __restrict__ slot_hint,
+                              unsigned char* __restrict__ atom_active)
 {
     // per type: does it have any non-zero LJ partner?  (every block recomputes the tiny table: no inter-block order)
     __shared__ int act_sh[MAX_TYPES];
@@ -154,9 +155,13 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
             t = 0;
         }
         const int st = t | (act_sh[t] ? STYPE_ACTIVE : 0);  // bit 30: the atom has LJ partners
-        // the rows were ordered by this bit (reorder_rows): if it changes for any atom, the pair kernel is told to
-        // evaluate LJ in every chunk until the next build
-        if (check_order && !pad && ((stype[s] ^ st) & STYPE_ACTIVE)) atomicOr(order_stale, 1);
+        // the builder ordered the rows by the LJ activity it ASSUMED (the flags of the last force call before the build,
+        // all active without one): an atom assumed LJ-free that has LJ partners would be skipped, so the pair kernels are
+        // told to evaluate LJ in every chunk until the next build; the flag seen now is the next build's hint
+        if (!pad) {
+            if (!slot_hint[s] && (st & STYPE_ACTIVE)) atomicOr(order_stale, 1);
+            atom_active[o] = (st & STYPE_ACTIVE) ? 1 : 0;
+        }
         stype[s] = st;
         Facc[s] = mk4((real)0, (real)0, (real)0, (real)0);
     }
@@ -319,13 +324,14 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
         acc_t w[6] = {0, 0, 0, 0, 0, 0};
 
         // software pipeline: (jslot, meta) two chunks ahead, (xyzq, stype) one chunk ahead
-        int64_t e = U * (int64_t)P.row_cap + P.m_res + lane;
+        const int64_t e0 = U * (int64_t)P.row_cap + P.m_res + lane;
+        const int n_am = n_a + (int)n_m, nu_cap = P.row_cap - P.m_res;
         unsigned jn = 0, jn2 = 0;  // packed entries
         int tjn = 0;
         unsigned mn = 0, mn2 = 0;  // i-masks
         real4 pjn = mk4((real)0, (real)0, (real)0, (real)0);
-        if (total > 0) { jn = P.entry[e]; mn = P.emask[e]; }
-        if (total > 1) { jn2 = P.entry[e + 32]; mn2 = P.emask[e + 32]; }
+        if (total > 0) { const int64_t e = e0 + row_chunk_offset(0, total, n_am, nu_cap); jn = P.entry[e]; mn = P.emask[e]; }
+        if (total > 1) { const int64_t e = e0 + row_chunk_offset(1, total, n_am, nu_cap); jn2 = P.entry[e]; mn2 = P.emask[e]; }
         if (total > 0) { pjn = P.xyzq[jn & ENTRY_SLOT_MASK]; tjn = P.stype[jn & ENTRY_SLOT_MASK] & STYPE_MASK; }
 
         for (int c = 0; c < total; ++c) {
@@ -336,8 +342,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const int tj = tjn;
             jn = jn2; mn = mn2;
             if (c + 1 < total) { pjn = P.xyzq[jn & ENTRY_SLOT_MASK]; tjn = P.stype[jn & ENTRY_SLOT_MASK] & STYPE_MASK; }
-            if (c + 2 < total) { jn2 = P.entry[e + 64]; mn2 = P.emask[e + 64]; }
-            e += 32;
+            if (c + 2 < total) { const int64_t e = e0 + row_chunk_offset(c + 2, total, n_am, nu_cap); jn2 = P.entry[e]; mn2 = P.emask[e]; }
 
             const real4 off = off_s[code];
             const real xj = pj.x + off.x, yj = pj.y + off.y, zj = pj.z + off.z;
@@ -718,6 +723,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     const unsigned nb_excl = ewald && nl->n_excl > 0 ? (unsigned)((nl->n_excl + 255) / 256) : 0;
     if ((rc = ensure(ctx, nl->xyzq, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->stype, nsl * sizeof(int), s))) return rc;
+    if ((rc = ensure(ctx, nl->atom_active, (size_t)nl->N, s))) return rc;
     if ((rc = ensure(ctx, nl->Facc, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->Fown, nsl * sizeof(real4), s))) return rc;
     if ((rc = ensure(ctx, nl->lj, (size_t)MAX_TYPES * MAX_TYPES * 4 * sizeof(double) + MAX_TYPES * sizeof(int), s))) return rc;
@@ -731,14 +737,10 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     gather_kernel<real><<<(unsigned)((nsl + T - 1) / T), T, 0, s>>>(pos, charge, type, (const int*)nl->perm.p, (const double*)nl->ref.p,
                                                                     nsl, (real4*)nl->xyzq.p, (int*)nl->stype.p, (real4*)nl->Facc.p,
                                                                     lj_table, nt, lj_dev, row_active, (double*)nl->accum.p,
-                                                                    (int*)nl->flags.p + 8, nl->rows_sorted ? 1 : 0);
+                                                                    (int*)nl->flags.p + 8, (const unsigned char*)nl->slot_hint.p,
+                                                                    (unsigned char*)nl->atom_active.p);
     DIMOS_LAUNCH_CHECK(ctx, "gather");
-    if (!nl->rows_sorted) {  // once per build: partition every row's mask-free entries, LJ-active j-atoms first
-        launch_reorder_rows((unsigned*)nl->entry.p, (unsigned char*)nl->emask.p, (int2*)nl->row_info.p, (const int*)nl->stype.p,
-                            nun, nl->row_cap, nl->m_res, s);
-        DIMOS_LAUNCH_CHECK(ctx, "reorder_rows");
-        nl->rows_sorted = true;
-    }
+    nl->hint_valid = true;  // atom_active now holds this call's LJ-activity flags: the next build files its entries by them
 
     ForceParams<real> P;
     P.n_units = nun; P.n_slots = nsl; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;

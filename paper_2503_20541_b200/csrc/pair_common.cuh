@@ -85,8 +85,6 @@ __device__ __forceinline__ T reduce8_scatter(T (&v)[8], int lane)
 }
 
 // packed-FP32 pair kernel (pair_f32x2.cu); returns false when the case is not covered (caller uses the generic kernel)
-void launch_reorder_rows(unsigned* entry, unsigned char* emask, int2* row_info, const int* stype, int64_t n_units,
-                         int row_cap, int m_res, cudaStream_t s);
 // rolled fp64 kernel (pair_f64.cu); false = not covered
 bool launch_pair_force_f64(const ForceParams<double>& P, int method, int pbc, unsigned nb, cudaStream_t s);
 bool launch_pair_force_f32x2(const ForceParams<float>& P, int method, unsigned nb, size_t dyn, cudaStream_t s);

@@ -253,7 +253,7 @@ __device__ __forceinline__ float4 lds_offset(unsigned base, unsigned w)
         }                                                                                                        \
         EC = lds_u32(sa + (SOFF) + 256u);                                                                        \
         unsigned mk = 0xFFu;                                                                                     \
-        if ((KIND) == 1) { mk = mk_n; mk_n = mp[32]; }                                                           \
+        if ((KIND) == 1) { mk = c_m < n_m_true ? mk_n : 0xFFu; mk_n = mp[32]; }                                  \
         const float nxj = off.x - PJ.x, nyj = off.y - PJ.y, nzj = off.z - PJ.z; /* -(x_j + image shift) */       \
         float sx, sy, sz;                                                                                        \
         const unsigned ljrow = (KIND) != 2 ? ljt_base + ((unsigned)(TJ & STYPE_MASK) << 4) : 0u;                  \
@@ -263,6 +263,19 @@ __device__ __forceinline__ float4 lds_offset(unsigned base, unsigned w)
         w[3] = fmaf(-nyj, sy, w[3]); w[4] = fmaf(-nyj, sz, w[4]); w[5] = fmaf(-nzj, sz, w[5]);                   \
         red_add_xyz(P.Facc + jc, sx, sy, sz);                                                                    \
     } while (0)
+
+// One unit's row into a shared-memory buffer: the chunks at the row's start (LJ-active and masked) and the chunks that
+// end at the row's capacity (see row_chunk_offset) become one contiguous sequence; one or two bulk copies, one mbarrier.
+__device__ __forceinline__ void copy_row(const ForceParams<float>& P, long long U, int2 ri, unsigned dst, unsigned bar, unsigned long long pol)
+{
+    const int total = ri.x & 0xFFFF;
+    const int n_am = (ri.y & 0xFFFF) + (int)((unsigned)ri.y >> 16);
+    const unsigned bytes1 = (unsigned)n_am * 128u, bytes2 = (unsigned)(total - n_am) * 128u;
+    const unsigned* row = P.entry + U * (int64_t)P.row_cap + P.m_res;
+    mbar_expect_tx(bar, bytes1 + bytes2);
+    if (bytes1) bulk_row_to_smem(dst, row, bytes1, bar, pol);
+    if (bytes2) bulk_row_to_smem(dst + bytes1, row + (P.row_cap - P.m_res) - (total - n_am) * 32, bytes2, bar, pol);
+}
 
 template <int METHOD, bool SW>
 __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x2_kernel(ForceParams<float> P)
@@ -316,11 +329,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     }
     int2 ri = P.row_info[U];
     unsigned kbuf = 0;  // units processed by this warp: buffer = kbuf & 1, mbarrier phase = (kbuf >> 1) & 1
-    if (lane == 0 && (ri.x & 0xFFFF) != 0) {
-        const unsigned bytes = (unsigned)(ri.x & 0xFFFF) * 128u;
-        mbar_expect_tx(bar0, bytes);
-        bulk_row_to_smem(buf0, P.entry + U * (int64_t)P.row_cap + P.m_res, bytes, bar0, pol_stream);
-    }
+    if (lane == 0 && (ri.x & 0xFFFF) != 0) copy_row(P, U, ri, buf0, bar0, pol_stream);
     // pipeline state handed from one unit to the next: first two entries, first j-atom, the unit's own atoms
     unsigned ea = 0, eb = 0;
     float4 pA = make_float4(0.f, 0.f, 0.f, 0.f), pB;
@@ -341,10 +350,13 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         long long Un = 0;
         if (lane == 0) Un = (long long)atomicAdd(P.unit_counter, 1ull);  // in flight during the first phase
         const int total = ri.x & 0xFFFF;                  // chunks in the row
-        // lj_all: every chunk takes the masked-with-LJ path (mask-free chunks carry all-ones masks)
-        const int n_a = lj_all ? 0 : (ri.y & 0xFFFF);                  // mask-free chunks whose j-atoms have LJ partners
-        const int n_m = lj_all ? total : (int)((unsigned)ri.y >> 16);  // masked chunks after them
-        const int n_b = total - n_a - n_m;                             // mask-free chunks without LJ
+        const int n_a = ri.y & 0xFFFF;                  // mask-free chunks whose j-atoms were assumed LJ-active
+        const int n_m_true = (int)((unsigned)ri.y >> 16);  // chunks after them that read their i-masks
+        // lj_all (an atom assumed LJ-free turned out to have LJ partners): the trailing mask-free chunks go through the
+        // masked-with-LJ loop as well, with all-ones masks
+        const int n_m = lj_all ? total - n_a : n_m_true;
+        const int n_b = total - n_a - n_m;                 // trailing mask-free chunks without LJ
+        int c_m = 0;                                       // index inside the masked loop
         const unsigned b = kbuf & 1u;
 
         const unsigned char* mp = P.emask + U * (int64_t)P.row_cap + P.m_res + lane + n_a * 32;
@@ -384,7 +396,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         const bool more = Un < P.n_units;
         int2 ri_n = make_int2(0, 0);
         if (more) ri_n = P.row_info[Un];
-        for (int c = 0; c < n_m; ++c) {
+        for (c_m = 0; c_m < n_m; ++c_m) {
             DIMOS_CHUNK_STEP(1, pA, tA, pB, tB, ea, eb, 0u);
             pA = pB; tA = tB;
             { const unsigned t_ = ea; ea = eb; eb = t_; }
@@ -394,11 +406,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         // the next unit's row: bulk copy into the other buffer (last read by the previous unit, which is finished)
         const int total_n = ri_n.x & 0xFFFF;
         __syncwarp();
-        if (lane == 0 && total_n != 0) {
-            const unsigned bytes = (unsigned)total_n * 128u;
-            mbar_expect_tx(bar0 + 8u * (b ^ 1u), bytes);
-            bulk_row_to_smem(buf0 + (b ^ 1u) * row_bytes, P.entry + Un * (int64_t)P.row_cap + P.m_res, bytes, bar0 + 8u * (b ^ 1u), pol_stream);
-        }
+        if (lane == 0 && total_n != 0) copy_row(P, Un, ri_n, buf0 + (b ^ 1u) * row_bytes, bar0 + 8u * (b ^ 1u), pol_stream);
         for (int c = 0; c < n_b; c += 2) {
             DIMOS_CHUNK_STEP(2, pA, tA, pB, tB, ea, eb, 0u);
             if (c + 1 < n_b) { DIMOS_CHUNK_STEP(2, pB, tB, pA, tA, eb, ea, 128u); }
@@ -457,92 +465,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
 }
 #undef DIMOS_CHUNK_STEP
 
-// Once per build (first force call): every full unit's row is rewritten as
-//   [ mask-free chunks of j-atoms WITH LJ partners | chunks that read their i-masks | mask-free chunks WITHOUT LJ ]
-// The middle region takes the entries whose mask is not all-ones (exclusions, the unit's own half, padding) and the
-// leftovers of the two mask-free classes that do not fill a chunk.  The pair kernel then needs the j-atom types only
-// for the first two regions and no per-chunk vote.  Should an atom's LJ activity change afterwards (gather_kernel
-// notices), the kernel evaluates LJ in every chunk: the order is an optimisation, never a correctness condition.
-constexpr int RO_WARPS = 4;
-__global__ __launch_bounds__(RO_WARPS * 32) void reorder_rows_kernel(unsigned* __restrict__ entry, unsigned char* __restrict__ emask,
-                                                                     int2* __restrict__ row_info,
-                                                                     const int* __restrict__ stype, int64_t n_units,
-                                                                     int row_cap, int m_res)
-{
-    extern __shared__ __align__(16) unsigned char ro_smem[];
-    const int cap = row_cap - m_res;
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int64_t U = (int64_t)blockIdx.x * RO_WARPS + wib;
-    if (U >= n_units) return;
-    unsigned* se = reinterpret_cast<unsigned*>(ro_smem) + (size_t)wib * cap;
-    unsigned short* sm = reinterpret_cast<unsigned short*>(reinterpret_cast<unsigned*>(ro_smem) + (size_t)RO_WARPS * cap) + (size_t)wib * cap;
-    const int2 ri = row_info[U];
-    if (ri.x & 0x10000) return;  // partial unit: every chunk stays masked
-    const int n = (ri.x & 0xFFFF) * 32 < cap ? (ri.x & 0xFFFF) * 32 : cap;
-    if (n == 0) return;
-    const int64_t base = U * (int64_t)row_cap + m_res;
-    const unsigned FULL = 0xffffffffu, lt = (1u << lane) - 1u;
-    // class of an entry: 0 = mask-free with LJ, 1 = masked (real), 2 = mask-free without LJ, 3 = padding (mask 0, goes last in the masked region)
-    int cnt[4] = {0, 0, 0, 0};
-    for (int k0 = 0; k0 < n; k0 += 32) {
-        const int k = k0 + lane;
-        const unsigned wd = entry[base + k];
-        const unsigned m = emask[base + k];
-        int cls;
-        if (m == 0u) cls = 3;
-        else if (m != 0xFFu) cls = 1;
-        else cls = (stype[wd & ENTRY_SLOT_MASK] & STYPE_ACTIVE) ? 0 : 2;
-        se[k] = wd;
-        sm[k] = (unsigned short)(m | (cls << 8));
-#pragma unroll
-        for (int q = 0; q < 4; ++q) cnt[q] += __popc(__ballot_sync(FULL, cls == q));
-    }
-    __syncwarp();
-    const int fullA = cnt[0] & ~31, fullB = cnt[2] & ~31;         // entries in whole mask-free chunks
-    const int remA = cnt[0] - fullA, remB = cnt[2] - fullB;
-    const int nM = cnt[1] + cnt[3] + remA + remB;                 // multiple of 32 because n, fullA, fullB are
-    // destination offsets: A_full | remA, masked, remB, padding | B_full
-    int posM = fullA + remA, posB = fullA + nM, posP = fullA + remA + cnt[1] + remB;
-    int seenA = 0, seenB = 0;
-    for (int k0 = 0; k0 < n; k0 += 32) {
-        const int k = k0 + lane;
-        const unsigned wd = se[k];
-        const unsigned short mm = sm[k];
-        const int cls = mm >> 8;
-        const unsigned b0 = __ballot_sync(FULL, cls == 0), b1 = __ballot_sync(FULL, cls == 1), b2 = __ballot_sync(FULL, cls == 2),
-                       b3 = __ballot_sync(FULL, cls == 3);
-        int dst;
-        if (cls == 0) {
-            const int r = seenA + __popc(b0 & lt);  // rank among the LJ class: the first fullA go to the front, the rest into the masked region
-            dst = r < fullA ? r : fullA + (r - fullA);
-        } else if (cls == 1) {
-            dst = posM + __popc(b1 & lt);
-        } else if (cls == 2) {
-            const int r = seenB + __popc(b2 & lt);
-            dst = r < fullB ? posB + r : fullA + remA + cnt[1] + (r - fullB);
-        } else {
-            dst = posP + __popc(b3 & lt);
-        }
-        entry[base + dst] = wd;
-        emask[base + dst] = (unsigned char)(mm & 0xFFu);
-        seenA += __popc(b0);
-        posM += __popc(b1);
-        seenB += __popc(b2);
-        posP += __popc(b3);
-    }
-    if (lane == 0) row_info[U] = make_int2(ri.x, (fullA >> 5) | ((nM >> 5) << 16));
-}
-
 }  // namespace
-
-void launch_reorder_rows(unsigned* entry, unsigned char* emask, int2* row_info, const int* stype, int64_t n_units,
-                         int row_cap, int m_res, cudaStream_t s)
-{
-    const size_t smem = (size_t)RO_WARPS * (row_cap - m_res) * 6;
-    if (smem > 48 * 1024) cudaFuncSetAttribute(reorder_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    const unsigned nb = (unsigned)((n_units + RO_WARPS - 1) / RO_WARPS);
-    reorder_rows_kernel<<<nb, RO_WARPS * 32, smem, s>>>(entry, emask, row_info, stype, n_units, row_cap, m_res);
-}
 
 template <int METHOD, bool SW>
 static bool launch_one(const ForceParams<float>& P, unsigned nb, size_t dyn, cudaStream_t s)

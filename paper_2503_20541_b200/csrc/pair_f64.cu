@@ -92,9 +92,10 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
         const int total = ri.x & 0xFFFF;
         const int n_a = ri.y & 0xFFFF;
         const unsigned n_m = (unsigned)ri.y >> 16;
-        int64_t e = U * (int64_t)P.row_cap + P.m_res + lane;
+        const int64_t e0 = U * (int64_t)P.row_cap + P.m_res + lane;
+        const int n_am = n_a + (int)n_m, nu_cap = P.row_cap - P.m_res;
         unsigned jn = 0, mn = 0;
-        if (total > 0) { jn = P.entry[e]; mn = P.emask[e]; }
+        if (total > 0) { const int64_t e = e0 + row_chunk_offset(0, total, n_am, nu_cap); jn = P.entry[e]; mn = P.emask[e]; }
         double4 pjn = make_double4(0, 0, 0, 0);
         int tjn = 0;
         if (total > 0) { pjn = P.xyzq[jn & ENTRY_SLOT_MASK]; tjn = P.stype[jn & ENTRY_SLOT_MASK] & STYPE_MASK; }
@@ -107,12 +108,12 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
             const double4 pj = pjn;
             const int tj = tjn;
             if (c + 1 < total) {  // next chunk: entry, mask, then the gathered atom (its latency is covered by this chunk's math)
-                jn = P.entry[e + 32];
-                mn = P.emask[e + 32];
+                const int64_t e = e0 + row_chunk_offset(c + 1, total, n_am, nu_cap);
+                jn = P.entry[e];
+                mn = P.emask[e];
                 pjn = P.xyzq[jn & ENTRY_SLOT_MASK];
                 tjn = P.stype[jn & ENTRY_SLOT_MASK] & STYPE_MASK;
             }
-            e += 32;
             const double4 off = off_s[code];
             const double xj = pj.x + off.x, yj = pj.y + off.y, zj = pj.z + off.z, qj = pj.w;
             const bool lj_chunk = lj_all || c < n_a + (int)n_m;
