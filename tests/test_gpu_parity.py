@@ -620,3 +620,37 @@ def test_needs_rebuild_on_two_streams_at_once():
             assert int(f1.item()) == 1 and int(f2.item()) == 0
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64", "mixed"])
+def test_lj_activity_changes_after_the_build(precision):
+    """The builder files the rows by the LJ-activity flags of the LAST force call (a hint).  If the types or the LJ table
+    change afterwards so that an atom assumed LJ-free has LJ partners, the pair kernels must notice and evaluate LJ in
+    every chunk: forces and energies still match the oracle, before and after the next rebuild; the opposite change
+    (atoms lose their LJ partners) needs no fallback and must match as well."""
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, precision)
+    pos64 = db.pos.double().cpu().numpy()
+    q64 = db.charge.double().cpu().numpy()
+    lj_water = lj_table_np(wb)                                     # LJ on O only
+    lj_all = oracle.lorentz_berthelot([wl.SIGMA_O, 0.12], [wl.EPS_O, 0.2])   # H gets a small LJ core too
+    lj_none = oracle.lorentz_berthelot([wl.SIGMA_O, 0.0], [0.0, 0.0])        # nobody has LJ
+    ctx = dimos.Context(0, precision)
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        for table in (lj_water, lj_water):  # second call: after a rebuild that used the first call's flags
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, torch.from_numpy(table).cuda())
+            nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)
+        for table in (lj_all, lj_all, lj_none, lj_water, lj_all):
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, torch.from_numpy(table).cuda())
+            orc = oracle.nonbonded(pos64, q64, wb.type, table, db.box, 1.0, excl_pairs=wb.excl_pairs, band=BAND)
+            check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision)
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)  # hint: everybody active
+        for table in (lj_all, lj_water):
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, torch.from_numpy(table).cuda())
+            orc = oracle.nonbonded(pos64, q64, wb.type, table, db.box, 1.0, excl_pairs=wb.excl_pairs, band=BAND)
+            check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision)
+        gp = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy()
+        check_neighbor_set(gp, pos64, db.box, 1.1, wb.excl_pairs)
+    finally:
+        ctx.close()
