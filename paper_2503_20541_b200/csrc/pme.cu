@@ -29,6 +29,8 @@ struct PmePlan {
     DevBuf grid;     // real[K1*K2*K3]
     DevBuf spec;     // complex[K1*K2*(K3/2+1)]
     DevBuf moduli;   // double[K1+K2+K3]: |b(m)|^2 per axis
+    DevBuf tables;   // double[2*(K1+K2+K3)]: per axis {m_k, |b|^2 exp(-pi^2 m_k^2/alpha^2)} for the alpha and box below
+    double tab_alpha = 0, tab_L[3] = {0, 0, 0};
     DevBuf work;     // cuFFT work area (shared by both plans)
     DevBuf acc;      // double[8]: E_recip, Wxx, Wxy, Wxz, Wyy, Wyz, Wzz, sum q^2
 };
@@ -123,52 +125,67 @@ template <typename real> struct cplx;
 template <> struct cplx<float> { using type = float2; };
 template <> struct cplx<double> { using type = double2; };
 
+// Per-axis tables of the influence function, one thread per mesh index: tab[0][k] = m_k = k'/L (k' = k or k - K),
+// tab[1][k] = |b(k)|^2 exp(-pi^2 m_k^2 / alpha^2).  exp(-pi^2 m^2 / alpha^2) is separable in the three axes, so the
+// per-wave-vector kernel below needs no exponential.
+__global__ void pme_axis_tables_kernel(const double* __restrict__ mod, int K, double L, double alpha, double* __restrict__ tab)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= K) return;
+    const double m = (double)(k <= K / 2 ? k : k - K) / L;
+    tab[k] = m;
+    tab[K + k] = mod[k] * exp(-M_PI * M_PI * m * m / (alpha * alpha));
+}
+
 // acc[0] += E, acc[1..6] += W (xx, xy, xz, yy, yz, zz)
 template <typename real>
-__global__ __launch_bounds__(256) void pme_solve_kernel(typename cplx<real>::type* __restrict__ spec, int K1, int K2, int K3, double Lx,
-                                                        double Ly, double Lz, double alpha, double ke_over_piV,
-                                                        const double* __restrict__ mod1, const double* __restrict__ mod2,
-                                                        const double* __restrict__ mod3, double* __restrict__ acc)
+__global__ __launch_bounds__(256) void pme_solve_kernel(typename cplx<real>::type* __restrict__ spec, int K1, int K2, int K3, double alpha,
+                                                        double ke_over_piV, const double* __restrict__ t1, const double* __restrict__ t2,
+                                                        const double* __restrict__ t3, double* __restrict__ acc)
 {
     const int K3h = K3 / 2 + 1;
-    const int64_t total = (int64_t)K1 * K2 * K3h;
+    const int64_t rows = (int64_t)K1 * K2;  // one (k1, k2) row of K3h wave vectors per warp iteration
     double v[7] = {0, 0, 0, 0, 0, 0, 0};
     const double pi2_a2 = M_PI * M_PI / (alpha * alpha);
-    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
-        const int k3 = (int)(t % K3h);
-        const int64_t r = t / K3h;
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t r = warp; r < rows; r += n_warps) {
         const int k2 = (int)(r % K2), k1 = (int)(r / K2);
-        if (k1 == 0 && k2 == 0 && k3 == 0) {
-            spec[t].x = (real)0;
-            spec[t].y = (real)0;
-            continue;
+        const double mx = t1[k1], my = t2[k2];
+        const double f12 = ke_over_piV * t1[K1 + k1] * t2[K2 + k2], m12 = mx * mx + my * my;
+        for (int k3 = lane; k3 < K3h; k3 += 32) {
+            const int64_t t = r * K3h + k3;
+            if (k1 == 0 && k2 == 0 && k3 == 0) {
+                spec[t].x = (real)0;
+                spec[t].y = (real)0;
+                continue;
+            }
+            const double mz = t3[k3];  // k3 <= K3/2 in the half spectrum
+            const double m2 = m12 + mz * mz;
+            const double inv_m2 = 1.0 / m2;
+            const double bc = f12 * t3[K3 + k3] * inv_m2;
+            const double re = (double)spec[t].x, im = (double)spec[t].y;
+            // the half spectrum holds every wave vector with 0 < k3 < K3/2 once for itself and once for its conjugate
+            const double wgt = (k3 == 0 || 2 * k3 == K3) ? 1.0 : 2.0;
+            const double e = 0.5 * wgt * bc * (re * re + im * im);
+            const double fac = 2.0 * (inv_m2 + pi2_a2);
+            v[0] += e;
+            v[1] += e * (1.0 - fac * mx * mx);
+            v[2] += e * (-fac * mx * my);
+            v[3] += e * (-fac * mx * mz);
+            v[4] += e * (1.0 - fac * my * my);
+            v[5] += e * (-fac * my * mz);
+            v[6] += e * (1.0 - fac * mz * mz);
+            spec[t].x = (real)(bc * re);
+            spec[t].y = (real)(bc * im);
         }
-        const double mx = (double)(k1 <= K1 / 2 ? k1 : k1 - K1) / Lx;
-        const double my = (double)(k2 <= K2 / 2 ? k2 : k2 - K2) / Ly;
-        const double mz = (double)k3 / Lz;  // k3 <= K3/2 in the half spectrum
-        const double m2 = mx * mx + my * my + mz * mz;
-        const double bc = ke_over_piV * exp(-pi2_a2 * m2) / m2 * mod1[k1] * mod2[k2] * mod3[k3];
-        const double re = (double)spec[t].x, im = (double)spec[t].y;
-        // the half spectrum holds every wave vector with 0 < k3 < K3/2 once for itself and once for its conjugate
-        const double wgt = (k3 == 0 || 2 * k3 == K3) ? 1.0 : 2.0;
-        const double e = 0.5 * wgt * bc * (re * re + im * im);
-        const double fac = 2.0 * (1.0 / m2 + pi2_a2);
-        v[0] += e;
-        v[1] += e * (1.0 - fac * mx * mx);
-        v[2] += e * (-fac * mx * my);
-        v[3] += e * (-fac * mx * mz);
-        v[4] += e * (1.0 - fac * my * my);
-        v[5] += e * (-fac * my * mz);
-        v[6] += e * (1.0 - fac * mz * mz);
-        spec[t].x = (real)(bc * re);
-        spec[t].y = (real)(bc * im);
     }
     __shared__ double sh[8][7];
 #pragma unroll
     for (int q = 0; q < 7; ++q)
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
-    const int lane = threadIdx.x & 31, wi = threadIdx.x >> 5;
+    const int wi = threadIdx.x >> 5;
     if (lane == 0)
         for (int q = 0; q < 7; ++q) sh[wi][q] = v[q];
     __syncthreads();
@@ -337,6 +354,7 @@ void pme_release(Ctx* ctx)
     release(ctx, p->grid);
     release(ctx, p->spec);
     release(ctx, p->moduli);
+    release(ctx, p->tables);
     release(ctx, p->work);
     release(ctx, p->acc);
     delete p;
@@ -368,6 +386,7 @@ static int pme_prepare(Ctx* ctx, const int* K, int order, bool dbl, cudaStream_t
     if ((rc = ensure(ctx, p->spec, n_spec * 2 * rs, s))) return rc;
     if ((rc = ensure(ctx, p->moduli, (size_t)(K[0] + K[1] + K[2]) * sizeof(double), s))) return rc;
     if ((rc = ensure(ctx, p->acc, 8 * sizeof(double), s))) return rc;
+    if ((rc = ensure(ctx, p->tables, (size_t)2 * (K[0] + K[1] + K[2]) * sizeof(double), s))) return rc;
     std::vector<double> mod(K[0] + K[1] + K[2]);
     host_moduli(order, K[0], mod.data());
     host_moduli(order, K[1], mod.data() + K[0]);
@@ -415,8 +434,21 @@ static int pme_recip_typed(Ctx* ctx, const real* pos, const real* charge, int64_
     int nb = (int)((n_spec + 255) / 256);
     if (nb > ctx->sm_count * 8) nb = ctx->sm_count * 8;
     const double* mod = (const double*)p->moduli.p;
-    pme_solve_kernel<real><<<nb, 256, 0, s>>>((typename cplx<real>::type*)p->spec.p, K[0], K[1], K[2], L[0], L[1], L[2], alpha,
-                                              ke / (M_PI * V), mod, mod + K[0], mod + K[0] + K[1], acc);
+    double* tab = (double*)p->tables.p;
+    if (p->tab_alpha != alpha || p->tab_L[0] != L[0] || p->tab_L[1] != L[1] || p->tab_L[2] != L[2]) {  // once per (alpha, box)
+        int off_m = 0, off_t = 0;
+        for (int a = 0; a < 3; ++a) {
+            pme_axis_tables_kernel<<<(K[a] + 255) / 256, 256, 0, s>>>(mod + off_m, K[a], L[a], alpha, tab + off_t);
+            DIMOS_LAUNCH_CHECK(ctx, "pme_axis_tables");
+            off_m += K[a];
+            off_t += 2 * K[a];
+        }
+        p->tab_alpha = alpha;
+        for (int a = 0; a < 3; ++a) p->tab_L[a] = L[a];
+    }
+    nb = ctx->sm_count * 8;
+    pme_solve_kernel<real><<<nb, 256, 0, s>>>((typename cplx<real>::type*)p->spec.p, K[0], K[1], K[2], alpha, ke / (M_PI * V), tab,
+                                              tab + 2 * K[0], tab + 2 * K[0] + 2 * K[1], acc);
     DIMOS_LAUNCH_CHECK(ctx, "pme_solve");
     if (sizeof(real) == 8) fr = cufftExecZ2D(p->inv, (cufftDoubleComplex*)p->spec.p, (cufftDoubleReal*)grid);
     else fr = cufftExecC2R(p->inv, (cufftComplex*)p->spec.p, (cufftReal*)grid);
