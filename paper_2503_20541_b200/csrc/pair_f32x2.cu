@@ -328,7 +328,9 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         return;
     }
     int2 ri = P.row_info[U];
-    unsigned kbuf = 0;  // units processed by this warp: buffer = kbuf & 1, mbarrier phase = (kbuf >> 1) & 1
+    unsigned kbuf = 0;  // units processed by this warp: buffer = kbuf & 1
+    unsigned phase = 0;  // bit b: parity of the next completion of buffer b's mbarrier (flips only when a row was copied into b:
+                         // a unit without entries copies nothing and waits for nothing)
     if (lane == 0 && (ri.x & 0xFFFF) != 0) copy_row(P, U, ri, buf0, bar0, pol_stream);
     // pipeline state handed from one unit to the next: first two entries, first j-atom, the unit's own atoms
     unsigned ea = 0, eb = 0;
@@ -338,6 +340,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     int my_t = 0;
     if ((ri.x & 0xFFFF) != 0) {
         mbar_wait(bar0, 0);
+        phase ^= 1u;
         ea = lds_u32(buf0 + lane * 4u);
         eb = lds_u32(buf0 + lane * 4u + 128u);
         const unsigned jj = min(ea & ENTRY_SLOT_MASK, slot_max);
@@ -419,7 +422,8 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         int my_t_n = 0;
         if (more) {
             if (total_n != 0) {
-                mbar_wait(bar0 + 8u * (b ^ 1u), ((kbuf + 1u) >> 1) & 1u);
+                mbar_wait(bar0 + 8u * (b ^ 1u), (phase >> (b ^ 1u)) & 1u);
+                phase ^= 1u << (b ^ 1u);
                 const unsigned sn = buf0 + (b ^ 1u) * row_bytes + lane * 4u;
                 ea = lds_u32(sn);
                 eb = lds_u32(sn + 128u);

@@ -654,3 +654,32 @@ def test_lj_activity_changes_after_the_build(precision):
         check_neighbor_set(gp, pos64, db.box, 1.1, wb.excl_pairs)
     finally:
         ctx.close()
+
+
+def test_sparse_gas_with_isolated_atoms_f32():
+    """A dilute gas in a box with many cells: most units hold one or two atoms and many have no list entry at all (the
+    packed kernel then copies no row for them and must keep its buffer bookkeeping straight); a few close pairs carry the
+    whole energy."""
+    rng = np.random.default_rng(31)
+    n = 1500
+    box = np.array([14.0, 13.0, 15.0])
+    pos = rng.uniform(0, 1, size=(n, 3)) * box
+    pos[1::2][:300] = pos[0::2][:300] + rng.normal(0, 0.2, size=(300, 3))  # 300 pairs at ~0.35 nm
+    pos = pos.astype(np.float32)
+    q = rng.choice([-0.5, 0.5], size=n).astype(np.float32)
+    typ = rng.integers(0, 2, size=n).astype(np.int32)
+    lj_np = oracle.lorentz_berthelot([0.3, 0.0], [0.5, 0.0])
+    ctx = dimos.Context(0, "f32")
+    try:
+        dp, dq, dt = torch.from_numpy(pos).cuda(), torch.from_numpy(q).cuda(), torch.from_numpy(typ).cuda()
+        lj = torch.from_numpy(lj_np).cuda()
+        nl = dimos.dimos_nl_build(ctx, dp, box, 1.0, 0.1, None)
+        assert nl.stats()["pbc_mode"] == 0
+        for _ in range(2):
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, dp, dq, dt, lj)
+            orc = oracle.nonbonded(pos.astype(np.float64), q, typ, lj_np, box, 1.0, band=BAND)
+            check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, "f32")
+            nl = dimos.dimos_nl_build(ctx, dp, box, 1.0, 0.1, None, nl=nl)
+        check_neighbor_set(dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy(), pos.astype(np.float64), box, 1.1, None)
+    finally:
+        ctx.close()
