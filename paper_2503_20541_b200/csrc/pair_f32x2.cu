@@ -218,6 +218,34 @@ __device__ __forceinline__ void bulk_row_to_smem(unsigned dst, const void* src, 
                  "l"(src), "r"(bytes), "r"(bar), "l"(pol)
                  : "memory");
 }
+// gathers of the next chunk's j-atom: volatile asm so that neither the compiler's scheduler nor its register-pressure
+// heuristics sink them below the arithmetic they are meant to overlap with
+__device__ __forceinline__ float4 ldg_f4(const float4* p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int ldg_s32(const int* p)
+{
+    int v;
+    asm volatile("ld.global.nc.s32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+// j-atom gather straight into shared memory (16 bytes per lane, cp.async): it holds no registers while in flight, so the
+// register allocator cannot turn its destination into scratch for the chunk's arithmetic and push the load behind it
+__device__ __forceinline__ void gather_to_smem(unsigned dst, const float4* p)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\ncp.async.commit_group;" ::"r"(dst), "l"(p) : "memory");
+}
+__device__ __forceinline__ void gather_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void gather_wait_but_one() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+__device__ __forceinline__ float4 lds_f4v(unsigned addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
 __device__ __forceinline__ unsigned lds_u32(unsigned addr)
 {
     unsigned v;
@@ -242,26 +270,30 @@ __device__ __forceinline__ float4 lds_offset(unsigned base, unsigned w)
 //   A row (reorder_rows) is three phases, each with its own loop: KIND 0 = mask-free chunks whose j-atoms have LJ
 //   partners, KIND 1 = chunks that read their i-masks (always with LJ), KIND 2 = mask-free chunks without LJ.  Only
 //   phases 0 and 1 gather the j-atom types (for the chunk after them, too: harmless at the phase boundary).
-#define DIMOS_CHUNK_STEP(KIND, PJ, TJ, PJn, TJn, EC, EN, SOFF)                                                   \
+#define DIMOS_CHUNK_STEP(KIND, GX, TJ, EC, SOFF)                                                                 \
     do {                                                                                                         \
         const float4 off = lds_offset(off_base, EC);                                                             \
+        const float4 PJ = lds_f4v(GX);  /* landed: every step ends with gather_wait_but_one() */                 \
         const unsigned jc = EC & ENTRY_SLOT_MASK;                                                                \
-        {                                                                                                        \
-            const unsigned jj = min(EN & ENTRY_SLOT_MASK, slot_max);                                             \
-            PJn = P.xyzq[jj];                                                                                    \
-            if ((KIND) != 2) TJn = P.stype[jj];                                                                  \
-        }                                                                                                        \
+        const unsigned ljrow = (KIND) != 2 ? ljt_base + ((unsigned)(TJ & STYPE_MASK) << 4) : 0u;                  \
+        /* refill this parity's set for chunk c + 2: entry from the row buffer, j-atom into the slot's twin */   \
         EC = lds_u32(sa + (SOFF) + 256u);                                                                        \
+        GX ^= 1024u;                                                                                             \
+        {                                                                                                        \
+            const unsigned jj = min(EC & ENTRY_SLOT_MASK, slot_max);                                             \
+            gather_to_smem(GX, P.xyzq + jj);                                                                     \
+            if ((KIND) != 2) TJ = ldg_s32(P.stype + jj);                                                         \
+        }                                                                                                        \
         unsigned mk = 0xFFu;                                                                                     \
         if ((KIND) == 1) { mk = c_m < n_m_true ? mk_n : 0xFFu; mk_n = mp[32]; }                                  \
         const float nxj = off.x - PJ.x, nyj = off.y - PJ.y, nzj = off.z - PJ.z; /* -(x_j + image shift) */       \
         float sx, sy, sz;                                                                                        \
-        const unsigned ljrow = (KIND) != 2 ? ljt_base + ((unsigned)(TJ & STYPE_MASK) << 4) : 0u;                  \
         chunk_body<METHOD, SW, (KIND) == 1, (KIND) != 2>(u, k, ljrow, ti16, nxj, nyj, nzj, PJ.w, mk, lj_pairs, sx, sy, sz);      \
         /* virial: x_j' (x) F_j in unit-local coordinates, x_j' = -nxj */                                        \
         w[0] = fmaf(-nxj, sx, w[0]); w[1] = fmaf(-nxj, sy, w[1]); w[2] = fmaf(-nxj, sz, w[2]);                   \
         w[3] = fmaf(-nyj, sy, w[3]); w[4] = fmaf(-nyj, sz, w[4]); w[5] = fmaf(-nzj, sz, w[5]);                   \
         red_add_xyz(P.Facc + jc, sx, sy, sz);                                                                    \
+        gather_wait_but_one();  /* the next chunk's j-atom has landed; the one after it may still be in flight */ \
     } while (0)
 
 // One unit's row into a shared-memory buffer: the chunks at the row's start (LJ-active and masked) and the chunks that
@@ -277,11 +309,20 @@ __device__ __forceinline__ void copy_row(const ForceParams<float>& P, long long 
     if (bytes2) bulk_row_to_smem(dst + bytes1, row + (P.row_cap - P.m_res) - (total - n_am) * 32, bytes2, bar, pol);
 }
 
+// after an odd number of chunks the even / odd register sets change roles
+#define DIMOS_SWAP_SETS()                                               \
+    do {                                                                \
+        const unsigned g_ = gA; gA = gB; gB = g_;                       \
+        const unsigned e_ = ea; ea = eb; eb = e_;                       \
+        const int t_ = tA; tA = tB; tB = t_;                            \
+    } while (0)
+
 template <int METHOD, bool SW>
 __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x2_kernel(ForceParams<float> P)
 {
     __shared__ float4 off_s[32];
     __shared__ __align__(8) unsigned long long bars[FX_WARPS][2];
+    __shared__ __align__(2048) float4 gat_s[FX_WARPS][4][32];  // four gathered-j-atom slots per lane: even chunks use 0 / 2, odd 1 / 3
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     // dynamic shared memory: FX_WARPS x 2 row buffers of P.row_words words (128-byte aligned), then the LJ table
     float4* ljt = reinterpret_cast<float4*>(dyn_smem + (size_t)FX_WARPS * 2 * P.row_words * 4);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
@@ -334,7 +375,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     if (lane == 0 && (ri.x & 0xFFFF) != 0) copy_row(P, U, ri, buf0, bar0, pol_stream);
     // pipeline state handed from one unit to the next: first two entries, first j-atom, the unit's own atoms
     unsigned ea = 0, eb = 0;
-    float4 pA = make_float4(0.f, 0.f, 0.f, 0.f), pB;
+    unsigned gA = smem_u32(&gat_s[wib][0][lane]), gB = smem_u32(&gat_s[wib][1][lane]);  // slot of the current even / odd chunk's j-atom (^ 1024: its twin)
     int tA = 0, tB = 0;
     float4 mine = make_float4(0.f, 0.f, 0.f, 0.f);
     int my_t = 0;
@@ -343,9 +384,11 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         phase ^= 1u;
         ea = lds_u32(buf0 + lane * 4u);
         eb = lds_u32(buf0 + lane * 4u + 128u);
-        const unsigned jj = min(ea & ENTRY_SLOT_MASK, slot_max);
-        pA = P.xyzq[jj];
-        tA = P.stype[jj];
+        const unsigned ja = min(ea & ENTRY_SLOT_MASK, slot_max), jb = min(eb & ENTRY_SLOT_MASK, slot_max);
+        gather_to_smem(gA, P.xyzq + ja);
+        gather_to_smem(gB, P.xyzq + jb);
+        tA = P.stype[ja];
+        tB = P.stype[jb];
     }
     if (lane < UNIT) { mine = P.xyzq[U * UNIT + lane]; my_t = P.stype[U * UNIT + lane]; }
 
@@ -387,22 +430,22 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         u.e_c = f2(0.f, 0.f);
         u.e_lj = f2(0.f, 0.f);
         float w[6] = {0, 0, 0, 0, 0, 0};
+        gather_wait_all();  // the first two chunks' j-atoms, requested at the hand-off
 
         // ---- the row: three phases, two chunks per iteration (ping-pong entry registers and coordinate buffers; a
         //      phase with an odd number of chunks ends with one swap) ----
         for (int c = 0; c < n_a; c += 2) {
-            DIMOS_CHUNK_STEP(0, pA, tA, pB, tB, ea, eb, 0u);
-            if (c + 1 < n_a) { DIMOS_CHUNK_STEP(0, pB, tB, pA, tA, eb, ea, 128u); sa += 256u; }
-            else { pA = pB; tA = tB; const unsigned t_ = ea; ea = eb; eb = t_; sa += 128u; }
+            DIMOS_CHUNK_STEP(0, gA, tA, ea, 0u);
+            if (c + 1 < n_a) { DIMOS_CHUNK_STEP(0, gB, tB, eb, 128u); sa += 256u; }
+            else { DIMOS_SWAP_SETS(); sa += 128u; }
         }
         Un = __shfl_sync(FULL, Un, 0);
         const bool more = Un < P.n_units;
         int2 ri_n = make_int2(0, 0);
         if (more) ri_n = P.row_info[Un];
         for (c_m = 0; c_m < n_m; ++c_m) {
-            DIMOS_CHUNK_STEP(1, pA, tA, pB, tB, ea, eb, 0u);
-            pA = pB; tA = tB;
-            { const unsigned t_ = ea; ea = eb; eb = t_; }
+            DIMOS_CHUNK_STEP(1, gA, tA, ea, 0u);
+            DIMOS_SWAP_SETS();
             sa += 128u;
             mp += 32;
         }
@@ -411,8 +454,8 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
         __syncwarp();
         if (lane == 0 && total_n != 0) copy_row(P, Un, ri_n, buf0 + (b ^ 1u) * row_bytes, bar0 + 8u * (b ^ 1u), pol_stream);
         for (int c = 0; c < n_b; c += 2) {
-            DIMOS_CHUNK_STEP(2, pA, tA, pB, tB, ea, eb, 0u);
-            if (c + 1 < n_b) { DIMOS_CHUNK_STEP(2, pB, tB, pA, tA, eb, ea, 128u); }
+            DIMOS_CHUNK_STEP(2, gA, tA, ea, 0u);
+            if (c + 1 < n_b) { DIMOS_CHUNK_STEP(2, gB, tB, eb, 128u); }
             sa += 256u;
         }
 
@@ -427,9 +470,12 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
                 const unsigned sn = buf0 + (b ^ 1u) * row_bytes + lane * 4u;
                 ea = lds_u32(sn);
                 eb = lds_u32(sn + 128u);
-                const unsigned jj = min(ea & ENTRY_SLOT_MASK, slot_max);
-                pA = P.xyzq[jj];
-                tA = P.stype[jj];
+                const unsigned ja = min(ea & ENTRY_SLOT_MASK, slot_max), jb = min(eb & ENTRY_SLOT_MASK, slot_max);
+                gather_wait_all();  // nothing of this row may still be landing in the slots
+                gather_to_smem(gA, P.xyzq + ja);
+                gather_to_smem(gB, P.xyzq + jb);
+                tA = P.stype[ja];
+                tB = P.stype[jb];
             }
             if (lane < UNIT) { mine_n = P.xyzq[Un * UNIT + lane]; my_t_n = P.stype[Un * UNIT + lane]; }
         }
@@ -468,6 +514,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     if (lane == 1) P.partials[prow + 8] = 0.0;
 }
 #undef DIMOS_CHUNK_STEP
+#undef DIMOS_SWAP_SETS
 
 }  // namespace
 
