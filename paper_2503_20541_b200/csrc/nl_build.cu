@@ -701,11 +701,14 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                 if (pj.w != (real)0) {  // not a padding slot
                     const real4 co = code_off[code];
                     const real px = pj.x + co.x, py = pj.y + co.y, pz = pj.z + co.z;
-                    unsigned bits = 0;
+                    mask = valid_i & ~excl_bits(slot);
                     if constexpr (sizeof(real) == 4 && PBC == 0) {
-                        // fp32, image from the cell offset: two i-atoms per packed instruction (FADD2/FMUL2/FFMA2)
+                        // fp32, image from the cell offset: two i-atoms per packed instruction (FADD2/FMUL2/FFMA2); the common
+                        // case (every i-atom counts) only needs "any i-atom in range": compares OR-ed into one predicate
                         const float2 nx = make_float2(-(float)px, -(float)px), ny = make_float2(-(float)py, -(float)py),
                                      nz = make_float2(-(float)pz, -(float)pz);
+                        float2 r2v[UNIT / 2];
+                        bool any = false;
 #pragma unroll
                         for (int q = 0; q < UNIT / 2; ++q) {
                             const float2 ddx = __fadd2_rn(make_float2((float)xi[2 * q], (float)xi[2 * q + 1]), nx);
@@ -714,10 +717,22 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                             float2 r2 = __fmul2_rn(ddx, ddx);
                             r2 = __ffma2_rn(ddy, ddy, r2);
                             r2 = __ffma2_rn(ddz, ddz, r2);
-                            bits |= (r2.x < (float)P.rnl2 ? 1u : 0u) << (2 * q);
-                            bits |= (r2.y < (float)P.rnl2 ? 1u : 0u) << (2 * q + 1);
+                            r2v[q] = r2;
+                            any = any || r2.x < (float)P.rnl2 || r2.y < (float)P.rnl2;
+                        }
+                        if (mask == 0xFFu) {
+                            acc = any;
+                        } else if (any) {  // exclusions or missing i-atoms: which i-atoms are in range matters
+                            unsigned bits = 0;
+#pragma unroll
+                            for (int q = 0; q < UNIT / 2; ++q) {
+                                bits |= (r2v[q].x < (float)P.rnl2 ? 1u : 0u) << (2 * q);
+                                bits |= (r2v[q].y < (float)P.rnl2 ? 1u : 0u) << (2 * q + 1);
+                            }
+                            acc = (bits & mask) != 0;
                         }
                     } else {
+                        unsigned bits = 0;
 #pragma unroll
                         for (int i = 0; i < UNIT; ++i) {
                             real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
@@ -729,9 +744,8 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
                             real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
                             bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
                         }
+                        acc = (bits & mask) != 0;
                     }
-                    mask = valid_i & ~excl_bits(slot);
-                    acc = (bits & mask) != 0;
                     cls_b = pj.w == (real)1;
                 }
             }
