@@ -7,9 +7,11 @@
 //       first the units whose bounding box is within r_nl of its own, then the individual j-atoms
 //       of those units that have at least one unit atom within r_nl.  Every unordered atom pair is
 //       owned by exactly one unit (circular half-ordering of unit indices; triangular mask inside a
-//       unit).  Entries carry an 8-bit mask (exclusions, intra-unit half, padding) and a stencil
-//       code that selects the periodic image; entries whose mask is not all-ones are stored in a
-//       reserved region in front of the row so the force kernel runs a mask-free loop over the rest.
+//       unit).  An entry is one 32-bit word (slot | stencil code selecting the periodic image); its
+//       8-bit i-mask (exclusions, intra-unit half, padding) goes to a byte array that only the masked
+//       chunks read.  A row is written in the three-phase layout the force kernels walk: j-atoms
+//       assumed LJ-active (the flags of the last force call) upwards from the row's start, the
+//       others downwards from the end of its capacity, masked entries and leftovers in between.
 //
 // All coordinates used here are cell-relative (x - cell origin - wrap*L, formed in fp64 and rounded
 // once), so fp32 distance tests across the periodic seam keep ~1e-7 nm absolute accuracy at any L.
@@ -194,23 +196,6 @@ __global__ void scatter_atoms_kernel(int64_t N, const int* __restrict__ atom_cel
 // ------------------------------------------------------------------------------------------------
 // A1d: per-cell k-d bisection -> compact units of 8 atoms
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void bitonic_sort_u64(unsigned long long* K, int npad)
-{
-    for (int k = 2; k <= npad; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int t = threadIdx.x; t < npad; t += blockDim.x) {
-                int ixj = t ^ j;
-                if (ixj > t) {
-                    unsigned long long a = K[t], b = K[ixj];
-                    bool asc = (t & k) == 0;
-                    if ((a > b) == asc) { K[t] = b; K[ixj] = a; }
-                }
-            }
-            __syncthreads();
-        }
-    }
-}
-
 // Rank sort inside segments: position p (< n) carries local id Kin[p] and the 32-bit key KEY[p]; if its segment
 // [st, st + cnt) is to be sorted (`sort_it`), p moves to st + #{q in the segment: KEY[q] < KEY[p], or equal and q < p}.
 // One pass, no barrier inside, ~3 instructions per comparison: a cell of ~150 atoms needs ~450 comparisons per thread

@@ -351,7 +351,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
             const unsigned mask = plain ? 0xFFu : m;
             real fjx = 0, fjy = 0, fjz = 0;
 
-            // after reorder_rows only the chunks in front of and inside the masked region hold j-atoms with LJ partners
+            // the builder put the j-atoms assumed to have LJ partners in front of and inside the masked region
             const bool lj_chunk = lj_all || c < n_a + (int)n_m;
             if (plain) {
 #pragma unroll

@@ -42,7 +42,7 @@ struct ForceParams {
     const typename vec4<real>::type* lj4;  // (c6, c12, 6 c6, 12 c12) per type pair
     unsigned long long* unit_counter;      // dynamic unit scheduling (zeroed by gather_kernel)
     const int* row_active;   // per type: any non-zero LJ partner
-    const int* order_stale;  // != 0: an atom's LJ activity changed since reorder_rows ran (evaluate LJ everywhere)
+    const int* order_stale;  // != 0: an atom the builder assumed LJ-free has LJ partners (evaluate LJ everywhere)
     real4* Facc;
     real4* Fown;
     double* partials;        // [gridDim.x][N_PART]

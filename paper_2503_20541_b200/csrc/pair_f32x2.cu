@@ -8,12 +8,14 @@
 // freed slots and the kernel is bound by the FMA pipe instead of by instruction issue.
 //
 // Covers: fp32 positions, fp32 accumulation (DIMOS_F32), image shift from the stencil code (pbc_mode 0), reaction
-// field (Eq. 8) and Ewald real space (Eq. 10).  Everything else (fp64, mixed, per-pair minimum image) stays on the
-// generic kernel.
+// field (Eq. 8) and Ewald real space (Eq. 10).  fp64 runs csrc/pair_f64.cu; mixed precision and per-pair minimum image
+// stay on the generic kernel of nonbonded.cu.
 //
-// LJ is evaluated only in chunks in which at least one j-atom has LJ partners (warp vote) and, there, only for
-// i-atom pairs with an LJ-active member; rows are reordered LJ-active-j-first after a build (reorder_rows_kernel
-// below), which is an optimisation only: correctness never depends on the order.
+// Data movement: a unit's row of list entries is staged in the warp's shared-memory buffer by a TMA bulk copy issued one
+// unit ahead; the gathered j-atoms pass through per-lane shared-memory slots filled by cp.async two chunks ahead.
+// LJ is evaluated only in the row's first two phases (the builder filed the j-atoms by the LJ activity of the last force
+// call, see nl_build.cu) and, there, only for i-atom pairs with an LJ-active member; that order is an optimisation:
+// gather_kernel checks the assumption against the real types and the kernel falls back to LJ everywhere.
 #include <math.h>
 
 #include "pair_common.cuh"
@@ -267,7 +269,7 @@ __device__ __forceinline__ float4 lds_offset(unsigned base, unsigned w)
 // replaces EC by the entry of chunk c+2 (two entry registers, two coordinate buffers: nothing is copied at the loop
 // back-edge), and evaluates chunk c.  Reads past the row's last chunk stay inside the buffer's slack and their slot
 // is clamped, so the pipeline needs no guards.
-//   A row (reorder_rows) is three phases, each with its own loop: KIND 0 = mask-free chunks whose j-atoms have LJ
+//   A row is three phases (written that way by build_list), each with its own loop: KIND 0 = mask-free chunks whose j-atoms have LJ
 //   partners, KIND 1 = chunks that read their i-masks (always with LJ), KIND 2 = mask-free chunks without LJ.  Only
 //   phases 0 and 1 gather the j-atom types (for the chunk after them, too: harmless at the phase boundary).
 #define DIMOS_CHUNK_STEP(KIND, GX, TJ, EC, SOFF)                                                                 \
