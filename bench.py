@@ -443,6 +443,14 @@ def run_ours(args, spec, precision):
         h_W = torch.empty((3, 3), dtype=torch.float64).pin_memory()
         hnl = None
         k = 0
+        # first DMA of a freshly page-locked buffer is up to 10x slower on this box (lazy mapping): touch every staging
+        # buffer once before anything is timed, as a caller's buffers would have been after its first step
+        scratch = torch.empty_like(pos)
+        for hp in host_pos:
+            scratch.copy_(hp, non_blocking=True)
+        h_F.copy_(scratch, non_blocking=True)
+        torch.cuda.synchronize()
+        del scratch
         # charge / type / lj_table travel once (first call); afterwards only the positions do
         hnl, _ = ctx.step_host(None, host_pos[0], h_charge, h_type, h_lj, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E, h_W, **kw)
         k = 1
@@ -450,6 +458,21 @@ def run_ours(args, spec, precision):
             hnl, _ = ctx.step_host(hnl, host_pos[k % ring], None, None, None, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E,
                                    h_W, ntypes=h_lj.shape[0], **kw)
             k += 1
+        # settle: up to 60 more untimed steps until 10 steps in a row without a rebuild take within 8 % of the fastest seen
+        # (the first CUDA process on a fresh box has shown host-side transfer times that take a while to come down)
+        best, streak = float("inf"), 0
+        for _ in range(60):
+            ts = time.perf_counter()
+            hnl, rb = ctx.step_host(hnl, host_pos[k % ring], None, None, None, box.box, spec.r_cut, spec.skin, h_excl, h_F, h_E,
+                                    h_W, ntypes=h_lj.shape[0], **kw)
+            k += 1
+            if rb:
+                continue
+            dt_ = time.perf_counter() - ts
+            best = min(best, dt_)
+            streak = streak + 1 if dt_ <= 1.08 * best else 0
+            if streak >= 10:
+                break
         torch.cuda.synchronize()
         if dist:
             dist.barrier()
