@@ -132,7 +132,7 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
                 if (!__any_sync(FULL, in)) continue;  // no lane has this i-atom inside the cutoff
                 double fs = 0.0;
                 if (in) {
-                    const double rinv = 1.0 / sqrt(r2);
+                    const double rinv = rsqrt(r2);  // 1 ulp (CUDA math library), far inside the 1e-10 bar
                     const double rinv2 = rinv * rinv;
                     const double qq = a.w * qj;
                     double fr2;
