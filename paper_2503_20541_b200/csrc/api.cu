@@ -173,6 +173,7 @@ DIMOS_API int dimos_nl_build(dimos_ctx* c, const void* pos, int64_t N, const dou
     const bool same_geom = !created && nl->N == N && nl->r_nl == r_nl && nl->box[0] == box[0] && nl->box[1] == box[1] &&
                            nl->box[2] == box[2];
     if (!same_geom) nl->row_cap = 0;  // re-estimate the row capacity
+    if (nl->N != N) nl->hint_valid = false;  // the LJ-activity flags of the last force call belong to another atom set
     nl->N = N;
     nl->r_cut = r_cut;
     nl->skin = skin;

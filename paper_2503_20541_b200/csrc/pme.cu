@@ -400,9 +400,11 @@ static int pme_prepare(Ctx* ctx, const int* K, int order, bool dbl, cudaStream_t
     cufftSetAutoAllocation(p->fwd, 0);
     cufftSetAutoAllocation(p->inv, 0);
     if (cufftMakePlan3d(p->fwd, K[0], K[1], K[2], dbl ? CUFFT_D2Z : CUFFT_R2C, &ws_f) != CUFFT_SUCCESS ||
-        cufftMakePlan3d(p->inv, K[0], K[1], K[2], dbl ? CUFFT_Z2D : CUFFT_C2R, &ws_i) != CUFFT_SUCCESS)
+        cufftMakePlan3d(p->inv, K[0], K[1], K[2], dbl ? CUFFT_Z2D : CUFFT_C2R, &ws_i) != CUFFT_SUCCESS) {
+        pme_release(ctx);  // no half-made plan may survive for the next call with the same mesh
         return set_error(ctx, DIMOS_ECUDA, "cufftMakePlan3d failed (mesh size not supported)");
-    if ((rc = ensure(ctx, p->work, std::max(ws_f, ws_i), s))) return rc;
+    }
+    if ((rc = ensure(ctx, p->work, std::max(ws_f, ws_i), s))) { pme_release(ctx); return rc; }
     cufftSetWorkArea(p->fwd, p->work.p);
     cufftSetWorkArea(p->inv, p->work.p);
     cufftSetStream(p->fwd, s);
