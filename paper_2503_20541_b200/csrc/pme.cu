@@ -361,7 +361,7 @@ void pme_release(Ctx* ctx)
     ctx->pme = nullptr;
 }
 
-static int pme_prepare(Ctx* ctx, const int* K, int order, bool dbl, cudaStream_t s)
+static int pme_prepare_impl(Ctx* ctx, const int* K, int order, bool dbl, cudaStream_t s)
 {
     PmePlan* p = ctx->pme;
     if (p && (p->K[0] != K[0] || p->K[1] != K[1] || p->K[2] != K[2] || p->order != order || p->dbl != dbl)) {
@@ -410,6 +410,14 @@ static int pme_prepare(Ctx* ctx, const int* K, int order, bool dbl, cudaStream_t
     cufftSetStream(p->fwd, s);
     cufftSetStream(p->inv, s);
     return DIMOS_OK;
+}
+
+// a plan that could not be completed (allocation, cuFFT) is torn down, so that the next call starts from scratch
+static int pme_prepare(Ctx* ctx, const int* K, int order, bool dbl, cudaStream_t s)
+{
+    const int rc = pme_prepare_impl(ctx, K, order, dbl, s);
+    if (rc != DIMOS_OK) pme_release(ctx);
+    return rc;
 }
 
 template <typename real>
