@@ -303,7 +303,9 @@ DIMOS_API int dimos_vv_kick(dimos_ctx* ctx, void* vel, const void* F, const void
  *   vel       dev, N x 3 or NULL: if given, v += (x_constrained - x_unconstrained) / dt, the half-step velocity that goes
  *             with the constrained positions (step 6 is dimos_settle_velocities)
  *   water     dev, n_w x 3 int32: atom indices (O, H1, H2) of each molecule; molecules must be whole (no atom of a molecule
- *             wrapped into another periodic image), which dimos_vv_kick_drift preserves since it never wraps
+ *             wrapped into another periodic image), which dimos_vv_kick_drift preserves since it never wraps.  Every index
+ *             must be a valid row of pos / vel and no atom may belong to two molecules; the call does not receive N, so
+ *             neither is checked (this holds for every call that takes `water`)
  *   m_O, m_H  masses; d_OH, d_HH the constraint lengths (0 < d_HH < 2 d_OH)
  * float or double per the context precision (coordinates enter only as differences to the old oxygen).  Asynchronous on
  * the stream; n_w = 0 is a no-op.  DIMOS_EINVAL for bad lengths, masses or dt. */
