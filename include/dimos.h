@@ -95,6 +95,11 @@ typedef struct {
     double r_switch;      /* LJ switching distance r_s of Eq. 6: for r_s < r < r_c the LJ term is
                            * multiplied by S(x) = 1 - 6x^5 + 15x^4 - 10x^3, x = (r - r_s)/(r_c - r_s); Coulomb terms are
                            * not switched.  <= 0 or >= r_cut: plain truncation at r_cut (reading C-8).  NaN: EINVAL */
+    const int32_t* skip_flag; /* NULL, or a DEVICE word (e.g. the flag_dev of dimos_nl_needs_rebuild): if it is
+                           * non-zero when the kernels of dimos_nonbonded run, they do nothing -- F, E and virial keep their
+                           * old contents -- so that the force call can be enqueued behind the trigger without waiting for the
+                           * host to read the flag; a caller that then finds the flag set rebuilds the list and calls again
+                           * with skip_flag = NULL.  Must be NULL for the *_host entry points (DIMOS_EINVAL otherwise). */
 } dimos_nb_params;
 
 typedef struct {
@@ -201,8 +206,9 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* ctx, dimos_nl* nl, const void* pos
  *   charge_host, type_host, lj_table_host   each may be NULL once a call on this list has passed it: the device copy
  *                 kept in the list is used again, so that only what changed travels (positions travel every step)
  *   rebuilt_host  host, may be NULL: receives 1 if this call (re)built the list, else 0
- * Other arguments as in dimos_nonbonded_host.  Synchronises the stream (twice: once to read the
- * trigger, once at the end). */
+ * Other arguments as in dimos_nonbonded_host.  Synchronises the stream: once on a step that keeps the list (the force
+ * kernels are enqueued behind the trigger, conditional on its device flag, and the results copied back behind them),
+ * otherwise once to read the trigger, inside the rebuild, and once at the end. */
 DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_host, const void* charge_host,
                               const int32_t* type_host, const double* lj_table_host, int32_t ntypes, int64_t N,
                               const double* box, double skin, const int32_t* excl_pairs_host, int64_t n_excl,

@@ -48,7 +48,8 @@ class _Allocator(ctypes.Structure):
 
 class _Params(ctypes.Structure):
     _fields_ = [("r_cut", ctypes.c_double), ("eps_rf", ctypes.c_double), ("alpha", ctypes.c_double),
-                ("coulomb_const", ctypes.c_double), ("method", ctypes.c_int32), ("r_switch", ctypes.c_double)]
+                ("coulomb_const", ctypes.c_double), ("method", ctypes.c_int32), ("r_switch", ctypes.c_double),
+                ("skip_flag", ctypes.c_void_p)]
 
 
 class _Stats(ctypes.Structure):
@@ -301,13 +302,19 @@ class Context:
         self._check(rc)
         return bool(host.value) if sync else (flag if flag is not None else self._flag)
 
-    def _params(self, nl, method, eps_rf, alpha, coulomb_const, r_switch=0.0):
+    def _params(self, nl, method, eps_rf, alpha, coulomb_const, r_switch=0.0, skip_flag=None):
+        skip = None
+        if skip_flag is not None:
+            if not skip_flag.is_cuda or skip_flag.dtype != torch.int32 or skip_flag.numel() < 1:
+                raise ValueError("skip_flag must be an int32 device tensor")
+            skip = skip_flag.data_ptr()
         return _Params(float(nl.r_cut), float(eps_rf), float(alpha), float(coulomb_const),
-                       _METHODS[method] if isinstance(method, str) else int(method), float(r_switch))
+                       _METHODS[method] if isinstance(method, str) else int(method), float(r_switch), skip)
 
     def nonbonded(self, nl: NeighborList, pos, charge, type_, lj_table, *, method="rf", eps_rf=78.5, alpha=3.12,
-                  coulomb_const=138.935456, r_switch=0.0, F=None, E=None, virial=None):
-        """dimos_nonbonded: returns (F (N,3) real, E (4,) float64, virial (3,3) float64) device tensors."""
+                  coulomb_const=138.935456, r_switch=0.0, F=None, E=None, virial=None, skip_flag=None):
+        """dimos_nonbonded: returns (F (N,3) real, E (4,) float64, virial (3,3) float64) device tensors.
+        skip_flag: dimos_nb_params.skip_flag, an int32 device tensor (the kernels do nothing if it is non-zero when they run)."""
         pos = self._dev(pos, self.real, 3)
         n = pos.shape[0]
         charge = self._dev(charge, self.real)
@@ -320,7 +327,7 @@ class Context:
         F = torch.empty_like(pos) if F is None else self._dev(F, self.real, 3)
         E = torch.empty(4, dtype=torch.float64, device=dev) if E is None else self._dev(E, torch.float64)
         virial = torch.empty(3, 3, dtype=torch.float64, device=dev) if virial is None else self._dev(virial, torch.float64)
-        prm = self._params(nl, method, eps_rf, alpha, coulomb_const, r_switch)
+        prm = self._params(nl, method, eps_rf, alpha, coulomb_const, r_switch, skip_flag)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_nonbonded(self.handle, nl.handle, pos.data_ptr(), charge.data_ptr(), type_.data_ptr(),
                                           lj_table.data_ptr(), nt, _box3(nl.box), ctypes.byref(prm), F.data_ptr(),
@@ -349,7 +356,7 @@ class Context:
         for t in (pos, charge, type_, lj_table, F, E, virial, excl_pairs):
             if t is not None and (t.is_cuda or not t.is_contiguous()):
                 raise ValueError("step_host takes contiguous host tensors")
-        prm = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method], float(r_switch))
+        prm = _Params(float(r_cut), float(eps_rf), float(alpha), float(coulomb_const), _METHODS[method], float(r_switch), None)
         h = ctypes.c_void_p(nl.handle.value if nl is not None else None)
         rebuilt = ctypes.c_int32(0)
         n_excl = 0 if excl_pairs is None else excl_pairs.shape[0]

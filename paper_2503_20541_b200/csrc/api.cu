@@ -590,6 +590,7 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* c, dimos_nl* l, const void* pos_ho
     NL* nl = reinterpret_cast<NL*>(l);
     int rc = check_nb_args(ctx, nl, ntypes, box, params);
     if (rc) return rc;
+    if (params->skip_flag) return set_error(ctx, DIMOS_EINVAL, "skip_flag must be NULL for the host entry points");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
     cudaStream_t s = (cudaStream_t)stream;
     const size_t rs = ctx->precision == DIMOS_F64 ? sizeof(double) : sizeof(float);
@@ -626,6 +627,7 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
     if (!c) return DIMOS_EINVAL;
     Ctx* ctx = reinterpret_cast<Ctx*>(c);
     if (!inout || !pos_host || !box || !params || !F_host || !E_host) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
+    if (params->skip_flag) return set_error(ctx, DIMOS_EINVAL, "skip_flag must be NULL for the host entry points");
     if (N <= 0 || n_excl < 0 || (n_excl > 0 && !excl_pairs_host)) return set_error(ctx, DIMOS_EINVAL, "bad N or exclusion list");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
     cudaStream_t s = (cudaStream_t)stream;
@@ -658,9 +660,33 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
             if (lj_table_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(nl->st_lj.p, lj_table_host, (size_t)ntypes * ntypes * 2 * sizeof(double), cudaMemcpyHostToDevice, s));
             static_uploaded = true;
         }
+        // Steady state: the force call goes out behind the trigger, conditional on the device flag (dimos_nb_params.skip_flag),
+        // and its results behind it, so that a step that keeps the list has ONE host synchronisation.  If the flag turns
+        // out set, the kernels did nothing, the copies below carried stale data, and the ordinary path after the rebuild
+        // overwrites them.
+        bool speculative = false;
+        if (static_uploaded && nl->st_F.p && nl->st_EW.p && nl->st_F.bytes >= 3 * (size_t)N * rs && nl->st_static_ntypes == ntypes) {
+            if ((rc = check_nb_args(ctx, nl, ntypes, box, params))) return rc;
+            dimos_nb_params cond = *params;
+            cond.skip_flag = (const int32_t*)nl->st_flag.p;
+            double* EW = (double*)nl->st_EW.p;
+            rc = nonbonded_impl(ctx, nl, nl->st_pos.p, nl->st_charge.p, (const int32_t*)nl->st_type.p, (const double*)nl->st_lj.p, ntypes,
+                                &cond, nl->st_F.p, EW, EW + 4, s);
+            if (rc) return rc;
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(F_host, nl->st_F.p, 3 * (size_t)N * rs, cudaMemcpyDeviceToHost, s));
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(E_host, EW, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
+            if (virial_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(virial_host, EW + 4, 9 * sizeof(double), cudaMemcpyDeviceToHost, s));
+            DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 35, (int*)nl->flags.p + 9, sizeof(int), cudaMemcpyDeviceToHost, s));
+            speculative = true;
+        }
         DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
         flag = ctx->h_pinned[33];
         fresh = flag != 0;
+        if (!fresh && speculative) {
+            if (rebuilt_host) *rebuilt_host = 0;
+            if (ctx->h_pinned[35]) return set_error(ctx, DIMOS_EINVAL, "type index out of range [0, ntypes)");
+            return DIMOS_OK;
+        }
     } else {
         // first call (or changed geometry): a throw-away device copy of pos/excl, then a normal build
         DevBuf tmp_pos, tmp_ref, tmp_excl;

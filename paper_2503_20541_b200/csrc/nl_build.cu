@@ -520,8 +520,11 @@ __device__ __forceinline__ real axis_gap(real lo1, real hi1, real lo2, real hi2,
     return g;
 }
 
+#ifndef BL_MIN_CTAS
+#define BL_MIN_CTAS 7  // 72 registers: 28 warps per SM (6 CTAs at 80+ registers measured 8 % slower, 8 CTAs spill)
+#endif
 template <typename real, int PBC>
-__global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<real> P)
+__global__ __launch_bounds__(BL_WARPS * 32, (sizeof(real) == 4 && PBC == 0) ? BL_MIN_CTAS : 1) void build_list_kernel(BuildParams<real> P)
 {
     using real4 = typename vec4<real>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -596,23 +599,34 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
     int nub = 0;  // mask-free entries of the others: written downwards from the end of the row's capacity
     bool lost = false;  // warp-uniform: the cursors met
     const int nu_cap = P.row_cap - P.m_res;
+    // the row's mask-free region: A upwards from [0], B downwards from [nu_cap - 1].  The pointer goes through an opaque
+    // move so that it stays ONE 64-bit register pair (ptxas otherwise re-adds row, m_res and the base for every store)
+    unsigned* row_up;
+    {
+        unsigned* t = P.entry + row + P.m_res;
+        asm volatile("mov.b64 %0, %1;" : "=l"(row_up) : "l"(t));
+    }
 
     // append one warp-wide batch of entries; cls_b: the j-atom is assumed to have no LJ partners
     auto append = [&](bool accept, unsigned mask, int j, int code, bool cls_b) {
         const bool is_masked = accept && mask != 0xFFu;
         const bool is_a = accept && !is_masked && !cls_b;
         const bool is_b = accept && !is_masked && cls_b;
-        const unsigned bm = __ballot_sync(FULL, is_masked), ba = __ballot_sync(FULL, is_a), bb = __ballot_sync(FULL, is_b);
-        if (is_masked) {
-            int pos = nm + __popc(bm & lt_mask);
-            if (pos < P.m_res) { st_j[pos] = (int)entry_pack(j, code); st_meta[pos] = (unsigned short)mask; }
+        const unsigned ba = __ballot_sync(FULL, is_a), bb = __ballot_sync(FULL, is_b);
+        const unsigned e = entry_pack(j, code);
+        if (__any_sync(FULL, is_masked)) {  // rare: a j-atom with an exclusion partner in the unit
+            const unsigned bm = __ballot_sync(FULL, is_masked);
+            if (is_masked) {
+                const int pos = nm + __popc(bm & lt_mask);
+                if (pos < P.m_res) { st_j[pos] = (int)e; st_meta[pos] = (unsigned short)mask; }
+            }
+            nm += __popc(bm);
         }
         // the two cursors never write into each other's current batch; once they would, nothing more is written and
         // the row is reported as overflowed (the host grows row_cap and rebuilds)
         if (nua + nub + 64 > nu_cap) lost = true;
-        if (is_a && !lost) P.entry[row + P.m_res + nua + __popc(ba & lt_mask)] = entry_pack(j, code);
-        if (is_b && !lost) P.entry[row + P.m_res + nu_cap - 1 - (nub + __popc(bb & lt_mask))] = entry_pack(j, code);
-        nm += __popc(bm);
+        if (is_a && !lost) row_up[nua + __popc(ba & lt_mask)] = e;
+        if (is_b && !lost) row_up[nu_cap - 1 - (nub + __popc(bb & lt_mask))] = e;
         nua += __popc(ba);
         nub += __popc(bb);
     };
@@ -631,13 +645,14 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
         nua += __popc(bp);
     };
 
+    // i-mask bits of the unit's atoms that exclude the atom in `slot`
     auto excl_bits = [&](int slot) -> unsigned {
         unsigned ex = 0;
-        if (slot >= ex_lo && slot <= ex_hi)
-            for (int k = 0; k < n_ex; ++k)
-                if (ex_slot[k] == slot) ex |= 1u << ex_i[k];
+        for (int k = 0; k < n_ex; ++k)
+            if (ex_slot[k] == slot) ex |= 1u << ex_i[k];
         return ex;
     };
+    const int ex_ulo = ex_lo >> 3, ex_uhi = ex_hi >> 3;  // range of the units that hold an exclusion partner (empty: lo > hi)
 
     // ---- own-unit entries: the i < j half ----
     {
@@ -670,79 +685,96 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
     }
 
     int ncand = 0;
-    // atom-level pass over the buffered candidate units
+    constexpr int CAND_EXCL = 0x20;  // cand_code bit: the candidate unit holds an exclusion partner of one of the unit's atoms
+    // atom-level pass over the buffered candidate units: one j-atom per lane, the next batch's atoms requested before the
+    // current batch is tested (the LDS -> LDG chain of a batch is as long as its arithmetic)
     auto flush = [&]() {
         const int T = ncand * UNIT;
-        for (int t0 = 0; t0 < T; t0 += 32) {
-            const int t = t0 + lane;
-            bool acc = false, cls_b = false;
-            unsigned mask = 0;
-            int slot = 0, code = SELF_CODE;
+        int slot_n = 0, code_n = SELF_CODE;
+        real4 pj_n = make4((real)0, (real)0, (real)0, (real)0);  // w = 0: padding, never accepted
+        auto fetch = [&](int t) {
+            slot_n = 0;
+            code_n = SELF_CODE;
+            pj_n.w = (real)0;
             if (t < T) {
-                const int v = cand_unit[t >> 3];
-                code = cand_code[t >> 3];
-                slot = v * UNIT + (t & 7);
-                const real4 pj = P.xyz[slot];
-                if (pj.w != (real)0) {  // not a padding slot
-                    const real4 co = code_off[code];
-                    const real px = pj.x + co.x, py = pj.y + co.y, pz = pj.z + co.z;
-                    mask = valid_i & ~excl_bits(slot);
-                    if constexpr (sizeof(real) == 4 && PBC == 0) {
-                        // fp32, image from the cell offset: two i-atoms per packed instruction (FADD2/FMUL2/FFMA2); the common
-                        // case (every i-atom counts) only needs "any i-atom in range": compares OR-ed into one predicate
-                        const float2 nx = make_float2(-(float)px, -(float)px), ny = make_float2(-(float)py, -(float)py),
-                                     nz = make_float2(-(float)pz, -(float)pz);
-                        float2 r2v[UNIT / 2];
-                        bool any = false;
+                code_n = cand_code[t >> 3];
+                slot_n = cand_unit[t >> 3] * UNIT + (t & 7);
+                pj_n = P.xyz[slot_n];
+            }
+        };
+        fetch(lane);
+        for (int t0 = 0; t0 < T; t0 += 32) {
+            const int slot = slot_n, code_f = code_n;
+            const real4 pj = pj_n;
+            fetch(t0 + 32 + lane);
+            const int code = code_f & 0x1F;
+            bool acc = false;
+            const bool cls_b = pj.w == (real)1;
+            unsigned mask = valid_i;
+            if (__any_sync(FULL, (code_f & CAND_EXCL) != 0)) {
+                if (code_f & CAND_EXCL) mask &= ~excl_bits(slot);
+            }
+            const real4 co = code_off[code];
+            const real px = pj.x + co.x, py = pj.y + co.y, pz = pj.z + co.z;
+            if constexpr (sizeof(real) == 4 && PBC == 0) {
+                // fp32, image from the cell offset: two i-atoms per packed instruction (FADD2/FMUL2/FFMA2); the common
+                // case (every i-atom counts) only needs "any i-atom in range": the smallest of the 8 squared distances
+                const float2 nx = make_float2(-(float)px, -(float)px), ny = make_float2(-(float)py, -(float)py),
+                             nz = make_float2(-(float)pz, -(float)pz);
+                float2 r2v[UNIT / 2];
+                bool any = false;
 #pragma unroll
-                        for (int q = 0; q < UNIT / 2; ++q) {
-                            const float2 ddx = __fadd2_rn(make_float2((float)xi[2 * q], (float)xi[2 * q + 1]), nx);
-                            const float2 ddy = __fadd2_rn(make_float2((float)yi[2 * q], (float)yi[2 * q + 1]), ny);
-                            const float2 ddz = __fadd2_rn(make_float2((float)zi[2 * q], (float)zi[2 * q + 1]), nz);
-                            float2 r2 = __fmul2_rn(ddx, ddx);
-                            r2 = __ffma2_rn(ddy, ddy, r2);
-                            r2 = __ffma2_rn(ddz, ddz, r2);
-                            r2v[q] = r2;
-                            any = any || r2.x < (float)P.rnl2 || r2.y < (float)P.rnl2;
-                        }
-                        if (mask == 0xFFu) {
-                            acc = any;
-                        } else if (any) {  // exclusions or missing i-atoms: which i-atoms are in range matters
-                            unsigned bits = 0;
-#pragma unroll
-                            for (int q = 0; q < UNIT / 2; ++q) {
-                                bits |= (r2v[q].x < (float)P.rnl2 ? 1u : 0u) << (2 * q);
-                                bits |= (r2v[q].y < (float)P.rnl2 ? 1u : 0u) << (2 * q + 1);
-                            }
-                            acc = (bits & mask) != 0;
-                        }
-                    } else {
-                        unsigned bits = 0;
-#pragma unroll
-                        for (int i = 0; i < UNIT; ++i) {
-                            real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
-                            if (PBC == 1) {
-                                ddx -= P.L[0] * rint_r(ddx / P.L[0]);
-                                ddy -= P.L[1] * rint_r(ddy / P.L[1]);
-                                ddz -= P.L[2] * rint_r(ddz / P.L[2]);
-                            }
-                            real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                            bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
-                        }
-                        acc = (bits & mask) != 0;
-                    }
-                    cls_b = pj.w == (real)1;
+                for (int q = 0; q < UNIT / 2; ++q) {
+                    const float2 ddx = __fadd2_rn(make_float2((float)xi[2 * q], (float)xi[2 * q + 1]), nx);
+                    const float2 ddy = __fadd2_rn(make_float2((float)yi[2 * q], (float)yi[2 * q + 1]), ny);
+                    const float2 ddz = __fadd2_rn(make_float2((float)zi[2 * q], (float)zi[2 * q + 1]), nz);
+                    float2 r2 = __fmul2_rn(ddx, ddx);
+                    r2 = __ffma2_rn(ddy, ddy, r2);
+                    r2 = __ffma2_rn(ddz, ddz, r2);
+                    r2v[q] = r2;
+                    any = any || r2.x < (float)P.rnl2 || r2.y < (float)P.rnl2;
                 }
+                any = any && pj.w != (real)0;
+                if (mask == 0xFFu) {
+                    acc = any;
+                } else if (any) {  // exclusions or missing i-atoms: which i-atoms are in range matters
+                    unsigned bits = 0;
+#pragma unroll
+                    for (int q = 0; q < UNIT / 2; ++q) {
+                        bits |= (r2v[q].x < (float)P.rnl2 ? 1u : 0u) << (2 * q);
+                        bits |= (r2v[q].y < (float)P.rnl2 ? 1u : 0u) << (2 * q + 1);
+                    }
+                    acc = (bits & mask) != 0;
+                }
+            } else {
+                unsigned bits = 0;
+#pragma unroll
+                for (int i = 0; i < UNIT; ++i) {
+                    real ddx = xi[i] - px, ddy = yi[i] - py, ddz = zi[i] - pz;
+                    if (PBC == 1) {
+                        ddx -= P.L[0] * rint_r(ddx / P.L[0]);
+                        ddy -= P.L[1] * rint_r(ddy / P.L[1]);
+                        ddz -= P.L[2] * rint_r(ddz / P.L[2]);
+                    }
+                    real r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                    bits |= (r2 < P.rnl2 ? 1u : 0u) << i;
+                }
+                acc = (bits & mask) != 0 && pj.w != (real)0;
             }
             append_any(acc, mask, slot, code, cls_b);
         }
         ncand = 0;
     };
 
-    // Stencil table, one lane per (de-duplicated) stencil cell: its unit range, image code, and whether any of its units
-    // can be owned by U.  Ownership is an arc of n_units/2 consecutive unit indices, far longer than a cell's range, so
-    // a cell neither of whose end units is owned (and that does not hold U itself) has no owned unit at all.
+    // Stencil table, one lane per (de-duplicated) stencil cell: the range of its units that U owns, and the image code.
+    // Ownership (owns()) is an arc of unit indices, U + 1 .. U + d_max modulo n_units, and a cell's units are consecutive
+    // indices, so the owned units of a cell are the cell's range clipped to the arc: the scan below then visits owned
+    // units only and needs no ownership test.  A range that meets both pieces of a wrapped arc (possible only when one
+    // cell holds about half of all units) is kept whole and the test is made per candidate (`test_owns`).
+    const int n_u = (int)P.n_units;  // n_slots <= 2^27 (checked by the host): unit indices fit in an int
+    const int iU = (int)U;
     int my_us = 0, my_cnt = 0, my_code = SELF_CODE;
+    bool both = false;
     {
         const int ns = sn[0] * sn[1] * sn[2];
         if (lane < ns) {
@@ -757,12 +789,18 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
             const int c2 = (scx * P.g.n[1] + scy) * P.g.n[2] + scz;
             my_code = stencil_code(sdx, sdy, sdz);
             const int us = P.unit_start[c2], ue = P.unit_start[c2 + 1];
-            my_us = us;
-            my_cnt = ue - us;
-            if (my_cnt > 0 && P.n_units >= 256 && !(U >= us && U < ue) && !owns(U, us, P.n_units) && !owns(U, ue - 1, P.n_units))
-                my_cnt = 0;
+            const int d_max = (n_u - 1) / 2 + (((n_u & 1) == 0 && iU < n_u / 2) ? 1 : 0);
+            const int a_hi = iU + d_max;  // last index of the arc, before wrapping
+            const int lo1 = max(us, iU + 1), hi1 = min(ue, min(a_hi, n_u - 1) + 1);  // [U + 1, min(a_hi, n - 1)]
+            const int lo2 = us, hi2 = a_hi >= n_u ? min(ue, a_hi - n_u + 1) : us;       // [0, a_hi - n]
+            const bool p1 = hi1 > lo1, p2 = hi2 > lo2;
+            both = p1 && p2;
+            if (both) { my_us = us; my_cnt = ue - us; }
+            else if (p1) { my_us = lo1; my_cnt = hi1 - lo1; }
+            else if (p2) { my_us = lo2; my_cnt = hi2 - lo2; }
         }
     }
+    const bool test_owns = __any_sync(FULL, both);
     int my_pre = my_cnt;  // exclusive prefix sum of the unit counts over the stencil lanes
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -784,16 +822,22 @@ __global__ __launch_bounds__(BL_WARPS * 32) void build_list_kernel(BuildParams<r
             const int pt = __shfl_sync(FULL, my_pre, t & 31);
             if (t < 32 && pt <= f) c = t;
         }
-        const int c_us = __shfl_sync(FULL, my_us, c), c_pre = __shfl_sync(FULL, my_pre, c), code = __shfl_sync(FULL, my_code, c);
+        const int c_us = __shfl_sync(FULL, my_us, c), c_pre = __shfl_sync(FULL, my_pre, c);
+        int code = __shfl_sync(FULL, my_code, c);
         const int v = c_us + (f - c_pre);
-        bool acc = false;
-        if (f < n_scan && v != U && owns(U, v, P.n_units)) {
+        bool acc = f < n_scan;
+        if (test_owns) acc = acc && v != iU && owns(U, v, P.n_units);
+        if (acc) {
             const real4 co = code_off[code];
             real4 lo = P.bb_lo[v], hi = P.bb_hi[v];
             real gx = axis_gap<real, PBC>(ulo.x, uhi.x, lo.x + co.x, hi.x + co.x, P.L[0]);
             real gy = axis_gap<real, PBC>(ulo.y, uhi.y, lo.y + co.y, hi.y + co.y, P.L[1]);
             real gz = axis_gap<real, PBC>(ulo.z, uhi.z, lo.z + co.z, hi.z + co.z, P.L[2]);
             acc = gx * gx + gy * gy + gz * gz < P.rnl2;
+            if (acc && v >= ex_ulo && v <= ex_uhi) {  // does this unit hold an exclusion partner?
+                for (int k = 0; k < n_ex; ++k)
+                    if ((ex_slot[k] >> 3) == v) code |= CAND_EXCL;
+            }
         }
         unsigned b = __ballot_sync(FULL, acc);
         if (acc) {

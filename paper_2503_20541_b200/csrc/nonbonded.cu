@@ -129,8 +129,9 @@ __global__ void gather_kernel(const real* __restrict__ pos, const real* __restri
                               typename vec4<real>::type* __restrict__ Facc, const double* __restrict__ lj_table, int nt,
                               real* __restrict__ lj_out, int* __restrict__ row_active, double* __restrict__ accum,
                               int* __restrict__ order_stale, const unsigned char* __restrict__ slot_hint,
-                              unsigned char* __restrict__ atom_active)
+                              unsigned char* __restrict__ atom_active, const int* __restrict__ skip)
 {
+    if (skip != nullptr && *skip != 0) return;  // dimos_nb_params.skip_flag: the list is stale, the caller rebuilds and calls again
     // per type: does it have any non-zero LJ partner?  (every block recomputes the tiny table: no inter-block order)
     __shared__ int act_sh[MAX_TYPES];
     for (int t = threadIdx.x; t < nt; t += blockDim.x) {
@@ -274,6 +275,7 @@ __global__ __launch_bounds__(PF_WARPS * 32, sizeof(real) == 4 ? 2 : 1) void pair
     extern __shared__ __align__(16) unsigned char dyn_smem[];
     real4* ljt = reinterpret_cast<real4*>(dyn_smem);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
 
+    if (P.skip != nullptr && *P.skip != 0) return;  // dimos_nb_params.skip_flag (the whole grid sees the same word)
     for (int k = threadIdx.x; k < P.nt * P.nt; k += blockDim.x) ljt[k] = P.lj4[k];
     if (threadIdx.x < 27) {
         const int c = threadIdx.x;
@@ -406,8 +408,10 @@ template <typename real>
 __global__ void excl_correction_kernel(const int2* __restrict__ pairs, int64_t n_excl, const int* __restrict__ inv_perm,
                                        const typename vec4<real>::type* __restrict__ xyzq, const double* __restrict__ ref,
                                        typename vec4<real>::type* __restrict__ Facc, double* __restrict__ partials,
-                                       real ke, real alpha, real two_a_sqrtpi, double Lx, double Ly, double Lz)
+                                       real ke, real alpha, real two_a_sqrtpi, double Lx, double Ly, double Lz,
+                                       const int* __restrict__ skip)
 {
+    if (skip != nullptr && *skip != 0) return;  // dimos_nb_params.skip_flag: the list is stale, the caller rebuilds and calls again
     using real4 = typename vec4<real>::type;
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     double e = 0, w[6] = {0, 0, 0, 0, 0, 0};
@@ -469,8 +473,9 @@ __global__ void exceptions_kernel(const int2* __restrict__ pairs, const double2*
                                   const int* __restrict__ stype, const double* __restrict__ ref,
                                   const double* __restrict__ lj_table, int nt,
                                   typename vec4<real>::type* __restrict__ Facc, double* __restrict__ partials, real ke,
-                                  double Lx, double Ly, double Lz)
+                                  double Lx, double Ly, double Lz, const int* __restrict__ skip)
 {
+    if (skip != nullptr && *skip != 0) return;  // dimos_nb_params.skip_flag: the list is stale, the caller rebuilds and calls again
     using real4 = typename vec4<real>::type;
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // E_lj, E_coul, Wxx, Wxy, Wxz, Wyy, Wyz, Wzz
@@ -551,8 +556,9 @@ __global__ void finalize_kernel(const int* __restrict__ perm, int64_t n_slots,
                                 const typename vec4<real>::type* __restrict__ Fown,
                                 const typename vec4<real>::type* __restrict__ Facc, real* __restrict__ F,
                                 const double* __restrict__ partials, int64_t n_part_rows, double* __restrict__ accum,
-                                double* __restrict__ E, double* __restrict__ W)
+                                double* __restrict__ E, double* __restrict__ W, const int* __restrict__ skip)
 {
+    if (skip != nullptr && *skip != 0) return;  // dimos_nb_params.skip_flag: the list is stale, the caller rebuilds and calls again
     using real4 = typename vec4<real>::type;
     for (int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; s < n_slots; s += (int64_t)gridDim.x * blockDim.x) {
         const int o = perm[s];
@@ -733,20 +739,24 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     real* lj_dev = (real*)nl->lj.p;
     int* row_active = (int*)((char*)nl->lj.p + (size_t)MAX_TYPES * MAX_TYPES * 4 * sizeof(double));
 
+    const int* skip = reinterpret_cast<const int*>(prm->skip_flag);
     const int T = 256;
     gather_kernel<real><<<(unsigned)((nsl + T - 1) / T), T, 0, s>>>(pos, charge, type, (const int*)nl->perm.p, (const double*)nl->ref.p,
                                                                     nsl, (real4*)nl->xyzq.p, (int*)nl->stype.p, (real4*)nl->Facc.p,
                                                                     lj_table, nt, lj_dev, row_active, (double*)nl->accum.p,
                                                                     (int*)nl->flags.p + 8, (const unsigned char*)nl->slot_hint.p,
-                                                                    (unsigned char*)nl->atom_active.p);
+                                                                    (unsigned char*)nl->atom_active.p, skip);
     DIMOS_LAUNCH_CHECK(ctx, "gather");
-    nl->hint_valid = true;  // atom_active now holds this call's LJ-activity flags: the next build files its entries by them
+    // atom_active now holds this call's LJ-activity flags: the next build files its entries by them (a call that may be
+    // skipped on the device proves nothing; the unconditional call after the rebuild does)
+    if (skip == nullptr) nl->hint_valid = true;
 
     ForceParams<real> P;
     P.n_units = nun; P.n_slots = nsl; P.row_cap = nl->row_cap; P.m_res = nl->m_res; P.nt = nt;
     P.xyzq = (const real4*)nl->xyzq.p; P.stype = (const int*)nl->stype.p;
     P.entry = (const unsigned*)nl->entry.p; P.emask = (const unsigned char*)nl->emask.p; P.row_info = (const int2*)nl->row_info.p;
     P.lj4 = (const real4*)lj_dev; P.row_active = row_active; P.order_stale = (const int*)nl->flags.p + 8;
+    P.skip = skip;
     P.unit_counter = reinterpret_cast<unsigned long long*>((double*)nl->accum.p + 14);
     P.Facc = (real4*)nl->Facc.p; P.Fown = (real4*)nl->Fown.p; P.partials = (double*)nl->partials.p;
     const double rc_ = prm->r_cut;
@@ -777,7 +787,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
         excl_correction_kernel<real><<<nb_excl, 256, 0, s>>>((const int2*)nl->excl_pairs.p, nl->n_excl, (const int*)nl->inv_perm.p,
                                                               (const real4*)nl->xyzq.p, (const double*)nl->ref.p, (real4*)nl->Facc.p,
                                                               (double*)nl->partials.p + n_force_rows * N_PART, P.ke, P.alpha,
-                                                              P.two_a_sqrtpi, nl->grid.L[0], nl->grid.L[1], nl->grid.L[2]);
+                                                              P.two_a_sqrtpi, nl->grid.L[0], nl->grid.L[1], nl->grid.L[2], skip);
         DIMOS_LAUNCH_CHECK(ctx, "excl_correction");
     }
     if (nb_exc) {
@@ -785,7 +795,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
                                                         (const int*)nl->inv_perm.p, (const real4*)nl->xyzq.p, (const int*)nl->stype.p,
                                                         (const double*)nl->ref.p, lj_table, nt, (real4*)nl->Facc.p,
                                                         (double*)nl->partials.p + (n_force_rows + nb_excl) * N_PART, P.ke,
-                                                        nl->grid.L[0], nl->grid.L[1], nl->grid.L[2]);
+                                                        nl->grid.L[0], nl->grid.L[1], nl->grid.L[2], skip);
         DIMOS_LAUNCH_CHECK(ctx, "exceptions");
     }
     int fb = (int)((nsl + T - 1) / T);
@@ -793,7 +803,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     if (fb > maxfb) fb = maxfb;
     if (fb < 1) fb = 1;
     finalize_kernel<real><<<fb, T, 0, s>>>((const int*)nl->perm.p, nsl, (const real4*)nl->Fown.p, (const real4*)nl->Facc.p, F,
-                                           (const double*)nl->partials.p, (int64_t)n_force_rows + nb_excl + nb_exc, (double*)nl->accum.p, E, W);
+                                           (const double*)nl->partials.p, (int64_t)n_force_rows + nb_excl + nb_exc, (double*)nl->accum.p, E, W, skip);
     DIMOS_LAUNCH_CHECK(ctx, "finalize");
     return DIMOS_OK;
 }

@@ -43,6 +43,7 @@ struct ForceParams {
     unsigned long long* unit_counter;      // dynamic unit scheduling (zeroed by gather_kernel)
     const int* row_active;   // per type: any non-zero LJ partner
     const int* order_stale;  // != 0: an atom the builder assumed LJ-free has LJ partners (evaluate LJ everywhere)
+    const int* skip;         // dimos_nb_params.skip_flag: NULL, or a device word; != 0 when the kernel runs: do nothing
     real4* Facc;
     real4* Fown;
     double* partials;        // [gridDim.x][N_PART]

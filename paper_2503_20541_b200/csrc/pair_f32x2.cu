@@ -329,6 +329,7 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
     // dynamic shared memory: FX_WARPS x 2 row buffers of P.row_words words (128-byte aligned), then the LJ table
     float4* ljt = reinterpret_cast<float4*>(dyn_smem + (size_t)FX_WARPS * 2 * P.row_words * 4);  // [nt*nt] (c6, c12, 6 c6, 12 c12)
 
+    if (P.skip != nullptr && *P.skip != 0) return;  // dimos_nb_params.skip_flag (the whole grid sees the same word)
     const unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int wib = threadIdx.x >> 5;

@@ -54,6 +54,7 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
     double4* ljt = reinterpret_cast<double4*>(dyn_smem);                          // [nt*nt] (c6, c12, 6 c6, 12 c12)
     double* facc = reinterpret_cast<double*>(ljt + P.nt * P.nt);                  // [F64_WARPS][UNIT*3][F64_PAD]
 
+    if (P.skip != nullptr && *P.skip != 0) return;  // dimos_nb_params.skip_flag (the whole grid sees the same word)
     for (int t = threadIdx.x; t < P.nt * P.nt; t += blockDim.x) ljt[t] = P.lj4[t];
     if (threadIdx.x < 27) {
         const int c = threadIdx.x;
