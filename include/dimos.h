@@ -206,9 +206,9 @@ DIMOS_API int dimos_nonbonded_host(dimos_ctx* ctx, dimos_nl* nl, const void* pos
  *   charge_host, type_host, lj_table_host   each may be NULL once a call on this list has passed it: the device copy
  *                 kept in the list is used again, so that only what changed travels (positions travel every step)
  *   rebuilt_host  host, may be NULL: receives 1 if this call (re)built the list, else 0
- * Other arguments as in dimos_nonbonded_host.  Synchronises the stream: once on a step that keeps the list (the force
- * kernels are enqueued behind the trigger, conditional on its device flag, and the results copied back behind them),
- * otherwise once to read the trigger, inside the rebuild, and once at the end. */
+ * Other arguments as in dimos_nonbonded_host.  Synchronises with the host: on a step that keeps the list the force
+ * kernels are enqueued behind the trigger, conditional on its device flag, the host waits for the flag alone while they
+ * run, then for the results; otherwise once to read the trigger, inside the rebuild, and once at the end. */
 DIMOS_API int dimos_step_host(dimos_ctx* ctx, dimos_nl** inout, const void* pos_host, const void* charge_host,
                               const int32_t* type_host, const double* lj_table_host, int32_t ntypes, int64_t N,
                               const double* box, double skin, const int32_t* excl_pairs_host, int64_t n_excl,

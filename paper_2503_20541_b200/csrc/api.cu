@@ -126,6 +126,7 @@ DIMOS_API int dimos_destroy(dimos_ctx* c)
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     if (ctx->d_rebuild_state) cudaFree(ctx->d_rebuild_state);
     for (cudaEvent_t e : ctx->prof_events) cudaEventDestroy(e);
+    if (ctx->ev_flag) cudaEventDestroy(ctx->ev_flag);
     delete ctx;
     return DIMOS_OK;
 }
@@ -661,28 +662,34 @@ DIMOS_API int dimos_step_host(dimos_ctx* c, dimos_nl** inout, const void* pos_ho
             static_uploaded = true;
         }
         // Steady state: the force call goes out behind the trigger, conditional on the device flag (dimos_nb_params.skip_flag),
-        // and its results behind it, so that a step that keeps the list has ONE host synchronisation.  If the flag turns
-        // out set, the kernels did nothing, the copies below carried stale data, and the ordinary path after the rebuild
-        // overwrites them.
+        // while the host waits only for the flag (an event behind its copy): a step that keeps the list never leaves the
+        // GPU idle between the trigger and the force kernels.  If the flag turns out set, the kernels did nothing and the
+        // ordinary path below rebuilds and computes.
         bool speculative = false;
         if (static_uploaded && nl->st_F.p && nl->st_EW.p && nl->st_F.bytes >= 3 * (size_t)N * rs && nl->st_static_ntypes == ntypes) {
             if ((rc = check_nb_args(ctx, nl, ntypes, box, params))) return rc;
+            if (!ctx->ev_flag) DIMOS_CUDA_TRY(ctx, cudaEventCreateWithFlags(&ctx->ev_flag, cudaEventDisableTiming));
+            DIMOS_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_flag, s));
             dimos_nb_params cond = *params;
             cond.skip_flag = (const int32_t*)nl->st_flag.p;
             double* EW = (double*)nl->st_EW.p;
             rc = nonbonded_impl(ctx, nl, nl->st_pos.p, nl->st_charge.p, (const int32_t*)nl->st_type.p, (const double*)nl->st_lj.p, ntypes,
                                 &cond, nl->st_F.p, EW, EW + 4, s);
             if (rc) return rc;
+            speculative = true;
+            DIMOS_CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_flag));
+        } else {
+            DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+        }
+        flag = ctx->h_pinned[33];
+        fresh = flag != 0;
+        if (!fresh && speculative) {
+            double* EW = (double*)nl->st_EW.p;
             DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(F_host, nl->st_F.p, 3 * (size_t)N * rs, cudaMemcpyDeviceToHost, s));
             DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(E_host, EW, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
             if (virial_host) DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(virial_host, EW + 4, 9 * sizeof(double), cudaMemcpyDeviceToHost, s));
             DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_pinned + 35, (int*)nl->flags.p + 9, sizeof(int), cudaMemcpyDeviceToHost, s));
-            speculative = true;
-        }
-        DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
-        flag = ctx->h_pinned[33];
-        fresh = flag != 0;
-        if (!fresh && speculative) {
+            DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
             if (rebuilt_host) *rebuilt_host = 0;
             if (ctx->h_pinned[35]) return set_error(ctx, DIMOS_EINVAL, "type index out of range [0, ntypes)");
             return DIMOS_OK;

@@ -58,6 +58,7 @@ struct Ctx {
     int* h_pinned = nullptr;        // 64 ints pinned scratch for read-backs
     unsigned long long* d_rebuild_state = nullptr;  // TRIGGER_RING x {max bits, ticket}: one pair per trigger call in flight
     unsigned trigger_seq = 0;
+    cudaEvent_t ev_flag = nullptr;  // dimos_step_host: marks the arrival of the trigger flag in pinned memory
     DevBuf scratch;  // small per-context device scratch (type histogram of dimos_dispersion_correction)
     std::vector<struct NL*> lists;
     struct PmePlan* pme = nullptr;  // cuFFT plans, mesh and accumulators of dimos_pme_recip (pme.cu), rebuilt when the mesh changes
