@@ -1,13 +1,14 @@
 // pme.cu -- reciprocal-space electrostatics by smooth particle-mesh Ewald (Eq. 11,
 // PAPER.md:227 Eq. 12, "we implement smooth PME ... B-splines based on the recursive definition").
 //
-//   pme_spread   one warp per atom: scaled fractional coordinate (fp64 from the raw position, so the spline argument is
-//                exact to the rounding of `real`), the 3 x n cardinal B-spline weights by the recursion, q * w1 w2 w3
-//                added to the n^3 mesh points (lanes over the n^2 (x, y) pairs, z contiguous in memory)
+//   pme_spread   one warp per 32 atoms: every lane computes the scaled fractional coordinate (fp64 from the raw position, so
+//                the spline argument is exact to the rounding of `real`) and the 3 x n cardinal B-spline weights of its
+//                atom by the recursion; the warp then adds q * w1 w2 w3 to the n^3 mesh points of one atom after the other,
+//                points dealt to the lanes with z (contiguous in memory) fastest
 //   cuFFT        real-to-complex 3-D transform of the charge mesh (library call; SURVEY.md §8(f) 3 names it)
 //   pme_solve    per wave vector: B(m) C(m), energy 1/2 B C |F(Q)|^2, virial, F(Q) *= B C  (half spectrum, weights 1 / 2)
 //   cuFFT        complex-to-real transform: the convolution theta_rec * Q
-//   pme_gather   one warp per atom: F_i = -q_i sum_k grad(theta_i)(k) (theta_rec * Q)(k)
+//   pme_gather   same decomposition: F_i = -q_i sum_k grad(theta_i)(k) (theta_rec * Q)(k)
 //   pme_self     Eq. 12: -k_e alpha / sqrt(pi) sum q^2
 //
 // The mesh is indexed [k1][k2][k3] with k3 fastest.  Energies and virial are reduced in fp64.
@@ -86,37 +87,82 @@ __device__ __forceinline__ void scaled_fraction(const real* __restrict__ pos, in
     w = (real)(u - (double)k);
 }
 
-template <typename real, int N>
-__global__ __launch_bounds__(256) void pme_spread_kernel(const real* __restrict__ pos, const real* __restrict__ charge, int64_t n_atoms,
-                                                         double Lx, double Ly, double Lz, int K1, int K2, int K3,
-                                                         real* __restrict__ grid)
+// Spread and gather: one warp per 32 consecutive atoms.  First every lane computes the spline weights of ITS atom (3 axes,
+// the recursion runs for 32 atoms at once) and leaves them in the warp's shared-memory table; then the warp walks over its
+// atoms one after the other with the N^3 mesh points of the atom dealt to the lanes, z (contiguous in memory) fastest, so
+// that the N points of a mesh row sit in adjacent lanes: one warp-wide RED / load touches ~32/N rows instead of 32.
+constexpr int PME_WARPS = 4;
+
+template <typename real, int N, bool DERIV>
+struct PmeWarpTable {
+    real th[32][3][N];                   // [atom of the warp][axis][j]: a lane's stores have the odd stride 3 N
+    real dth[DERIV ? 32 : 1][3][N];
+};
+
+template <typename real, int N, bool DERIV>
+__device__ __forceinline__ void pme_warp_weights(const real* __restrict__ pos, int64_t i, bool have, double Lx, double Ly, double Lz,
+                                                 int K1, int K2, int K3, PmeWarpTable<real, N, DERIV>& tab, int lane, int& f1, int& f2,
+                                                 int& f3)
 {
-    const int lane = threadIdx.x & 31;
-    const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (i >= n_atoms) return;
-    int f1, f2, f3;
-    real w1, w2, w3;
-    scaled_fraction(pos, i, 0, Lx, K1, f1, w1);
-    scaled_fraction(pos, i, 1, Ly, K2, f2, w2);
-    scaled_fraction(pos, i, 2, Lz, K3, f3, w3);
-    real t1[PME_MAX_ORDER], t2[PME_MAX_ORDER], t3[PME_MAX_ORDER], d_[PME_MAX_ORDER];
-    bspline_weights<real, N>(w1, t1, d_);
-    bspline_weights<real, N>(w2, t2, d_);
-    bspline_weights<real, N>(w3, t3, d_);
-    const real q = charge[i];
-    for (int p = lane; p < N * N; p += 32) {
-        const int j1 = p / N, j2 = p - j1 * N;
-        int k1 = f1 - j1; if (k1 < 0) k1 += K1;
-        int k2 = f2 - j2; if (k2 < 0) k2 += K2;
-        real s1 = (real)0, s2 = (real)0;
+    f1 = f2 = f3 = 0;
+    if (have) {
 #pragma unroll
-        for (int j = 0; j < N; ++j) { if (j == j1) s1 = t1[j]; if (j == j2) s2 = t2[j]; }
-        const real q12 = q * s1 * s2;
-        real* row = grid + ((int64_t)k1 * K2 + k2) * K3;
+        for (int a = 0; a < 3; ++a) {
+            const double L = a == 0 ? Lx : (a == 1 ? Ly : Lz);
+            const int K = a == 0 ? K1 : (a == 1 ? K2 : K3);
+            int fl;
+            real w;
+            scaled_fraction(pos, i, a, L, K, fl, w);
+            real t[PME_MAX_ORDER], d[PME_MAX_ORDER];
+            bspline_weights<real, N>(w, t, d);
 #pragma unroll
-        for (int j3 = 0; j3 < N; ++j3) {
-            int k3 = f3 - j3; if (k3 < 0) k3 += K3;
-            atomicAdd(row + k3, q12 * t3[j3]);
+            for (int j = 0; j < N; ++j) {
+                tab.th[lane][a][j] = t[j];
+                if (DERIV) tab.dth[lane][a][j] = d[j];
+            }
+            if (a == 0) f1 = fl; else if (a == 1) f2 = fl; else f3 = fl;
+        }
+    }
+    __syncwarp();
+}
+
+template <typename real, int N>
+__global__ __launch_bounds__(PME_WARPS * 32) void pme_spread_kernel(const real* __restrict__ pos, const real* __restrict__ charge,
+                                                                     int64_t n_atoms, double Lx, double Ly, double Lz, int K1, int K2,
+                                                                     int K3, real* __restrict__ grid)
+{
+    __shared__ PmeWarpTable<real, N, false> tabs[PME_WARPS];
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int64_t a0 = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 32;
+    if (a0 >= n_atoms) return;  // whole warps leave; there is no block-wide barrier
+    const int cnt = (int)((n_atoms - a0) < 32 ? (n_atoms - a0) : 32);
+    PmeWarpTable<real, N, false>& tab = tabs[wib];
+    int f1m, f2m, f3m;
+    pme_warp_weights<real, N, false>(pos, a0 + lane, lane < cnt, Lx, Ly, Lz, K1, K2, K3, tab, lane, f1m, f2m, f3m);
+    const real qm = lane < cnt ? charge[a0 + lane] : (real)0;
+    // this lane's mesh points inside an atom's N^3 block do not depend on the atom: decompose the point indices once
+    constexpr int NP = N * N * N, NIT = (NP + 31) / 32;
+    int j1[NIT], j2[NIT], j3[NIT];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+        const int p = it * 32 + lane, j12 = p / N;
+        j3[it] = p - j12 * N;
+        j1[it] = j12 / N;
+        j2[it] = j12 - j1[it] * N;
+    }
+    for (int a = 0; a < cnt; ++a) {
+        const int f1 = __shfl_sync(FULL, f1m, a), f2 = __shfl_sync(FULL, f2m, a), f3 = __shfl_sync(FULL, f3m, a);
+        const real q = __shfl_sync(FULL, qm, a);
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            if (it * 32 + lane < NP) {
+                int k1 = f1 - j1[it]; if (k1 < 0) k1 += K1;
+                int k2 = f2 - j2[it]; if (k2 < 0) k2 += K2;
+                int k3 = f3 - j3[it]; if (k3 < 0) k3 += K3;
+                const real v = q * tab.th[a][0][j1[it]] * tab.th[a][1][j2[it]] * tab.th[a][2][j3[it]];
+                atomicAdd(grid + ((int64_t)k1 * K2 + k2) * K3 + k3, v);
+            }
         }
     }
 }
@@ -153,31 +199,47 @@ __global__ __launch_bounds__(256) void pme_solve_kernel(typename cplx<real>::typ
         const int k2 = (int)(r % K2), k1 = (int)(r / K2);
         const double mx = t1[k1], my = t2[k2];
         const double f12 = ke_over_piV * t1[K1 + k1] * t2[K2 + k2], m12 = mx * mx + my * my;
-        for (int k3 = lane; k3 < K3h; k3 += 32) {
-            const int64_t t = r * K3h + k3;
-            if (k1 == 0 && k2 == 0 && k3 == 0) {
-                spec[t].x = (real)0;
-                spec[t].y = (real)0;
-                continue;
+        // four wave vectors per lane at a time: their loads are issued together (one row is K3h <= 4 x 32 for meshes up to
+        // 254, i.e. one batch), the arithmetic and the stores follow
+        constexpr int UB = 4;
+        for (int kb = 0; kb < K3h; kb += 32 * UB) {
+            typename cplx<real>::type c[UB];
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int k3 = kb + u * 32 + lane;
+                if (k3 < K3h) c[u] = spec[r * K3h + k3];
             }
-            const double mz = t3[k3];  // k3 <= K3/2 in the half spectrum
-            const double m2 = m12 + mz * mz;
-            const double inv_m2 = 1.0 / m2;
-            const double bc = f12 * t3[K3 + k3] * inv_m2;
-            const double re = (double)spec[t].x, im = (double)spec[t].y;
-            // the half spectrum holds every wave vector with 0 < k3 < K3/2 once for itself and once for its conjugate
-            const double wgt = (k3 == 0 || 2 * k3 == K3) ? 1.0 : 2.0;
-            const double e = 0.5 * wgt * bc * (re * re + im * im);
-            const double fac = 2.0 * (inv_m2 + pi2_a2);
-            v[0] += e;
-            v[1] += e * (1.0 - fac * mx * mx);
-            v[2] += e * (-fac * mx * my);
-            v[3] += e * (-fac * mx * mz);
-            v[4] += e * (1.0 - fac * my * my);
-            v[5] += e * (-fac * my * mz);
-            v[6] += e * (1.0 - fac * mz * mz);
-            spec[t].x = (real)(bc * re);
-            spec[t].y = (real)(bc * im);
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int k3 = kb + u * 32 + lane;
+                if (k3 >= K3h) continue;
+                const int64_t t = r * K3h + k3;
+                if (k1 == 0 && k2 == 0 && k3 == 0) {
+                    spec[t].x = (real)0;
+                    spec[t].y = (real)0;
+                    continue;
+                }
+                const double mz = t3[k3];  // k3 <= K3/2 in the half spectrum
+                const double m2 = m12 + mz * mz;
+                const double inv_m2 = 1.0 / m2;
+                const double bc = f12 * t3[K3 + k3] * inv_m2;
+                const double re = (double)c[u].x, im = (double)c[u].y;
+                // the half spectrum holds every wave vector with 0 < k3 < K3/2 once for itself and once for its conjugate
+                const double wgt = (k3 == 0 || 2 * k3 == K3) ? 1.0 : 2.0;
+                const double e = 0.5 * wgt * bc * (re * re + im * im);
+                const double fac = 2.0 * (inv_m2 + pi2_a2);
+                v[0] += e;
+                v[1] += e * (1.0 - fac * mx * mx);
+                v[2] += e * (-fac * mx * my);
+                v[3] += e * (-fac * mx * mz);
+                v[4] += e * (1.0 - fac * my * my);
+                v[5] += e * (-fac * my * mz);
+                v[6] += e * (1.0 - fac * mz * mz);
+                typename cplx<real>::type o;
+                o.x = (real)(bc * re);
+                o.y = (real)(bc * im);
+                spec[t] = o;
+            }
         }
     }
     __shared__ double sh[8][7];
@@ -197,55 +259,58 @@ __global__ __launch_bounds__(256) void pme_solve_kernel(typename cplx<real>::typ
 }
 
 template <typename real, int N>
-__global__ __launch_bounds__(256) void pme_gather_kernel(const real* __restrict__ pos, const real* __restrict__ charge, int64_t n_atoms,
-                                                         double Lx, double Ly, double Lz, int K1, int K2, int K3,
-                                                         const real* __restrict__ grid, real* __restrict__ F, int accumulate)
+__global__ __launch_bounds__(PME_WARPS * 32) void pme_gather_kernel(const real* __restrict__ pos, const real* __restrict__ charge,
+                                                                     int64_t n_atoms, double Lx, double Ly, double Lz, int K1, int K2,
+                                                                     int K3, const real* __restrict__ grid, real* __restrict__ F,
+                                                                     int accumulate)
 {
-    const int lane = threadIdx.x & 31;
-    const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (i >= n_atoms) return;
-    int f1, f2, f3;
-    real w1, w2, w3;
-    scaled_fraction(pos, i, 0, Lx, K1, f1, w1);
-    scaled_fraction(pos, i, 1, Ly, K2, f2, w2);
-    scaled_fraction(pos, i, 2, Lz, K3, f3, w3);
-    real t1[PME_MAX_ORDER], t2[PME_MAX_ORDER], t3[PME_MAX_ORDER], d1[PME_MAX_ORDER], d2[PME_MAX_ORDER], d3[PME_MAX_ORDER];
-    bspline_weights<real, N>(w1, t1, d1);
-    bspline_weights<real, N>(w2, t2, d2);
-    bspline_weights<real, N>(w3, t3, d3);
-    real fx = (real)0, fy = (real)0, fz = (real)0;
-    for (int p = lane; p < N * N; p += 32) {
-        const int j1 = p / N, j2 = p - j1 * N;
-        int k1 = f1 - j1; if (k1 < 0) k1 += K1;
-        int k2 = f2 - j2; if (k2 < 0) k2 += K2;
-        real s1 = (real)0, s2 = (real)0, e1 = (real)0, e2 = (real)0;
+    __shared__ PmeWarpTable<real, N, true> tabs[PME_WARPS];
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int64_t a0 = (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5) * 32;
+    if (a0 >= n_atoms) return;
+    const int cnt = (int)((n_atoms - a0) < 32 ? (n_atoms - a0) : 32);
+    PmeWarpTable<real, N, true>& tab = tabs[wib];
+    int f1m, f2m, f3m;
+    pme_warp_weights<real, N, true>(pos, a0 + lane, lane < cnt, Lx, Ly, Lz, K1, K2, K3, tab, lane, f1m, f2m, f3m);
+    constexpr int NP = N * N * N, NIT = (NP + 31) / 32;
+    int j1[NIT], j2[NIT], j3[NIT];
 #pragma unroll
-        for (int j = 0; j < N; ++j) {
-            if (j == j1) { s1 = t1[j]; e1 = d1[j]; }
-            if (j == j2) { s2 = t2[j]; e2 = d2[j]; }
-        }
-        const real* row = grid + ((int64_t)k1 * K2 + k2) * K3;
-        real a0 = (real)0, a1 = (real)0;  // sum_j3 theta3 phi, sum_j3 dtheta3 phi
-#pragma unroll
-        for (int j3 = 0; j3 < N; ++j3) {
-            int k3 = f3 - j3; if (k3 < 0) k3 += K3;
-            const real ph = row[k3];
-            a0 += t3[j3] * ph;
-            a1 += d3[j3] * ph;
-        }
-        fx += e1 * s2 * a0;
-        fy += s1 * e2 * a0;
-        fz += s1 * s2 * a1;
+    for (int it = 0; it < NIT; ++it) {
+        const int p = it * 32 + lane, j12 = p / N;
+        j3[it] = p - j12 * N;
+        j1[it] = j12 / N;
+        j2[it] = j12 - j1[it] * N;
     }
+    real Fx = (real)0, Fy = (real)0, Fz = (real)0;  // lane a ends up with the sums of atom a
+    for (int a = 0; a < cnt; ++a) {
+        const int f1 = __shfl_sync(FULL, f1m, a), f2 = __shfl_sync(FULL, f2m, a), f3 = __shfl_sync(FULL, f3m, a);
+        real fx = (real)0, fy = (real)0, fz = (real)0;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        fx += __shfl_xor_sync(0xffffffffu, fx, o);
-        fy += __shfl_xor_sync(0xffffffffu, fy, o);
-        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+        for (int it = 0; it < NIT; ++it) {
+            if (it * 32 + lane < NP) {
+                int k1 = f1 - j1[it]; if (k1 < 0) k1 += K1;
+                int k2 = f2 - j2[it]; if (k2 < 0) k2 += K2;
+                int k3 = f3 - j3[it]; if (k3 < 0) k3 += K3;
+                const real ph = grid[((int64_t)k1 * K2 + k2) * K3 + k3];
+                const real s1 = tab.th[a][0][j1[it]], s2 = tab.th[a][1][j2[it]], s3 = tab.th[a][2][j3[it]];
+                fx += tab.dth[a][0][j1[it]] * s2 * s3 * ph;
+                fy += s1 * tab.dth[a][1][j2[it]] * s3 * ph;
+                fz += s1 * s2 * tab.dth[a][2][j3[it]] * ph;
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            fx += __shfl_xor_sync(FULL, fx, o);
+            fy += __shfl_xor_sync(FULL, fy, o);
+            fz += __shfl_xor_sync(FULL, fz, o);
+        }
+        if (lane == a) { Fx = fx; Fy = fy; Fz = fz; }
     }
-    if (lane == 0) {
+    if (lane < cnt) {
+        const int64_t i = a0 + lane;
         const real q = charge[i];
-        const real gx = -q * (real)((double)K1 / Lx) * fx, gy = -q * (real)((double)K2 / Ly) * fy, gz = -q * (real)((double)K3 / Lz) * fz;
+        const real gx = -q * (real)((double)K1 / Lx) * Fx, gy = -q * (real)((double)K2 / Ly) * Fy, gz = -q * (real)((double)K3 / Lz) * Fz;
         if (accumulate) { F[3 * i] += gx; F[3 * i + 1] += gy; F[3 * i + 2] += gz; }
         else { F[3 * i] = gx; F[3 * i + 1] = gy; F[3 * i + 2] = gz; }
     }
@@ -320,12 +385,12 @@ template <typename real, int N>
 int launch_spread_gather(Ctx* ctx, bool gather, const real* pos, const real* charge, int64_t n, const double* L, const int* K, real* grid,
                          real* F, int accumulate, cudaStream_t s)
 {
-    const unsigned nb = (unsigned)((n * 32 + 255) / 256);
+    const unsigned nb = (unsigned)((n + 32 * PME_WARPS - 1) / (32 * PME_WARPS));  // one warp per 32 atoms
     if (!gather) {
-        pme_spread_kernel<real, N><<<nb, 256, 0, s>>>(pos, charge, n, L[0], L[1], L[2], K[0], K[1], K[2], grid);
+        pme_spread_kernel<real, N><<<nb, PME_WARPS * 32, 0, s>>>(pos, charge, n, L[0], L[1], L[2], K[0], K[1], K[2], grid);
         DIMOS_LAUNCH_CHECK(ctx, "pme_spread");
     } else {
-        pme_gather_kernel<real, N><<<nb, 256, 0, s>>>(pos, charge, n, L[0], L[1], L[2], K[0], K[1], K[2], grid, F, accumulate);
+        pme_gather_kernel<real, N><<<nb, PME_WARPS * 32, 0, s>>>(pos, charge, n, L[0], L[1], L[2], K[0], K[1], K[2], grid, F, accumulate);
         DIMOS_LAUNCH_CHECK(ctx, "pme_gather");
     }
     return DIMOS_OK;
