@@ -82,3 +82,30 @@ def test_lj_table_fill_is_eq5_and_matches_the_oracle():
     assert t[1, 1, 1] == 0.0 and t[0, 1, 1] == 0.0  # a type with eps = 0 has no LJ partner
     with pytest.raises(binding.DimosError):
         binding.dimos_lj_table_fill([0.3, -1.0], [0.1, 0.1])
+
+
+def test_binding_structs_match_the_header_layout(tmp_path):
+    """The ctypes mirrors of dimos_nb_params and dimos_nl_stats_t have the size and field offsets a C compiler gives the
+    structs of include/dimos.h (the header is plain C: it must compile with gcc, too)."""
+    import shutil
+    import subprocess
+
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no C compiler")
+    fields_p = [name for name, _ in binding._Params._fields_]
+    fields_s = [name for name, _ in binding._Stats._fields_]
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "dimos.h"', "int main(void) {",
+             '  printf("%zu\\n", sizeof(dimos_nb_params));']
+    lines += [f'  printf("%zu\\n", offsetof(dimos_nb_params, {f}));' for f in fields_p]
+    lines += ['  printf("%zu\\n", sizeof(dimos_nl_stats_t));']
+    lines += [f'  printf("%zu\\n", offsetof(dimos_nl_stats_t, {f}));' for f in fields_s]
+    lines += ["  return 0;", "}"]
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run([gcc, "-std=c99", "-Wall", "-Werror", "-I", build_ext.INCLUDE, str(src), "-o", str(exe)], check=True)
+    got = [int(x) for x in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()]
+    want = [ctypes.sizeof(binding._Params)] + [getattr(binding._Params, f).offset for f in fields_p]
+    want += [ctypes.sizeof(binding._Stats)] + [getattr(binding._Stats, f).offset for f in fields_s]
+    assert got == want
