@@ -164,6 +164,24 @@ DIMOS_API int dimos_nl_destroy(dimos_ctx* ctx, dimos_nl* nl);
 DIMOS_API int dimos_nl_needs_rebuild(dimos_ctx* ctx, const void* pos, const void* pos_at_build, int64_t N,
                                      double skin, int32_t* flag_dev, int32_t* flag_host, void* stream);
 
+/* dimos_nl_needs_rebuild_static -- the same trigger (reading C-5) for callers that must not allocate: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call allocates nothing (no
+ * cudaMalloc / cudaFree, no dimos_allocator callback, no allocating library routine) and does not synchronise: its whole
+ * scratch -- one block maximum per 1024 atoms and a ticket -- is a fixed __device__ array of 64.25 KiB inside the library,
+ * held by every GPU that loads the library until the process exits.  The first call on a device looks the array's device
+ * address up (cudaGetSymbolAddress; make one call outside any capture).
+ *   pos, pos_at_build  dev, N x 3, element type of the context
+ *   N                  1 .. DIMOS_STATIC_MAX_ATOMS; beyond it the call returns DIMOS_EOVERFLOW and launches nothing
+ *   flag_dev           dev, one int32, written with 0 or 1 (required): the flag dimos_nl_needs_rebuild writes
+ *   max_disp2_dev      dev, one double, may be NULL: receives max_i |pos_i - pos_at_build_i|^2 as computed in the context's
+ *                      element type (+inf if a coordinate is NaN)
+ * Enqueues one memset of the ticket and one kernel on `stream`.  ALL calls of a process on one GPU share the array, which
+ * keeps the last call's contents: two calls that overlap on the GPU (different streams, or different contexts on the same
+ * device) race and may both write wrong flags -- order them on one stream or with events. */
+#define DIMOS_STATIC_MAX_ATOMS 8388608 /* 8192 blocks x 1024 atoms */
+DIMOS_API int dimos_nl_needs_rebuild_static(dimos_ctx* ctx, const void* pos, const void* pos_at_build, int64_t N,
+                                            double skin, int32_t* flag_dev, double* max_disp2_dev, void* stream);
+
 /* dimos_nonbonded -- PAPER.md:189-213, 222, 243; SURVEY/DESIGN reading C-7 for the virial.
  * Evaluates, over the pairs of the list that are not excluded and have minimum-image r < r_cut
  * (strict, fp32 r^2 in F32/MIXED contexts), the Lennard-Jones energy (Eq. 4) and the Coulomb

@@ -33,6 +33,7 @@ EXPORTED_SYMBOLS = (
     "dimos_dispersion_correction", "dimos_settle", "dimos_settle_velocities",
     "dimos_kinetic_energy", "dimos_berendsen", "dimos_water_kick_drift_settle", "dimos_water_kick_settle_velocities",
     "dimos_berendsen_scale", "dimos_pme_recip", "dimos_pme_mesh_size", "dimos_lj_table_fill", "dimos_langevin_ou",
+    "dimos_nl_needs_rebuild_static",
 )
 
 
@@ -88,6 +89,7 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_nl_build.argtypes = [vp, vp, i64, ctypes.POINTER(dbl), dbl, dbl, vp, i64, vp, vp, ctypes.POINTER(vp)]
     lib.dimos_nl_destroy.argtypes = [vp, vp]
     lib.dimos_nl_needs_rebuild.argtypes = [vp, vp, vp, i64, dbl, vp, ctypes.POINTER(i32), vp]
+    lib.dimos_nl_needs_rebuild_static.argtypes = [vp, vp, vp, i64, dbl, vp, vp, vp]
     lib.dimos_nonbonded.argtypes = [vp, vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), ctypes.POINTER(_Params), vp, vp, vp, vp]
     lib.dimos_nonbonded_host.argtypes = [vp, vp, vp, vp, vp, vp, i32, ctypes.POINTER(dbl), ctypes.POINTER(_Params), vp, vp, vp, vp]
     lib.dimos_nl_export_pairs.argtypes = [vp, vp, vp, i64, ctypes.POINTER(i64), vp]
@@ -301,6 +303,21 @@ class Context:
                                                  ctypes.byref(host) if sync else None, _stream_ptr())
         self._check(rc)
         return bool(host.value) if sync else (flag if flag is not None else self._flag)
+
+    def nl_needs_rebuild_static(self, pos, pos_at_build, skin, flag, max_disp2=None):
+        """dimos_nl_needs_rebuild_static: the trigger with its scratch in a fixed device array (no allocation, no host
+        synchronisation).  flag: int32 device tensor (required, caller-owned); max_disp2: float64 device tensor or None."""
+        pos = self._dev(pos, self.real, 3)
+        ref = self._dev(pos_at_build, self.real, 3)
+        flag = self._dev(flag, torch.int32)
+        if max_disp2 is not None:
+            max_disp2 = self._dev(max_disp2, torch.float64)
+        with torch.cuda.device(self.device):
+            rc = self.lib.dimos_nl_needs_rebuild_static(self.handle, pos.data_ptr(), ref.data_ptr(), pos.shape[0], float(skin),
+                                                        flag.data_ptr(), max_disp2.data_ptr() if max_disp2 is not None else None,
+                                                        _stream_ptr())
+        self._check(rc)
+        return flag
 
     def _params(self, nl, method, eps_rf, alpha, coulomb_const, r_switch=0.0, skip_flag=None):
         skip = None
@@ -644,6 +661,10 @@ class Context:
 # -- module-level functions with the C names -------------------------------------------------------
 def dimos_nl_build(ctx: Context, pos, box, r_cut, skin, excl_pairs=None, pos_at_build=None, nl=None) -> NeighborList:
     return ctx.nl_build(pos, box, r_cut, skin, excl_pairs, pos_at_build, nl)
+
+
+def dimos_nl_needs_rebuild_static(ctx: Context, pos, pos_at_build, skin, flag, max_disp2=None):
+    return ctx.nl_needs_rebuild_static(pos, pos_at_build, skin, flag, max_disp2)
 
 
 def dimos_nl_needs_rebuild(ctx: Context, pos, pos_at_build, skin, sync: bool = True, flag=None):

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OUT = os.path.join(HERE, "libdimos_b200.so")
-SOURCES = ("api.cu", "nl_build.cu", "nonbonded.cu", "pair_f32x2.cu", "integrator.cu", "pme.cu", "pair_f64.cu")
+SOURCES = ("api.cu", "nl_build.cu", "nonbonded.cu", "pair_f32x2.cu", "integrator.cu", "pme.cu", "pair_f64.cu", "static_scratch.cu")
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC,-fvisibility=hidden", "--expt-relaxed-constexpr",
