@@ -722,7 +722,7 @@ static int nonbonded_typed(Ctx* ctx, NL* nl, const real* pos, const real* charge
     const bool fx = sizeof(real) == 4 && use_f32x2(ctx, nl, prm->method);
     const int wpb = fx ? FX_WARPS : PF_WARPS;  // warps per CTA
     const unsigned nb_full = (unsigned)((nun + wpb - 1) / wpb);
-    const unsigned nb_res = (unsigned)ctx->sm_count * (fx ? (unsigned)FX_CTAS_PER_SM : 2u);
+    const unsigned nb_res = (unsigned)ctx->sm_count * (fx ? (unsigned)FX_CTAS_PER_SM : (sizeof(real) == 8 ? (unsigned)F64_MIN_CTAS : 2u));
     const unsigned nb_force = nb_full < nb_res ? nb_full : nb_res;
     const size_t n_force_rows = (size_t)nb_force * wpb;  // one fp64 partial row per warp
     const bool ewald = prm->method == DIMOS_EWALD_REAL;

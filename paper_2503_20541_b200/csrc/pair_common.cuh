@@ -4,6 +4,10 @@
 
 #include "common.cuh"
 
+#ifndef F64_MIN_CTAS
+#define F64_MIN_CTAS 3  // resident CTAs per SM the fp64 pair kernel is compiled (80 registers) and launched for
+#endif
+
 namespace dimos {
 
 __device__ __forceinline__ float4 mk4(float x, float y, float z, float w) { return make_float4(x, y, z, w); }

@@ -2,11 +2,16 @@
 // configs[0] and configs[4] in fp64).
 //
 // Same decomposition as the other pair kernels (one warp per unit of 8 i-atoms, one lane per j-atom of a 32-entry chunk,
-// one vector of REDs per j-atom), but written for double precision, where one pair slot costs a few hundred instructions
-// (IEEE 1/sqrt, exp, the erfc series): the loop over the 8 i-atoms is ROLLED, the i-atoms live in shared memory and the
-// per-lane F_i partial sums in a padded shared-memory array, so that the whole kernel is ~1,500 instructions.  The unrolled
-// generic kernel (nonbonded.cu) is 13,000 instructions in fp64 and spends 95 % of its cycles waiting for instruction
-// fetch (profiles/r2_f64_pair_force_ncu.md).  A warp-wide vote skips an i-atom that no lane has inside the cutoff.
+// one vector of REDs per j-atom), but written for double precision, where one pair inside the cutoff costs a few hundred
+// instructions (IEEE 1/sqrt, exp, the erfc series) and only 44 % of the listed pair slots are inside the cutoff:
+//   pass 1  every lane tests its j-atom against the 8 i-atoms (distance only) and the warp writes the in-cutoff pairs of
+//           the chunk, j-major, into a dense queue in shared memory;
+//   pass 2  the queue is worked off 32 pairs at a time, one pair per lane, so that the expensive arithmetic runs on full
+//           warps (~4 batches per chunk instead of 8 half-empty passes over the i-atoms).  F_i goes to a per-lane column
+//           of a padded shared-memory array (summed once per unit), F_j through a segmented warp sum over the consecutive
+//           lanes that hold the same j-atom.
+// The i-atoms live in shared memory and the code is rolled: the unrolled generic kernel (nonbonded.cu) is 13,000
+// instructions in fp64 and spends 95 % of its cycles waiting for instruction fetch (profiles/r2_f64_pair_force_ncu.md).
 #include <math.h>
 
 #include "pair_common.cuh"
@@ -16,7 +21,7 @@ namespace dimos {
 namespace {
 
 constexpr int F64_WARPS = 8;
-constexpr int F64_PAD = 33;  // per-(i, component) row of 32 lane partials, padded against bank conflicts in the final sum
+constexpr int F64_PAD = 32;  // per-(i, component) row of 32 lane partials: a lane's column is its own bank whatever i it works on
 
 __constant__ double CHEB[28] = {
 #include "erfc_cheb.inc"
@@ -45,11 +50,16 @@ __device__ __forceinline__ void erfc_exp(double x, bool fast, double& erfc_x, do
 }
 
 template <int METHOD, int PBC>
-__global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(ForceParams<double> P)
+__global__ __launch_bounds__(F64_WARPS * 32, F64_MIN_CTAS) void pair_force_f64_kernel(ForceParams<double> P)
 {
     __shared__ double4 off_s[27];
     __shared__ double4 iat_s[F64_WARPS][UNIT];  // the warp's current i-atoms: x, y, z, k_e q
     __shared__ int ti_s[F64_WARPS][UNIT];       // their LJ table row offset (type * nt), or -1 without LJ partners
+    __shared__ double4 jat_s[F64_WARPS][32];    // the chunk's j-atoms (image-shifted x, y, z, q), one per lane
+    __shared__ double fj_s[F64_WARPS][32 * 3];  // F_j of the chunk's j-atoms, summed over the batches
+    __shared__ int tj_s[F64_WARPS][32];         // their types
+    __shared__ double ftot_s[F64_WARPS][UNIT * 3];  // F_i of the unit, summed over the lanes' columns
+    __shared__ unsigned char que_s[F64_WARPS][32 * UNIT];  // the chunk's in-cutoff pairs: j-lane << 3 | i
     extern __shared__ __align__(16) unsigned char dyn_smem[];
     double4* ljt = reinterpret_cast<double4*>(dyn_smem);                          // [nt*nt] (c6, c12, 6 c6, 12 c12)
     double* facc = reinterpret_cast<double*>(ljt + P.nt * P.nt);                  // [F64_WARPS][UNIT*3][F64_PAD]
@@ -67,6 +77,12 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
     const int wib = threadIdx.x >> 5;
     double4* iat = iat_s[wib];
     int* tis = ti_s[wib];
+    double4* jat = jat_s[wib];
+    double* fjs = fj_s[wib];
+    int* tjs = tj_s[wib];
+    double* ftot = ftot_s[wib];
+    unsigned char* que = que_s[wib];
+    for (int k = lane; k < 32 * 3; k += 32) fjs[k] = 0.0;
     double* fw = facc + (size_t)wib * UNIT * 3 * F64_PAD;
     const bool lj_all = *P.order_stale != 0;
     const bool fast = P.erfc_fast != 0;
@@ -118,8 +134,9 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
             const double4 off = off_s[code];
             const double xj = pj.x + off.x, yj = pj.y + off.y, zj = pj.z + off.z, qj = pj.w;
             const bool lj_chunk = lj_all || c < n_a + (int)n_m;
-            double fjx = 0, fjy = 0, fjz = 0;
-#pragma unroll 1
+            // ---- pass 1 (cheap): which of the 8 i-atoms does this lane's j-atom have inside the cutoff ----
+            unsigned bits = 0;
+#pragma unroll
             for (int i = 0; i < UNIT; ++i) {
                 const double4 a = iat[i];
                 double dx = a.x - xj, dy = a.y - yj, dz = a.z - zj;
@@ -129,13 +146,43 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
                     dz -= P.L[2] * rint(dz * P.invL[2]);
                 }
                 const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-                const bool in = r2 < P.rc2 && ((mask >> i) & 1u);
-                if (!__any_sync(FULL, in)) continue;  // no lane has this i-atom inside the cutoff
+                bits |= (r2 < P.rc2 ? 1u : 0u) << i;
+            }
+            bits &= mask;
+            // ---- the in-cutoff pairs of the chunk as a dense queue, j-major: entry = j-lane << 3 | i ----
+            jat[lane] = make_double4(xj, yj, zj, qj);
+            tjs[lane] = tj;
+            const int cnt = __popc(bits);
+            int o = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int y = __shfl_up_sync(FULL, o, d);
+                if (lane >= d) o += y;
+            }
+            const int T = __shfl_sync(FULL, o, 31);
+            o -= cnt;
+            for (unsigned b = bits; b; b &= b - 1u) que[o++] = (unsigned char)((lane << 3) | (__ffs(b) - 1));
+            __syncwarp();
+            // ---- pass 2 (the expensive arithmetic): one pair per lane, 32 pairs per batch ----
+            for (int q0 = 0; q0 < T; q0 += 32) {
+                const int q = q0 + lane;
+                const bool valid = q < T;
+                const unsigned e = valid ? (unsigned)que[q] : 0u;
+                const int i = (int)(e & 7u), jl = valid ? (int)(e >> 3) : 32 + lane;  // invalid lanes: a segment of their own
+                const double4 a = iat[i];
+                const double4 b = jat[jl & 31];
+                double dx = a.x - b.x, dy = a.y - b.y, dz = a.z - b.z;
+                if (PBC == 1) {
+                    dx -= P.L[0] * rint(dx * P.invL[0]);
+                    dy -= P.L[1] * rint(dy * P.invL[1]);
+                    dz -= P.L[2] * rint(dz * P.invL[2]);
+                }
                 double fs = 0.0;
-                if (in) {
+                if (valid) {
+                    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));  // the same expression as in pass 1: inside the cutoff
                     const double rinv = rsqrt(r2);  // 1 ulp (CUDA math library), far inside the 1e-10 bar
                     const double rinv2 = rinv * rinv;
-                    const double qq = a.w * qj;
+                    const double qq = a.w * b.w;
                     double fr2;
                     if (METHOD == DIMOS_RF) {  // Eq. 8, reading C-1
                         acc[1] += qq * (fma(P.krf, r2, rinv) - P.crf);
@@ -150,7 +197,7 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
                     }
                     const int ti = tis[i];
                     if (ti >= 0 && lj_chunk) {  // Eq. 4 (+ Eq. 6)
-                        const double4 cc = ljt[ti + tj];
+                        const double4 cc = ljt[ti + tjs[jl]];
                         const double rinv6 = rinv2 * rinv2 * rinv2;
                         double elj = fma(cc.y, rinv6, -cc.x) * rinv6;
                         double flj = fma(cc.w, rinv6, -cc.z) * rinv6;
@@ -171,31 +218,51 @@ __global__ __launch_bounds__(F64_WARPS * 32, 2) void pair_force_f64_kernel(Force
                     fs = fr2 * rinv2;
                 }
                 const double fx = fs * dx, fy = fs * dy, fz = fs * dz;
-                fw[(3 * i) * F64_PAD + lane] += fx;
-                fw[(3 * i + 1) * F64_PAD + lane] += fy;
-                fw[(3 * i + 2) * F64_PAD + lane] += fz;
-                fjx -= fx; fjy -= fy; fjz -= fz;
+                if (valid) {  // F_i: this lane's own column of the i-atom's three rows
+                    fw[(3 * i) * F64_PAD + lane] += fx;
+                    fw[(3 * i + 1) * F64_PAD + lane] += fy;
+                    fw[(3 * i + 2) * F64_PAD + lane] += fz;
+                }
                 if (PBC == 1) {  // the image can differ per pair: direct per-pair virial
                     acc[2] += dx * fx; acc[3] += dx * fy; acc[4] += dx * fz;
                     acc[5] += dy * fy; acc[6] += dy * fz; acc[7] += dz * fz;
                 }
+                // F_j: the pairs of one j-atom are consecutive lanes (at most 8): segmented sum, the segment's first lane adds
+                // it to the j-atom's accumulator (one segment per j-atom and batch: plain read-modify-write)
+                double sx = -fx, sy = -fy, sz = -fz;
+#pragma unroll
+                for (int d = 1; d < UNIT; d <<= 1) {
+                    const int jo = __shfl_down_sync(FULL, jl, d);
+                    const double tx = __shfl_down_sync(FULL, sx, d), ty = __shfl_down_sync(FULL, sy, d), tz = __shfl_down_sync(FULL, sz, d);
+                    if (lane + d < 32 && jo == jl) { sx += tx; sy += ty; sz += tz; }
+                }
+                const int jprev = __shfl_up_sync(FULL, jl, 1);
+                if (valid && (lane == 0 || jprev != jl)) {
+                    fjs[3 * jl] += sx;
+                    fjs[3 * jl + 1] += sy;
+                    fjs[3 * jl + 2] += sz;
+                }
+                __syncwarp();  // a j-atom's segment can continue in the next batch
             }
+            const double fjx = fjs[3 * lane], fjy = fjs[3 * lane + 1], fjz = fjs[3 * lane + 2];
+            fjs[3 * lane] = 0.0; fjs[3 * lane + 1] = 0.0; fjs[3 * lane + 2] = 0.0;
             if (PBC == 0) {  // x_j' (x) F_j^entry in unit-local coordinates
                 acc[2] = fma(xj, fjx, acc[2]); acc[3] = fma(xj, fjy, acc[3]); acc[4] = fma(xj, fjz, acc[4]);
                 acc[5] = fma(yj, fjy, acc[5]); acc[6] = fma(yj, fjz, acc[6]); acc[7] = fma(zj, fjz, acc[7]);
             }
             if (mask) red_add_xyz(&P.Facc[j], fjx, fjy, fjz);
+            __syncwarp();  // every lane is done with jat / tjs / que before the next chunk overwrites them
         }
         __syncwarp();
         // F_i of the unit: lane l < 24 sums row l (i = l / 3, component l % 3) of the padded array
         if (lane < UNIT * 3) {
             double s = 0.0;
-            for (int k = 0; k < 32; ++k) s += fw[lane * F64_PAD + k];
-            fw[lane * F64_PAD + 32] = s;
+            for (int k = 0; k < 32; ++k) s += fw[lane * F64_PAD + ((k + lane) & 31)];  // rotated: the rows' banks differ
+            ftot[lane] = s;
         }
         __syncwarp();
         if (lane < UNIT) {
-            const double rx = fw[(3 * lane) * F64_PAD + 32], ry = fw[(3 * lane + 1) * F64_PAD + 32], rz = fw[(3 * lane + 2) * F64_PAD + 32];
+            const double rx = ftot[3 * lane], ry = ftot[3 * lane + 1], rz = ftot[3 * lane + 2];
             P.Fown[U * UNIT + lane] = make_double4(rx, ry, rz, 0.0);
             if (PBC == 0) {  // x_i (x) F_i^unit
                 const double4 v = iat[lane];
