@@ -690,7 +690,8 @@ static int launch_pair_force(Ctx* ctx, const NL* nl, const ForceParams<real>& P,
     }
 #define DIMOS_PF(M, B)                                                                                            \
     do {                                                                                                          \
-        if (dyn > 48 * 1024) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
+        /* 48 KB without the opt-in, static (offset table, < 1 KB) + dynamic */                                   \
+        if (dyn > 46 * 1024) cudaFuncSetAttribute(pair_force_kernel<real, acc_t, M, B>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
         pair_force_kernel<real, acc_t, M, B><<<nb, PF_WARPS * 32, dyn, s>>>(P);                                   \
     } while (0)
     bool done = false;

@@ -524,7 +524,9 @@ __global__ __launch_bounds__(FX_WARPS * 32, FX_CTAS_PER_SM) void pair_force_f32x
 template <int METHOD, bool SW>
 static bool launch_one(const ForceParams<float>& P, unsigned nb, size_t dyn, cudaStream_t s)
 {
-    if (dyn > 48 * 1024 &&
+    // Without the opt-in a CTA may use 48 KB of shared memory, STATIC + dynamic: the kernel's static part (gather slots,
+    // offset table, barriers) is ~17 KB, so short rows (dyn of 25 .. 48 KB) need the attribute as well
+    if (dyn > 24 * 1024 &&
         cudaFuncSetAttribute(pair_force_f32x2_kernel<METHOD, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn) != cudaSuccess) {
         cudaGetLastError();
         return false;

@@ -683,3 +683,59 @@ def test_sparse_gas_with_isolated_atoms_f32():
         check_neighbor_set(dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy(), pos.astype(np.float64), box, 1.1, None)
     finally:
         ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,method,nt", [("f32", "rf", 17), ("f32", "ewald", 40), ("f32", "rf", 64), ("mixed", "rf", 64),
+                                                 ("f64", "ewald", 64), ("f64", "rf", 23)])
+def test_many_atom_types(precision, method, nt):
+    """Up to MAX_TYPES = 64 atom types (Eq. 5 table of nt x nt entries in shared memory; the packed kernel hands over to the
+    generic one when the table does not fit beside its row buffers): the mixture of _mixture_box with random types, a third
+    of the types without LJ partners, compared with the oracle as a whole system."""
+    import dataclasses
+
+    wb = _mixture_box(16, 4.6, 99 + nt)
+    rng = np.random.default_rng(nt)
+    sigma = rng.uniform(0.18, 0.30, size=nt)
+    eps = rng.uniform(0.1, 0.8, size=nt)
+    eps[rng.random(nt) < 0.33] = 0.0
+    eps[0] = 0.5  # at least one LJ-active type
+    wb = dataclasses.replace(wb, type=rng.integers(0, nt, size=wb.n_atoms).astype(np.int32), sigma=sigma, epsilon=eps)
+    rep = run_case(wb, precision, 1.0, 0.1, method, check_set=False)
+    assert rep["stats"]["pbc_mode"] == 0
+
+
+@pytest.mark.gpu
+def test_more_than_64_types_is_rejected():
+    wb = _mixture_box(12, 3.5, 5)
+    db = DeviceBox(wb, "f32")
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        lj = torch.ones(65, 65, 2, dtype=torch.float64, device=db.pos.device)
+        with pytest.raises(dimos.DimosError) as err:
+            dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, lj)
+        assert err.value.args[0].endswith("(status -1)")
+    finally:
+        ctx.close()
+
+
+@pytest.mark.gpu
+def test_short_rows_as_the_first_call_of_a_process_f32():
+    """Regression: a list with short rows (a box of a third of water's density: row capacity 576) gives the packed kernel
+    25 .. 48 KB of dynamic shared memory, which together with its ~17 KB of static shared memory needs the opt-in attribute;
+    the launch failed with `invalid argument` unless an earlier call of the same process (a water box) had raised the
+    attribute.  Runs the mixture as the FIRST force call of a fresh process, against the oracle."""
+    import os
+    import subprocess
+    import sys
+
+    here = os.path.dirname(os.path.abspath(__file__))
+    script = ("import sys; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+              "from test_gpu_parity import _mixture_box\n"
+              "from gpu_harness import run_case\n"
+              "rep = run_case(_mixture_box(16, 4.6, 2024), 'f32', 1.0, 0.1, 'rf')\n"
+              "assert rep['stats']['row_capacity'] < 1000, rep['stats']\n"
+              "print('fresh-process ok', rep['stats']['row_capacity'])\n") % (os.path.dirname(here), here)
+    res = subprocess.run([sys.executable, "-c", script], capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0 and "fresh-process ok" in res.stdout, res.stdout[-2000:] + res.stderr[-4000:]
