@@ -739,3 +739,42 @@ def test_short_rows_as_the_first_call_of_a_process_f32():
               "print('fresh-process ok', rep['stats']['row_capacity'])\n") % (os.path.dirname(here), here)
     res = subprocess.run([sys.executable, "-c", script], capture_output=True, text=True, timeout=600)
     assert res.returncode == 0 and "fresh-process ok" in res.stdout, res.stdout[-2000:] + res.stderr[-4000:]
+
+
+def _ortho_mixture_box(n_sites, a, seed):
+    """_mixture_box on an nx x ny x nz lattice: an orthorhombic box with different edges (and cell counts) per axis."""
+    import dataclasses
+
+    rng = np.random.default_rng(seed)
+    n_sites = np.asarray(n_sites)
+    box = np.array([np.float32(k * a) for k in n_sites], dtype=np.float64)
+    sites = np.stack(np.meshgrid(*[np.arange(k) for k in n_sites], indexing="ij"), axis=-1).reshape(-1, 3)
+    sites = sites[rng.random(sites.shape[0]) > 0.1]
+    n = sites.shape[0]
+    pos = ((sites + 0.5) * (box / n_sites) + rng.uniform(-0.06, 0.06, size=(n, 3))) % box
+    pos = np.minimum(pos.astype(np.float32), np.nextafter(box.astype(np.float32), np.float32(0)))
+    charge = rng.choice(np.array([-0.6, -0.2, 0.0, 0.3, 0.5]), size=n)
+    charge -= charge.mean()
+    pick = np.arange(0, n - 1, dtype=np.int32)[rng.random(n - 1) < 0.3]
+    base = wl.make_water_box(2, 5.0, 3)
+    return dataclasses.replace(base, box=box, pos=pos, charge=charge.astype(np.float32), type=rng.integers(0, 3, size=n).astype(np.int32),
+                               sigma=np.array([0.28, 0.22, 0.0]), epsilon=np.array([0.6, 0.3, 0.0]),
+                               excl_pairs=np.stack([pick, pick + 1], axis=1).astype(np.int32), mass=np.ones(n))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,method", [("f32", "rf"), ("f32", "ewald"), ("mixed", "rf"), ("f64", "ewald"), ("f64", "rf")])
+def test_orthorhombic_box_with_different_cell_counts_per_axis(precision, method):
+    """3 x 4 x 6 cells (edges 3.45, 4.6, 6.61 nm): the image shift of a list entry comes from the cell offsets, whose edge
+    differs per axis; pair set, forces, energies and virial of the whole system against the oracle."""
+    wb = _ortho_mixture_box((12, 16, 23), 0.2875, 31)
+    rep = run_case(wb, precision, 1.0, 0.1, method)
+    assert rep["stats"]["pbc_mode"] == 0 and list(rep["stats"]["n_cells"]) == [3, 4, 6]
+    # the same system with the axes permuted: another assignment of lengths to the fastest / slowest cell index
+    import dataclasses
+
+    perm = [2, 0, 1]
+    wb2 = dataclasses.replace(wb, box=wb.box[perm].copy(), pos=np.ascontiguousarray(wb.pos[:, perm]))
+    rep2 = run_case(wb2, precision, 1.0, 0.1, method)
+    assert list(rep2["stats"]["n_cells"]) == [6, 3, 4]
+    assert rep2["n_pairs_cut"] == rep["n_pairs_cut"]

@@ -122,3 +122,22 @@ def test_pme_recip_config4_full_size_f32():
     mesh = dimos.dimos_pme_mesh_size(3.12, wb.box, delta)
     F, E, W, p64, q64 = run(wb.pos, wb.charge, wb.box, 3.12, mesh, 5, "f32")
     compare(F, E, W, pme.pme_recip(p64, q64, wb.box, 3.12, mesh, 5), "f32", q64, 3.12)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("order", [3, 5])
+def test_pme_recip_orthorhombic_box_and_mesh(precision, order):
+    """Box edges 2.1 x 3.3 x 2.7 nm and a mesh of 21 x 36 x 25 points (odd sizes included: the half spectrum of the
+    real-to-complex transform then has no Nyquist plane): 700 point charges, neutral, at random positions, a tail of 21
+    atoms beyond the last full warp of 32."""
+    rng = np.random.default_rng(17)
+    n = 32 * 21 + 21 + 7
+    box = np.array([2.1, 3.3, 2.7])
+    pos = rng.uniform(0.0, 1.0, size=(n, 3)) * box
+    q = rng.uniform(-1.0, 1.0, size=n)
+    q -= q.mean()
+    if precision == "f32":
+        pos, q = pos.astype(np.float32), q.astype(np.float32)
+    mesh = (21, 36, 25)
+    F, E, W, p64, q64 = run(pos, q, box, 3.0, mesh, order, precision)
+    compare(F, E, W, pme.pme_recip(p64, q64, box, 3.0, mesh, order), precision, q64, 3.0)
