@@ -104,7 +104,10 @@ def check_nonbonded(F, E, W, orc, precision, use_allow=True, e_floor=0.0):
     dF = np.sqrt(((F - orc.F) ** 2).sum(axis=1))
     allow = orc.allow if (use_allow and orc.allow is not None and precision != "f64") else np.zeros_like(dF)
     # reading C-10: the allowance is rare (SURVEY expects ~2.8 % of atoms own a pair within 1e-5 nm of r_c)
-    assert (allow > 0).mean() <= 0.05, f"{(allow > 0).mean():.3f} of the atoms carry a cutoff-band allowance"
+    # in a uniform fluid: 2 atoms per pair in the shell r_c +- BAND, i.e. a fraction 2 (n_pairs / N) 6 BAND / r_c with r_c ~ 1 nm
+    # (2.5 % for water); the bound is twice that, and never below the 5 % that holds for every water box
+    expect = 2.0 * orc.n_pairs / max(len(dF), 1) * 6.0 * BAND
+    assert (allow > 0).mean() <= max(0.05, 2.0 * expect), f"{(allow > 0).mean():.3f} of the atoms carry a cutoff-band allowance"
     excess = dF - allow
     worst = int(np.argmax(excess))
     assert excess[worst] <= f_tol * rms, (

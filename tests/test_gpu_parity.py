@@ -778,3 +778,37 @@ def test_orthorhombic_box_with_different_cell_counts_per_axis(precision, method)
     rep2 = run_case(wb2, precision, 1.0, 0.1, method)
     assert list(rep2["stats"]["n_cells"]) == [6, 3, 4]
     assert rep2["n_pairs_cut"] == rep["n_pairs_cut"]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision,method", [("f32", "rf"), ("f32", "ewald"), ("mixed", "rf"), ("f64", "ewald")])
+def test_short_cutoff_many_cells(precision, method):
+    """configs[1]'s water box with r_c = 0.45 nm, skin 0.05 nm: 8 cells per axis of ~16 atoms each, two units per cell, rows
+    of ~60 entries (the smallest row capacity the builder uses)."""
+    wb = wl.make_config(1)
+    rep = run_case(wb, precision, 0.45, 0.05, method)
+    assert rep["stats"]["pbc_mode"] == 0 and min(rep["stats"]["n_cells"]) >= 8
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_dense_fluid_with_rows_beyond_the_packed_kernels_buffers(precision):
+    """Point particles at four times water's atom density (400 nm^-3): ~1,600 list entries per unit, so the row capacity
+    grows past what the packed kernel can stage in shared memory and the fp32 call runs on the generic kernel; cells hold
+    ~580 atoms (the in-cell sorter's multi-pass path)."""
+    import dataclasses
+
+    rng = np.random.default_rng(404)
+    n_side, edge = 25, 3.4
+    a = edge / n_side
+    sites = np.stack(np.meshgrid(*[np.arange(n_side)] * 3, indexing="ij"), axis=-1).reshape(-1, 3)
+    n = sites.shape[0]
+    pos = (((sites + 0.5) * a + rng.uniform(-0.03, 0.03, size=(n, 3))) % edge).astype(np.float32)
+    charge = rng.choice(np.array([-0.3, 0.0, 0.3]), size=n)
+    charge -= charge.mean()
+    base = wl.make_water_box(2, 5.0, 3)
+    wb = dataclasses.replace(base, box=np.array([np.float32(edge)] * 3, dtype=np.float64), pos=pos, charge=charge.astype(np.float32),
+                             type=rng.integers(0, 2, size=n).astype(np.int32), sigma=np.array([0.10, 0.08]),
+                             epsilon=np.array([0.4, 0.0]), excl_pairs=np.zeros((0, 2), np.int32), mass=np.ones(n))
+    rep = run_case(wb, precision, 1.0, 0.1, "rf")
+    assert rep["stats"]["row_capacity"] > 1500 and rep["stats"]["pbc_mode"] == 0
