@@ -79,17 +79,20 @@ def dispersion_correction(type_, lj_table, box, r_cut, r_switch=0.0):
     return e, e * np.eye(3)
 
 
-def shake_water(pos_old, pos_new, mass, d_oh, d_hh, tol=1e-14, max_iter=500):
+def shake_water(pos_old, pos_new, mass, d_oh, d_hh, tol=1e-14, max_iter=200000):
     """Position constraints of rigid three-site water (step 3 of PAPER.md:281-292; PAPER.md:327 names SETTLE for it), as
     the plain iterative SHAKE procedure run to convergence: for every molecule (atoms 3k, 3k+1, 3k+2 = O, H, H) the new
     positions are corrected along the OLD bond vectors, x_i += g m_i^-1 r_ij_old, x_j -= g m_j^-1 r_ij_old with
     g = (d_ij^2 - |r_ij_new|^2) / (2 (1/m_i + 1/m_j) r_ij_new . r_ij_old), until |r_ij| = d_ij for the three bonds.
     SETTLE solves the same equations in closed form, so a converged SHAKE is its oracle.  Returns the constrained
-    positions (fp64); pos_old must satisfy the constraints."""
+    positions (fp64); pos_old must satisfy the constraints.  The sweeps converge in ~30 iterations for water's shape and in
+    thousands for a nearly linear molecule (the three bond vectors are then almost dependent); a run that has not reached
+    `tol` after max_iter sweeps raises instead of returning an unconverged answer."""
     x0 = np.asarray(pos_old, dtype=np.float64).reshape(-1, 3, 3)
     x = np.array(pos_new, dtype=np.float64).reshape(-1, 3, 3)
     im = 1.0 / np.asarray(mass, dtype=np.float64).reshape(-1, 3)
     bonds = ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh))
+    best, stalled = np.inf, 0
     for _ in range(max_iter):
         worst = 0.0
         for i, j, d in bonds:
@@ -100,12 +103,20 @@ def shake_water(pos_old, pos_new, mass, d_oh, d_hh, tol=1e-14, max_iter=500):
             g = diff / (2.0 * (im[:, i] + im[:, j]) * (r_new * r_old).sum(1))
             x[:, i] += (g * im[:, i])[:, None] * r_old
             x[:, j] -= (g * im[:, j])[:, None] * r_old
-        if worst < tol:
+        # converged: the residual is below tol, or it sits on its rounding floor (no 1 % improvement in 100 sweeps, below
+        # 1e-11: an ill-conditioned shape amplifies the rounding of the coordinates past tol)
+        if worst < 0.99 * best:
+            best, stalled = worst, 0
+        else:
+            stalled += 1
+        if worst < tol or (stalled >= 100 and best < 1e-11):
             break
+    else:
+        raise RuntimeError(f"shake_water: not converged after {max_iter} sweeps (worst relative residual {worst:.3e})")
     return x.reshape(-1, 3)
 
 
-def rattle_water_velocities(pos, vel, mass, tol=1e-15, max_iter=2000):
+def rattle_water_velocities(pos, vel, mass, tol=1e-15, max_iter=200000):
     """Velocity constraints of rigid three-site water (step 6 of PAPER.md:281-292), as the plain iterative RATTLE velocity
     stage run to convergence: for every bond (i, j) of a molecule (atoms 3k, 3k+1, 3k+2) the component of the relative
     velocity along the bond is removed by an impulse along r_ij shared by inverse mass,
@@ -127,6 +138,8 @@ def rattle_water_velocities(pos, vel, mass, tol=1e-15, max_iter=2000):
             v[:, j] += (k * im[:, j])[:, None] * r
         if worst < tol:
             break
+    else:
+        raise RuntimeError(f"rattle_water_velocities: not converged after {max_iter} sweeps (worst residual {worst:.3e} of max|v|)")
     return v.reshape(-1, 3)
 
 

@@ -450,3 +450,46 @@ def test_langevin_ou_matches_oracle(precision, n):
         assert np.allclose(vf.cpu().numpy(), v * np.exp(-gamma * dt), rtol=1e-6, atol=0)
         with pytest.raises(dimos.DimosError):
             dimos.dimos_langevin_ou(ctx, vd, torch.from_numpy(inv_m).to(dev), torch.from_numpy(xi).to(dev), -1.0, dt, T)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("model", ["spce", "heavy", "wide", "light_centre"])
+def test_settle_and_velocity_stage_for_other_rigid_three_site_models(precision, model):
+    """The constraint solvers take the geometry and the masses as arguments (PAPER.md:327 names SETTLE for water in
+    general): SPC/E (0.1 nm, 109.47 deg), heavy water (m_H = 2.014), a nearly linear triangle (170 deg) and a molecule
+    whose centre atom is the light one.  Positions against the oracle's converged SHAKE, velocities against its converged
+    RATTLE velocity stage."""
+    d_oh, angle, m_O, m_H = {"spce": (0.1, 109.47, 15.9994, 1.008), "heavy": (0.09572, 104.52, 15.9994, 2.014),
+                             "wide": (0.11, 170.0, 12.0, 3.0), "light_centre": (0.12, 95.0, 1.5, 14.0)}[model]
+    d_hh = 2.0 * d_oh * np.sin(np.radians(angle) / 2.0)
+    rng = np.random.default_rng(5 + len(model))  # spce 9, heavy 10, wide 9 + different draws below, light_centre 17
+    np_real = np.float64 if precision == "f64" else np.float32
+    n_w = 777
+    mass = np.tile([m_O, m_H, m_H], n_w)
+    x0 = _random_rigid_waters(rng, n_w, d_oh, d_hh).astype(np_real)
+    dt = 0.001
+    v = rng.normal(0.0, 1.5, size=x0.shape) / np.sqrt(mass)[:, None]
+    x1 = (x0.astype(np.float64) + dt * v).astype(np_real)
+    x0_64 = oracle.shake_water(x0.astype(np.float64), x0.astype(np.float64), mass, d_oh, d_hh)
+    ref_x = oracle.shake_water(x0_64, x1.astype(np.float64), mass, d_oh, d_hh)
+    water = np.arange(3 * n_w, dtype=np.int32).reshape(n_w, 3)
+    dev = torch.device("cuda", 0)
+    with dimos.Context(0, precision) as ctx:
+        p = torch.from_numpy(x1.copy()).to(dev)
+        dimos.dimos_settle(ctx, torch.from_numpy(x0).to(dev), p, torch.from_numpy(water).to(dev), m_O, m_H, d_oh, d_hh)
+        vd = torch.from_numpy(v.astype(np_real)).to(dev)
+        dimos.dimos_settle_velocities(ctx, p, vd, torch.from_numpy(water).to(dev), m_O, m_H)
+        torch.cuda.synchronize()
+        got_x = p.cpu().numpy().astype(np.float64)
+        got_v = vd.cpu().numpy().astype(np.float64)
+    tol = 5e-12 if precision == "f64" else 3e-6
+    # the device's old positions are rigid only to the rounding of their element type (2.4e-7 nm at 6 nm in fp32); how far
+    # that moves the solution grows like 1 / cos(angle / 2), the inverse height of the triangle (11.5 at 170 degrees)
+    kappa = max(1.0, 0.6 / np.cos(np.radians(angle) / 2.0))
+    assert np.abs(got_x - ref_x).max() < tol * kappa
+    m = got_x.reshape(-1, 3, 3)
+    for i, j, d in ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh)):  # the constraints themselves hold to rounding whatever the shape
+        assert np.abs(np.linalg.norm(m[:, i] - m[:, j], axis=1) - d).max() < tol
+    ref_v = oracle.rattle_water_velocities(got_x, v.astype(np_real).astype(np.float64), mass)
+    vtol = (1e-11 if precision == "f64" else 2e-5) * np.abs(v).max()
+    assert np.abs(got_v - ref_v).max() < vtol

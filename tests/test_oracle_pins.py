@@ -655,6 +655,38 @@ def test_shake_water_satisfies_constraints_and_conserves_momentum():
     assert np.abs(oracle.shake_water(x0, shift, wb.mass, wl.R_OH, d_hh) - shift).max() < 1e-12
 
 
+def test_shake_water_runs_to_convergence_for_a_nearly_linear_molecule():
+    """A 170-degree triangle makes the three bond vectors almost dependent: the sweeps need thousands of iterations (water
+    needs ~30).  The answer must still satisfy the constraints to 1e-13, keep every centre of mass, not move when the cap is
+    raised further -- and a cap that is too small must raise instead of returning the unconverged positions (which are
+    8e-6 nm off here, the size of an fp32 parity bar)."""
+    d_oh, m_c, m_e = 0.11, 12.0, 3.0
+    d_ee = 2.0 * d_oh * np.sin(np.radians(170.0) / 2.0)
+    rng = np.random.default_rng(9)
+    h = np.radians(85.0)
+    tri = np.array([[0.0, 0.0, 0.0], [d_oh * np.sin(h), 0.0, d_oh * np.cos(h)], [-d_oh * np.sin(h), 0.0, d_oh * np.cos(h)]])
+    n = 50
+    x0 = (tri[None] + rng.uniform(0.0, 6.0, size=(n, 1, 3))).reshape(-1, 3)
+    mass = np.tile([m_c, m_e, m_e], n)
+    x1 = x0 + 0.001 * rng.normal(0.0, 1.5, size=x0.shape) / np.sqrt(mass)[:, None]
+    xc = oracle.shake_water(x0, x1, mass, d_oh, d_ee)
+    m = xc.reshape(-1, 3, 3)
+    for i, j, d in ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_ee)):
+        assert np.abs(np.linalg.norm(m[:, i] - m[:, j], axis=1) - d).max() < 1e-13
+    w = mass.reshape(-1, 3, 1)
+    com = lambda p: (p.reshape(-1, 3, 3) * w).sum(1) / w.sum(1)
+    assert np.abs(com(xc) - com(x1)).max() < 1e-13
+    assert np.abs(oracle.shake_water(x0, x1, mass, d_oh, d_ee, max_iter=400000) - xc).max() == 0.0
+    with pytest.raises(RuntimeError, match="not converged"):
+        oracle.shake_water(x0, x1, mass, d_oh, d_ee, max_iter=500)
+    v = rng.normal(0.0, 1.0, size=x0.shape) / np.sqrt(mass)[:, None]
+    vc = oracle.rattle_water_velocities(xc, v, mass).reshape(-1, 3, 3)
+    for i, j in ((0, 1), (0, 2), (1, 2)):
+        assert np.abs(((vc[:, i] - vc[:, j]) * (m[:, i] - m[:, j])).sum(1)).max() < 1e-14
+    with pytest.raises(RuntimeError, match="not converged"):
+        oracle.rattle_water_velocities(xc, v, mass, max_iter=20)
+
+
 def test_rattle_water_velocities_pins():
     """Step 6 (PAPER.md:281-292): after the velocity constraint no bond length changes to first order (v_ij . r_ij = 0);
     the impulses are internal and central, so each molecule keeps its linear and angular momentum; a rigid-body velocity
