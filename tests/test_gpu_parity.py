@@ -219,14 +219,22 @@ def test_exceptions_survive_rebuild_and_can_be_cleared_f32():
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("precision,index", [("f32", 1), ("f64", 1), ("f32", 0), ("f64", 0)])
+@pytest.mark.parametrize("precision,index", [("f32", 1), ("f64", 1), ("f32", 0), ("f64", 0), ("f32", "ortho"), ("f64", "ortho"),
+                                             ("f64", "ortho_unwrapped")])
 def test_edge_list_with_vectors_and_shifts(precision, index):
     """dimos_nl_export_edges: the edge set within r_cut equals the oracle's (outside the +-1e-5 nm
     band), and every edge carries d = r_a - r_b - shift L and the shift the oracle computes.  configs[1] has 4 cells per
     axis (image from the cell offsets), configs[0] a single cell (per-pair minimum image)."""
-    wb = wl.make_config(index)
-    r_cut = 1.0 if index == 1 else 0.9
-    db = DeviceBox(wb, precision)
+    pos = None
+    if isinstance(index, str):  # 3 x 4 x 6 cells with different edges; "unwrapped": atoms moved by whole boxes, so that the
+        wb = _ortho_mixture_box((12, 16, 23), 0.2875, 32)  # shifts of an edge are large and differ from atom to atom
+        if index == "ortho_unwrapped":
+            k = np.random.default_rng(3).integers(-3, 4, size=wb.pos.shape)
+            pos = wb.pos.astype(np.float64) + k * wb.box
+    else:
+        wb = wl.make_config(index)
+    r_cut = 0.9 if index == 0 else 1.0
+    db = DeviceBox(wb, precision, pos=pos)
     ctx = dimos.Context(0, precision)
     try:
         nl = dimos.dimos_nl_build(ctx, db.pos, db.box, r_cut, 0.1, db.excl)
