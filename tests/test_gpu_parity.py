@@ -820,3 +820,38 @@ def test_dense_fluid_with_rows_beyond_the_packed_kernels_buffers(precision):
                              epsilon=np.array([0.4, 0.0]), excl_pairs=np.zeros((0, 2), np.int32), mass=np.ones(n))
     rep = run_case(wb, precision, 1.0, 0.1, "rf")
     assert rep["stats"]["row_capacity"] > 1500 and rep["stats"]["pbc_mode"] == 0
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_one_list_handle_rebuilt_for_different_systems(precision):
+    """dimos_nl_build with an existing handle takes ANY new system: another atom count, box, cutoff, cell grid (one cell
+    with per-pair minimum image <-> 3 x 4 x 6 cells), exclusion list (none, water's, random) and type count.  Nothing of the
+    previous system may survive in the handle's buffers: after every rebuild the pair set, forces, energies and virial are
+    compared with the oracle, and the sequence returns to the first system at the end."""
+    import dataclasses
+
+    water216, water3k = wl.make_config(0), wl.make_config(1)
+    ortho = _ortho_mixture_box((12, 16, 23), 0.2875, 77)
+    gas = dataclasses.replace(ortho, pos=ortho.pos[::9].copy(), charge=(ortho.charge[::9] - ortho.charge[::9].mean()).astype(np.float32),
+                              type=ortho.type[::9].copy(), excl_pairs=np.zeros((0, 2), np.int32), mass=ortho.mass[::9].copy())
+    cases = [(water3k, 1.0, 0.1, "rf"), (water216, 0.9, 0.1, "rf"), (ortho, 1.0, 0.1, "ewald"), (gas, 0.8, 0.3, "rf"),
+             (water3k, 0.7, 0.05, "ewald"), (water216, 0.9, 0.1, "rf")]
+    ctx = dimos.Context(0, precision)
+    nl = None
+    try:
+        for k, (wb, r_cut, skin, method) in enumerate(cases):
+            db = DeviceBox(wb, precision)
+            nl = dimos.dimos_nl_build(ctx, db.pos, db.box, r_cut, skin, db.excl if wb.excl_pairs.shape[0] else None, nl=nl)
+            assert torch.equal(nl.pos_at_build, db.pos)
+            pos64 = db.pos.double().cpu().numpy()
+            gp = dimos.dimos_nl_export_pairs(ctx, nl).cpu().numpy()
+            check_neighbor_set(gp, pos64, db.box, r_cut + skin, wb.excl_pairs)
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, method=method)
+            torch.cuda.synchronize()
+            orc = oracle.nonbonded(pos64, db.charge.double().cpu().numpy(), wb.type, db.lj_np, db.box, r_cut, method=METHOD[method],
+                                   excl_pairs=wb.excl_pairs, band=BAND)
+            check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision)
+            assert nl.stats()["n_atoms"] == wb.n_atoms, k
+    finally:
+        ctx.close()
