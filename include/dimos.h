@@ -404,9 +404,10 @@ DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* ctx, const void* pos
  *   pairs   dev, n_exc x 2 int32, (i, j) with i < j, original atom indices; read (copied into the list)
  *   scale   dev, n_exc x 2 double, (s_c, s_lj) per pair; read (copied)
  *   n_exc   >= 0; 0 removes the exceptions.  The copy belongs to the list and survives rebuilds in place.
- * The list is checked once here (indices in range, i < j, every pair among the list's excluded pairs: DIMOS_EINVAL
- * otherwise); the call synchronises the stream.
- * Not checked: that the pairs are excluded pairs (the caller's precondition). */
+ * The list is checked here (indices in range, i < j, every pair among the list's excluded pairs: DIMOS_EINVAL
+ * otherwise); the call synchronises the stream.  Every later dimos_nl_build into the same handle repeats the check against
+ * the atom count and the exclusion list it is given: if the stored exceptions no longer fit, that build removes them and
+ * returns DIMOS_EINVAL (build again, then set the exceptions that belong to the new system). */
 DIMOS_API int dimos_nl_set_exceptions(dimos_ctx* ctx, dimos_nl* nl, const int32_t* pairs, const double* scale,
                                       int64_t n_exc, void* stream);
 

@@ -1099,11 +1099,22 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
         DIMOS_LAUNCH_CHECK(ctx, "excl_fill");
     }
 
+    // the 1-4 exceptions the list holds (dimos_nl_set_exceptions) survive a rebuild only if they still fit the system: indices
+    // below the new N and every pair among the new excluded pairs; checked against the adjacency just built (flags[10])
+    if (nl->n_exc > 0 && (rc = check_exceptions_impl(ctx, nl, (const int32_t*)nl->exc_pairs.p, nl->n_exc, flags + 10, s))) return rc;
+
     // ---- read back: number of units, max cell population, early error flags (sync #1) ----
     int* h = ctx->h_pinned;
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h, flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h + 2, (int*)nl->unit_start.p + ncells, sizeof(int), cudaMemcpyDeviceToHost, s));
+    DIMOS_CUDA_TRY(ctx, cudaMemcpyAsync(h + 3, flags + 10, sizeof(int), cudaMemcpyDeviceToHost, s));
     DIMOS_CUDA_TRY(ctx, cudaStreamSynchronize(s));
+    if (nl->n_exc > 0 && h[3] != 0) {
+        nl->n_exc = 0;  // they cannot be used with this system; the handle itself stays usable for the next build
+        return set_error(ctx, DIMOS_EINVAL,
+                         "the list's 1-4 exceptions do not fit the system it is rebuilt for (index out of range, or a pair that is "
+                         "not among the excluded pairs): they have been removed; set them again after the build");
+    }
     if (h[0] & FLAG_NONFINITE) return set_error(ctx, DIMOS_EINVAL, "non-finite coordinate in pos");
     if (h[0] & FLAG_EXCL_RANGE) return set_error(ctx, DIMOS_EINVAL, "excl_pairs row out of range or not i<j");
     if (h[0] & FLAG_EXCL_OVERFLOW) return set_error(ctx, DIMOS_EINVAL, "an atom has more than 32 exclusion partners");

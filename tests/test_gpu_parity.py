@@ -855,3 +855,40 @@ def test_one_list_handle_rebuilt_for_different_systems(precision):
             assert nl.stats()["n_atoms"] == wb.n_atoms, k
     finally:
         ctx.close()
+
+
+@pytest.mark.gpu
+def test_exceptions_are_revalidated_when_the_handle_is_rebuilt_for_another_system():
+    """The 1-4 exceptions stored in a list index atoms and must be excluded pairs.  Rebuilding the handle for fewer atoms
+    (indices out of range) or with an exclusion list that lacks them (they would be counted twice) must not use them:
+    the build removes them and returns DIMOS_EINVAL; the next build succeeds and the forces are those without exceptions."""
+    big, small = wl.make_config(1), wl.make_config(0)
+    dbig, dsmall = DeviceBox(big, "f32"), DeviceBox(small, "f32")
+    dev = dbig.pos.device
+    exc = torch.from_numpy(big.excl_pairs[-30:].copy()).to(dev)  # pairs of the last molecules: beyond the small system's N
+    scale = torch.full((30, 2), 0.5, dtype=torch.float64, device=dev)
+    ctx = dimos.Context(0, "f32")
+    try:
+        nl = dimos.dimos_nl_build(ctx, dbig.pos, dbig.box, 1.0, 0.1, dbig.excl)
+        dimos.dimos_nl_set_exceptions(ctx, nl, exc, scale)
+        nl = dimos.dimos_nl_build(ctx, dbig.pos, dbig.box, 1.0, 0.1, dbig.excl, nl=nl)  # same system: they stay
+        with pytest.raises(dimos.DimosError, match="exceptions do not fit"):
+            dimos.dimos_nl_build(ctx, dsmall.pos, dsmall.box, 0.9, 0.1, dsmall.excl, nl=nl)
+        nl = dimos.dimos_nl_build(ctx, dsmall.pos, dsmall.box, 0.9, 0.1, dsmall.excl, nl=nl)
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, dsmall.pos, dsmall.charge, dsmall.type, dsmall.lj)
+        orc = oracle.nonbonded(dsmall.pos.double().cpu().numpy(), small.charge, small.type, dsmall.lj_np, dsmall.box, 0.9,
+                               excl_pairs=small.excl_pairs, band=BAND)
+        check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, "f32")
+        # same atoms, but an exclusion list without the exception pairs
+        nl = dimos.dimos_nl_build(ctx, dbig.pos, dbig.box, 1.0, 0.1, dbig.excl, nl=nl)
+        dimos.dimos_nl_set_exceptions(ctx, nl, exc, scale)
+        fewer = torch.from_numpy(big.excl_pairs[:-30].copy()).to(dev)
+        with pytest.raises(dimos.DimosError, match="exceptions do not fit"):
+            dimos.dimos_nl_build(ctx, dbig.pos, dbig.box, 1.0, 0.1, fewer, nl=nl)
+        nl = dimos.dimos_nl_build(ctx, dbig.pos, dbig.box, 1.0, 0.1, dbig.excl, nl=nl)
+        F, E, W = dimos.dimos_nonbonded(ctx, nl, dbig.pos, dbig.charge, dbig.type, dbig.lj)
+        orc = oracle.nonbonded(dbig.pos.double().cpu().numpy(), big.charge, big.type, dbig.lj_np, dbig.box, 1.0,
+                               excl_pairs=big.excl_pairs, band=BAND)
+        check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, "f32")
+    finally:
+        ctx.close()
