@@ -198,6 +198,7 @@ __global__ __launch_bounds__(256) void pme_solve_kernel(typename cplx<real>::typ
     for (int64_t r = warp; r < rows; r += n_warps) {
         const int k2 = (int)(r % K2), k1 = (int)(r / K2);
         const double mx = t1[k1], my = t2[k2];
+        const bool nyq_x = 2 * k1 == K1, nyq_y = 2 * k2 == K2;
         const double f12 = ke_over_piV * t1[K1 + k1] * t2[K2 + k2], m12 = mx * mx + my * my;
         // four wave vectors per lane at a time: their loads are issued together (one row is K3h <= 4 x 32 for meshes up to
         // 254, i.e. one batch), the arithmetic and the stores follow
@@ -228,12 +229,17 @@ __global__ __launch_bounds__(256) void pme_solve_kernel(typename cplx<real>::typ
                 const double wgt = (k3 == 0 || 2 * k3 == K3) ? 1.0 : 2.0;
                 const double e = 0.5 * wgt * bc * (re * re + im * im);
                 const double fac = 2.0 * (inv_m2 + pi2_a2);
+                // The conjugate sits at mesh index (K1 - k1, K2 - k2, K3 - k3); its wave vector is -m, except that an index
+                // K/2 of an even mesh maps to +K/2 for both (m' = m for m <= K/2, Essmann's convention, which the oracle
+                // follows): the off-diagonal virial terms of the pair then cancel instead of doubling
+                const double sx = (wgt == 2.0 && nyq_x) ? 0.0 : 1.0, sy = (wgt == 2.0 && nyq_y) ? 0.0 : 1.0;
+                const double sxy = (wgt == 2.0 && (nyq_x != nyq_y)) ? 0.0 : 1.0;
                 v[0] += e;
                 v[1] += e * (1.0 - fac * mx * mx);
-                v[2] += e * (-fac * mx * my);
-                v[3] += e * (-fac * mx * mz);
+                v[2] += sxy * e * (-fac * mx * my);
+                v[3] += sx * e * (-fac * mx * mz);
                 v[4] += e * (1.0 - fac * my * my);
-                v[5] += e * (-fac * my * mz);
+                v[5] += sy * e * (-fac * my * mz);
                 v[6] += e * (1.0 - fac * mz * mz);
                 typename cplx<real>::type o;
                 o.x = (real)(bc * re);

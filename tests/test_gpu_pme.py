@@ -141,3 +141,29 @@ def test_pme_recip_orthorhombic_box_and_mesh(precision, order):
     mesh = (21, 36, 25)
     F, E, W, p64, q64 = run(pos, q, box, 3.0, mesh, order, precision)
     compare(F, E, W, pme.pme_recip(p64, q64, box, 3.0, mesh, order), precision, q64, 3.0)
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_pme_plan_is_rebuilt_when_mesh_order_or_system_change_within_one_context(precision):
+    """One context, a sequence of calls with different meshes, spline orders, boxes, Ewald parameters and atom counts (the
+    cuFFT plans, the mesh and the per-axis tables are cached in the context and must follow), each against the oracle."""
+    real = torch.float64 if precision == "f64" else torch.float32
+    rng = np.random.default_rng(23)
+    ctx = dimos.Context(0, precision)
+    try:
+        for n, box, alpha, mesh, order in [(300, (2.0, 2.0, 2.0), 3.0, (20, 20, 20), 5), (300, (2.0, 2.0, 2.0), 3.0, (32, 30, 28), 5),
+                                           (1000, (2.0, 2.6, 3.1), 2.6, (32, 30, 28), 4), (300, (2.0, 2.0, 2.0), 3.4, (20, 20, 20), 6),
+                                           (300, (2.2, 2.0, 2.0), 3.4, (20, 20, 20), 6)]:
+            box = np.array(box)
+            pos = rng.uniform(0.0, 1.0, size=(n, 3)) * box
+            q = rng.uniform(-1.0, 1.0, size=n)
+            q -= q.mean()
+            dp = torch.from_numpy(pos).to("cuda", real)
+            dq = torch.from_numpy(q).to("cuda", real)
+            F, E, W = dimos.dimos_pme_recip(ctx, dp, dq, box, alpha, mesh, order=order)
+            torch.cuda.synchronize()
+            p64, q64 = dp.double().cpu().numpy(), dq.double().cpu().numpy()
+            compare(F.double().cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), pme.pme_recip(p64, q64, box, alpha, mesh, order),
+                    precision, q64, alpha)
+    finally:
+        ctx.close()
