@@ -892,3 +892,38 @@ def test_exceptions_are_revalidated_when_the_handle_is_rebuilt_for_another_syste
         check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, "f32")
     finally:
         ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("precision", ["f32", "mixed", "f64"])
+@pytest.mark.parametrize("kind", ["pure_lj", "pure_coulomb", "nothing"])
+def test_systems_without_charges_or_without_lj(precision, kind):
+    """An argon-like fluid (no charges: every row is in the LJ phase, E_coul = 0 exactly), point charges without any LJ
+    parameters (every row in the LJ-free phase after the first call's hint, E_lj = 0 exactly) and a system with neither
+    (all outputs exactly zero).  Two force calls with a rebuild in between, so that the second list is filed by the hint."""
+    import dataclasses
+
+    wb = _mixture_box(16, 4.6, 11)
+    n = wb.n_atoms
+    if kind == "pure_lj":
+        wb = dataclasses.replace(wb, charge=np.zeros(n, np.float32), type=np.zeros(n, np.int32), sigma=np.array([0.26]), epsilon=np.array([0.9]))
+    elif kind == "pure_coulomb":
+        wb = dataclasses.replace(wb, sigma=np.array([0.3, 0.2, 0.0]), epsilon=np.zeros(3))
+    else:
+        wb = dataclasses.replace(wb, charge=np.zeros(n, np.float32), sigma=np.zeros(3), epsilon=np.zeros(3))
+    db = DeviceBox(wb, precision)
+    ctx = dimos.Context(0, precision)
+    try:
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        orc = oracle.nonbonded(db.pos.double().cpu().numpy(), wb.charge, wb.type, db.lj_np, db.box, 1.0, excl_pairs=wb.excl_pairs, band=BAND)
+        for rep in range(2):
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj)
+            F, E, W = F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy()
+            if kind == "nothing":
+                assert not F.any() and not E.any() and not W.any()
+            else:
+                check_nonbonded(F, E, W, orc, precision)
+                assert E[2 if kind == "pure_lj" else 1] == 0.0  # E = (total, LJ, Coulomb, exclusion correction)
+            nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)
+    finally:
+        ctx.close()
