@@ -927,3 +927,37 @@ def test_systems_without_charges_or_without_lj(precision, kind):
             nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)
     finally:
         ctx.close()
+
+
+@pytest.mark.gpu
+def test_two_contexts_and_two_lists_interleaved():
+    """Two contexts of different precision on one device, and two lists in one of them, used in alternation on two streams:
+    a context's workspace, a list's buffers and the per-call reduction state belong to their owner only."""
+    a, b = wl.make_config(1), _mixture_box(16, 4.6, 5)
+    da32, db32, da64 = DeviceBox(a, "f32"), DeviceBox(b, "f32"), DeviceBox(a, "f64")
+    c32, c64 = dimos.Context(0, "f32"), dimos.Context(0, "f64")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    try:
+        with torch.cuda.stream(s1):
+            nl_a = dimos.dimos_nl_build(c32, da32.pos, da32.box, 1.0, 0.1, da32.excl)
+        with torch.cuda.stream(s2):
+            nl_b = dimos.dimos_nl_build(c32, db32.pos, db32.box, 1.0, 0.1, db32.excl)
+            nl_c = dimos.dimos_nl_build(c64, da64.pos, da64.box, 1.0, 0.1, da64.excl)
+        torch.cuda.synchronize()
+        out = {}
+        for rep in range(3):
+            with torch.cuda.stream(s1):
+                out["a"] = dimos.dimos_nonbonded(c32, nl_a, da32.pos, da32.charge, da32.type, da32.lj)
+            with torch.cuda.stream(s2):
+                out["c"] = dimos.dimos_nonbonded(c64, nl_c, da64.pos, da64.charge, da64.type, da64.lj, method="ewald")
+            with torch.cuda.stream(s1):
+                out["b"] = dimos.dimos_nonbonded(c32, nl_b, db32.pos, db32.charge, db32.type, db32.lj, method="ewald")
+        torch.cuda.synchronize()
+        for key, dbx, wb, prec, method in (("a", da32, a, "f32", "rf"), ("b", db32, b, "f32", "ewald"), ("c", da64, a, "f64", "ewald")):
+            F, E, W = out[key]
+            orc = oracle.nonbonded(dbx.pos.double().cpu().numpy(), dbx.charge.double().cpu().numpy(), wb.type, dbx.lj_np, dbx.box, 1.0,
+                                   method=METHOD[method], excl_pairs=wb.excl_pairs, band=BAND)
+            check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, prec)
+    finally:
+        c32.close()
+        c64.close()
