@@ -961,3 +961,14 @@ def test_two_contexts_and_two_lists_interleaved():
     finally:
         c32.close()
         c64.close()
+
+
+@pytest.mark.gpu
+def test_list_beyond_two_to_the_31_entries_f32():
+    """12.6 million atoms (4.2 million waters, edge 50.1 nm): 1.61 million units x a row capacity of 1,344 = 2.17e9 entry
+    slots, beyond the range of a 32-bit index.  Every atom's force, the energies, the virial and the in-cutoff pair count
+    (2.64e9) against the oracle's cell list (~35 s on 16 cores)."""
+    wb = wl.make_scaled(4200000, seed=wl.SEED_BASE + 99, method="rf")
+    rep = run_case(wb, "f32", 1.0, 0.1, "rf", check_set=False, on_device=True)
+    assert rep["stats"]["n_units"] * rep["stats"]["row_capacity"] > 2**31
+    assert rep["n_pairs_cut"] > 2.6e9
