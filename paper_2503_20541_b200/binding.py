@@ -180,6 +180,7 @@ class Context:
         self._alloc_struct = None
         self._guard = int(guard_bytes)
         self._guard_violations: list[tuple[int, int]] = []
+        self.fail_alloc_after: int | None = None  # tests: the allocator callback succeeds this many more times, then returns NULL
         if self._guard % 256 != 0:
             raise ValueError("guard_bytes must be a multiple of 256")
         if torch_allocator:
@@ -187,6 +188,10 @@ class Context:
 
             def _alloc(nbytes, _stream, _user):
                 g = self._guard
+                if self.fail_alloc_after is not None:  # fault injection for the error-path tests
+                    if self.fail_alloc_after <= 0:
+                        return None
+                    self.fail_alloc_after -= 1
                 try:
                     t = torch.empty(int(nbytes) + 2 * g, dtype=torch.uint8, device=dev)
                     if g:

@@ -62,3 +62,59 @@ def test_the_guard_check_itself_detects_a_stray_write():
         assert len(ctx.check_guards()) == 1
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_every_allocation_failure_is_reported_and_leaves_the_context_usable(precision):
+    """The dimos_allocator callback returns NULL at the k-th request, for every k until the whole sequence (list build,
+    force call, exceptions, PME, in-place rebuild) succeeds: each failure must come back as DIMOS_ENOMEM (-3) -- no crash, no
+    other status -- and afterwards the same calls on the same context must succeed and agree with the oracle."""
+    import oracle
+    from gpu_harness import BAND, DeviceBox, METHOD, check_nonbonded
+    from oracle import pme_oracle as pme
+
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, precision)
+    dev = db.pos.device
+    exc = torch.from_numpy(wb.excl_pairs[:50].copy()).to(dev)
+    scale = torch.full((50, 2), 0.5, dtype=torch.float64, device=dev)
+    mesh = (30, 32, 36)
+    ctx = dimos.Context(0, precision)
+
+    def sequence():
+        nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl)
+        try:
+            dimos.dimos_nl_set_exceptions(ctx, nl, exc, scale)
+            out = dimos.dimos_nonbonded(ctx, nl, db.pos, db.charge, db.type, db.lj, method="ewald")
+            rec = dimos.dimos_pme_recip(ctx, db.pos, db.charge, db.box, 3.12, mesh, order=5)
+            nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 1.0, 0.1, db.excl, nl=nl)
+            torch.cuda.synchronize()
+            return out, rec
+        finally:
+            ctx.lib.dimos_nl_destroy(ctx.handle, nl.handle)
+
+    try:
+        failures = 0
+        for k in range(400):
+            ctx.fail_alloc_after = k
+            try:
+                out, rec = sequence()
+                break
+            except dimos.DimosError as err:
+                assert err.args[0].endswith("(status -3)"), err.args[0]
+                failures += 1
+            finally:
+                ctx.fail_alloc_after = None
+        else:
+            raise AssertionError("the sequence never completed")
+        assert failures >= 10, failures  # the sequence makes dozens of requests
+        out, rec = sequence()  # and once more with a healthy allocator
+        F, E, W = out
+        pos64 = db.pos.double().cpu().numpy()
+        orc = oracle.nonbonded(pos64, db.charge.double().cpu().numpy(), wb.type, db.lj_np, db.box, 1.0, method=METHOD["ewald"],
+                               excl_pairs=wb.excl_pairs, band=BAND, exceptions=(wb.excl_pairs[:50], np.full((50, 2), 0.5)))
+        check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, precision)
+        U0, _, _ = pme.pme_recip(pos64, db.charge.double().cpu().numpy(), db.box, 3.12, mesh, 5)
+        assert abs(float(rec[1][0]) - U0) <= (1e-10 if precision == "f64" else 1e-5) * abs(U0)
+    finally:
+        ctx.close()
