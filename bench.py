@@ -549,7 +549,9 @@ def run_ours(args, spec, precision):
     if precision == "f64":
         fp32_peak = 40.0  # NVIDIA's nominal B200 FP64 vector rate (no measured figure on this pool); context only
     # the packed kernel runs fp32 boxes with at least three cells per axis, either method (csrc/nonbonded.cu use_f32x2)
-    kernel_name = "pair_force_f32x2_kernel" if (precision == "f32" and stats["pbc_mode"] == 0) else "pair_force_kernel"
+    # ... the fp64 kernel every DIMOS_F64 call (csrc/pair_f64.cu), the generic kernel the rest (mixed; small fp32 boxes)
+    kernel_name = ("pair_force_f32x2_kernel" if (precision == "f32" and stats["pbc_mode"] == 0)
+                   else "pair_force_f64_kernel" if precision == "f64" else "pair_force_kernel")
     list_bytes = stats["list_bytes"] + stats["n_slots"] * (16 + 4 + 16 + 16)
     roofline = {
         "bound": "alu", "kernel": kernel_name, "achieved": achieved_tflops, "peak": fp32_peak, "unit": "TFLOP/s",
