@@ -3,7 +3,8 @@
 //   A3  needs_rebuild: warp-reduced max of |pos - pos_at_build|^2.
 //   gather: current positions -> cell-relative sorted float4 (x,y,z,q), LJ type, zeroed j-side force
 //           accumulators; block 0 also converts the (sigma, eps) table to (c6, c12).
-//   A4  pair_force: one warp per unit of 8 i-atoms held in registers; every lane owns one j-atom of
+//   A4  pair_force (the generic kernel: DIMOS_MIXED, fp32 boxes with fewer than three cells per axis, rows or LJ tables too
+//       large for the others; fp32 boxes otherwise run pair_f32x2.cu, DIMOS_F64 runs pair_f64.cu): one warp per unit of 8 i-atoms held in registers; every lane owns one j-atom of
 //       a 32-wide chunk of the unit's list, evaluates it against the 8 i-atoms (LJ Eq. 4 + reaction
 //       field Eq. 8, or + Ewald direct space Eq. 10), accumulates F_i in registers over the whole
 //       row and F_j over the 8 slots, then issues ONE vector reduction (red.global.add.v4.f32) per
