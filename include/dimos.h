@@ -28,6 +28,8 @@
  *   Host calls on one context must not overlap in time (no internal locking).  Their device work may: calls may use
  *   different streams and several lists, and up to 64 rebuild-trigger evaluations (dimos_nl_needs_rebuild and the
  *   integrator steps that fuse it) may be in flight at once, each with its own reduction state.
+ *   Every call that touches the device makes the context's device the calling thread's current CUDA device
+ *   (cudaSetDevice) and leaves it current on return; `stream` must belong to that device.
  *   There is no CPU fallback: without a usable CUDA device every compute call fails with
  *   DIMOS_ECUDA.
  */
