@@ -256,9 +256,29 @@ def tau_vs_n(ctx, dimos, dev, spec, precision, timed, tau_force_main, tau_build_
         for _ in range(3):
             dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw)
         t_f = timed(lambda: dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, **kw), reps=20)
+        # a step that keeps the list (trigger with the flag left on the device -> conditional force call), launched call by
+        # call and replayed as one CUDA graph: small boxes are launch-bound (tests/test_gpu_graph.py checks the replayed results)
+        flag = torch.zeros(1, dtype=torch.int32, device=dev)
+
+        def step_body():
+            dimos.dimos_nl_needs_rebuild_static(ctx, pos, nl.pos_at_build, spec.skin, flag)
+            dimos.dimos_nonbonded(ctx, nl, pos, charge, typ, lj, F=F, E=E, virial=W, skip_flag=flag, **kw)
+
+        t_eager = t_graph = None
+        try:
+            step_body()
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                step_body()
+            t_eager = timed(step_body, reps=50)
+            t_graph = timed(graph.replay, reps=50)
+            del graph
+        except Exception as exc:  # the measurement is context: never let it take the bench line down
+            print(f"tau_vs_n: graph capture failed at {b.n_atoms} atoms: {exc}", file=sys.stderr)
         t_b = timed(lambda: dimos.dimos_nl_build(ctx, pos, b.box, spec.r_cut, spec.skin, excl, nl=nl), reps=5)
         rows.append({"n_atoms": int(b.n_atoms), "tau_force_s": t_f, "tau_build_s": t_b, "pairs_in_cutoff": int(n_cut),
-                     "pairs_per_s_force_only": n_cut / t_f})
+                     "pairs_per_s_force_only": n_cut / t_f, "tau_step_eager_s": t_eager, "tau_step_cuda_graph_s": t_graph})
     rows.append({"n_atoms": int(n_main), "tau_force_s": tau_force_main, "tau_build_s": tau_build_main,
                  "pairs_in_cutoff": int(n_cut_main), "pairs_per_s_force_only": n_cut_main / tau_force_main})
     return rows
