@@ -276,9 +276,42 @@ def tau_vs_n(ctx, dimos, dev, spec, precision, timed, tau_force_main, tau_build_
             del graph
         except Exception as exc:  # the measurement is context: never let it take the bench line down
             print(f"tau_vs_n: graph capture failed at {b.n_atoms} atoms: {exc}", file=sys.stderr)
+        # the same for one whole rigid-water MD step that keeps the list (the three calls of md_step_tau, the last two conditional
+        # on the fused trigger's flag); started at rest with dt = 1e-4 fs so that the ~150 timed steps of the unrelaxed box (forces up
+        # to 1e5 kJ mol^-1 nm^-1) stay far below the trigger: the kernels' work does not depend on dt
+        t_md_eager = t_md_graph = None
+        try:
+            water = torch.arange(b.n_atoms, dtype=torch.int32, device=dev).reshape(-1, 3)
+            m_O, m_H = float(b.mass[0]), float(b.mass[1])
+            d_oh = wl.R_OH
+            d_hh = 2.0 * wl.R_OH * float(np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0))
+            x, v = pos.clone(), torch.zeros_like(pos)
+            nl_md = dimos.dimos_nl_build(ctx, x, b.box, spec.r_cut, spec.skin, excl)
+            dimos.dimos_nonbonded(ctx, nl_md, x, charge, typ, lj, F=F, E=E, virial=W, **kw)
+
+            def md_body():
+                fl = dimos.dimos_water_kick_drift_settle(ctx, x, v, F, water, m_O, m_H, d_oh, d_hh, 1e-7, pos_at_build=nl_md.pos_at_build,
+                                                         skin=spec.skin, sync=False)
+                dimos.dimos_nonbonded(ctx, nl_md, x, charge, typ, lj, F=F, E=E, virial=W, skip_flag=fl, **kw)
+                dimos.dimos_water_kick_settle_velocities(ctx, x, v, F, water, m_O, m_H, 1e-7, skip_flag=fl)
+                return fl
+
+            fl = md_body()
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                md_body()
+            t_e, t_g = timed(md_body, reps=50), timed(graph.replay, reps=50)
+            assert int(fl.item()) == 0 and bool(torch.isfinite(x).all()), "the timed MD steps crossed the rebuild trigger"
+            t_md_eager, t_md_graph = t_e, t_g
+            del graph
+            ctx.lib.dimos_nl_destroy(ctx.handle, nl_md.handle)
+        except Exception as exc:
+            print(f"tau_vs_n: MD-step graph measurement failed at {b.n_atoms} atoms: {exc}", file=sys.stderr)
         t_b = timed(lambda: dimos.dimos_nl_build(ctx, pos, b.box, spec.r_cut, spec.skin, excl, nl=nl), reps=5)
         rows.append({"n_atoms": int(b.n_atoms), "tau_force_s": t_f, "tau_build_s": t_b, "pairs_in_cutoff": int(n_cut),
-                     "pairs_per_s_force_only": n_cut / t_f, "tau_step_eager_s": t_eager, "tau_step_cuda_graph_s": t_graph})
+                     "pairs_per_s_force_only": n_cut / t_f, "tau_step_eager_s": t_eager, "tau_step_cuda_graph_s": t_graph,
+                     "tau_md_step_eager_s": t_md_eager, "tau_md_step_cuda_graph_s": t_md_graph})
     rows.append({"n_atoms": int(n_main), "tau_force_s": tau_force_main, "tau_build_s": tau_build_main,
                  "pairs_in_cutoff": int(n_cut_main), "pairs_per_s_force_only": n_cut_main / tau_force_main})
     return rows

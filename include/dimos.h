@@ -319,12 +319,17 @@ DIMOS_API int dimos_virtual_box(dimos_ctx* ctx, const void* pos, int64_t N, doub
  *   inv_mass      dev, N, same type: 1 / m_i
  *   pos_at_build, skin, flag_dev, flag_host (kick_drift only; pos_at_build and flag_dev both NULL to skip): the rebuild
  *                 trigger of dimos_nl_needs_rebuild evaluated on the NEW positions in the same pass.
- *                 A non-NULL flag_host synchronises the stream. */
+ *                 A non-NULL flag_host synchronises the stream.
+ *   skip_flag     (kick only) NULL, or a device word as in dimos_nb_params.skip_flag: if it is non-zero when the kernel runs,
+ *                 vel is left untouched.  With it a whole step -- kick_drift (sets the flag), dimos_nonbonded and this kick, all
+ *                 given the same word -- can be enqueued or recorded in a CUDA graph without the host knowing the flag: on
+ *                 the step where it fires the forces and the second kick do nothing, and the host finishes that step
+ *                 (dimos_nl_build, dimos_nonbonded, this kick, all without skip_flag). */
 DIMOS_API int dimos_vv_kick_drift(dimos_ctx* ctx, void* pos, void* vel, const void* F, const void* inv_mass, int64_t N,
                                   double dt, const void* pos_at_build, double skin, int32_t* flag_dev, int32_t* flag_host,
                                   void* stream);
 DIMOS_API int dimos_vv_kick(dimos_ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt,
-                            void* stream);
+                            const int32_t* skip_flag, void* stream);
 
 /* dimos_settle -- step 3 of velocity Verlet for rigid three-site water: the SETTLE closed form that
  * PAPER.md:327 names, i.e. the positions the three distance constraints |O-H1| = |O-H2| = d_OH, |H1-H2| = d_HH admit when
@@ -393,13 +398,15 @@ DIMOS_API int dimos_berendsen_scale(dimos_ctx* ctx, void* vel, int64_t N, int64_
  *                            the kinetic energy of the constrained velocities (step 8; one double, fp64 accumulation)
  * Same arithmetic as the separate calls, in the same order.  Only atoms listed in `water` (dev, n_w x 3 int32: O, H1, H2)
  * are moved; masses come from m_O, m_H.  pos must satisfy the constraints on entry to kick_drift_settle.  Asynchronous on
- * the stream unless flag_host is given. */
+ * the stream unless flag_host is given.  kick_settle_velocities takes skip_flag as dimos_vv_kick does (vel untouched, and
+ * *ke_dev = 0, when the word is non-zero). */
 DIMOS_API int dimos_water_kick_drift_settle(dimos_ctx* ctx, void* pos, void* vel, const void* F, const int32_t* water,
                                             int64_t n_w, double m_O, double m_H, double d_OH, double d_HH, double dt,
                                             const void* pos_at_build, double skin, int32_t* flag_dev, int32_t* flag_host,
                                             void* stream);
 DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* ctx, const void* pos, void* vel, const void* F, const int32_t* water,
-                                                 int64_t n_w, double m_O, double m_H, double dt, double* ke_dev, void* stream);
+                                                 int64_t n_w, double m_O, double m_H, double dt, double* ke_dev,
+                                                 const int32_t* skip_flag, void* stream);
 
 /* dimos_nl_set_exceptions -- PAPER.md:243 ("1-4 exceptions ... scale the strength of the non-bonded interactions by
  * some common factor", or an individual factor per pair; "handled explicitly by the non-bonded interaction method").

@@ -99,12 +99,12 @@ def load_library() -> ctypes.CDLL:
     lib.dimos_nl_count_within.argtypes = [vp, vp, dbl, ctypes.POINTER(i64), vp]
     lib.dimos_nl_set_exceptions.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.dimos_vv_kick_drift.argtypes = [vp, vp, vp, vp, vp, i64, dbl, vp, dbl, vp, ctypes.POINTER(i32), vp]
-    lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp]
+    lib.dimos_vv_kick.argtypes = [vp, vp, vp, vp, i64, dbl, vp, vp]
     lib.dimos_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp]
     lib.dimos_settle_velocities.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, vp]
     lib.dimos_water_kick_drift_settle.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, dbl, dbl, vp, dbl, vp,
                                                   ctypes.POINTER(i32), vp]
-    lib.dimos_water_kick_settle_velocities.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, vp, vp]
+    lib.dimos_water_kick_settle_velocities.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, vp, vp, vp]
     lib.dimos_berendsen_scale.argtypes = [vp, vp, i64, i64, dbl, dbl, dbl, vp, vp]
     lib.dimos_kinetic_energy.argtypes = [vp, vp, vp, i64, vp, ctypes.POINTER(dbl), vp]
     lib.dimos_berendsen.argtypes = [vp, vp, vp, i64, i64, dbl, dbl, dbl, vp, ctypes.POINTER(dbl), vp]
@@ -467,14 +467,21 @@ class Context:
             return None
         return bool(host.value) if sync else self._flag
 
-    def vv_kick(self, vel, F, inv_mass, dt):
-        """dimos_vv_kick: velocity-Verlet step 5 in place."""
+    def _skip_ptr(self, skip_flag):
+        if skip_flag is None:
+            return None
+        if not skip_flag.is_cuda or skip_flag.dtype != torch.int32 or skip_flag.numel() < 1:
+            raise ValueError("skip_flag must be an int32 device tensor")
+        return skip_flag.data_ptr()
+
+    def vv_kick(self, vel, F, inv_mass, dt, skip_flag=None):
+        """dimos_vv_kick: velocity-Verlet step 5 in place (not at all if the device word skip_flag is non-zero)."""
         vel = self._dev(vel, self.real, 3)
         F = self._dev(F, self.real, 3)
         inv_mass = self._dev(inv_mass, self.real)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_vv_kick(self.handle, vel.data_ptr(), F.data_ptr(), inv_mass.data_ptr(), vel.shape[0], float(dt),
-                                        _stream_ptr())
+                                        self._skip_ptr(skip_flag), _stream_ptr())
         self._check(rc)
 
     def langevin_ou(self, vel, inv_mass, xi, gamma, dt, T):
@@ -531,7 +538,7 @@ class Context:
             return None
         return bool(host.value) if sync else self._flag
 
-    def water_kick_settle_velocities(self, pos, vel, F, water, m_O, m_H, dt, want_ke=False):
+    def water_kick_settle_velocities(self, pos, vel, F, water, m_O, m_H, dt, want_ke=False, skip_flag=None):
         """dimos_water_kick_settle_velocities: steps 5 + 6 for rigid waters in one pass; with want_ke returns the device
         tensor (1 double) that receives the kinetic energy of the constrained velocities."""
         pos = self._dev(pos, self.real, 3)
@@ -542,7 +549,8 @@ class Context:
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_water_kick_settle_velocities(self.handle, pos.data_ptr(), vel.data_ptr(), F.data_ptr(),
                                                              water.data_ptr(), water.shape[0], float(m_O), float(m_H), float(dt),
-                                                             ke.data_ptr() if want_ke else None, _stream_ptr())
+                                                             ke.data_ptr() if want_ke else None, self._skip_ptr(skip_flag),
+                                                             _stream_ptr())
         self._check(rc)
         return ke
 
@@ -706,8 +714,8 @@ def dimos_vv_kick_drift(ctx: Context, pos, vel, F, inv_mass, dt, **kw):
     return ctx.vv_kick_drift(pos, vel, F, inv_mass, dt, **kw)
 
 
-def dimos_vv_kick(ctx: Context, vel, F, inv_mass, dt):
-    return ctx.vv_kick(vel, F, inv_mass, dt)
+def dimos_vv_kick(ctx: Context, vel, F, inv_mass, dt, skip_flag=None):
+    return ctx.vv_kick(vel, F, inv_mass, dt, skip_flag)
 
 
 def dimos_langevin_ou(ctx: Context, vel, inv_mass, xi, gamma, dt, T):
@@ -726,8 +734,8 @@ def dimos_water_kick_drift_settle(ctx: Context, pos, vel, F, water, m_O, m_H, d_
     return ctx.water_kick_drift_settle(pos, vel, F, water, m_O, m_H, d_OH, d_HH, dt, **kw)
 
 
-def dimos_water_kick_settle_velocities(ctx: Context, pos, vel, F, water, m_O, m_H, dt, want_ke=False):
-    return ctx.water_kick_settle_velocities(pos, vel, F, water, m_O, m_H, dt, want_ke=want_ke)
+def dimos_water_kick_settle_velocities(ctx: Context, pos, vel, F, water, m_O, m_H, dt, want_ke=False, skip_flag=None):
+    return ctx.water_kick_settle_velocities(pos, vel, F, water, m_O, m_H, dt, want_ke=want_ke, skip_flag=skip_flag)
 
 
 def dimos_berendsen_scale(ctx: Context, vel, n_dof, T0, tau, dt, ke):

@@ -409,14 +409,15 @@ DIMOS_API int dimos_vv_kick_drift(dimos_ctx* c, void* pos, void* vel, const void
     return DIMOS_OK;
 }
 
-DIMOS_API int dimos_vv_kick(dimos_ctx* c, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, void* stream)
+DIMOS_API int dimos_vv_kick(dimos_ctx* c, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, const int32_t* skip_flag,
+                            void* stream)
 {
     if (!c) return DIMOS_EINVAL;
     Ctx* ctx = reinterpret_cast<Ctx*>(c);
     if (!vel || !F || !inv_mass) return set_error(ctx, DIMOS_EINVAL, "NULL argument");
     if (N <= 0 || !(dt == dt)) return set_error(ctx, DIMOS_EINVAL, "bad N or dt");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
-    return vv_kick_impl(ctx, vel, F, inv_mass, N, dt, (cudaStream_t)stream);
+    return vv_kick_impl(ctx, vel, F, inv_mass, N, dt, skip_flag, (cudaStream_t)stream);
 }
 
 DIMOS_API int dimos_settle(dimos_ctx* c, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w,
@@ -473,7 +474,8 @@ DIMOS_API int dimos_water_kick_drift_settle(dimos_ctx* c, void* pos, void* vel, 
 }
 
 DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* c, const void* pos, void* vel, const void* F, const int32_t* water,
-                                                 int64_t n_w, double m_O, double m_H, double dt, double* ke_dev, void* stream)
+                                                 int64_t n_w, double m_O, double m_H, double dt, double* ke_dev,
+                                                 const int32_t* skip_flag, void* stream)
 {
     if (!c) return DIMOS_EINVAL;
     Ctx* ctx = reinterpret_cast<Ctx*>(c);
@@ -481,7 +483,7 @@ DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* c, const void* pos, 
     if (n_w <= 0) return set_error(ctx, DIMOS_EINVAL, "n_w must be > 0");
     if (!(m_O > 0) || !(m_H > 0) || !(dt == dt)) return set_error(ctx, DIMOS_EINVAL, "bad masses or dt");
     if (cudaSetDevice(ctx->device) != cudaSuccess) return set_error(ctx, DIMOS_ECUDA, "cudaSetDevice failed");
-    return water_step_b_impl(ctx, pos, vel, F, water, n_w, m_O, m_H, dt, ke_dev, (cudaStream_t)stream);
+    return water_step_b_impl(ctx, pos, vel, F, water, n_w, m_O, m_H, dt, ke_dev, skip_flag, (cudaStream_t)stream);
 }
 
 DIMOS_API int dimos_kinetic_energy(dimos_ctx* c, const void* vel, const void* inv_mass, int64_t N, double* ke_dev,

@@ -175,14 +175,14 @@ int vv_kick_drift_impl(Ctx* ctx, void* pos, void* vel, const void* F, const void
 int bbox_impl(Ctx* ctx, const void* pos, int64_t N, unsigned* out_dev, cudaStream_t s);
 int type_histogram_impl(Ctx* ctx, const int32_t* type, int64_t N, int nt, unsigned long long* counts_dev, int* bad_dev,
                         cudaStream_t s);
-int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, cudaStream_t s);
+int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, const int32_t* skip, cudaStream_t s);
 int langevin_ou_impl(Ctx* ctx, void* vel, const void* inv_mass, const void* xi, int64_t N, double gamma, double dt, double T, cudaStream_t s);
 int settle_impl(Ctx* ctx, const void* pos_old, void* pos, void* vel, const int32_t* water, int64_t n_w, double m_O,
                 double m_H, double d_OH, double d_HH, double dt, cudaStream_t s);
 int water_step_a_impl(Ctx* ctx, void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O, double m_H,
                       double d_OH, double d_HH, double dt, const void* ref, double skin, int32_t* flag_dev, cudaStream_t s);
 int water_step_b_impl(Ctx* ctx, const void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O,
-                      double m_H, double dt, double* ke_dev, cudaStream_t s);
+                      double m_H, double dt, double* ke_dev, const int32_t* skip, cudaStream_t s);
 int kinetic_energy_impl(Ctx* ctx, const void* vel, const void* inv_mass, int64_t N, double* ke_dev, cudaStream_t s);
 int berendsen_scale_impl(Ctx* ctx, void* vel, int64_t N, const double* ke_dev, double two_over_dof_kb, double T0,
                          double dt_over_tau, cudaStream_t s);

@@ -45,8 +45,9 @@ __global__ void vv_kick_drift_kernel(real* __restrict__ pos, real* __restrict__ 
 // step 5:  v += (dt/2) F / m
 template <typename real>
 __global__ void vv_kick_kernel(real* __restrict__ vel, const real* __restrict__ F, const real* __restrict__ inv_mass,
-                               int64_t N, real dt)
+                               int64_t N, real dt, const int* __restrict__ skip)
 {
+    if (skip != nullptr && *skip != 0) return;  // the caller's list is stale (see dimos_nb_params.skip_flag): this step is finished by the host
     const real hdt = (real)0.5 * dt;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) {
         const real s = hdt * inv_mass[i];
@@ -254,8 +255,9 @@ __device__ __forceinline__ void settle_vel_molecule(const real (*x)[3], real (*v
 template <typename real, bool KICK>
 __global__ void settle_vel_kernel(const real* __restrict__ pos, real* __restrict__ vel, const real* __restrict__ F,
                                   const int32_t* __restrict__ water, int64_t n_w, real imO, real imH, real hdt,
-                                  double* __restrict__ ke)
+                                  double* __restrict__ ke, const int* __restrict__ skip)
 {
+    if (skip != nullptr && *skip != 0) return;  // the caller's list is stale (see dimos_nb_params.skip_flag): this step is finished by the host
     double acc = 0.0;
     for (int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_w; w += (int64_t)gridDim.x * blockDim.x) {
         const int64_t id[3] = {water[3 * w], water[3 * w + 1], water[3 * w + 2]};
@@ -460,13 +462,13 @@ int langevin_ou_impl(Ctx* ctx, void* vel, const void* inv_mass, const void* xi, 
     return DIMOS_OK;
 }
 
-int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, cudaStream_t s)
+int vv_kick_impl(Ctx* ctx, void* vel, const void* F, const void* inv_mass, int64_t N, double dt, const int32_t* skip, cudaStream_t s)
 {
     const int blocks = grid_for(ctx, N);
     if (ctx->precision == DIMOS_F64)
-        vv_kick_kernel<double><<<blocks, 256, 0, s>>>((double*)vel, (const double*)F, (const double*)inv_mass, N, dt);
+        vv_kick_kernel<double><<<blocks, 256, 0, s>>>((double*)vel, (const double*)F, (const double*)inv_mass, N, dt, skip);
     else
-        vv_kick_kernel<float><<<blocks, 256, 0, s>>>((float*)vel, (const float*)F, (const float*)inv_mass, N, (float)dt);
+        vv_kick_kernel<float><<<blocks, 256, 0, s>>>((float*)vel, (const float*)F, (const float*)inv_mass, N, (float)dt, skip);
     DIMOS_LAUNCH_CHECK(ctx, "vv_kick");
     return DIMOS_OK;
 }
@@ -500,10 +502,10 @@ int settle_vel_impl(Ctx* ctx, const void* pos, void* vel, const int32_t* water, 
     const int blocks = grid_for(ctx, n_w);
     if (ctx->precision == DIMOS_F64)
         settle_vel_kernel<double, false><<<blocks, 256, 0, s>>>((const double*)pos, (double*)vel, nullptr, water, n_w, 1.0 / m_O,
-                                                                1.0 / m_H, 0.0, nullptr);
+                                                                1.0 / m_H, 0.0, nullptr, nullptr);
     else
         settle_vel_kernel<float, false><<<blocks, 256, 0, s>>>((const float*)pos, (float*)vel, nullptr, water, n_w,
-                                                               (float)(1.0 / m_O), (float)(1.0 / m_H), 0.f, nullptr);
+                                                               (float)(1.0 / m_O), (float)(1.0 / m_H), 0.f, nullptr, nullptr);
     DIMOS_LAUNCH_CHECK(ctx, "settle_velocities");
     return DIMOS_OK;
 }
@@ -536,16 +538,16 @@ int water_step_a_impl(Ctx* ctx, void* pos, void* vel, const void* F, const int32
 }
 
 int water_step_b_impl(Ctx* ctx, const void* pos, void* vel, const void* F, const int32_t* water, int64_t n_w, double m_O,
-                      double m_H, double dt, double* ke_dev, cudaStream_t s)
+                      double m_H, double dt, double* ke_dev, const int32_t* skip, cudaStream_t s)
 {
     if (ke_dev) DIMOS_CUDA_TRY(ctx, cudaMemsetAsync(ke_dev, 0, sizeof(double), s));
     const int blocks = grid_for(ctx, n_w);
     if (ctx->precision == DIMOS_F64)
         settle_vel_kernel<double, true><<<blocks, 256, 0, s>>>((const double*)pos, (double*)vel, (const double*)F, water, n_w,
-                                                               1.0 / m_O, 1.0 / m_H, 0.5 * dt, ke_dev);
+                                                               1.0 / m_O, 1.0 / m_H, 0.5 * dt, ke_dev, skip);
     else
         settle_vel_kernel<float, true><<<blocks, 256, 0, s>>>((const float*)pos, (float*)vel, (const float*)F, water, n_w,
-                                                              (float)(1.0 / m_O), (float)(1.0 / m_H), (float)(0.5 * dt), ke_dev);
+                                                              (float)(1.0 / m_O), (float)(1.0 / m_H), (float)(0.5 * dt), ke_dev, skip);
     DIMOS_LAUNCH_CHECK(ctx, "water_kick_settle_velocities");
     return DIMOS_OK;
 }

@@ -75,3 +75,78 @@ def test_steps_between_rebuilds_replayed_as_a_cuda_graph(precision, method):
         assert ctx.launch_count() - launches0 <= (rebuilds + 1) * per_capture + rebuilds * 60
     finally:
         ctx.close()
+
+
+def test_rigid_water_md_steps_replayed_as_a_cuda_graph_f32():
+    """The whole velocity-Verlet step of PAPER.md:281-292 for rigid water as ONE graph: dimos_water_kick_drift_settle (steps
+    1-3 and the trigger, which leaves its flag on the device), dimos_nonbonded (step 4) and dimos_water_kick_settle_velocities
+    (steps 5-6), the last two conditional on that flag.  On the step where the trigger fires the replay has advanced the
+    positions and done nothing else; the host rebuilds the list, computes the forces, applies the second kick and records
+    the graph again.  Every step's forces against the oracle at the trajectory's own positions; the molecules stay rigid;
+    and the trajectory equals, to the rounding of the force sums, the one the same calls produce without a graph."""
+    wb = wl.make_config(1)
+    db = DeviceBox(wb, "f32")
+    dev = db.pos.device
+    n = wb.n_atoms
+    m_O, m_H = float(wb.mass[0]), float(wb.mass[1])
+    d_oh = wl.R_OH
+    d_hh = 2.0 * wl.R_OH * float(np.sin(np.radians(wl.ANGLE_HOH_DEG) / 2.0))
+    water = torch.arange(n, dtype=torch.int32, device=dev).reshape(-1, 3)
+    v0 = torch.from_numpy(wl.maxwell_boltzmann_velocities(wb.mass, 300.0, wl.SEED_BASE + 31).astype(np.float32)).to(dev)
+    dt, skin, n_steps = 0.001, 0.1, 36
+
+    def run(use_graph):
+        ctx = dimos.Context(0, "f32")
+        try:
+            x, v = db.pos.clone(), v0.clone()
+            dimos.dimos_settle_velocities(ctx, x, v, water, m_O, m_H)
+            nl = dimos.dimos_nl_build(ctx, x, db.box, 1.0, skin, db.excl)
+            F, E, W = dimos.dimos_nonbonded(ctx, nl, x, db.charge, db.type, db.lj)
+            e_scale = abs(float(E[0]))
+
+            def body():
+                flag = dimos.dimos_water_kick_drift_settle(ctx, x, v, F, water, m_O, m_H, d_oh, d_hh, dt, pos_at_build=nl.pos_at_build,
+                                                           skin=skin, sync=False)
+                dimos.dimos_nonbonded(ctx, nl, x, db.charge, db.type, db.lj, F=F, E=E, virial=W, skip_flag=flag)
+                dimos.dimos_water_kick_settle_velocities(ctx, x, v, F, water, m_O, m_H, dt, skip_flag=flag)
+                return flag
+
+            def capture():
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g):
+                    body()
+                return g
+
+            flag = ctx._flag  # the word the fused trigger writes when no flag tensor is passed
+            graph = capture() if use_graph else None
+            rebuilds = 0
+            for step in range(n_steps):
+                if use_graph:
+                    graph.replay()
+                else:
+                    body()
+                torch.cuda.synchronize()
+                if int(flag.item()):
+                    nl = dimos.dimos_nl_build(ctx, x, db.box, 1.0, skin, db.excl, nl=nl)
+                    dimos.dimos_nonbonded(ctx, nl, x, db.charge, db.type, db.lj, F=F, E=E, virial=W)
+                    dimos.dimos_water_kick_settle_velocities(ctx, x, v, F, water, m_O, m_H, dt)
+                    rebuilds += 1
+                    if use_graph:
+                        graph = capture()
+                if use_graph:  # forces of this step against the oracle at this step's positions
+                    orc = oracle.nonbonded(x.double().cpu().numpy(), wb.charge, wb.type, db.lj_np, db.box, 1.0,
+                                           excl_pairs=wb.excl_pairs, band=BAND)
+                    check_nonbonded(F.cpu().numpy(), E.cpu().numpy(), W.cpu().numpy(), orc, "f32", e_floor=e_scale)
+            torch.cuda.synchronize()
+            return x.double().cpu().numpy(), v.double().cpu().numpy(), rebuilds
+        finally:
+            ctx.close()
+
+    xg, vg, rebuilds_g = run(True)
+    xe, ve, rebuilds_e = run(False)
+    assert rebuilds_g == rebuilds_e and 2 <= rebuilds_g <= 20, (rebuilds_g, rebuilds_e)
+    mol = xg.reshape(-1, 3, 3)
+    for i, j, d in ((0, 1, d_oh), (0, 2, d_oh), (1, 2, d_hh)):
+        assert np.abs(np.linalg.norm(mol[:, i] - mol[:, j], axis=1) - d).max() < 3e-6
+    # same calls, same order: the two trajectories differ only by the summation order of the force reductions
+    assert np.abs(xg - xe).max() < 2e-5 and np.abs(vg - ve).max() < 2e-3 * np.abs(ve).max()
