@@ -113,3 +113,39 @@ def test_host_entry_points_reject_a_skip_flag():
         assert rc == -1  # DIMOS_EINVAL
     finally:
         ctx.close()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_second_kick_honours_the_skip_flag(precision):
+    """dimos_vv_kick and dimos_water_kick_settle_velocities with the device word set leave the velocities untouched (the
+    kinetic-energy output is 0); with it clear they are the plain calls, bit for bit."""
+    real = torch.float64 if precision == "f64" else torch.float32
+    dev = torch.device("cuda", 0)
+    n_w = 1000
+    g = torch.Generator(device="cpu").manual_seed(5)
+    wb = wl.make_scaled(n_w, seed=wl.SEED_BASE + 8)
+    pos = torch.from_numpy(wb.pos).to(dev, real)
+    vel = torch.randn(3 * n_w, 3, generator=g, dtype=torch.float64).to(dev, real)
+    F = (100.0 * torch.randn(3 * n_w, 3, generator=g, dtype=torch.float64)).to(dev, real)
+    inv_m = torch.from_numpy(1.0 / wb.mass).to(dev, real)
+    water = torch.arange(3 * n_w, dtype=torch.int32, device=dev).reshape(-1, 3)
+    m_O, m_H = float(wb.mass[0]), float(wb.mass[1])
+    flag = torch.ones(1, dtype=torch.int32, device=dev)
+    ctx = dimos.Context(0, precision)
+    try:
+        v = vel.clone()
+        dimos.dimos_vv_kick(ctx, v, F, inv_m, 0.002, skip_flag=flag)
+        assert torch.equal(v, vel)
+        ke = dimos.dimos_water_kick_settle_velocities(ctx, pos, v, F, water, m_O, m_H, 0.002, want_ke=True, skip_flag=flag)
+        assert torch.equal(v, vel) and float(ke.item()) == 0.0
+        flag.zero_()
+        v_plain, v_flag = vel.clone(), vel.clone()
+        dimos.dimos_vv_kick(ctx, v_plain, F, inv_m, 0.002)
+        dimos.dimos_vv_kick(ctx, v_flag, F, inv_m, 0.002, skip_flag=flag)
+        assert torch.equal(v_plain, v_flag) and not torch.equal(v_plain, vel)
+        ke_plain = float(dimos.dimos_water_kick_settle_velocities(ctx, pos, v_plain, F, water, m_O, m_H, 0.002, want_ke=True).item())
+        ke_flag = float(dimos.dimos_water_kick_settle_velocities(ctx, pos, v_flag, F, water, m_O, m_H, 0.002, want_ke=True,
+                                                                 skip_flag=flag).item())
+        assert torch.equal(v_plain, v_flag) and ke_plain > 0.0 and abs(ke_flag - ke_plain) <= 1e-12 * ke_plain
+    finally:
+        ctx.close()
