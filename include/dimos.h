@@ -35,6 +35,8 @@
  *   enqueue only kernels and memsets, allocate nothing and do not synchronise: they may be recorded by a stream capture
  *   and replayed.  The recorded arguments include the list's buffers and sizes, so capture again after every
  *   dimos_nl_build; dimos_nb_params.skip_flag lets the recorded force kernels return at once on the step that needs one.
+ *   A recorded trigger keeps the reduction-state slot (one of the 64) it was recorded with: replay it on one stream, and
+ *   do not run other trigger calls of the same context on another stream at the same time.
  *   There is no CPU fallback: without a usable CUDA device every compute call fails with
  *   DIMOS_ECUDA.
  */
