@@ -31,7 +31,8 @@
  *   Every call that touches the device makes the context's device the calling thread's current CUDA device
  *   (cudaSetDevice) and leaves it current on return; `stream` must belong to that device.
  *   CUDA graphs: dimos_nl_needs_rebuild_static, dimos_nl_needs_rebuild with flag_host = NULL, the integrator calls
- *   without a host flag, and dimos_nonbonded (once an ordinary call on the same list has created its per-step workspace)
+ *   without a host flag, dimos_pme_recip (once a call with the same mesh, order, alpha and box has made its plans), and
+ *   dimos_nonbonded (once an ordinary call on the same list has created its per-step workspace)
  *   enqueue only kernels and memsets, allocate nothing and do not synchronise: they may be recorded by a stream capture
  *   and replayed.  The recorded arguments include the list's buffers and sizes, so capture again after every
  *   dimos_nl_build; dimos_nb_params.skip_flag lets the recorded force kernels return at once on the step that needs one.

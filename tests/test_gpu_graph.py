@@ -150,3 +150,43 @@ def test_rigid_water_md_steps_replayed_as_a_cuda_graph_f32():
         assert np.abs(np.linalg.norm(mol[:, i] - mol[:, j], axis=1) - d).max() < 3e-6
     # same calls, same order: the two trajectories differ only by the summation order of the force reductions
     assert np.abs(xg - xe).max() < 2e-5 and np.abs(vg - ve).max() < 2e-3 * np.abs(ve).max()
+
+
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+def test_pme_recip_replayed_as_a_cuda_graph(precision):
+    """dimos_pme_recip after a first call with the same mesh, order, alpha and box (which makes the cuFFT plans and the
+    per-axis tables) only enqueues kernels, memsets and the two cuFFT executions: recorded once, replayed for moved atoms,
+    against the numpy PME oracle."""
+    from oracle import pme_oracle as pme
+
+    wb = wl.make_config(1)
+    real = torch.float64 if precision == "f64" else torch.float32
+    dev = torch.device("cuda", 0)
+    pos = torch.from_numpy(wb.pos).to(dev, real)
+    q = torch.from_numpy(wb.charge).to(dev, real)
+    mesh, order, alpha = (36, 40, 42), 5, 3.12
+    F = torch.zeros_like(pos)
+    E = torch.zeros(2, dtype=torch.float64, device=dev)
+    W = torch.zeros(3, 3, dtype=torch.float64, device=dev)
+    ctx = dimos.Context(0, precision)
+    try:
+        dimos.dimos_pme_recip(ctx, pos, q, wb.box, alpha, mesh, order=order, F=F, E=E, virial=W)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            dimos.dimos_pme_recip(ctx, pos, q, wb.box, alpha, mesh, order=order, F=F, E=E, virial=W)
+        rng = np.random.default_rng(2)
+        for rep in range(3):
+            pos.add_(torch.from_numpy(rng.normal(0.0, 0.02, size=tuple(pos.shape))).to(dev, real))
+            F.fill_(7.0)
+            E.fill_(-1.0)
+            graph.replay()
+            torch.cuda.synchronize()
+            U0, F0, W0 = pme.pme_recip(pos.double().cpu().numpy(), q.double().cpu().numpy(), wb.box, alpha, mesh, order)
+            e_tol, f_tol, w_tol = (1e-10, 1e-10, 1e-9) if precision == "f64" else (1e-5, 1e-4, 1e-4)
+            assert abs(float(E[0]) - U0) <= e_tol * abs(U0)
+            rms = np.sqrt((F0 ** 2).sum(axis=1).mean())
+            assert np.sqrt(((F.double().cpu().numpy() - F0) ** 2).sum(axis=1)).max() <= f_tol * rms
+            assert np.abs(W.cpu().numpy() - W0).max() <= w_tol * np.abs(W0).max()
+    finally:
+        ctx.close()
