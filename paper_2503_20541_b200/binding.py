@@ -446,7 +446,7 @@ class Context:
         self._check(rc)
         return np.array(list(box), dtype=np.float64), np.array(list(lo), dtype=np.float64)
 
-    def vv_kick_drift(self, pos, vel, F, inv_mass, dt, pos_at_build=None, skin=0.0, sync=True):
+    def vv_kick_drift(self, pos, vel, F, inv_mass, dt, pos_at_build=None, skin=0.0, sync=True, flag=None):
         """dimos_vv_kick_drift: velocity-Verlet steps 1 + 2 in place; with pos_at_build also the rebuild flag (bool when
         sync, else the device flag tensor)."""
         pos = self._dev(pos, self.real, 3)
@@ -455,17 +455,18 @@ class Context:
         inv_mass = self._dev(inv_mass, self.real)
         host = ctypes.c_int32(0)
         trig = pos_at_build is not None
+        flag = self._flag if flag is None else self._dev(flag, torch.int32)  # the device word that receives the trigger's result
         if trig:
             pos_at_build = self._dev(pos_at_build, self.real, 3)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_vv_kick_drift(self.handle, pos.data_ptr(), vel.data_ptr(), F.data_ptr(), inv_mass.data_ptr(),
                                               pos.shape[0], float(dt), pos_at_build.data_ptr() if trig else None, float(skin),
-                                              self._flag.data_ptr() if trig else None,
+                                              flag.data_ptr() if trig else None,
                                               ctypes.byref(host) if (trig and sync) else None, _stream_ptr())
         self._check(rc)
         if not trig:
             return None
-        return bool(host.value) if sync else self._flag
+        return bool(host.value) if sync else flag
 
     def _skip_ptr(self, skip_flag):
         if skip_flag is None:
@@ -517,7 +518,8 @@ class Context:
                                                   float(m_O), float(m_H), _stream_ptr())
         self._check(rc)
 
-    def water_kick_drift_settle(self, pos, vel, F, water, m_O, m_H, d_OH, d_HH, dt, pos_at_build=None, skin=0.0, sync=True):
+    def water_kick_drift_settle(self, pos, vel, F, water, m_O, m_H, d_OH, d_HH, dt, pos_at_build=None, skin=0.0, sync=True,
+                                flag=None):
         """dimos_water_kick_drift_settle: steps 1 + 2 + 3 for rigid waters in one pass; returns the rebuild flag like
         vv_kick_drift (None without pos_at_build)."""
         pos = self._dev(pos, self.real, 3)
@@ -526,17 +528,18 @@ class Context:
         water = self._dev(water, torch.int32, 3)
         host = ctypes.c_int32(0)
         trig = pos_at_build is not None
+        flag = self._flag if flag is None else self._dev(flag, torch.int32)  # the device word that receives the trigger's result
         if trig:
             pos_at_build = self._dev(pos_at_build, self.real, 3)
         with torch.cuda.device(self.device):
             rc = self.lib.dimos_water_kick_drift_settle(
                 self.handle, pos.data_ptr(), vel.data_ptr(), F.data_ptr(), water.data_ptr(), water.shape[0], float(m_O),
                 float(m_H), float(d_OH), float(d_HH), float(dt), pos_at_build.data_ptr() if trig else None, float(skin),
-                self._flag.data_ptr() if trig else None, ctypes.byref(host) if (trig and sync) else None, _stream_ptr())
+                flag.data_ptr() if trig else None, ctypes.byref(host) if (trig and sync) else None, _stream_ptr())
         self._check(rc)
         if not trig:
             return None
-        return bool(host.value) if sync else self._flag
+        return bool(host.value) if sync else flag
 
     def water_kick_settle_velocities(self, pos, vel, F, water, m_O, m_H, dt, want_ke=False, skip_flag=None):
         """dimos_water_kick_settle_velocities: steps 5 + 6 for rigid waters in one pass; with want_ke returns the device

@@ -105,8 +105,8 @@ def test_rigid_water_md_steps_replayed_as_a_cuda_graph_f32():
             e_scale = abs(float(E[0]))
 
             def body():
-                flag = dimos.dimos_water_kick_drift_settle(ctx, x, v, F, water, m_O, m_H, d_oh, d_hh, dt, pos_at_build=nl.pos_at_build,
-                                                           skin=skin, sync=False)
+                dimos.dimos_water_kick_drift_settle(ctx, x, v, F, water, m_O, m_H, d_oh, d_hh, dt, pos_at_build=nl.pos_at_build,
+                                                    skin=skin, sync=False, flag=flag)
                 dimos.dimos_nonbonded(ctx, nl, x, db.charge, db.type, db.lj, F=F, E=E, virial=W, skip_flag=flag)
                 dimos.dimos_water_kick_settle_velocities(ctx, x, v, F, water, m_O, m_H, dt, skip_flag=flag)
                 return flag
@@ -117,7 +117,7 @@ def test_rigid_water_md_steps_replayed_as_a_cuda_graph_f32():
                     body()
                 return g
 
-            flag = ctx._flag  # the word the fused trigger writes when no flag tensor is passed
+            flag = torch.zeros(1, dtype=torch.int32, device=dev)  # the device word the trigger writes and the other two calls read
             graph = capture() if use_graph else None
             rebuilds = 0
             for step in range(n_steps):
