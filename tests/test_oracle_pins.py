@@ -776,3 +776,32 @@ def test_langevin_ou_pins():
         if k in (10, 30):
             c = ((v * v0) / kT_m).mean()
             assert c == pytest.approx(math.exp(-gamma * k * dt), abs=8 / math.sqrt(3 * n))
+
+
+def test_count_pairs_equals_the_length_of_the_pair_list_and_a_kd_tree_count():
+    """oracle.count_pairs (the count-only call that brackets the metric's numerator at the full-size configs) against
+    (a) the length of the pair list both algorithms return and (b) scipy's periodic k-d tree minus the excluded pairs in
+    range, on configs[1] (4 cells per axis), a single-cell box and a non-cubic box, with and without exclusions."""
+    from scipy.spatial import cKDTree
+
+    cases = [(wl.make_config(1), None, 1.0), (wl.make_config(1), None, 0.37), (small_box(m=40, edge=2.4, seed=4), None, 1.1),
+             (small_box(m=60, edge=2.6, seed=9), np.array([2.6, 3.1, 2.9]), 1.2)]
+    for wb, box, r in cases:
+        box = wb.box if box is None else box
+        pos = wb.pos.astype(np.float64)
+        for excl in (wb.excl_pairs, None):
+            n_list = len(oracle.neighbor_pairs(pos, box, r, excl, "celllist"))
+            assert oracle.count_pairs(pos, box, r, excl) == n_list
+            assert oracle.count_pairs(pos, box, r, excl, algorithm="bruteforce") == n_list
+            if r <= 0.5 * box.min():  # scipy's periodic tree needs r < L/2
+                pairs = cKDTree(pos % box, boxsize=box).query_pairs(r, output_type="ndarray")
+                d = pos[pairs[:, 0]] - pos[pairs[:, 1]]
+                d -= box * np.rint(d / box)
+                inside = (d * d).sum(1) < r * r  # the tree's test is <=; the oracle's is strict (reading C-4)
+                n_tree = int(inside.sum())
+                if excl is not None:
+                    i, j = excl[:, 0], excl[:, 1]
+                    de = pos[i] - pos[j]
+                    de -= box * np.rint(de / box)
+                    n_tree -= int(((de * de).sum(1) < r * r).sum())
+                assert n_list == n_tree, (r, n_list, n_tree)

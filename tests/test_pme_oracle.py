@@ -180,3 +180,22 @@ def test_pme_madelung_constant_through_the_mesh():
     want = -0.5 * len(q) * MADELUNG_NACL * KE / 0.5
     assert e_real + e_rec + pme.ewald_self(q, alpha) == pytest.approx(want, rel=2e-6)
     assert np.abs(F).max() < 1e-3 * abs(want)  # forces vanish by symmetry up to the mesh error
+
+
+def test_bspline_moduli_special_values():
+    """|b(m)|^2 (Essmann Eq. 4.4): 1 at m = 0 for every order (the weights M_n(k + 1) sum to one); identically 1 for order 2
+    (M_2(1) = 1 is the only weight); symmetric under m -> K - m (complex conjugation); never below 1 (|sum w e^{i..}| <= sum w
+    = 1 for non-negative weights); for order 4 at m = K/2 the closed value 1 / (M_4(1) - M_4(2) + M_4(3))^2 = 1 / (1/3)^2 = 9;
+    and for an odd order the vanishing denominator at 2 m = K is replaced by the neighbours' average (reading C-25)."""
+    for n in (2, 3, 4, 5, 6):
+        for K in (16, 21, 30):
+            mod = pme.bspline_moduli(n, K)
+            assert mod[0] == pytest.approx(1.0, rel=1e-14)
+            assert np.allclose(mod[1:], mod[1:][::-1], rtol=1e-12)
+            assert np.all(mod >= 1.0 - 1e-12)
+            if n == 2:
+                assert np.allclose(mod, 1.0, rtol=1e-14)
+    assert pme.bspline_moduli(4, 16)[8] == pytest.approx(9.0, rel=1e-12)
+    mod = pme.bspline_moduli(5, 16)  # odd order, even mesh: sum_k M_5(k + 1) (-1)^k = 1/24 - 11/24 + 11/24 - 1/24 = 0
+    den = 1.0 / mod
+    assert den[8] == pytest.approx(0.5 * (den[7] + den[9]), rel=1e-12)
