@@ -149,7 +149,8 @@ DIMOS_API int dimos_destroy(dimos_ctx* ctx);
  *   box           host, 3 doubles: orthorhombic box edges in nm
  *   r_cut, skin   nm; r_cut > 0, skin >= 0, r_cut <= min(box)/2 else DIMOS_EBOX
  *   excl_pairs    dev, n_excl x 2 int32, each row (i, j) with i < j, rows unique (reading C-17);
- *                 may be NULL when n_excl == 0.  At most 32 exclusion partners per atom.
+ *                 may be NULL when n_excl == 0.  At most 32 exclusion partners per atom.  Rows out of range, with i >= j,
+ *                 or listed twice, and atoms with more partners, are reported as DIMOS_EINVAL.
  *   pos_at_build  dev, N x 3, same type as pos, caller-owned; written with a copy of pos (the
  *                 reference positions of the rebuild trigger)
  *   stream        cudaStream_t

@@ -35,7 +35,8 @@ enum : int {
     FLAG_NONFINITE = 4,        // non-finite coordinate
     FLAG_CELL_OVERFLOW = 8,    // more than KD_MAX atoms in one cell
     FLAG_EXCL_OVERFLOW = 16,   // more than MAX_EXCL_PER_ATOM partners for one atom
-    FLAG_EXCL_RANGE = 32       // exclusion index out of range / not i<j
+    FLAG_EXCL_RANGE = 32,      // exclusion index out of range / not i<j
+    FLAG_EXCL_DUP = 64         // the same exclusion pair listed twice
 };
 
 template <typename real> struct vec4;

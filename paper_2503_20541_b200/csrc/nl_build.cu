@@ -462,6 +462,19 @@ __global__ void excl_fill_kernel(const int2* __restrict__ pairs, int64_t n_excl,
     adj[start[p.x] + atomicAdd(&cursor[p.x], 1)] = p.y;
     adj[start[p.y] + atomicAdd(&cursor[p.y], 1)] = p.x;
 }
+// every pair must be listed once (reading C-17): a duplicate would be corrected twice by the Ewald exclusion correction
+__global__ void excl_unique_kernel(const int2* __restrict__ pairs, int64_t n_excl, int64_t N, const int* __restrict__ start,
+                                   const int* __restrict__ adj, int* __restrict__ flags)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_excl) return;
+    int2 p = pairs[k];
+    if (p.x < 0 || p.y < 0 || p.x >= N || p.y >= N || p.x >= p.y) return;
+    int seen = 0;
+    const int e = min(start[p.x + 1], start[p.x] + MAX_EXCL_PER_ATOM);
+    for (int q = start[p.x]; q < e; ++q) seen += adj[q] == p.y ? 1 : 0;
+    if (seen > 1) atomicOr(&flags[0], FLAG_EXCL_DUP);
+}
 __global__ void zero_int_kernel(int* __restrict__ p, int64_t n)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1097,6 +1110,9 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
         excl_fill_kernel<<<(unsigned)((n_excl + T - 1) / T), T, 0, s>>>((const int2*)nl->excl_pairs.p, n_excl, N,
                                                                         (const int*)nl->excl_start.p, excl_deg, (int*)nl->excl_adj.p);
         DIMOS_LAUNCH_CHECK(ctx, "excl_fill");
+        excl_unique_kernel<<<(unsigned)((n_excl + T - 1) / T), T, 0, s>>>((const int2*)nl->excl_pairs.p, n_excl, N, (const int*)nl->excl_start.p,
+                                                                          (const int*)nl->excl_adj.p, flags);
+        DIMOS_LAUNCH_CHECK(ctx, "excl_unique");
     }
 
     // the 1-4 exceptions the list holds (dimos_nl_set_exceptions) survive a rebuild only if they still fit the system: indices
@@ -1118,6 +1134,7 @@ static int nl_build_typed(Ctx* ctx, NL* nl, const real* pos, const int32_t* excl
     if (h[0] & FLAG_NONFINITE) return set_error(ctx, DIMOS_EINVAL, "non-finite coordinate in pos");
     if (h[0] & FLAG_EXCL_RANGE) return set_error(ctx, DIMOS_EINVAL, "excl_pairs row out of range or not i<j");
     if (h[0] & FLAG_EXCL_OVERFLOW) return set_error(ctx, DIMOS_EINVAL, "an atom has more than 32 exclusion partners");
+    if (h[0] & FLAG_EXCL_DUP) return set_error(ctx, DIMOS_EINVAL, "excl_pairs lists a pair more than once");
     nl->max_cell_count = h[1];
     if (h[1] > KD_MAX) return set_error(ctx, DIMOS_EOVERFLOW, "more than 4096 atoms in one cell (r_cut+skin too large for this density)");
     nl->n_units = h[2];

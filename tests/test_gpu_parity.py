@@ -528,6 +528,10 @@ def test_error_codes():
         with pytest.raises(dimos.DimosError) as ei:
             dimos.dimos_nl_build(ctx, db.pos, db.box, 0.9, 0.1, bad_excl)
         assert ei.value.status == -1
+        dup_excl = torch.cat([db.excl, db.excl[7:8]])  # one pair listed twice (reading C-17: rows are unique)
+        with pytest.raises(dimos.DimosError, match="more than once") as ei:
+            dimos.dimos_nl_build(ctx, db.pos, db.box, 0.9, 0.1, dup_excl)
+        assert ei.value.status == -1
         nl = dimos.dimos_nl_build(ctx, db.pos, db.box, 0.9, 0.1, db.excl)
         nl.r_cut = 0.8  # params.r_cut differs from the build r_cut
         with pytest.raises(dimos.DimosError) as ei:
