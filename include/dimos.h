@@ -419,7 +419,8 @@ DIMOS_API int dimos_water_kick_settle_velocities(dimos_ctx* ctx, const void* pos
  * then adds, for every exception, s_lj * U_LJ(r) (Eq. 4) + s_c * k_e q_i q_j / r (Eq. 7) at the minimum-image distance,
  * without cutoff, switch, reaction-field or Ewald modification, and the matching forces and virial.  The LJ part goes
  * into E[1], the Coulomb part into E[2].
- *   pairs   dev, n_exc x 2 int32, (i, j) with i < j, original atom indices; read (copied into the list)
+ *   pairs   dev, n_exc x 2 int32, (i, j) with i < j, original atom indices, each pair once (a repeated row is applied
+ *           repeatedly; not checked); read (copied into the list)
  *   scale   dev, n_exc x 2 double, (s_c, s_lj) per pair; read (copied)
  *   n_exc   >= 0; 0 removes the exceptions.  The copy belongs to the list and survives rebuilds in place.
  * The list is checked here (indices in range, i < j, every pair among the list's excluded pairs: DIMOS_EINVAL
