@@ -484,6 +484,19 @@ def run_ours(args, spec, precision):
     clocks = sampler.stop() if rank == 0 else None
     rebuilds = state["rebuilds"]
     assert bool(torch.isfinite(E).all()), "non-finite energy in the timed region"
+    # the forces the timed loop left behind are those of its last step's positions: a fresh, unconditional evaluation on a
+    # list rebuilt at these positions must reproduce them (to the summation order of the reductions)
+    F_loop, E_loop = F.clone(), E.clone()
+    nl_chk = dimos.dimos_nl_build(ctx, pos, box.box, spec.r_cut, spec.skin, excl)
+    F_chk, E_chk, _ = dimos.dimos_nonbonded(ctx, nl_chk, pos, charge, typ, lj, **kw)
+    torch.cuda.synchronize()
+    f_rms = float(F_chk.double().pow(2).sum(1).mean().sqrt())
+    last_step_check = {"max_dF_over_rms": float((F_loop.double() - F_chk.double()).pow(2).sum(1).sqrt().max()) / f_rms,
+                       "dE_over_E": abs(float(E_loop[0] - E_chk[0])) / max(abs(float(E_chk[0])), 1e-300)}
+    tol_f, tol_e = (1e-9, 1e-10) if precision == "f64" else (2e-4, 1e-5)
+    assert last_step_check["max_dF_over_rms"] < tol_f and last_step_check["dE_over_E"] < tol_e, last_step_check
+    ctx.lib.dimos_nl_destroy(ctx.handle, nl_chk.handle)
+    del F_chk, E_chk, nl_chk
 
     # separate timings of the three calls (tau_force, tau_build, tau_check), list valid, median of 20
     def timed(fn, reps=20):
@@ -632,6 +645,7 @@ def run_ours(args, spec, precision):
         "tau": {"force_s": tau_force, "check_s": tau_check, "build_s": tau_build, "rebuilds": rebuilds,
                 "pairs_per_s_force_only": n_cut / tau_force},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "pme": pme,
+        "last_step_check": last_step_check,
         "list": {k: stats[k] for k in ("n_units", "n_entries", "n_entries_padded", "n_pair_slots", "list_bytes", "row_capacity")},
     }
     if not args.no_scan and world == 1 and precision != "f64":

@@ -46,6 +46,7 @@ def test_bench_line_has_the_contracts_keys_and_consistent_numbers():
     assert r["frac"] == pytest.approx(r["achieved"] / r["peak"], rel=1e-9) and 0 < r["frac"] < 1
     assert r["achieved"] == pytest.approx(r["flops_per_launch"] / (r["kernel_ms"] * 1e-3) * 1e-12, rel=1e-6)
     assert r["kernel"] == "pair_force_f32x2_kernel" and r["kernel_launches_timed"] + r["kernel_launches_skipped_on_device"] >= d["steps"]
+    assert d["last_step_check"]["max_dF_over_rms"] < 2e-4 and d["last_step_check"]["dE_over_E"] < 1e-5  # the loop's last forces are real
     b = d["cpu_baseline"]
     assert b["kind"] == "oracle" and b["cores"] >= 1 and b["value"] > 0 and b["unit"] == d["unit"] and b["same_config"] is True
     assert b["value"] < d["value"]
